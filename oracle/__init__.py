@@ -1,0 +1,229 @@
+"""CPU oracle -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+ctypes binding over oracle/liboracle.so (oracle.cpp + oracle_bp.cpp, double
+precision, no code shared with the CUDA path).  Only tests/,
+__graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference arm may
+import this package; the product package paper_2209_08450_b200 never does.
+
+Every wrapper below only marshals numpy arrays; the arithmetic is in the C++
+files, each function citing the PAPER.md passage / DESIGN.md reading it follows.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "liboracle.so")
+_SRC = [os.path.join(_HERE, "oracle.cpp"), os.path.join(_HERE, "oracle_bp.cpp")]
+
+FILTERS = {"ramp": 0, "shepp": 1, "parzen": 2}
+METHODS = {"grid": 0, "exact": 1, "lin": 2}
+DEFAULT_M = 4
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ (building the checker is not using it)."""
+    stale = force or not os.path.exists(_SO) or any(
+        os.path.getmtime(s) > os.path.getmtime(_SO) for s in _SRC)
+    if stale:
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared",
+                               "-o", _SO] + _SRC)
+    return _SO
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_kernel_alpha.restype = C.c_double
+        _lib.orc_kernel_alpha.argtypes = [C.c_int]
+        _lib.orc_num_threads.restype = C.c_int
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _c128(a):
+    return np.ascontiguousarray(a, dtype=np.complex128)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def kernel_alpha(m: int = DEFAULT_M) -> float:
+    return float(lib().orc_kernel_alpha(int(m)))
+
+
+def dft(x, sign=-1):
+    x = _c128(x)
+    X = np.empty_like(x)
+    lib().orc_dft(_p(x), _p(X), C.c_int(x.size), C.c_int(sign))
+    return X
+
+
+def fft(x, sign=-1):
+    x = _c128(x)
+    X = np.empty_like(x)
+    lib().orc_fft(_p(x), _p(X), C.c_int(x.size), C.c_int(sign))
+    return X
+
+
+def neglog(raw, flat, dark):
+    """raw u16 [nproj][nz][n], flat/dark f32 [nz][n] -> p f64 [nz][nproj][n]  (S1+S2)."""
+    raw = np.ascontiguousarray(raw, dtype=np.uint16)
+    nproj, nz, n = raw.shape
+    flat, dark = _f32(flat), _f32(dark)
+    assert flat.shape == (nz, n) and dark.shape == (nz, n)
+    p = np.empty((nz, nproj, n))
+    lib().orc_neglog(_p(raw), _p(flat), _p(dark), C.c_int(nproj), C.c_int(nz), C.c_int(n), _p(p))
+    return p
+
+
+def filter_table(M, filt="ramp"):
+    H = np.empty(M)
+    lib().orc_filter(C.c_int(M), C.c_int(FILTERS[filt]), _p(H))
+    return H
+
+
+def filter_rows(p, filt="ramp"):
+    """p [rows][n] -> q [rows][n]  (S3)."""
+    p = _f64(p)
+    rows, n = p.shape
+    q = np.empty_like(p)
+    lib().orc_filter_rows(_p(p), C.c_int(rows), C.c_int(n), C.c_int(FILTERS[filt]), _p(q))
+    return q
+
+
+def spectrum(q, center):
+    """q [nproj][n] -> G complex [nproj][2n], FFT order  (S4)."""
+    q = _f64(q)
+    nproj, n = q.shape
+    G = np.empty((nproj, 2 * n), dtype=np.complex128)
+    lib().orc_spectrum(_p(q), C.c_int(nproj), C.c_int(n), C.c_double(center), _p(G))
+    return G
+
+
+def _bp(fn, G, theta, n, m=None):
+    G = _c128(G)
+    theta = _f32(theta)
+    nproj = theta.size
+    assert G.shape == (nproj, 2 * n)
+    fre, fim = np.empty((n, n)), np.empty((n, n))
+    if m is None:
+        fn(_p(G), _p(theta), C.c_int(nproj), C.c_int(n), _p(fre), _p(fim))
+    else:
+        fn(_p(G), _p(theta), C.c_int(nproj), C.c_int(n), C.c_int(m), _p(fre), _p(fim))
+    return fre + 1j * fim
+
+
+def backproject_exact(G, theta, n):
+    """B_exact: complex image [n][n] (real part = the slice; imag = packed second slice)."""
+    return _bp(lib().orc_backproject_exact, G, theta, n)
+
+
+def backproject_grid(G, theta, n, m=DEFAULT_M):
+    """B_grid = S5 -> S6 -> S7: complex image [n][n]."""
+    return _bp(lib().orc_backproject_grid, G, theta, n, m)
+
+
+def backproject_lin(q, theta, center):
+    q = _f64(q)
+    theta = _f32(theta)
+    nproj, n = q.shape
+    f = np.empty((n, n))
+    lib().orc_backproject_lin(_p(q), _p(theta), C.c_int(nproj), C.c_int(n), C.c_double(center), _p(f))
+    return f
+
+
+def project_lin_adjoint(f, theta, center):
+    f = _f64(f)
+    theta = _f32(theta)
+    n = f.shape[0]
+    q = np.empty((theta.size, n))
+    lib().orc_project_lin_adjoint(_p(f), _p(theta), C.c_int(theta.size), C.c_int(n),
+                                  C.c_double(center), _p(q))
+    return q
+
+
+def grid(G, theta, n, m=DEFAULT_M):
+    """S5: G [nproj][2n] -> F [2n][2n] (FFT order, row = l2)."""
+    G = _c128(G)
+    theta = _f32(theta)
+    F = np.empty((2 * n, 2 * n), dtype=np.complex128)
+    lib().orc_grid(_p(G), _p(theta), C.c_int(theta.size), C.c_int(n), C.c_int(m), _p(F))
+    return F
+
+
+def grid_adjoint(F, theta, n, m=DEFAULT_M):
+    F = _c128(F)
+    theta = _f32(theta)
+    G = np.empty((theta.size, 2 * n), dtype=np.complex128)
+    lib().orc_grid_adjoint(_p(F), _p(theta), C.c_int(theta.size), C.c_int(n), C.c_int(m), _p(G))
+    return G
+
+
+def fft2(F, sign=+1):
+    """S6 (sign=+1: unnormalised inverse; -1: forward)."""
+    F = _c128(F)
+    g = np.empty_like(F)
+    lib().orc_fft2(_p(F), C.c_int(F.shape[0]), C.c_int(sign), _p(g))
+    return g
+
+
+def deapod_crop(g, n, m=DEFAULT_M):
+    """S7: g [2n][2n] -> complex f [n][n]."""
+    g = _c128(g)
+    fre, fim = np.empty((n, n)), np.empty((n, n))
+    lib().orc_deapod_crop(_p(g), C.c_int(n), C.c_int(m), _p(fre), _p(fim))
+    return fre + 1j * fim
+
+
+def deapod_crop_adjoint(f, n, m=DEFAULT_M):
+    f = _c128(f)
+    fre, fim = _f64(f.real), _f64(f.imag)
+    g = np.empty((2 * n, 2 * n), dtype=np.complex128)
+    lib().orc_deapod_crop_adjoint(_p(fre), _p(fim), C.c_int(n), C.c_int(m), _p(g))
+    return g
+
+
+def fbp_from_sino(p, theta, center, filt="ramp", m=DEFAULT_M, method="grid", return_q=False):
+    """p f64 [nz][nproj][n] -> out f64 [nz][n][n] (S3..S7 or the two definitions)."""
+    p = _f64(p)
+    theta = _f32(theta)
+    nz, nproj, n = p.shape
+    out = np.empty((nz, n, n))
+    q = np.empty_like(p) if return_q else None
+    lib().orc_fbp_from_sino(_p(p), _p(theta), C.c_int(nproj), C.c_int(nz), C.c_int(n),
+                            C.c_double(center), C.c_int(FILTERS[filt]), C.c_int(m),
+                            C.c_int(METHODS[method]), _p(out), _p(q) if return_q else None)
+    return (out, q) if return_q else out
+
+
+def recon(raw, flat, dark, theta, center, filt="ramp", m=DEFAULT_M, method="grid"):
+    """uint16 counts -> reconstruction, S1..S7.  raw [nproj][nz][n] -> out [nz][n][n]."""
+    raw = np.ascontiguousarray(raw, dtype=np.uint16)
+    nproj, nz, n = raw.shape
+    flat, dark, theta = _f32(flat), _f32(dark), _f32(theta)
+    out = np.empty((nz, n, n))
+    lib().orc_recon(_p(raw), _p(flat), _p(dark), _p(theta), C.c_int(nproj), C.c_int(nz), C.c_int(n),
+                    C.c_double(center), C.c_int(FILTERS[filt]), C.c_int(m), C.c_int(METHODS[method]),
+                    _p(out))
+    return out

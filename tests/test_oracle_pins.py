@@ -1,0 +1,313 @@
+"""Pins P1..P9: the CPU oracle checked against what the paper and the mathematics fix
+(closed forms, definitions, invariants) -- never against itself or the CUDA path.
+DESIGN.md "Oracle and pins" lists what each pin would catch.  CPU only.
+"""
+import numpy as np
+import pytest
+
+import oracle as orc
+import synthgen as sg
+
+
+def rl2(a, b):
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+# ---------------------------------------------------------------- P1: S1 + S2
+def test_p1_neglog_closed_form_and_guards():
+    rng = np.random.default_rng(1)
+    nproj, nz, n = 5, 3, 16
+    p_true = rng.uniform(0.0, 3.0, (nproj, nz, n))
+    flat = rng.uniform(20000, 30000, (nz, n)).astype(np.float32)
+    dark = rng.uniform(90, 110, (nz, n)).astype(np.float32)
+    flat64, dark64 = flat.astype(np.float64), dark.astype(np.float64)
+    cnt = (flat64 - dark64)[None] * np.exp(-p_true) + dark64[None]
+    raw = np.rint(cnt).astype(np.uint16)
+    p = orc.neglog(raw, flat, dark)                       # [nz][nproj][n]
+    # closed form per element; layout transposes projection-major -> slice-major
+    expect = -np.log((raw.astype(np.float64) - dark64[None]) / (flat64 - dark64)[None]).transpose(1, 0, 2)
+    assert np.abs(p - expect).max() < 1e-13
+    # count rounding bound: |dp| <= 0.5 e^p / (flat - dark)
+    bound = 0.5 * np.exp(p_true) / (flat64 - dark64)[None] * 1.01 + 1e-12
+    assert np.all(np.abs(p.transpose(1, 0, 2) - p_true) <= bound)
+    # guards: raw <= dark clamps t to 1e-6; flat == dark clamps the denominator to 1e-3
+    raw2 = np.array([[[50, 200]]], dtype=np.uint16)
+    flat2 = np.array([[1000.0, 100.0]], dtype=np.float32)
+    dark2 = np.array([[100.0, 100.0]], dtype=np.float32)
+    p2 = orc.neglog(raw2, flat2, dark2)
+    assert p2[0, 0, 0] == pytest.approx(-np.log(1e-6), abs=1e-12)
+    assert p2[0, 0, 1] == pytest.approx(-np.log(100.0 / 1e-3), abs=1e-12)
+
+
+# ---------------------------------------------------------------- P2: FFT
+@pytest.mark.parametrize("N", [2, 4, 8, 64, 256])
+def test_p2_fft_matches_definition_and_library(N):
+    rng = np.random.default_rng(N)
+    x = rng.standard_normal(N) + 1j * rng.standard_normal(N)
+    for sign in (-1, +1):
+        X = orc.fft(x, sign)
+        assert np.abs(X - orc.dft(x, sign)).max() < 1e-11 * N
+        lib = np.fft.fft(x) if sign < 0 else np.fft.ifft(x) * N
+        assert np.abs(X - lib).max() < 1e-11 * N
+    # Parseval and round trip
+    X = orc.fft(x, -1)
+    assert np.sum(np.abs(X) ** 2) == pytest.approx(N * np.sum(np.abs(x) ** 2), rel=1e-12)
+    assert np.abs(orc.fft(X, +1) / N - x).max() < 1e-12
+    # a delta at i0 transforms to e^{-2 pi i k i0 / N} (sign and index convention)
+    d = np.zeros(N, complex)
+    d[1 % N] = 1.0
+    assert np.abs(orc.fft(d, -1) - np.exp(-2j * np.pi * np.arange(N) * (1 % N) / N)).max() < 1e-12
+
+
+def test_p2_fft2_is_separable_library_ifft2():
+    rng = np.random.default_rng(3)
+    F = rng.standard_normal((16, 16)) + 1j * rng.standard_normal((16, 16))
+    assert np.abs(orc.fft2(F, +1) - np.fft.ifft2(F) * 256).max() < 1e-10
+    assert np.abs(orc.fft2(F, -1) - np.fft.fft2(F)).max() < 1e-10
+    # index convention: a delta at (l2, l1) = (2, 5) gives e^{+2 pi i (5 x1 + 2 x2)/M}
+    D = np.zeros((16, 16), complex)
+    D[2, 5] = 1.0
+    x = np.arange(16)
+    ref = np.exp(2j * np.pi * (5 * x[None, :] + 2 * x[:, None]) / 16)
+    assert np.abs(orc.fft2(D, +1) - ref).max() < 1e-12
+
+
+# ---------------------------------------------------------------- P3: filter table
+@pytest.mark.parametrize("M", [64, 256, 1024])
+def test_p3_filter_tables(M):
+    k = np.arange(M)
+    ks = np.where(k < M // 2, k, k - M)
+    i = ks.astype(np.float64)
+    alt = np.where(ks % 2 == 0, 1.0, -1.0)                    # (-1)^i: the zeroed Nyquist bin
+    for name in ("ramp", "shepp", "parzen"):
+        H = orc.filter_table(M, name)
+        assert H[M // 2] == 0.0
+        assert np.abs(H[1:] - H[1:][::-1]).max() < 1e-14          # real and even
+    # ramp: impulse response is the closed-form band-limited kernel (Kak & Slaney)
+    H = orc.filter_table(M, "ramp")
+    h = np.fft.ifft(H).real
+    href = np.where(ks == 0, 0.25, np.where(ks % 2 != 0, -1.0 / (np.pi ** 2 * np.maximum(i * i, 1)), 0.0))
+    r_nyq = np.sum(href * alt)                                  # the bin H[M/2] := 0 removed
+    assert np.abs(h + r_nyq / M * alt - href).max() < 1e-14
+    assert np.abs(H * M - np.abs(ks))[k != M // 2].max() < 0.21  # R ~ |k|/M, small positive DC
+    assert 0 < H[0] < 0.25 / M
+    # shepp: impulse response -2 / (pi^2 (4 i^2 - 1)) up to O(1/M^2) after restoring Nyquist
+    H = orc.filter_table(M, "shepp")
+    h = np.fft.ifft(H).real + (1.0 / np.pi) / M * alt
+    sref = -2.0 / (np.pi ** 2 * (4.0 * i * i - 1.0))
+    assert np.abs(h - sref).max() < 3.0 / M ** 2 + 2e-3 / M
+    # parzen: window values at u = 0, 1/4, 1/2, 3/4 against the ramp table
+    Hp, Hr = orc.filter_table(M, "parzen"), orc.filter_table(M, "ramp")
+    for u, wv in ((0.0, 1.0), (0.25, 1 - 6 * 0.0625 * 0.75), (0.5, 0.25), (0.75, 2 * 0.25 ** 3)):
+        kk = int(u * M / 2)
+        assert Hp[kk] == pytest.approx(Hr[kk] * wv, rel=1e-12)
+        assert Hp[(M - kk) % M] == pytest.approx(Hr[(M - kk) % M] * wv, rel=1e-12)
+
+
+def test_p3_filter_rows_is_linear_convolution_with_kernel():
+    # zero padding to M = 2n makes the FFT product a LINEAR convolution on [0, n)
+    n, M = 32, 64
+    rng = np.random.default_rng(5)
+    p = rng.standard_normal((3, n))
+    q = orc.filter_rows(p, "ramp")
+    h = np.fft.ifft(orc.filter_table(M, "ramp")).real          # wrapped signed kernel
+    for r in range(3):
+        for i in (0, 7, n - 1):
+            ref = sum(p[r, i2] * h[(i - i2) % M] for i2 in range(n))
+            assert q[r, i] == pytest.approx(ref, abs=1e-13)
+
+
+# ---------------------------------------------------------------- P4: plane wave
+@pytest.mark.parametrize("m", [3, 4, 5])
+def test_p4_plane_wave(m):
+    n, M, nproj = 32, 64, 24
+    theta = sg.make_theta(nproj)
+    xs = np.arange(n) - n // 2
+    X, Y = np.meshgrid(xs, xs)                                  # X varies along ix (last axis)
+    for j, k in [(0, 0), (3, 5), (10, -17), (23, 31), (12, 1), (12, -31)]:
+        G = np.zeros((nproj, M), complex)
+        G[j, k % M] = 1.0
+        t = float(theta[j])
+        ref = np.exp(2j * np.pi * (k / M) * (X * np.cos(t) + Y * np.sin(t)))
+        assert np.abs(orc.backproject_exact(G, theta, n) - ref).max() < 1e-11
+        # k = 0: a constant image -- any deapodisation / scale slip shows as curvature or offset
+        assert np.abs(orc.backproject_grid(G, theta, n, m) - ref).max() < 4.0 * np.exp(-2.22 * m)
+
+
+# ---------------------------------------------------------------- P5: analytic phantoms
+def _disc(mu, rad):
+    return sg.Ellipsoids(np.zeros((1, 3)), np.array([[rad, rad, 1e6]]), np.eye(3)[None], np.array([mu]))
+
+
+@pytest.mark.parametrize("method", ["exact", "grid", "lin"])
+def test_p5_uniform_disc_is_flat_and_scaled(method):
+    n, nproj, mu = 64, 96, 0.01
+    theta = sg.make_theta(nproj)
+    p = sg.line_integrals(_disc(mu, 20.0), theta, n, n / 2, [0], 1).transpose(1, 0, 2)
+    # closed form p = 2 mu sqrt(r^2 - s^2) (pins the generator too)
+    s = np.arange(n) - n / 2
+    assert np.abs(p[0, 7] - 2 * mu * np.sqrt(np.clip(400.0 - s * s, 0, None))).max() < 1e-12
+    f = orc.fbp_from_sino(p, theta, n / 2, "ramp", 4, method)[0]
+    Y, X = np.mgrid[0:n, 0:n] - n / 2
+    R = np.hypot(X, Y)
+    assert f[R < 17].mean() == pytest.approx(mu, rel=0.01)
+    assert np.abs(f[(R > 24) & (R < 30)]).mean() < 0.03 * mu
+
+
+@pytest.mark.parametrize("method", ["exact", "grid", "lin"])
+@pytest.mark.parametrize("center", [32.0, 32.5, 35.25])
+def test_p5_gaussian_blob_closed_form(method, center):
+    """Radon transform of mu exp(-r^2/2 sigma^2) about (x0, y0) is
+    mu sigma sqrt(2 pi) exp(-(s - s0)^2 / 2 sigma^2), s0 = x0 cos + y0 sin + c: an essentially
+    band-limited object, so FBP must return it; pins scale, orientation (x0 != y0, both signs),
+    centre phase sign and fractional centres."""
+    n, nproj = 64, 128
+    theta = sg.make_theta(nproj)
+    x0, y0, sig, mu = 7.3, -4.6, 3.0, 0.02
+    th = theta.astype(np.float64)
+    s0 = x0 * np.cos(th) + y0 * np.sin(th) + center
+    p = mu * sig * np.sqrt(2 * np.pi) * np.exp(-(np.arange(n)[None, :] - s0[:, None]) ** 2 / (2 * sig * sig))
+    Y, X = np.mgrid[0:n, 0:n] - n / 2
+    ref = mu * np.exp(-((X - x0) ** 2 + (Y - y0) ** 2) / (2 * sig * sig))
+    f = orc.fbp_from_sino(p[None], theta, center, "ramp", 4, method)[0]
+    tol = 0.01 if method != "lin" else 0.03
+    assert np.abs(f - ref).max() < tol * mu
+    iy, ix = np.unravel_index(np.argmax(f), f.shape)
+    assert (ix, iy) == (round(x0 + n / 2), round(y0 + n / 2))   # not flipped / transposed
+
+
+def test_p5_head_phantom_means_and_orientation():
+    w = sg.make_workload("C1", scale=2)
+    n = w.n
+    rows = [w.nz_total // 2]
+    p = sg.line_integrals(w.phantom, w.theta, n, w.center, rows, w.nz_total).transpose(1, 0, 2)
+    ph = sg.rasterize(w.phantom, n, rows, w.nz_total)[0]
+    f = orc.fbp_from_sino(p, w.theta, w.center, "shepp", 4, "grid")[0]
+    Y, X = np.mgrid[0:n, 0:n] - n / 2
+    brain = (X / (0.18 * n)) ** 2 + ((Y + 0.16 * n) / (0.08 * n)) ** 2 < 1    # featureless brain region
+    assert f[brain].mean() == pytest.approx(ph[brain].mean(), rel=0.02)
+    # the +y blob (top, cy = +0.19 n) is brighter than the mirrored -y location
+    top = (X / (0.05 * n)) ** 2 + ((Y - 0.19 * n) / (0.06 * n)) ** 2 < 1
+    bot = (X / (0.05 * n)) ** 2 + ((Y + 0.19 * n) / (0.06 * n)) ** 2 < 1
+    assert f[top].mean() > f[bot].mean() + 0.5 * 0.1 * 0.02
+    assert rl2(f, ph) < 0.35          # Gibbs-limited; reported, not a parity gate
+
+
+# ---------------------------------------------------------------- P6: centre handling
+def test_p6_integer_centre_shift():
+    w = sg.make_workload("C1", scale=2)
+    n, d = w.n, 3
+    row = [1]
+    p0 = sg.line_integrals(w.phantom, w.theta, n, w.center, row, w.nz_total).transpose(1, 0, 2)
+    p1 = sg.line_integrals(w.phantom, w.theta, n, w.center + d, row, w.nz_total).transpose(1, 0, 2)
+    assert np.abs(p1[0, :, d:] - p0[0, :, :-d]).max() < 1e-12      # the sinogram just shifts
+    Y, X = np.mgrid[0:n, 0:n] - n / 2
+    disc = np.hypot(X, Y) < 0.4 * n
+    f0 = orc.fbp_from_sino(p0, w.theta, w.center, "ramp", 4, "lin")[0]
+    f1 = orc.fbp_from_sino(p1, w.theta, w.center + d, "ramp", 4, "lin")[0]
+    assert rl2(f1[disc], f0[disc]) < 1e-12     # exact: those pixels never see the cropped tails
+    for meth in ("grid", "exact"):
+        f0 = orc.fbp_from_sino(p0, w.theta, w.center, "ramp", 4, meth)[0]
+        f1 = orc.fbp_from_sino(p1, w.theta, w.center + d, "ramp", 4, meth)[0]
+        assert rl2(f1[disc], f0[disc]) < 1e-2  # only the cropped filter tails differ
+
+
+# ---------------------------------------------------------------- P7: gridding vs exact sum
+@pytest.mark.parametrize("n", [16, 32, 64])
+def test_p7_grid_vs_exact_random_spectrum(n):
+    rng = np.random.default_rng(n)
+    nproj = 3 * n // 2
+    theta = sg.make_theta(nproj)
+    q = rng.standard_normal((nproj, n))
+    G = orc.spectrum(orc.filter_rows(q, "ramp"), n / 2 + 0.25)
+    fe = orc.backproject_exact(G, theta, n)
+    for m, bound in ((3, 2e-3), (4, 3e-4), (5, 4e-5)):
+        assert rl2(orc.backproject_grid(G, theta, n, m), fe) < bound
+
+
+def test_p7_grid_vs_exact_c1_phantom_with_noise():
+    """BASELINE.json gate: gridding vs direct summation <= 2e-3 rel-L2 on the phantom (C1)."""
+    w = sg.make_workload("C1")
+    rows = [3]
+    raw, _ = sg.make_counts(w, rows)
+    flat, dark, _, _ = sg.make_flat_dark(w, rows)
+    fe = orc.recon(raw, flat, dark, w.theta, w.center, "shepp", 4, "exact")
+    e3 = rl2(orc.recon(raw, flat, dark, w.theta, w.center, "shepp", 3, "grid"), fe)
+    e4 = rl2(orc.recon(raw, flat, dark, w.theta, w.center, "shepp", 4, "grid"), fe)
+    assert e4 < 2e-4
+    assert e3 < 1e-3          # m = 3 clears the 2e-3 gate with 2x margin (why it is the default)
+    fl = orc.recon(raw, flat, dark, w.theta, w.center, "shepp", 4, "lin")
+    assert 0.01 < rl2(fl, fe) < 0.2    # linear interpolation low-passes: reported, loosely gated (Q17)
+
+
+# ---------------------------------------------------------------- P8: adjoint identities
+def test_p8_adjoints():
+    rng = np.random.default_rng(8)
+    n, nproj, c, m = 16, 20, 8.4, 3
+    M = 2 * n
+    theta = sg.make_theta(nproj)
+
+    def cdot(a, b):
+        return np.vdot(b, a)   # <a, b> = sum a conj(b)
+
+    # B_lin and its literal transpose
+    q = rng.standard_normal((nproj, n))
+    f = rng.standard_normal((n, n))
+    lhs = np.sum(orc.backproject_lin(q, theta, c) * f)
+    rhs = np.sum(q * orc.project_lin_adjoint(f, theta, c))
+    assert lhs == pytest.approx(rhs, rel=1e-12)
+    # S5
+    G = rng.standard_normal((nproj, M)) + 1j * rng.standard_normal((nproj, M))
+    F = rng.standard_normal((M, M)) + 1j * rng.standard_normal((M, M))
+    assert cdot(orc.grid(G, theta, n, m), F) == pytest.approx(cdot(G, orc.grid_adjoint(F, theta, n, m)), rel=1e-12)
+    # S6: the forward transform is the adjoint of the unnormalised inverse
+    F2 = rng.standard_normal((M, M)) + 1j * rng.standard_normal((M, M))
+    assert cdot(orc.fft2(F, +1), F2) == pytest.approx(cdot(F, orc.fft2(F2, -1)), rel=1e-12)
+    # S7
+    fc = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+    assert cdot(orc.deapod_crop(F, n, m), fc) == pytest.approx(cdot(F, orc.deapod_crop_adjoint(fc, n, m)), rel=1e-12)
+    # whole B_grid against the composed transposes
+    lhs = cdot(orc.backproject_grid(G, theta, n, m), fc)
+    rhs = cdot(G, orc.grid_adjoint(orc.fft2(orc.deapod_crop_adjoint(fc, n, m), -1), theta, n, m))
+    assert abs(lhs - rhs) / abs(lhs) < 1e-6
+
+
+# ---------------------------------------------------------------- P9: independence, packing
+def test_p9_slice_independence_and_pair_packing():
+    rng = np.random.default_rng(9)
+    n, nproj, c = 16, 24, 8.5
+    theta = sg.make_theta(nproj)
+    p = rng.uniform(0, 2, (3, nproj, n))
+    stack = orc.fbp_from_sino(p, theta, c, "parzen", 3, "grid")
+    for z in range(3):
+        assert np.array_equal(stack[z], orc.fbp_from_sino(p[z:z + 1], theta, c, "parzen", 3, "grid")[0])
+    # two real slices ride one complex transform: G_A + i G_B -> f_A + i f_B
+    GA = orc.spectrum(orc.filter_rows(p[0], "parzen"), c)
+    GB = orc.spectrum(orc.filter_rows(p[1], "parzen"), c)
+    fa = orc.backproject_grid(GA, theta, n, 3)
+    fb = orc.backproject_grid(GB, theta, n, 3)
+    assert np.abs(fa.imag).max() < 1e-15 * np.abs(fa.real).max() + 1e-18   # Hermitian input -> real image
+    fp = orc.backproject_grid(GA + 1j * GB, theta, n, 3)
+    assert np.abs(fp.real - fa.real).max() < 1e-15 and np.abs(fp.imag - fb.real).max() < 1e-15
+
+
+def test_brute_force_python_gridding_tiny():
+    """S5 written out again as pure-Python loops on a tiny case (index / wrap / tap range)."""
+    n, M, m, nproj = 4, 8, 2, 3
+    theta = sg.make_theta(nproj)
+    rng = np.random.default_rng(10)
+    G = rng.standard_normal((nproj, M)) + 1j * rng.standard_normal((nproj, M))
+    alpha = np.pi / (np.sqrt(2.0) * m)
+    assert orc.kernel_alpha(m) == pytest.approx(alpha, rel=1e-15)
+    F = np.zeros((M, M), complex)
+    for j in range(nproj):
+        cs, sn = np.cos(float(theta[j])), np.sin(float(theta[j]))
+        for k in range(M):
+            ks = k if k < M // 2 else k - M
+            n1, n2 = ks * cs, ks * sn
+            for l2 in range(int(np.floor(n2)) - m - 1, int(np.floor(n2)) + m + 2):
+                for l1 in range(int(np.floor(n1)) - m - 1, int(np.floor(n1)) + m + 2):
+                    if abs(l1 - n1) >= m or abs(l2 - n2) >= m:      # open box |l - nu| < m
+                        continue
+                    F[l2 % M, l1 % M] += G[j, k] * np.exp(-alpha * (l1 - n1) ** 2) * np.exp(-alpha * (l2 - n2) ** 2)
+    assert np.abs(orc.grid(G, theta, n, m) - F).max() < 1e-13
