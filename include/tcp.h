@@ -1,0 +1,128 @@
+/* tcp.h -- C ABI of the B200-native parallel-beam FBP hot path (Fourier gridding).
+ *
+ * What is computed (per chunk of nz detector rows = slices), after arXiv 2209.08450
+ * (TomocuPy) sec. 2.2: "dark-flat field correction, taking negative logarithm of the
+ * data, one-dimensional filtering with the Shepp-Logan, Parzen or other filter"
+ * (PAPER.md:57), then the backprojection by the "Fourier-based method with
+ * exponential functions for interpolation in the frequency domain",
+ * oversampling 2.  Stage by stage:
+ *   S1+S2  t = (raw-dark)/max(flat-dark,1e-3), p = -ln max(t,1e-6)
+ *   S3     q = crop_n( IFFT_M( FFT_M([p,0]) * H ) ),  M = 2n, H = ramp kernel * window
+ *   S4     G[j][k] = C * FFT_M([q,0])[k] * exp(+2 pi i k c / M),  C = pi/(nproj*M)
+ *   S5     F[l2][l1] += G[j][k] phi(l1 - k cos_j) phi(l2 - k sin_j), |l - nu| < m,
+ *          phi(t) = exp(-alpha t^2), alpha = pi/(sqrt(2) m), periodic in M
+ *   S6     g = unnormalised inverse 2D FFT of F
+ *   S7     out[z][iy][ix] = Re g[y][x] / (Phi(x) Phi(y)),  x = ix - n/2, y = iy - n/2
+ * Two adjacent slices ride one complex transform (slice z -> real part, z+1 -> imaginary).
+ *
+ * Every step runs in hand-written sm_100a CUDA kernels inside this library.  There is
+ * no CPU fallback: if no CUDA device is usable the calls fail with TCP_ECUDA.
+ *
+ * Pointers: unless a parameter says HOST, every pointer is a DEVICE pointer owned by
+ * the caller; the library never frees or retains it beyond the call's stream work.
+ * Errors: functions returning int give TCP_OK (0) or a negative code; tcp_create*
+ * return NULL on error.  tcp_last_error() gives a thread-local message.
+ */
+#ifndef TCP_H_
+#define TCP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tcp_ctx tcp_ctx;                 /* opaque */
+typedef void* tcp_stream_t;                     /* a cudaStream_t (NULL = legacy default stream) */
+
+/* compute/storage dtype of the intermediates and dtype of `out` (FP16 storage
+ * with FP32 arithmetic where FP16 would lose accuracy).  F16_OUT32 exists for config C5. */
+enum { TCP_F32 = 0, TCP_F16 = 1, TCP_F16_OUT32 = 2 };
+/* "--fbp-filter": windows multiplying the band-limited ramp. */
+enum { TCP_FILTER_RAMP = 0, TCP_FILTER_SHEPP = 1, TCP_FILTER_PARZEN = 2 };
+enum { TCP_OK = 0, TCP_EINVAL = -1, TCP_ENOMEM = -2, TCP_ECUDA = -3, TCP_EUNSUPPORTED = -4 };
+/* intermediates a test may inspect through tcp_workspace() */
+enum { TCP_WS_SINOGRAM = 0, TCP_WS_SPECTRUM = 1, TCP_WS_GRID = 2, TCP_WS_PASS1 = 3, TCP_WS_TRIG = 4 };
+/* gridding implementations (tcp_set_option(TCP_OPT_GRID_IMPL, ...)) */
+enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1 };
+enum { TCP_OPT_GRID_IMPL = 0, TCP_OPT_PROFILE = 1 };
+/* stages timed when TCP_OPT_PROFILE is on, in launch order */
+enum { TCP_ST_TRIG = 0, TCP_ST_NORMALIZE = 1, TCP_ST_ROWS = 2, TCP_ST_GRID = 3, TCP_ST_IFFT_COLS = 4,
+       TCP_ST_IFFT_ROWS = 5, TCP_NSTAGES = 6 };
+
+/* Create a context for chunks of nz_chunk slices.
+ *   n        detector width = image side; a power of two in [64, 4096] (FP16
+ *            FFTs need power-of-two sizes; applied to FP32 too)
+ *   nproj    number of projection angles (>= 1)
+ *   nz_chunk slices per tcp_recon call (>= 1; "--nsino-per-chunk").
+ *            An odd count pairs its last slice with zeros.
+ *   center   rotation axis in detector pixels ("--rotation-axis"), 0 <= c <= n-1
+ *   dtype    TCP_F32 | TCP_F16 | TCP_F16_OUT32        filter   TCP_FILTER_*
+ * All workspaces and tables are allocated here (cudaMalloc); tcp_recon allocates nothing.
+ * Returns NULL on error (see tcp_last_error). */
+tcp_ctx* tcp_create(int n, int nproj, int nz_chunk, float center, int dtype, int filter);
+
+/* As tcp_create, with the gridding kernel half-width m in {3, 4} (taps per axis = 2m;
+ * 0 = default 3, which meets the 2e-3 gridding-vs-exact gate with 3x margin). */
+tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, int filter, int m);
+
+/* Reconstruct one chunk, S1..S7, asynchronously on `stream` (no host synchronisation).
+ *   raw_u16 [nproj][nz_chunk][n] uint16 counts, projection-major as a detector delivers them
+ *   flat, dark [nz_chunk][n] float32, already averaged over frames
+ *   theta   [nproj] float32 radians, strictly increasing, spanning less than pi
+ *   out     [nz_chunk][n][n], float32 (TCP_F32, TCP_F16_OUT32) or IEEE half (TCP_F16)
+ * One tcp_recon may be in flight per context.  Bitwise reproducible run to run. */
+int tcp_recon(tcp_ctx* ctx, const uint16_t* raw_u16, const float* flat, const float* dark,
+              const float* theta, void* out, tcp_stream_t stream);
+
+void tcp_destroy(tcp_ctx* ctx);                 /* NULL is allowed */
+const char* tcp_last_error(void);
+
+/* Mean of nframes uint16 frames [nframes][nz][n] -> float32 [nz][n] (config C4: "10 flat and
+ * 10 dark frames to be averaged").  Sum in fp32 (exact below 2^24), one division. */
+int tcp_mean_frames_u16(const uint16_t* frames, int nframes, int nz, int n, float* mean,
+                        tcp_stream_t stream);
+
+/* S1+S2 alone: raw -> the context's sinogram workspace [nz_chunk][nproj][n] (float or half). */
+int tcp_normalize(tcp_ctx* ctx, const uint16_t* raw_u16, const float* flat, const float* dark,
+                  tcp_stream_t stream);
+
+/* Device pointer and byte size of an intermediate left by the last tcp_recon (tests only):
+ *   TCP_WS_SINOGRAM [nz][nproj][n] real; TCP_WS_SPECTRUM [npair][nproj][M] complex (FFT order,
+ *   scaled by tcp_scale()); TCP_WS_GRID [npair][M l2][M l1] complex; TCP_WS_TRIG [nproj] double2. */
+int tcp_workspace(tcp_ctx* ctx, int which, void** ptr, size_t* bytes);
+/* Copy an intermediate into the caller's device buffer dst (>= the size tcp_workspace reports),
+ * asynchronously on `stream` (tests only). */
+int tcp_read_workspace(tcp_ctx* ctx, int which, void* dst, size_t dst_bytes, tcp_stream_t stream);
+/* Power-of-two factor by which SPECTRUM/GRID/PASS1 are scaled relative to S4's G (1 in fp32). */
+double tcp_scale(const tcp_ctx* ctx);
+/* Total device bytes the context allocated; kernels launched by one tcp_recon. */
+size_t tcp_workspace_bytes(const tcp_ctx* ctx);
+int tcp_launches_per_recon(const tcp_ctx* ctx);
+int tcp_set_option(tcp_ctx* ctx, int option, int value);
+
+/* Per-kernel device times.  With tcp_set_option(ctx, TCP_OPT_PROFILE, 1) every tcp_recon records
+ * CUDA events around each of its kernels on the caller's stream (no host synchronisation; a ring
+ * of 512 calls).  tcp_profile_collect synchronises on those events, adds the elapsed
+ * milliseconds of every call recorded since the last collect into ms_sum[TCP_NSTAGES] (HOST) and
+ * returns the number of calls in *ncalls (HOST). */
+int tcp_profile_collect(tcp_ctx* ctx, double* ms_sum, int* ncalls);
+
+/* The chunk pipeline (Fig. 1): reconstruct nz_total slices from HOST memory
+ * to HOST memory in chunks of nz_chunk, overlapping the H2D copy of chunk N, the compute of
+ * chunk N-1 and the D2H copy of chunk N-2 on three CUDA streams with nbuf (2 or 3) device
+ * buffer sets.  Host buffers should be pinned (cudaHostAlloc / torch pin_memory) or the
+ * copies will not overlap.  Blocks until the volume is done.
+ *   raw_host [nproj][nz_total][n] uint16; flat_host, dark_host [nz_total][n] float32;
+ *   theta_host [nproj] float32; out_host [nz_total][n][n] in the context's output dtype.
+ * A last partial chunk is allowed.  ms_out (HOST, may be NULL) receives the elapsed device time
+ * in milliseconds between the first copy and the last, measured with CUDA events. */
+int tcp_recon_volume_host(tcp_ctx* ctx, const uint16_t* raw_host, const float* flat_host,
+                          const float* dark_host, const float* theta_host, void* out_host,
+                          int nz_total, int nbuf, float* ms_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TCP_H_ */

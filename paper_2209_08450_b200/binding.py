@@ -1,0 +1,242 @@
+"""ctypes binding of include/tcp.h.  Same names as the C ABI; marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libtcp.so")
+
+DTYPES = {"f32": 0, "f16": 1, "f16_out32": 2}
+FILTERS = {"ramp": 0, "shepp": 1, "parzen": 2}
+WS = {"sinogram": 0, "spectrum": 1, "grid": 2, "pass1": 3, "trig": 4}
+GRID_IMPLS = {"gather": 0, "scatter": 1}
+
+# every symbol include/tcp.h declares (tests check the library exports them all)
+EXPORTS = [
+    "tcp_create", "tcp_create_ex", "tcp_recon", "tcp_destroy", "tcp_last_error",
+    "tcp_mean_frames_u16", "tcp_normalize", "tcp_workspace", "tcp_read_workspace", "tcp_scale",
+    "tcp_workspace_bytes", "tcp_launches_per_recon", "tcp_set_option", "tcp_profile_collect",
+    "tcp_recon_volume_host",
+]
+
+
+class TcpError(RuntimeError):
+    pass
+
+
+def lib_path() -> str:
+    return _SO
+
+
+_lib = None
+
+
+def lib():
+    """Load libtcp.so (built in-tree by paper_2209_08450_b200.build).  Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_SO):
+        raise TcpError("libtcp.so is not built: run `python -m paper_2209_08450_b200.build` "
+                       "(there is no CPU fallback)")
+    L = C.CDLL(_SO)
+    vp, ci, cf = C.c_void_p, C.c_int, C.c_float
+    L.tcp_create.restype = vp
+    L.tcp_create.argtypes = [ci, ci, ci, cf, ci, ci]
+    L.tcp_create_ex.restype = vp
+    L.tcp_create_ex.argtypes = [ci, ci, ci, cf, ci, ci, ci]
+    L.tcp_recon.restype = ci
+    L.tcp_recon.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    L.tcp_destroy.restype = None
+    L.tcp_destroy.argtypes = [vp]
+    L.tcp_last_error.restype = C.c_char_p
+    L.tcp_mean_frames_u16.restype = ci
+    L.tcp_mean_frames_u16.argtypes = [vp, ci, ci, ci, vp, vp]
+    L.tcp_normalize.restype = ci
+    L.tcp_normalize.argtypes = [vp, vp, vp, vp, vp]
+    L.tcp_workspace.restype = ci
+    L.tcp_workspace.argtypes = [vp, ci, C.POINTER(vp), C.POINTER(C.c_size_t)]
+    L.tcp_read_workspace.restype = ci
+    L.tcp_read_workspace.argtypes = [vp, ci, vp, C.c_size_t, vp]
+    L.tcp_scale.restype = C.c_double
+    L.tcp_scale.argtypes = [vp]
+    L.tcp_workspace_bytes.restype = C.c_size_t
+    L.tcp_workspace_bytes.argtypes = [vp]
+    L.tcp_launches_per_recon.restype = ci
+    L.tcp_launches_per_recon.argtypes = [vp]
+    L.tcp_set_option.restype = ci
+    L.tcp_set_option.argtypes = [vp, ci, ci]
+    L.tcp_profile_collect.restype = ci
+    L.tcp_profile_collect.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(ci)]
+    L.tcp_recon_volume_host.restype = ci
+    L.tcp_recon_volume_host.argtypes = [vp, vp, vp, vp, vp, vp, ci, ci, C.POINTER(cf)]
+    _lib = L
+    return L
+
+
+def tcp_last_error() -> str:
+    return lib().tcp_last_error().decode()
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise TcpError("tcp error %d: %s" % (rc, tcp_last_error()))
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _dev(t: torch.Tensor, dtype, shape=None) -> int:
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise TcpError("expected a contiguous CUDA tensor of dtype %s" % dtype)
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise TcpError("expected shape %s, got %s" % (tuple(shape), tuple(t.shape)))
+    return t.data_ptr()
+
+
+def tcp_create(n, nproj, nz_chunk, center, dtype, filter):
+    h = lib().tcp_create(n, nproj, nz_chunk, float(center), DTYPES.get(dtype, dtype), FILTERS.get(filter, filter))
+    if not h:
+        raise TcpError("tcp_create failed: " + tcp_last_error())
+    return h
+
+
+def tcp_create_ex(n, nproj, nz_chunk, center, dtype, filter, m):
+    h = lib().tcp_create_ex(n, nproj, nz_chunk, float(center), DTYPES.get(dtype, dtype),
+                            FILTERS.get(filter, filter), int(m))
+    if not h:
+        raise TcpError("tcp_create_ex failed: " + tcp_last_error())
+    return h
+
+
+def tcp_destroy(h):
+    lib().tcp_destroy(h)
+
+
+def tcp_recon(h, raw_u16, flat, dark, theta, out, stream=None):
+    """All arguments are CUDA tensors (uint16 as torch.uint16 or int16 storage)."""
+    _check(lib().tcp_recon(h, raw_u16.data_ptr(), flat.data_ptr(), dark.data_ptr(), theta.data_ptr(),
+                           out.data_ptr(), _stream(stream)))
+
+
+def tcp_normalize(h, raw_u16, flat, dark, stream=None):
+    _check(lib().tcp_normalize(h, raw_u16.data_ptr(), flat.data_ptr(), dark.data_ptr(), _stream(stream)))
+
+
+def tcp_mean_frames_u16(frames, mean, stream=None):
+    k, nz, n = frames.shape
+    _check(lib().tcp_mean_frames_u16(frames.data_ptr(), k, nz, n, _dev(mean, torch.float32, (nz, n)), _stream(stream)))
+
+
+def tcp_recon_volume_host(h, raw_host, flat_host, dark_host, theta_host, out_host, nz_total, nbuf=3):
+    """Host (pinned) tensors in, host tensor out; returns the device-timed milliseconds."""
+    ms = C.c_float(0.0)
+    _check(lib().tcp_recon_volume_host(h, raw_host.data_ptr(), flat_host.data_ptr(), dark_host.data_ptr(),
+                                       theta_host.data_ptr(), out_host.data_ptr(), int(nz_total), int(nbuf),
+                                       C.byref(ms)))
+    return float(ms.value)
+
+
+def _as_u16(t: torch.Tensor) -> torch.Tensor:
+    if t.dtype == torch.uint16:
+        return t
+    if t.dtype == torch.int16:
+        return t.view(torch.uint16)
+    raise TcpError("raw projections must be uint16")
+
+
+class Recon:
+    """Convenience owner of a tcp context (still only marshalling)."""
+
+    def __init__(self, n, nproj, nz_chunk, center, dtype="f32", filter="parzen", m=0):
+        if not torch.cuda.is_available():
+            raise TcpError("no CUDA device: this library has no CPU fallback")
+        self.n, self.nproj, self.nz, self.center = n, nproj, nz_chunk, float(center)
+        self.dtype, self.filter = dtype, filter
+        self.h = tcp_create_ex(n, nproj, nz_chunk, center, dtype, filter, m)
+        self.out_dtype = torch.float16 if dtype == "f16" else torch.float32
+        self.store_dtype = torch.float32 if dtype == "f32" else torch.float16
+
+    def close(self):
+        if getattr(self, "h", None):
+            tcp_destroy(self.h)
+            self.h = None
+
+    __del__ = close
+
+    def set_grid_impl(self, name: str):
+        _check(lib().tcp_set_option(self.h, 0, GRID_IMPLS[name]))
+
+    STAGES = ("trig", "normalize", "rows", "grid", "ifft_cols", "ifft_rows")
+
+    def set_profile(self, on: bool):
+        _check(lib().tcp_set_option(self.h, 1, 1 if on else 0))
+
+    def profile_collect(self):
+        """(dict stage -> summed ms, number of tcp_recon calls) since the last collect."""
+        ms = (C.c_double * 6)()
+        nc = C.c_int(0)
+        _check(lib().tcp_profile_collect(self.h, ms, C.byref(nc)))
+        return {k: float(ms[i]) for i, k in enumerate(self.STAGES)}, int(nc.value)
+
+    @property
+    def scale(self) -> float:
+        return float(lib().tcp_scale(self.h))
+
+    @property
+    def launches_per_recon(self) -> int:
+        return int(lib().tcp_launches_per_recon(self.h))
+
+    @property
+    def workspace_bytes(self) -> int:
+        return int(lib().tcp_workspace_bytes(self.h))
+
+    def recon(self, raw_u16, flat, dark, theta, out=None, stream=None):
+        raw_u16 = _as_u16(raw_u16)
+        _dev(raw_u16, torch.uint16, (self.nproj, self.nz, self.n))
+        _dev(flat, torch.float32, (self.nz, self.n))
+        _dev(dark, torch.float32, (self.nz, self.n))
+        _dev(theta, torch.float32, (self.nproj,))
+        if out is None:
+            out = torch.empty((self.nz, self.n, self.n), dtype=self.out_dtype, device=raw_u16.device)
+        _dev(out, self.out_dtype, (self.nz, self.n, self.n))
+        tcp_recon(self.h, raw_u16, flat, dark, theta, out, stream)
+        return out
+
+    def normalize(self, raw_u16, flat, dark, stream=None):
+        raw_u16 = _as_u16(raw_u16)
+        _dev(raw_u16, torch.uint16, (self.nproj, self.nz, self.n))
+        tcp_normalize(self.h, raw_u16, flat, dark, stream)
+        return self.workspace("sinogram")
+
+    def workspace(self, name: str) -> torch.Tensor:
+        """Copy of an intermediate of the last recon, as a torch tensor (tests only)."""
+        ptr, nbytes = C.c_void_p(), C.c_size_t()
+        _check(lib().tcp_workspace(self.h, WS[name], C.byref(ptr), C.byref(nbytes)))
+        npair, M = (self.nz + 1) // 2, 2 * self.n
+        buf = torch.empty(nbytes.value, dtype=torch.uint8, device="cuda")
+        _check(lib().tcp_read_workspace(self.h, WS[name], buf.data_ptr(), nbytes.value, _stream(None)))
+        torch.cuda.synchronize()
+        if name == "trig":
+            return buf.view(torch.float64).view(self.nproj, 2)
+        if name == "sinogram":
+            return buf.view(self.store_dtype).view(self.nz, self.nproj, self.n)
+        shape = {"spectrum": (npair, self.nproj, M), "grid": (npair, M, M), "pass1": (npair, self.n, M)}[name]
+        v = buf.view(self.store_dtype).view(*shape, 2).float()
+        return torch.complex(v[..., 0], v[..., 1])
+
+    def recon_volume_host(self, raw_host, flat_host, dark_host, theta_host, out_host=None, nbuf=3):
+        raw_host = _as_u16(raw_host)
+        nproj, nz_total, n = raw_host.shape
+        assert (nproj, n) == (self.nproj, self.n)
+        if out_host is None:
+            out_host = torch.empty((nz_total, n, n), dtype=self.out_dtype).pin_memory()
+        ms = tcp_recon_volume_host(self.h, raw_host, flat_host, dark_host, theta_host, out_host, nz_total, nbuf)
+        return out_host, ms

@@ -1,0 +1,136 @@
+// k_ifft2.cu -- S6 + S7: unnormalised inverse 2D FFT of the oversampled grid as two passes of
+// 1D shared-memory transforms ("2D FFT as a combination of 1D FFTs"), pruned to
+// the central n outputs per axis, with deapodisation, crop and cast fused into the second pass
+// ("accuracy controls").
+//
+// pass 1 (columns): for each l1, IFFT over l2 -> x2; keep iy = x2 + n/2 in [0, n);
+//                   T[pair][iy][l1].  A CTA owns W adjacent columns, so every global access is
+//                   a W-wide segment; lines sit in shared memory with a stride chosen to keep
+//                   the W-interleaved accesses bank-conflict free.
+// pass 2 (rows):    for each iy, IFFT over l1 -> x1; keep ix = x1 + n/2;
+//                   out[2 pair][iy][ix] = Re * deay[iy] * deax[ix], out[2 pair + 1] = Im * ...
+#include "fft.cuh"
+#include "tcp_internal.h"
+
+namespace tcpk {
+
+__host__ __device__ constexpr int cols_w(int M) { return (16384 / M) < 32 ? (16384 / M) : 32; }
+__host__ __device__ constexpr int cols_stride(int M) {   // float2 units; stride = 16/W (mod 16)
+    return padded_len(M) + (cols_w(M) >= 16 ? 1 : 16 / cols_w(M));
+}
+
+template <int M, class TC>
+__global__ void __launch_bounds__(cols_w(M) * M / 16) ifft_cols_kernel(const TC* __restrict__ grid,
+                                                                       TC* __restrict__ pass1,
+                                                                       const float2* __restrict__ tw) {
+    constexpr int n = M / 2, W = cols_w(M), LS = cols_stride(M);
+    extern __shared__ float2 smem[];
+    const int w = threadIdx.x % W;            // column inside the CTA's strip (fastest: coalescing)
+    const int tid = threadIdx.x / W;          // thread inside the column's FFT group
+    float2* s = smem + (size_t)w * LS;
+    const int pair = blockIdx.y;
+    const int l1 = blockIdx.x * W + w;
+    const TC* src = grid + (size_t)pair * M * M + l1;
+    TC* dst = pass1 + (size_t)pair * n * M + l1;
+    fft_line<M, true>(
+        s, tid, tw, [&](int l2) { return ld_c(src, (size_t)l2 * M); },
+        [&](int x2, float2 v) {
+            // signed x2 in [-n/2, n/2)  <->  FFT index x2 mod M
+            if (x2 < n / 2) st_c(dst, (size_t)(x2 + n / 2) * M, v);
+            else if (x2 >= M - n / 2) st_c(dst, (size_t)(x2 - (M - n / 2)) * M, v);
+        });
+}
+
+template <int M, int ROWS, class TC, class TO>
+__global__ void __launch_bounds__(ROWS* M / 16) ifft_rows_kernel(const TC* __restrict__ pass1, TO* __restrict__ out,
+                                                                 const float2* __restrict__ tw,
+                                                                 const float* __restrict__ deax,
+                                                                 const float* __restrict__ deay, int nz) {
+    constexpr int n = M / 2, TG = M / 16;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / TG, tid = threadIdx.x % TG;
+    float2* s = smem + (size_t)g * padded_len(M);
+    const int pair = blockIdx.y;
+    const int iy = blockIdx.x * ROWS + g;     // n is a multiple of ROWS
+    const TC* src = pass1 + ((size_t)pair * n + iy) * M;
+    const float dy = __ldg(&deay[iy]);
+    const int zA = 2 * pair, zB = 2 * pair + 1;
+    TO* oA = out + ((size_t)zA * n + iy) * n;
+    TO* oB = out + ((size_t)zB * n + iy) * n;
+    const bool hasB = zB < nz;
+    fft_line<M, true>(
+        s, tid, tw, [&](int l1) { return ld_c(src, (size_t)l1); },
+        [&](int x1, float2 v) {
+            int ix = -1;
+            if (x1 < n / 2) ix = x1 + n / 2;
+            else if (x1 >= M - n / 2) ix = x1 - (M - n / 2);
+            if (ix >= 0) {
+                const float d = dy * __ldg(&deax[ix]);
+                st_r(oA, ix, v.x * d);
+                if (hasB) st_r(oB, ix, v.y * d);
+            }
+        });
+}
+
+template <int M, class TC>
+static int launch_cols_t(const tcp_ctx* c, cudaStream_t st) {
+    constexpr int W = cols_w(M);
+    const size_t smem = (size_t)W * cols_stride(M) * sizeof(float2);
+    auto kern = ifft_cols_kernel<M, TC>;
+    TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    dim3 grid(M / W, c->npair);
+    kern<<<grid, W * M / 16, smem, st>>>((const TC*)c->grid, (TC*)c->pass1, c->tw);
+    TCP_CUDA_CHECK(cudaGetLastError());
+    return TCP_OK;
+}
+
+template <int M, class TC, class TO>
+static int launch_rows_t(const tcp_ctx* c, void* out, cudaStream_t st) {
+    constexpr int TG = M / 16;
+    constexpr int ROWS = (TG >= 128) ? 1 : 128 / TG;
+    const size_t smem = (size_t)ROWS * padded_len(M) * sizeof(float2);
+    auto kern = ifft_rows_kernel<M, ROWS, TC, TO>;
+    TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    dim3 grid((M / 2) / ROWS, c->npair);
+    kern<<<grid, ROWS * TG, smem, st>>>((const TC*)c->pass1, (TO*)out, c->tw, c->deax, c->deay, c->nz);
+    TCP_CUDA_CHECK(cudaGetLastError());
+    return TCP_OK;
+}
+
+template <int M>
+static int cols_m(const tcp_ctx* c, cudaStream_t st) {
+    return c->half_store ? launch_cols_t<M, __half2>(c, st) : launch_cols_t<M, float2>(c, st);
+}
+template <int M>
+static int rows_m(const tcp_ctx* c, void* out, cudaStream_t st) {
+    if (!c->half_store) return launch_rows_t<M, float2, float>(c, out, st);
+    return c->half_out ? launch_rows_t<M, __half2, __half>(c, out, st) : launch_rows_t<M, __half2, float>(c, out, st);
+}
+
+int launch_ifft_cols(const tcp_ctx* c, cudaStream_t st) {
+    switch (c->M) {
+        case 128: return cols_m<128>(c, st);
+        case 256: return cols_m<256>(c, st);
+        case 512: return cols_m<512>(c, st);
+        case 1024: return cols_m<1024>(c, st);
+        case 2048: return cols_m<2048>(c, st);
+        case 4096: return cols_m<4096>(c, st);
+        case 8192: return cols_m<8192>(c, st);
+    }
+    return set_error(TCP_EUNSUPPORTED, "unsupported M=%d", c->M);
+}
+
+int launch_ifft_rows(const tcp_ctx* c, void* out, cudaStream_t st) {
+    switch (c->M) {
+        case 128: return rows_m<128>(c, out, st);
+        case 256: return rows_m<256>(c, out, st);
+        case 512: return rows_m<512>(c, out, st);
+        case 1024: return rows_m<1024>(c, out, st);
+        case 2048: return rows_m<2048>(c, out, st);
+        case 4096: return rows_m<4096>(c, out, st);
+        case 8192: return rows_m<8192>(c, out, st);
+    }
+    return set_error(TCP_EUNSUPPORTED, "unsupported M=%d", c->M);
+}
+
+}  // namespace tcpk

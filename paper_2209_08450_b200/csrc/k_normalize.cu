@@ -1,0 +1,119 @@
+// k_normalize.cu -- S1+S2: dark/flat-field correction, negative logarithm and cast
+// (fp16 rule PAPER.md:53: arithmetic in fp32, one rounding to the storage type),
+// the frame-averaging helper, and the fp64 cos/sin table of the projection angles.
+//
+// HBM-bound: 2 B read + B_r written per sample.  Each thread moves 8 detector pixels:
+// one 128-bit load of uint16, 2x2 128-bit loads of flat/dark (L2 resident: nz*n floats are
+// reused by all nproj projections) and one (half) or two (float) 128-bit stores.  The
+// projection-major -> slice-major transpose only permutes whole rows, so both sides stay
+// fully coalesced.
+#include "tcp_internal.h"
+
+namespace tcpk {
+
+__device__ __forceinline__ float neglog1(float raw, float flat, float dark) {
+    const float eps_d = 1e-3f, t_min = 1e-6f;
+    const float den = flat - dark;
+    // near t = 1 (air) -ln t cancels: use t - 1 = (raw - flat)/den, exact numerator (Sterbenz),
+    // and log1p, so p keeps fp32 RELATIVE accuracy even where p ~ 0
+    if (den >= eps_d) {
+        const float u = (raw - flat) / den;
+        if (u > -0.5f) return -log1pf(u);
+    }
+    const float t = fmaxf((raw - dark) / fmaxf(den, eps_d), t_min);
+    return -logf(t);
+}
+
+template <class TS>
+__global__ void __launch_bounds__(256) normalize_kernel(const uint4* __restrict__ raw, const float4* __restrict__ flat,
+                                                        const float4* __restrict__ dark, TS* __restrict__ sino,
+                                                        int nproj, int nz, int n8) {
+    // one thread per 8 pixels; index space [nproj][nz][n8] in raw order
+    const size_t total = (size_t)nproj * nz * n8;
+    for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < total; v += (size_t)gridDim.x * blockDim.x) {
+        const int i8 = (int)(v % n8);
+        const size_t row = v / n8;
+        const int z = (int)(row % nz);
+        const int j = (int)(row / nz);
+        const uint4 r = __ldcs(&raw[v]);                       // streamed once
+        const size_t fo = ((size_t)z * n8 + i8) * 2;
+        const float4 f0 = __ldg(&flat[fo]), f1 = __ldg(&flat[fo + 1]);
+        const float4 d0 = __ldg(&dark[fo]), d1 = __ldg(&dark[fo + 1]);
+        float p[8];
+        p[0] = neglog1((float)(r.x & 0xffffu), f0.x, d0.x);
+        p[1] = neglog1((float)(r.x >> 16), f0.y, d0.y);
+        p[2] = neglog1((float)(r.y & 0xffffu), f0.z, d0.z);
+        p[3] = neglog1((float)(r.y >> 16), f0.w, d0.w);
+        p[4] = neglog1((float)(r.z & 0xffffu), f1.x, d1.x);
+        p[5] = neglog1((float)(r.z >> 16), f1.y, d1.y);
+        p[6] = neglog1((float)(r.w & 0xffffu), f1.z, d1.z);
+        p[7] = neglog1((float)(r.w >> 16), f1.w, d1.w);
+        const size_t o = (((size_t)z * nproj + j) * n8 + i8) * 8;   // element offset in sino
+        if constexpr (sizeof(TS) == 4) {
+            float4* dst = reinterpret_cast<float4*>(sino + o);
+            dst[0] = make_float4(p[0], p[1], p[2], p[3]);
+            dst[1] = make_float4(p[4], p[5], p[6], p[7]);
+        } else {
+            __half2 h0 = __floats2half2_rn(p[0], p[1]), h1 = __floats2half2_rn(p[2], p[3]);
+            __half2 h2 = __floats2half2_rn(p[4], p[5]), h3 = __floats2half2_rn(p[6], p[7]);
+            uint4 w;
+            w.x = *reinterpret_cast<unsigned*>(&h0);
+            w.y = *reinterpret_cast<unsigned*>(&h1);
+            w.z = *reinterpret_cast<unsigned*>(&h2);
+            w.w = *reinterpret_cast<unsigned*>(&h3);
+            *reinterpret_cast<uint4*>(sino + o) = w;
+        }
+    }
+}
+
+int launch_normalize(const tcp_ctx* c, const uint16_t* raw, const float* flat, const float* dark, cudaStream_t st) {
+    const int n8 = c->n / 8;
+    const size_t total = (size_t)c->nproj * c->nz * n8;
+    int blocks = (int)((total + 255) / 256);
+    const int cap = 148 * 8 * 4;                  // a few waves of 8 resident CTAs per SM
+    if (blocks > cap) blocks = cap;
+    if (c->half_store)
+        normalize_kernel<__half><<<blocks, 256, 0, st>>>((const uint4*)raw, (const float4*)flat, (const float4*)dark,
+                                                         (__half*)c->sino, c->nproj, c->nz, n8);
+    else
+        normalize_kernel<float><<<blocks, 256, 0, st>>>((const uint4*)raw, (const float4*)flat, (const float4*)dark,
+                                                        (float*)c->sino, c->nproj, c->nz, n8);
+    TCP_CUDA_CHECK(cudaGetLastError());
+    return TCP_OK;
+}
+
+// mean of K uint16 frames: sum in fp32 (exact below 2^24), one division
+__global__ void mean_frames_kernel(const uint16_t* __restrict__ frames, int nframes, size_t npix, float* __restrict__ mean) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < npix; i += (size_t)gridDim.x * blockDim.x) {
+        float s = 0.f;
+        for (int k = 0; k < nframes; ++k) s += (float)frames[(size_t)k * npix + i];
+        mean[i] = s / (float)nframes;
+    }
+}
+
+int launch_mean_frames(const uint16_t* frames, int nframes, int nz, int n, float* mean, cudaStream_t st) {
+    const size_t npix = (size_t)nz * n;
+    int blocks = (int)((npix + 255) / 256);
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    mean_frames_kernel<<<blocks, 256, 0, st>>>(frames, nframes, npix, mean);
+    TCP_CUDA_CHECK(cudaGetLastError());
+    return TCP_OK;
+}
+
+// cos/sin of the float32 angles in fp64: k*cos(theta) with
+// k up to 4096 must be good to ~1e-6 grid cells for the 1e-5 fp32 gate.
+__global__ void trig_kernel(const float* __restrict__ theta, int nproj, double2* __restrict__ trig) {
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < nproj) {
+        double t = (double)theta[j];
+        trig[j] = make_double2(cos(t), sin(t));
+    }
+}
+
+int launch_trig(const tcp_ctx* c, const float* theta, cudaStream_t st) {
+    trig_kernel<<<(c->nproj + 127) / 128, 128, 0, st>>>(theta, c->nproj, c->trig);
+    TCP_CUDA_CHECK(cudaGetLastError());
+    return TCP_OK;
+}
+
+}  // namespace tcpk

@@ -1,0 +1,89 @@
+// k_rows.cu -- S3 + S4 for one detector row of a slice pair, entirely in shared memory:
+//   a = [pA + i pB, 0]  -> FFT_M -> * H/M -> IFFT_M -> crop to [0,n), zero-pad -> FFT_M
+//   -> * S C e^{+2 pi i k c / M}  -> spectrum G[pair][j][k]
+// Two adjacent slices ride one complex transform (slice 2p -> real, 2p+1 -> imaginary):
+// H is real and even and the Nyquist bin is zeroed, so the packing survives the filter.
+// HBM sees one read of the two sinogram rows and one write of the spectrum row.
+#include "fft.cuh"
+#include "tcp_internal.h"
+
+namespace tcpk {
+
+template <int M, int ROWS, class TS, class TC>
+__global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict__ sino, TC* __restrict__ spec,
+                                                            const float2* __restrict__ tw,
+                                                            const float* __restrict__ hfilt,
+                                                            const float2* __restrict__ ptab, int nproj, int nz) {
+    constexpr int n = M / 2;
+    constexpr int TG = M / 16;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / TG;       // row group inside the CTA
+    const int tid = threadIdx.x % TG;
+    float2* s = smem + (size_t)g * padded_len(M);
+    int j = blockIdx.x * ROWS + g;
+    const bool live = j < nproj;
+    if (!live) j = nproj - 1;             // keep the group in the barriers; its stores are masked
+    const int pair = blockIdx.y;
+    const int zA = 2 * pair, zB = 2 * pair + 1;
+    const TS* pA = sino + ((size_t)zA * nproj + j) * n;
+    const TS* pB = sino + ((size_t)(zB < nz ? zB : zA) * nproj + j) * n;
+    const bool hasB = zB < nz;
+
+    // FFT #1: zero-padded load, filter on store
+    fft_line<M, false>(
+        s, tid, tw,
+        [&](int i) {
+            if (i < n) return make_float2(ld_r(pA, i), hasB ? ld_r(pB, i) : 0.f);
+            return make_float2(0.f, 0.f);
+        },
+        [&](int k, float2 v) {
+            const float h = __ldg(&hfilt[k]);
+            s[pad_idx(k)] = make_float2(v.x * h, v.y * h);
+        });
+    __syncthreads();
+    // FFT #2 (inverse): crop to the detector on store
+    fft_line<M, true>(
+        s, tid, tw, [&](int i) { return s[pad_idx(i)]; },
+        [&](int i, float2 v) { s[pad_idx(i)] = (i < n) ? v : make_float2(0.f, 0.f); });
+    __syncthreads();
+    // FFT #3: spectrum, centre phase and scale on store
+    TC* out = spec + ((size_t)pair * nproj + j) * M;
+    fft_line<M, false>(
+        s, tid, tw, [&](int i) { return s[pad_idx(i)]; },
+        [&](int k, float2 v) {
+            if (live) st_c(out, k, cmul(v, __ldg(&ptab[k])));
+        });
+}
+
+template <int M, class TS, class TC>
+static int launch_rows_t(const tcp_ctx* c, cudaStream_t st) {
+    constexpr int TG = M / 16;
+    constexpr int ROWS = (TG >= 128) ? 1 : 128 / TG;
+    const size_t smem = (size_t)ROWS * padded_len(M) * sizeof(float2);
+    auto kern = rows_kernel<M, ROWS, TS, TC>;
+    TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    dim3 grid((c->nproj + ROWS - 1) / ROWS, c->npair);
+    kern<<<grid, ROWS * TG, smem, st>>>((const TS*)c->sino, (TC*)c->spec, c->tw, c->hfilt, c->ptab, c->nproj, c->nz);
+    TCP_CUDA_CHECK(cudaGetLastError());
+    return TCP_OK;
+}
+
+template <int M>
+static int launch_rows_m(const tcp_ctx* c, cudaStream_t st) {
+    return c->half_store ? launch_rows_t<M, __half, __half2>(c, st) : launch_rows_t<M, float, float2>(c, st);
+}
+
+int launch_rows(const tcp_ctx* c, cudaStream_t st) {
+    switch (c->M) {
+        case 128: return launch_rows_m<128>(c, st);
+        case 256: return launch_rows_m<256>(c, st);
+        case 512: return launch_rows_m<512>(c, st);
+        case 1024: return launch_rows_m<1024>(c, st);
+        case 2048: return launch_rows_m<2048>(c, st);
+        case 4096: return launch_rows_m<4096>(c, st);
+        case 8192: return launch_rows_m<8192>(c, st);
+    }
+    return set_error(TCP_EUNSUPPORTED, "unsupported M=%d", c->M);
+}
+
+}  // namespace tcpk

@@ -1,0 +1,313 @@
+// tcp_api.cu -- the C ABI of include/tcp.h: context, tables (built in fp64 on the host),
+// validation, error reporting and the per-chunk launch sequence S1..S7.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "tcp_internal.h"
+
+namespace tcpk {
+
+static thread_local char g_err[512] = "";
+
+int set_error(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+static const int kProfileRing = 512;
+static const double kPi = 3.14159265358979323846264338327950288;
+
+// H[k]/M: band-limited ramp (h[0] = 1/4, h[i] = -1/(pi^2 i^2) for odd i) transformed as a real
+// cosine series, times the window; Nyquist bin zeroed (reading Q4).
+static void build_filter(int M, int filter, std::vector<float>& out) {
+    out.resize(M);
+    std::vector<double> coef;   // 2 h[i] for odd i in (0, M/2)
+    for (int i = 1; i < M / 2; i += 2) coef.push_back(-2.0 / (kPi * kPi * (double)i * (double)i));
+    for (int k = 0; k <= M / 2; ++k) {
+        double r = 0.25;
+        // sum small terms first for accuracy
+        for (int t = (int)coef.size() - 1; t >= 0; --t) {
+            long long ki = ((long long)k * (2 * t + 1)) % M;
+            r += coef[t] * cos(2.0 * kPi * (double)ki / (double)M);
+        }
+        double w = 1.0;
+        if (filter == TCP_FILTER_SHEPP) {
+            double a = kPi * (double)k / (double)M;
+            w = (k == 0) ? 1.0 : sin(a) / a;
+        } else if (filter == TCP_FILTER_PARZEN) {
+            double u = (double)k / (double)(M / 2);
+            w = (u <= 0.5) ? 1.0 - 6.0 * u * u * (1.0 - u) : 2.0 * (1.0 - u) * (1.0 - u) * (1.0 - u);
+        }
+        double h = (k == M / 2) ? 0.0 : r * w / (double)M;
+        out[k] = (float)h;
+        if (k > 0 && k < M / 2) out[M - k] = (float)h;
+    }
+}
+
+template <class T>
+static int upload(T** dptr, const std::vector<T>& h, size_t* bytes) {
+    TCP_CUDA_CHECK(cudaMalloc((void**)dptr, h.size() * sizeof(T)));
+    TCP_CUDA_CHECK(cudaMemcpy(*dptr, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+    *bytes += h.size() * sizeof(T);
+    return TCP_OK;
+}
+
+static int dev_alloc(void** p, size_t nbytes, size_t* bytes) {
+    cudaError_t e = cudaMalloc(p, nbytes);
+    if (e != cudaSuccess) {
+        *p = nullptr;
+        return set_error(e == cudaErrorMemoryAllocation ? TCP_ENOMEM : TCP_ECUDA, "cudaMalloc(%zu) failed: %s", nbytes,
+                         cudaGetErrorString(e));
+    }
+    *bytes += nbytes;
+    return TCP_OK;
+}
+
+static int build_context(tcp_ctx* c) {
+    const int n = c->n, M = c->M, m = c->m;
+    const size_t rb = c->half_store ? 2 : 4, cb = 2 * rb;
+    int rc;
+    if ((rc = dev_alloc(&c->sino, (size_t)c->nz * c->nproj * n * rb, &c->bytes))) return rc;
+    if ((rc = dev_alloc(&c->spec, (size_t)c->npair * c->nproj * M * cb, &c->bytes))) return rc;
+    if ((rc = dev_alloc(&c->grid, (size_t)c->npair * M * M * cb, &c->bytes))) return rc;
+    if ((rc = dev_alloc(&c->pass1, (size_t)c->npair * n * M * cb, &c->bytes))) return rc;
+    if ((rc = dev_alloc((void**)&c->trig, (size_t)c->nproj * sizeof(double2), &c->bytes))) return rc;
+
+    std::vector<float2> tw(M);
+    for (int t = 0; t < M; ++t) {
+        double a = -2.0 * kPi * (double)t / (double)M;
+        tw[t] = make_float2((float)cos(a), (float)sin(a));
+    }
+    if ((rc = upload(&c->tw, tw, &c->bytes))) return rc;
+
+    std::vector<float> hf;
+    build_filter(M, c->filter, hf);
+    if ((rc = upload(&c->hfilt, hf, &c->bytes))) return rc;
+
+    const double C = kPi / ((double)c->nproj * (double)M);
+    std::vector<float2> pt(M);
+    for (int k = 0; k < M; ++k) {
+        int ks = (k < M / 2) ? k : k - M;
+        double fr = fmod((double)ks * (double)c->center, (double)M) / (double)M;
+        double a = 2.0 * kPi * fr;
+        pt[k] = make_float2((float)(c->scale * C * cos(a)), (float)(c->scale * C * sin(a)));
+    }
+    pt[M / 2] = make_float2(0.f, 0.f);
+    if ((rc = upload(&c->ptab, pt, &c->bytes))) return rc;
+
+    const double alpha = kPi / (sqrt(2.0) * (double)m);
+    std::vector<float> dx(n), dy(n);
+    for (int i = 0; i < n; ++i) {
+        double x = (double)(i - n / 2);
+        double phi = sqrt(kPi / alpha) * exp(-kPi * kPi * x * x / (alpha * (double)M * (double)M));
+        dy[i] = (float)(1.0 / phi);
+        dx[i] = (float)(1.0 / (phi * c->scale));
+    }
+    if ((rc = upload(&c->deax, dx, &c->bytes))) return rc;
+    if ((rc = upload(&c->deay, dy, &c->bytes))) return rc;
+
+    // gather tiles, heaviest (closest to DC) first: sample density falls as 1/radius
+    const int T = 16, tx = M / T;
+    std::vector<std::pair<long long, int>> key;
+    auto mind = [&](int t) {
+        long long best = 1LL << 60;
+        for (int q = 0; q < T; ++q) {
+            int L = t * T + q, l = (L < n) ? L : L - M;
+            best = std::min<long long>(best, llabs((long long)l));
+        }
+        return best;
+    };
+    for (int ty = 0; ty < tx; ++ty)
+        for (int txi = 0; txi < tx; ++txi) {
+            long long a = mind(txi), b = mind(ty);
+            key.push_back({a * a + b * b, ty * tx + txi});
+        }
+    std::sort(key.begin(), key.end());
+    std::vector<int> order;
+    for (auto& kv : key) order.push_back(kv.second);
+    c->ntiles = (int)order.size();
+    if ((rc = upload(&c->tile_order, order, &c->bytes))) return rc;
+    return TCP_OK;
+}
+
+}  // namespace tcpk
+
+using namespace tcpk;
+
+extern "C" {
+
+const char* tcp_last_error(void) { return g_err; }
+
+tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, int filter, int m) {
+    g_err[0] = 0;
+    if (m == 0) m = 3;
+    if (n < 64 || n > 4096 || (n & (n - 1)) != 0) {
+        set_error(TCP_EINVAL, "n=%d must be a power of two in [64, 4096]", n);
+        return nullptr;
+    }
+    if (nproj < 1 || nz_chunk < 1) { set_error(TCP_EINVAL, "nproj=%d and nz_chunk=%d must be >= 1", nproj, nz_chunk); return nullptr; }
+    if (!(center >= 0.f && center <= (float)(n - 1))) { set_error(TCP_EINVAL, "center=%g outside [0, n-1]", (double)center); return nullptr; }
+    if (dtype < TCP_F32 || dtype > TCP_F16_OUT32) { set_error(TCP_EINVAL, "unknown dtype %d", dtype); return nullptr; }
+    if (filter < TCP_FILTER_RAMP || filter > TCP_FILTER_PARZEN) { set_error(TCP_EINVAL, "unknown filter %d", filter); return nullptr; }
+    if (m != 3 && m != 4) { set_error(TCP_EINVAL, "kernel half-width m=%d must be 3 or 4", m); return nullptr; }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        set_error(TCP_ECUDA, "no usable CUDA device (this library has no CPU fallback)");
+        return nullptr;
+    }
+    tcp_ctx* c = (tcp_ctx*)calloc(1, sizeof(tcp_ctx));
+    if (!c) { set_error(TCP_ENOMEM, "out of host memory"); return nullptr; }
+    c->n = n; c->M = 2 * n; c->nproj = nproj; c->nz = nz_chunk; c->npair = (nz_chunk + 1) / 2;
+    c->dtype = dtype; c->filter = filter; c->m = m; c->center = center;
+    c->half_store = dtype != TCP_F32;
+    c->half_out = dtype == TCP_F16;
+    // fp16 storage: S = 2^13 puts |f| Phi^2 S <= 65504 for |f| < 1.9 per pixel while keeping
+    // noise-level spectrum samples above the half subnormal range
+    c->scale = c->half_store ? 8192.0 : 1.0;
+    c->grid_impl = TCP_GRID_GATHER;
+    cudaGetDevice(&c->device);
+    if (build_context(c) != TCP_OK || setup_kernel_attributes(c) != TCP_OK) {
+        char keep[512];
+        strncpy(keep, g_err, sizeof(keep));
+        tcp_destroy(c);
+        strncpy(g_err, keep, sizeof(g_err));
+        return nullptr;
+    }
+    return c;
+}
+
+tcp_ctx* tcp_create(int n, int nproj, int nz_chunk, float center, int dtype, int filter) {
+    return tcp_create_ex(n, nproj, nz_chunk, center, dtype, filter, 0);
+}
+
+void tcp_destroy(tcp_ctx* c) {
+    if (!c) return;
+    pipe_destroy(c);
+    if (c->pev) {
+        for (int i = 0; i < kProfileRing * (TCP_NSTAGES + 1); ++i) cudaEventDestroy(c->pev[i]);
+        free(c->pev);
+    }
+    cudaFree(c->sino); cudaFree(c->spec); cudaFree(c->grid); cudaFree(c->pass1); cudaFree(c->trig);
+    cudaFree(c->tw); cudaFree(c->hfilt); cudaFree(c->ptab); cudaFree(c->deax); cudaFree(c->deay);
+    cudaFree(c->tile_order);
+    free(c);
+}
+
+int tcp_normalize(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* dark, tcp_stream_t stream) {
+    if (!c || !raw || !flat || !dark) return set_error(TCP_EINVAL, "NULL argument");
+    return launch_normalize(c, raw, flat, dark, (cudaStream_t)stream);
+}
+
+int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* dark, const float* theta, void* out,
+              tcp_stream_t stream) {
+    if (!c || !raw || !flat || !dark || !theta || !out) return set_error(TCP_EINVAL, "NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    cudaEvent_t* ev = nullptr;
+    if (c->profile) {
+        if (c->pcalls >= kProfileRing) return set_error(TCP_EINVAL, "profile ring full: call tcp_profile_collect");
+        ev = c->pev + (size_t)c->pcalls * (TCP_NSTAGES + 1);
+        c->pcalls++;
+    }
+#define TCP_MARK(i) do { if (ev) TCP_CUDA_CHECK(cudaEventRecord(ev[i], st)); } while (0)
+    TCP_MARK(0);
+    if ((rc = launch_trig(c, theta, st))) return rc;
+    TCP_MARK(1);
+    if ((rc = launch_normalize(c, raw, flat, dark, st))) return rc;
+    TCP_MARK(2);
+    if ((rc = launch_rows(c, st))) return rc;
+    TCP_MARK(3);
+    if (c->grid_impl == TCP_GRID_SCATTER_ATOMIC) rc = launch_grid_scatter(c, st);
+    else rc = launch_grid_gather(c, theta, st);
+    if (rc) return rc;
+    TCP_MARK(4);
+    if ((rc = launch_ifft_cols(c, st))) return rc;
+    TCP_MARK(5);
+    if ((rc = launch_ifft_rows(c, out, st))) return rc;
+    TCP_MARK(6);
+#undef TCP_MARK
+    return TCP_OK;
+}
+
+int tcp_profile_collect(tcp_ctx* c, double* ms_sum, int* ncalls) {
+    if (!c || !ms_sum || !ncalls) return set_error(TCP_EINVAL, "NULL argument");
+    for (int s = 0; s < TCP_NSTAGES; ++s) ms_sum[s] = 0.0;
+    *ncalls = c->pcalls;
+    for (int k = 0; k < c->pcalls; ++k) {
+        cudaEvent_t* ev = c->pev + (size_t)k * (TCP_NSTAGES + 1);
+        TCP_CUDA_CHECK(cudaEventSynchronize(ev[TCP_NSTAGES]));
+        for (int s = 0; s < TCP_NSTAGES; ++s) {
+            float ms = 0.f;
+            TCP_CUDA_CHECK(cudaEventElapsedTime(&ms, ev[s], ev[s + 1]));
+            ms_sum[s] += (double)ms;
+        }
+    }
+    c->pcalls = 0;
+    return TCP_OK;
+}
+
+int tcp_launches_per_recon(const tcp_ctx* c) { return c ? 6 : 0; }
+
+int tcp_mean_frames_u16(const uint16_t* frames, int nframes, int nz, int n, float* mean, tcp_stream_t stream) {
+    if (!frames || !mean || nframes < 1 || nz < 1 || n < 1) return set_error(TCP_EINVAL, "bad argument");
+    return launch_mean_frames(frames, nframes, nz, n, mean, (cudaStream_t)stream);
+}
+
+int tcp_workspace(tcp_ctx* c, int which, void** ptr, size_t* bytes) {
+    if (!c || !ptr || !bytes) return set_error(TCP_EINVAL, "NULL argument");
+    const size_t rb = c->half_store ? 2 : 4, cb = 2 * rb;
+    switch (which) {
+        case TCP_WS_SINOGRAM: *ptr = c->sino; *bytes = (size_t)c->nz * c->nproj * c->n * rb; return TCP_OK;
+        case TCP_WS_SPECTRUM: *ptr = c->spec; *bytes = (size_t)c->npair * c->nproj * c->M * cb; return TCP_OK;
+        case TCP_WS_GRID: *ptr = c->grid; *bytes = (size_t)c->npair * c->M * c->M * cb; return TCP_OK;
+        case TCP_WS_PASS1: *ptr = c->pass1; *bytes = (size_t)c->npair * c->n * c->M * cb; return TCP_OK;
+        case TCP_WS_TRIG: *ptr = c->trig; *bytes = (size_t)c->nproj * sizeof(double2); return TCP_OK;
+    }
+    return set_error(TCP_EINVAL, "unknown workspace %d", which);
+}
+
+int tcp_read_workspace(tcp_ctx* c, int which, void* dst, size_t dst_bytes, tcp_stream_t stream) {
+    void* src = nullptr;
+    size_t nb = 0;
+    int rc = tcp_workspace(c, which, &src, &nb);
+    if (rc) return rc;
+    if (!dst || dst_bytes < nb) return set_error(TCP_EINVAL, "dst too small: %zu < %zu", dst_bytes, nb);
+    TCP_CUDA_CHECK(cudaMemcpyAsync(dst, src, nb, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return TCP_OK;
+}
+
+double tcp_scale(const tcp_ctx* c) { return c ? c->scale : 0.0; }
+size_t tcp_workspace_bytes(const tcp_ctx* c) { return c ? c->bytes : 0; }
+
+int tcp_set_option(tcp_ctx* c, int option, int value) {
+    if (!c) return set_error(TCP_EINVAL, "NULL context");
+    if (option == TCP_OPT_GRID_IMPL) {
+        if (value != TCP_GRID_GATHER && value != TCP_GRID_SCATTER_ATOMIC) return set_error(TCP_EINVAL, "bad grid impl %d", value);
+        if (value == TCP_GRID_SCATTER_ATOMIC && c->half_store) return set_error(TCP_EUNSUPPORTED, "scatter gridding supports TCP_F32 only");
+        c->grid_impl = value;
+        return TCP_OK;
+    }
+    if (option == TCP_OPT_PROFILE) {
+        if (value && !c->pev) {
+            c->pev = (cudaEvent_t*)calloc((size_t)kProfileRing * (TCP_NSTAGES + 1), sizeof(cudaEvent_t));
+            if (!c->pev) return set_error(TCP_ENOMEM, "out of host memory");
+            for (int i = 0; i < kProfileRing * (TCP_NSTAGES + 1); ++i) TCP_CUDA_CHECK(cudaEventCreate(&c->pev[i]));
+        }
+        c->profile = value != 0;
+        c->pcalls = 0;
+        return TCP_OK;
+    }
+    return set_error(TCP_EINVAL, "unknown option %d", option);
+}
+
+}  // extern "C"

@@ -1,0 +1,75 @@
+// tcp_internal.h -- context layout and kernel launchers shared by the .cu files of libtcp.
+#pragma once
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/tcp.h"
+
+struct tcp_ctx {
+    int n, M, nproj, nz, npair, dtype, filter, m;
+    float center;
+    bool half_store;      // intermediates in half / half2 (TCP_F16, TCP_F16_OUT32)
+    bool half_out;        // out in half (TCP_F16)
+    double scale;         // power-of-two scale S of SPECTRUM / GRID / PASS1 (1 in fp32)
+    int grid_impl;
+    int device;
+    // workspaces (device)
+    void* sino;           // [nz][nproj][n]      float | half
+    void* spec;           // [npair][nproj][M]   float2 | half2   (S * G of stage S4, FFT order)
+    void* grid;           // [npair][M][M]       float2 | half2   (row = l2, FFT order)
+    void* pass1;          // [npair][n][M]       float2 | half2   (row = iy, col = l1)
+    double2* trig;        // [nproj] (cos, sin) of theta, fp64
+    // tables (device), built in fp64 on the host at create
+    float2* tw;           // [M] e^{-2 pi i t / M}
+    float* hfilt;         // [M] H[k] / M
+    float2* ptab;         // [M] S * C * e^{+2 pi i k c / M}, k signed; 0 at k = M/2
+    float* deax;          // [n] 1 / (S * Phi(x))
+    float* deay;          // [n] 1 / Phi(y)
+    int* tile_order;      // gather gridding: tiles sorted by decreasing work
+    int ntiles;
+    size_t bytes;
+    // per-kernel profiling (TCP_OPT_PROFILE): ring of event sets, TCP_NSTAGES + 1 events per call
+    bool profile;
+    cudaEvent_t* pev;
+    int pcalls;           // calls recorded since the last collect
+    // chunk pipeline (lazily created by tcp_recon_volume_host)
+    struct Pipe* pipe;
+};
+
+namespace tcpk {
+
+int set_error(int code, const char* fmt, ...);
+#define TCP_CUDA_CHECK(expr)                                                                   \
+    do {                                                                                       \
+        cudaError_t e__ = (expr);                                                              \
+        if (e__ != cudaSuccess)                                                                \
+            return tcpk::set_error(TCP_ECUDA, "%s failed: %s (%s:%d)", #expr,                  \
+                                   cudaGetErrorString(e__), __FILE__, __LINE__);               \
+    } while (0)
+
+// kernel launchers: each enqueues on `st` and returns TCP_OK or an error code
+int launch_trig(const tcp_ctx* c, const float* theta, cudaStream_t st);
+int launch_normalize(const tcp_ctx* c, const uint16_t* raw, const float* flat, const float* dark,
+                     cudaStream_t st);
+int launch_rows(const tcp_ctx* c, cudaStream_t st);
+int launch_grid_scatter(const tcp_ctx* c, cudaStream_t st);
+int launch_grid_gather(const tcp_ctx* c, const float* theta, cudaStream_t st);
+int launch_ifft_cols(const tcp_ctx* c, cudaStream_t st);
+int launch_ifft_rows(const tcp_ctx* c, void* out, cudaStream_t st);
+int launch_mean_frames(const uint16_t* frames, int nframes, int nz, int n, float* mean, cudaStream_t st);
+int setup_kernel_attributes(const tcp_ctx* c);
+void pipe_destroy(tcp_ctx* c);
+
+// storage <-> fp32 helpers
+__device__ __forceinline__ float2 ld_c(const float2* p, size_t i) { return p[i]; }
+__device__ __forceinline__ float2 ld_c(const __half2* p, size_t i) { return __half22float2(p[i]); }
+__device__ __forceinline__ void st_c(float2* p, size_t i, float2 v) { p[i] = v; }
+__device__ __forceinline__ void st_c(__half2* p, size_t i, float2 v) { p[i] = __float22half2_rn(v); }
+__device__ __forceinline__ float ld_r(const float* p, size_t i) { return p[i]; }
+__device__ __forceinline__ float ld_r(const __half* p, size_t i) { return __half2float(p[i]); }
+__device__ __forceinline__ void st_r(float* p, size_t i, float v) { p[i] = v; }
+__device__ __forceinline__ void st_r(__half* p, size_t i, float v) { p[i] = __float2half_rn(v); }
+
+}  // namespace tcpk

@@ -26,5 +26,6 @@ from .counts import (  # noqa: F401
     make_theta,
     make_workload,
     make_counts,
+    make_counts_torch,
     make_flat_dark,
 )

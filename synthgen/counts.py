@@ -135,3 +135,38 @@ def make_counts(w: Workload, z_rows, noise: bool = True):
             cnt = sig * (1.0 + 0.005 * rng.standard_normal(sig.shape))
         raw[:, r, :] = np.clip(np.rint(cnt + doff[None, :]), 0, 65535).astype(np.uint16)
     return raw, p
+
+
+def make_counts_torch(w: Workload, z_rows, device="cuda"):
+    """The same recipe as make_counts/make_flat_dark evaluated with torch on `device`, for the
+    large configs (C3..C5) where numpy would take minutes.  Random draws come from a torch
+    generator seeded with (w.seed, first row), so they differ from the numpy path; the SAME
+    arrays are given to the CUDA path and (copied to the host) to the oracle.
+    Returns (raw_u16[nproj][r][n], flat_frames_u16[K][r][n], dark_frames_u16[K][r][n]) on device."""
+    import torch
+
+    z_rows = np.asarray(z_rows)
+    g = torch.Generator(device=device)
+    g.manual_seed(int(w.seed) * 100003 + int(z_rows[0]))
+    p = line_integrals(w.phantom, w.theta, w.n, w.center, z_rows, w.nz_total, xp=torch,
+                       dtype=torch.float32, device=device)
+    R, n, K = len(z_rows), w.n, w.nframes
+    gain = w.flat_level * (1.0 + 0.02 * torch.randn((R, n), generator=g, device=device))
+    doff = w.dark_level + 3.0 * torch.randn((R, n), generator=g, device=device)
+    sig = gain.clamp_min(0)[None] * torch.exp(-p)
+    if w.noise == "poisson":
+        cnt = torch.poisson(sig, generator=g)
+    elif w.noise == "none":
+        cnt = sig
+    else:
+        cnt = sig * (1.0 + 0.005 * torch.randn(sig.shape, generator=g, device=device))
+    raw = (cnt + doff[None]).round().clamp(0, 65535).to(torch.int32).to(torch.uint16)
+    if K == 1:
+        ff, df = (gain + doff)[None], doff[None]
+    else:
+        ff = torch.poisson(gain.clamp_min(0)[None].expand(K, R, n), generator=g) + doff[None] \
+            + 1.5 * torch.randn((K, R, n), generator=g, device=device)
+        df = doff[None] + 1.5 * torch.randn((K, R, n), generator=g, device=device)
+    ff = ff.round().clamp(0, 65535).to(torch.int32).to(torch.uint16)
+    df = df.round().clamp(0, 65535).to(torch.int32).to(torch.uint16)
+    return raw, ff, df

@@ -124,7 +124,11 @@ def line_integrals(ell: Ellipsoids, theta, n: int, center: float, z_rows, nz_tot
     for e in range(len(ell)):
         a = A[e]
         x0, y0, z0 = ell.center[e]
-        # cull: slices the ellipsoid cannot reach contribute nothing
+        # cull: slices the ellipsoid cannot reach contribute nothing (z half-extent of the
+        # ellipsoid is sqrt((Q diag(a^2) Q^T)_zz))
+        zext = float(np.sqrt(np.sum((ell.rot[e][2, :] * ell.axes[e]) ** 2)))
+        if np.all(np.abs(z_rows - nz_total / 2.0 - z0) > zext):
+            continue
         vx = u * c - x0
         vy = u * s - y0
         vz = zz - z0
@@ -139,6 +143,8 @@ def line_integrals(ell: Ellipsoids, theta, n: int, center: float, z_rows, nz_tot
         chord = 2.0 * xp.sqrt(xp.clip(disc, 0.0, None)) / alpha
         term = float(ell.mu[e]) * chord
         out = term if out is None else out + term
+    if out is None:
+        out = (u * c) * 0.0 + zz * 0.0
     return out
 
 

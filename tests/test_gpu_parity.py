@@ -1,0 +1,193 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Gates (BASELINE.json north_star): fp32 vs oracle gridding <= 1e-5
+rel-L2 per slice; fp16 <= 5e-3 rel-L2 and <= 1e-2 max-abs on the normalised volume."""
+import numpy as np
+import pytest
+import torch
+
+import oracle as orc
+import synthgen as sg
+
+pytestmark = pytest.mark.gpu
+
+FP32_GATE = 1e-5
+FP16_GATE_L2 = 5e-3
+FP16_GATE_MAX = 1e-2
+
+
+def rl2(a, b):
+    a = np.asarray(a).astype(np.complex128 if np.iscomplexobj(a) or np.iscomplexobj(b) else np.float64)
+    b = np.asarray(b).astype(a.dtype)
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def _tcp():
+    import paper_2209_08450_b200 as tcp
+    return tcp
+
+
+def _inputs(w, rows):
+    raw, _ = sg.make_counts(w, rows)
+    flat, dark, _, _ = sg.make_flat_dark(w, rows)
+    return raw, flat, dark, w.theta
+
+
+def _to_dev(raw, flat, dark, theta):
+    return (torch.from_numpy(raw.view(np.int16)).cuda().view(torch.uint16), torch.from_numpy(flat).cuda(),
+            torch.from_numpy(dark).cuda(), torch.from_numpy(theta).cuda())
+
+
+def _gpu_recon(w, rows, dtype, m=3, filt=None, impl="gather", keep=False):
+    tcp = _tcp()
+    raw, flat, dark, theta = _inputs(w, rows)
+    r = tcp.Recon(w.n, w.nproj, len(rows), w.center, dtype, filt or w.filter, m)
+    if impl != "gather":
+        r.set_grid_impl(impl)
+    out = r.recon(*_to_dev(raw, flat, dark, theta))
+    torch.cuda.synchronize()
+    res = out.float().cpu().numpy()
+    if keep:
+        return res, r, (raw, flat, dark, theta)
+    r.close()
+    return res, None, (raw, flat, dark, theta)
+
+
+# ------------------------------------------------------------------ C1, stage by stage
+@pytest.mark.parametrize("m", [3, 4])
+def test_c1_fp32_stages_and_volume(m):
+    w = sg.make_workload("C1")
+    rows = list(range(w.nz_total))
+    out, r, (raw, flat, dark, theta) = _gpu_recon(w, rows, "f32", m=m, keep=True)
+    n, M = w.n, 2 * w.n
+    # S1+S2
+    p = orc.neglog(raw, flat, dark)
+    sino = r.workspace("sinogram").cpu().numpy()
+    assert np.abs(sino - p).max() < 2e-6 * max(1.0, np.abs(p).max())
+    # S3+S4 (pairs packed: slice 2p real, 2p+1 imaginary)
+    spec = r.workspace("spectrum").cpu().numpy()
+    for pair in (0, 3):
+        GA = orc.spectrum(orc.filter_rows(p[2 * pair], w.filter), w.center)
+        GB = orc.spectrum(orc.filter_rows(p[2 * pair + 1], w.filter), w.center)
+        assert rl2(spec[pair], GA + 1j * GB) < 2e-6
+    # S5
+    grid = r.workspace("grid").cpu().numpy()
+    GA = orc.spectrum(orc.filter_rows(p[0], w.filter), w.center)
+    GB = orc.spectrum(orc.filter_rows(p[1], w.filter), w.center)
+    Fo = orc.grid(GA + 1j * GB, theta, n, m)
+    assert rl2(grid[0], Fo) < 3e-6
+    # S1..S7
+    ref = orc.recon(raw, flat, dark, theta, w.center, w.filter, m, "grid")
+    for z in rows:
+        assert rl2(out[z], ref[z]) < FP32_GATE, (z, rl2(out[z], ref[z]))
+    r.close()
+
+
+def test_c1_scatter_matches_gather():
+    w = sg.make_workload("C1")
+    rows = list(range(w.nz_total))
+    a, _, _ = _gpu_recon(w, rows, "f32", impl="gather")
+    b, _, _ = _gpu_recon(w, rows, "f32", impl="scatter")
+    assert rl2(a, b) < 3e-6
+
+
+def test_c1_bitwise_reproducible_and_chunk_independent():
+    w = sg.make_workload("C1")
+    rows = list(range(w.nz_total))
+    a, _, _ = _gpu_recon(w, rows, "f32")
+    b, _, _ = _gpu_recon(w, rows, "f32")
+    assert np.array_equal(a, b)
+    # a chunk equals its slice pairs reconstructed alone
+    c, _, _ = _gpu_recon(w, rows[2:4], "f32")
+    assert np.array_equal(a[2:4], c)
+    # odd chunk: the last slice is paired with zeros
+    d, _, _ = _gpu_recon(w, rows[:3], "f32")
+    assert np.array_equal(a[:2], d[:2])
+    ref = orc.recon(*_inputs(w, rows[2:3])[:3], w.theta, w.center, w.filter, 3, "grid")
+    assert rl2(d[2], ref[0]) < FP32_GATE
+
+
+@pytest.mark.parametrize("dtype", ["f16", "f16_out32"])
+def test_c1_fp16(dtype):
+    w = sg.make_workload("C1")
+    rows = list(range(w.nz_total))
+    out, _, (raw, flat, dark, theta) = _gpu_recon(w, rows, dtype)
+    ref = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, "grid")
+    scale = np.abs(ref).max()
+    for z in rows:
+        assert rl2(out[z], ref[z]) < FP16_GATE_L2
+    assert np.abs(out - ref).max() / scale < FP16_GATE_MAX
+
+
+# ------------------------------------------------------------------ other sizes / filters / centres
+@pytest.mark.parametrize("cfg,scale,dtype", [
+    ("C2", 8, "f32"), ("C2", 4, "f32"), ("C2", 2, "f32"), ("C2", 2, "f16"),
+    ("C3", 8, "f32"), ("C3", 4, "f16"), ("C4", 16, "f16"), ("C4", 8, "f32"), ("C5", 16, "f16_out32"),
+    ("C2", 1, "f32"), ("C2", 1, "f16"), ("C3", 1, "f16"),
+])
+def test_downscaled_configs(cfg, scale, dtype):
+    w = sg.make_workload(cfg, scale=scale)
+    # pairs of ADJACENT slices, as in a real chunk: the two slices of a pair share one complex
+    # transform, so rounding error is relative to the larger of the two
+    h = w.nz_total // 2
+    rows = [0, 1, h, h + 1, w.nz_total - 2, w.nz_total - 1]
+    out, _, (raw, flat, dark, theta) = _gpu_recon(w, rows, dtype)
+    ref = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, "grid")
+    if dtype == "f32":
+        for z in range(len(rows)):
+            assert rl2(out[z], ref[z]) < FP32_GATE, (cfg, scale, z, rl2(out[z], ref[z]))
+    else:
+        for z in range(len(rows)):
+            assert rl2(out[z], ref[z]) < FP16_GATE_L2, (cfg, scale, z, rl2(out[z], ref[z]))
+        assert np.abs(out - ref).max() / np.abs(ref).max() < FP16_GATE_MAX
+
+
+@pytest.mark.parametrize("filt", ["ramp", "shepp", "parzen"])
+def test_filters_and_offcentre(filt):
+    w = sg.make_workload("C1")
+    w.center = 61.75
+    rows = [3, 4]
+    out, _, (raw, flat, dark, theta) = _gpu_recon(w, rows, "f32", filt=filt)
+    ref = orc.recon(raw, flat, dark, theta, w.center, filt, 3, "grid")
+    for z in range(2):
+        assert rl2(out[z], ref[z]) < FP32_GATE
+
+
+def test_mean_frames_and_errors():
+    tcp = _tcp()
+    rng = np.random.default_rng(0)
+    fr = rng.integers(0, 65536, (10, 5, 64), dtype=np.uint16)
+    d = torch.from_numpy(fr.view(np.int16)).cuda().view(torch.uint16)
+    mean = torch.empty((5, 64), dtype=torch.float32, device="cuda")
+    tcp.tcp_mean_frames_u16(d, mean)
+    torch.cuda.synchronize()
+    ref = (fr.astype(np.float64).sum(0) / 10.0)
+    assert np.abs(mean.cpu().numpy() - ref).max() <= np.abs(ref).max() * 2 ** -23
+    for bad in [(100, 10, 2, 50.0), (128, 0, 2, 50.0), (128, 10, 0, 50.0), (128, 10, 2, 200.0), (8192, 10, 2, 50.0)]:
+        with pytest.raises(tcp.TcpError):
+            tcp.tcp_create(bad[0], bad[1], bad[2], bad[3], "f32", "ramp")
+    with pytest.raises(tcp.TcpError):
+        tcp.tcp_create_ex(128, 10, 2, 50.0, "f32", "ramp", 7)
+
+
+def test_pipeline_host_matches_direct():
+    """a7: chunked, stream-overlapped host->host pipeline equals chunk-by-chunk tcp_recon."""
+    tcp = _tcp()
+    w = sg.make_workload("C2", scale=4)           # 128^2 x 128 slices
+    nzt = 22                                       # 5 chunks of 4 + a partial chunk of 2
+    rows = list(range(nzt))
+    raw, flat, dark, theta = _inputs(w, rows)
+    r = tcp.Recon(w.n, w.nproj, 4, w.center, "f32", w.filter)
+    raw_h = torch.from_numpy(raw.view(np.int16)).view(torch.uint16).pin_memory()
+    out_h, ms = r.recon_volume_host(raw_h, torch.from_numpy(flat).pin_memory(), torch.from_numpy(dark).pin_memory(),
+                                    torch.from_numpy(theta).pin_memory(), nbuf=3)
+    assert ms > 0
+    out_h = out_h.numpy()
+    for z0 in range(0, 20, 4):
+        sl = slice(z0, z0 + 4)
+        d = r.recon(*_to_dev(np.ascontiguousarray(raw[:, sl]), flat[sl], dark[sl], theta))
+        torch.cuda.synchronize()
+        assert np.array_equal(out_h[sl], d.cpu().numpy())
+    ref = orc.recon(np.ascontiguousarray(raw[:, 20:22]), flat[20:22], dark[20:22], theta, w.center, w.filter, 3, "grid")
+    for z in range(2):
+        assert rl2(out_h[20 + z], ref[z]) < FP32_GATE
+    r.close()
