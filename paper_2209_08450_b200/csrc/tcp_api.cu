@@ -136,7 +136,7 @@ static int build_context(tcp_ctx* c) {
     for (auto& kv : key) order.push_back(kv.second);
     c->ntiles = (int)order.size();
     if ((rc = upload(&c->tile_order, order, &c->bytes))) return rc;
-    return TCP_OK;
+    return grid_tile_setup(c);
 }
 
 }  // namespace tcpk
@@ -174,7 +174,7 @@ tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, 
     // fp16 storage: S = 2^13 puts |f| Phi^2 S <= 65504 for |f| < 1.9 per pixel while keeping
     // noise-level spectrum samples above the half subnormal range
     c->scale = c->half_store ? 8192.0 : 1.0;
-    c->grid_impl = TCP_GRID_GATHER;
+    c->grid_impl = TCP_GRID_TILE;
     cudaGetDevice(&c->device);
     if (build_context(c) != TCP_OK || setup_kernel_attributes(c) != TCP_OK) {
         char keep[512];
@@ -200,6 +200,7 @@ void tcp_destroy(tcp_ctx* c) {
     cudaFree(c->sino); cudaFree(c->spec); cudaFree(c->grid); cudaFree(c->pass1); cudaFree(c->trig);
     cudaFree(c->tw); cudaFree(c->hfilt); cudaFree(c->ptab); cudaFree(c->deax); cudaFree(c->deay);
     cudaFree(c->tile_order);
+    grid_tile_free(c);
     free(c);
 }
 
@@ -228,7 +229,8 @@ int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* d
     if ((rc = launch_rows(c, st))) return rc;
     TCP_MARK(3);
     if (c->grid_impl == TCP_GRID_SCATTER_ATOMIC) rc = launch_grid_scatter(c, st);
-    else rc = launch_grid_gather(c, theta, st);
+    else if (c->grid_impl == TCP_GRID_GATHER) rc = launch_grid_gather(c, theta, st);
+    else rc = launch_grid_tile(c, theta, st);
     if (rc) return rc;
     TCP_MARK(4);
     if ((rc = launch_ifft_cols(c, st))) return rc;
@@ -256,7 +258,11 @@ int tcp_profile_collect(tcp_ctx* c, double* ms_sum, int* ncalls) {
     return TCP_OK;
 }
 
-int tcp_launches_per_recon(const tcp_ctx* c) { return c ? 6 : 0; }
+int tcp_launches_per_recon(const tcp_ctx* c) {
+    if (!c) return 0;
+    if (c->grid_impl == TCP_GRID_TILE) return 7 + (c->g_nred ? 1 : 0);   // + plan (+ reduce)
+    return c->grid_impl == TCP_GRID_SCATTER_ATOMIC ? 6 : 6;              // (scatter adds a memset, not a kernel)
+}
 
 int tcp_mean_frames_u16(const uint16_t* frames, int nframes, int nz, int n, float* mean, tcp_stream_t stream) {
     if (!frames || !mean || nframes < 1 || nz < 1 || n < 1) return set_error(TCP_EINVAL, "bad argument");
@@ -292,7 +298,7 @@ size_t tcp_workspace_bytes(const tcp_ctx* c) { return c ? c->bytes : 0; }
 int tcp_set_option(tcp_ctx* c, int option, int value) {
     if (!c) return set_error(TCP_EINVAL, "NULL context");
     if (option == TCP_OPT_GRID_IMPL) {
-        if (value != TCP_GRID_GATHER && value != TCP_GRID_SCATTER_ATOMIC) return set_error(TCP_EINVAL, "bad grid impl %d", value);
+        if (value != TCP_GRID_GATHER && value != TCP_GRID_SCATTER_ATOMIC && value != TCP_GRID_TILE) return set_error(TCP_EINVAL, "bad grid impl %d", value);
         if (value == TCP_GRID_SCATTER_ATOMIC && c->half_store) return set_error(TCP_EUNSUPPORTED, "scatter gridding supports TCP_F32 only");
         c->grid_impl = value;
         return TCP_OK;

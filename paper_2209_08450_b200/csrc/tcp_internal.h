@@ -29,6 +29,12 @@ struct tcp_ctx {
     float* deay;          // [n] 1 / Phi(y)
     int* tile_order;      // gather gridding: tiles sorted by decreasing work
     int ntiles;
+    // tile gridding (k_grid_tile.cu): work items, split-tile reduce list, partial tiles, per-call plan
+    int4* g_items;
+    int4* g_red;
+    float2* g_partial;
+    int2* g_plan;
+    int g_nitems, g_nred;
     size_t bytes;
     // per-kernel profiling (TCP_OPT_PROFILE): ring of event sets, TCP_NSTAGES + 1 events per call
     bool profile;
@@ -56,6 +62,9 @@ int launch_normalize(const tcp_ctx* c, const uint16_t* raw, const float* flat, c
 int launch_rows(const tcp_ctx* c, cudaStream_t st);
 int launch_grid_scatter(const tcp_ctx* c, cudaStream_t st);
 int launch_grid_gather(const tcp_ctx* c, const float* theta, cudaStream_t st);
+int launch_grid_tile(const tcp_ctx* c, const float* theta, cudaStream_t st);
+int grid_tile_setup(tcp_ctx* c);
+void grid_tile_free(tcp_ctx* c);
 int launch_ifft_cols(const tcp_ctx* c, cudaStream_t st);
 int launch_ifft_rows(const tcp_ctx* c, void* out, cudaStream_t st);
 int launch_mean_frames(const uint16_t* frames, int nframes, int nz, int n, float* mean, cudaStream_t st);
