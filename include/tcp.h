@@ -45,9 +45,11 @@ enum { TCP_OK = 0, TCP_EINVAL = -1, TCP_ENOMEM = -2, TCP_ECUDA = -3, TCP_EUNSUPP
 /* intermediates a test may inspect through tcp_workspace() */
 enum { TCP_WS_SINOGRAM = 0, TCP_WS_SPECTRUM = 1, TCP_WS_GRID = 2, TCP_WS_PASS1 = 3, TCP_WS_TRIG = 4 };
 /* gridding implementations (tcp_set_option(TCP_OPT_GRID_IMPL, ...)) */
-/* TILE (default): tile-owned, atomics-free, bitwise reproducible; GATHER: per-cell gather
- * (atomics-free, slow; cross-check); SCATTER_ATOMIC: fp32 atomics (TCP_F32 only; cross-check) */
-enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1, TCP_GRID_TILE = 2 };
+/* TILE: tile-owned, atomics-free, bitwise reproducible, CUDA-core FMAs (default for TCP_F32);
+ * MMA: the same tiles with the multiply-accumulate on the tcgen05 tensor cores (fp16 storage only;
+ * default for TCP_F16 / TCP_F16_OUT32); GATHER: per-cell gather (atomics-free, slow; cross-check);
+ * SCATTER_ATOMIC: fp32 atomics (TCP_F32 only; cross-check) */
+enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1, TCP_GRID_TILE = 2, TCP_GRID_MMA = 3 };
 enum { TCP_OPT_GRID_IMPL = 0, TCP_OPT_PROFILE = 1 };
 /* stages timed when TCP_OPT_PROFILE is on, in launch order */
 enum { TCP_ST_TRIG = 0, TCP_ST_NORMALIZE = 1, TCP_ST_ROWS = 2, TCP_ST_GRID = 3, TCP_ST_IFFT_COLS = 4,

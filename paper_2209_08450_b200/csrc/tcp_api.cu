@@ -174,7 +174,7 @@ tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, 
     // fp16 storage: S = 2^13 puts |f| Phi^2 S <= 65504 for |f| < 1.9 per pixel while keeping
     // noise-level spectrum samples above the half subnormal range
     c->scale = c->half_store ? 8192.0 : 1.0;
-    c->grid_impl = TCP_GRID_TILE;
+    c->grid_impl = c->half_store ? TCP_GRID_MMA : TCP_GRID_TILE;
     cudaGetDevice(&c->device);
     if (build_context(c) != TCP_OK || setup_kernel_attributes(c) != TCP_OK) {
         char keep[512];
@@ -260,7 +260,7 @@ int tcp_profile_collect(tcp_ctx* c, double* ms_sum, int* ncalls) {
 
 int tcp_launches_per_recon(const tcp_ctx* c) {
     if (!c) return 0;
-    if (c->grid_impl == TCP_GRID_TILE) return 7 + (c->g_nred ? 1 : 0);   // + plan (+ reduce)
+    if (c->grid_impl == TCP_GRID_TILE || c->grid_impl == TCP_GRID_MMA) return 7 + (c->g_nred ? 1 : 0);   // + plan (+ reduce)
     return c->grid_impl == TCP_GRID_SCATTER_ATOMIC ? 6 : 6;              // (scatter adds a memset, not a kernel)
 }
 
@@ -298,8 +298,9 @@ size_t tcp_workspace_bytes(const tcp_ctx* c) { return c ? c->bytes : 0; }
 int tcp_set_option(tcp_ctx* c, int option, int value) {
     if (!c) return set_error(TCP_EINVAL, "NULL context");
     if (option == TCP_OPT_GRID_IMPL) {
-        if (value != TCP_GRID_GATHER && value != TCP_GRID_SCATTER_ATOMIC && value != TCP_GRID_TILE) return set_error(TCP_EINVAL, "bad grid impl %d", value);
+        if (value < TCP_GRID_GATHER || value > TCP_GRID_MMA) return set_error(TCP_EINVAL, "bad grid impl %d", value);
         if (value == TCP_GRID_SCATTER_ATOMIC && c->half_store) return set_error(TCP_EUNSUPPORTED, "scatter gridding supports TCP_F32 only");
+        if (value == TCP_GRID_MMA && !c->half_store) return set_error(TCP_EUNSUPPORTED, "tensor-core gridding needs fp16 storage");
         c->grid_impl = value;
         return TCP_OK;
     }

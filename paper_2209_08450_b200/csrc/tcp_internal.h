@@ -63,6 +63,7 @@ int launch_rows(const tcp_ctx* c, cudaStream_t st);
 int launch_grid_scatter(const tcp_ctx* c, cudaStream_t st);
 int launch_grid_gather(const tcp_ctx* c, const float* theta, cudaStream_t st);
 int launch_grid_tile(const tcp_ctx* c, const float* theta, cudaStream_t st);
+int launch_grid_mma_main(const tcp_ctx* c, cudaStream_t st);
 int grid_tile_setup(tcp_ctx* c);
 void grid_tile_free(tcp_ctx* c);
 int launch_ifft_cols(const tcp_ctx* c, cudaStream_t st);

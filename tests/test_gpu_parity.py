@@ -37,11 +37,11 @@ def _to_dev(raw, flat, dark, theta):
             torch.from_numpy(dark).cuda(), torch.from_numpy(theta).cuda())
 
 
-def _gpu_recon(w, rows, dtype, m=3, filt=None, impl="tile", keep=False):
+def _gpu_recon(w, rows, dtype, m=3, filt=None, impl=None, keep=False):
     tcp = _tcp()
     raw, flat, dark, theta = _inputs(w, rows)
     r = tcp.Recon(w.n, w.nproj, len(rows), w.center, dtype, filt or w.filter, m)
-    if impl != "tile":          # the library's default
+    if impl is not None:        # default: "tile" for f32, "mma" (tensor cores) for fp16 storage
         r.set_grid_impl(impl)
     out = r.recon(*_to_dev(raw, flat, dark, theta))
     torch.cuda.synchronize()
@@ -93,12 +93,16 @@ def test_c1_gridding_implementations_agree():
     assert rl2(t, a) < 3e-6
     th, _, _ = _gpu_recon(w, rows, "f16", impl="tile")
     ah, _, _ = _gpu_recon(w, rows, "f16", impl="gather")
+    mh, _, _ = _gpu_recon(w, rows, "f16", impl="mma")
     assert rl2(th, ah) < 2e-3
+    # tile (FHFMA) and mma (tcgen05) accumulate in fp32; mma rounds wx, wy and wx*wy to fp16 (three roundings, tile one)
+    assert rl2(mh, th) < 1e-3
 
 
-@pytest.mark.parametrize("dtype,nz", [("f32", 18), ("f16", 18), ("f16", 5)])
+@pytest.mark.parametrize("dtype,nz", [("f32", 18), ("f16", 18), ("f16", 5), ("f16", 32), ("f16", 36)])
 def test_several_pair_groups_and_ragged_chunk(dtype, nz):
-    """nz = 18 -> 9 slice pairs = two pair groups of 8, the second ragged; nz = 5 -> odd, one group of 4."""
+    """nz = 18 -> 9 slice pairs = two pair groups of 8 (tile) / one of 16 (mma), ragged; nz = 5 -> odd;
+    nz = 32 -> one full group of 16 pairs; nz = 36 -> 18 pairs = two mma groups."""
     w = sg.make_workload("C2", scale=4)
     rows = list(range(40, 40 + nz))
     out, _, (raw, flat, dark, theta) = _gpu_recon(w, rows, dtype)
