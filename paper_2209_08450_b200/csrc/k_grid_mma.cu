@@ -19,9 +19,12 @@
 // (8 x NN TMEM columns).  Per batch, the samples that can touch a sub-tile are listed (a chord crosses
 // a sub-tile box in one run), the lists are laid end to end in 16-column segments, and for every
 // 64 columns: phase 1 writes the separable 1D weights (6 + 6 taps) and copies the B rows, phase 2
-// forms the outer products into the MN-major A stage, and one thread issues the MMAs; two stages
-// are ring-buffered on mbarriers signalled by tcgen05.commit.  Deterministic: fixed order, no atomics.
+// forms the outer products into the MN-major A stage.  Warp-specialised: 7 producer warps each build
+// whole 32-column stages (one lane = one column, no block barrier inside the loop), 1 warp issues the
+// MMAs in column order (fixed summation order => bitwise reproducible) from a ring of 4 stages
+// guarded by full/empty mbarriers (tcgen05.commit frees a stage).
 #include <math.h>
+#include <stdio.h>
 
 #include "grid_common.cuh"
 #include "tcp_internal.h"
@@ -29,12 +32,14 @@
 namespace tcpk {
 
 constexpr int SUBX = 16, SUBY = 8, NSUB = 8;      // sub-tile = 128 cells; 2 x 4 sub-tiles per region
-constexpr int MPB = 12;                           // chords per batch
-constexpr int KC = 64;                            // columns (samples) per A/B stage
-constexpr int NST = 2;                            // stages
+constexpr int MPB = 10;                           // chords per batch
+constexpr int SC = 32;                            // columns (samples) per A/B stage = one producer warp
+constexpr int NST = 4;                            // stages in the ring
+constexpr int NPROD = 7;                          // producer warps; warp 7 issues the MMAs
 constexpr int RUNMAX = 32;                        // >= samples of one chord inside a sub-tile's sample box
 constexpr int COLMAX = NSUB * MPB * RUNMAX;       // flat column list capacity (segments are 16-aligned)
 constexpr int A_LBO = (128 / 8) * 128;            // bytes between k-blocks of 8 columns in an A stage
+constexpr int A_STAGE = SC * 256;                 // bytes of one A stage: [SC/8][16][8 columns][8 cells] half
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -46,13 +51,24 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t addr, uint32_t lbo, uint3
 __device__ __forceinline__ void mbar_init(uint64_t* b, int count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count));
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
+__device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity, int tag = 0, int info = 0) {
     uint32_t done = 0;
-    while (!done)
+#ifdef TCP_MBAR_WATCHDOG
+    unsigned spins = 0;
+#endif
+    while (!done) {
         asm volatile("{.reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p;}"
                      : "=r"(done)
                      : "r"(smem_u32(b)), "r"(parity)
                      : "memory");
+#ifdef TCP_MBAR_WATCHDOG
+        if (!done && ++spins > (1u << 22)) {
+            if ((threadIdx.x & 31) == 0)
+                printf("mbar stuck: block %d,%d warp %d tag %d parity %u info %d\n", blockIdx.x, blockIdx.y, threadIdx.x >> 5, tag, parity, info);
+            __trap();
+        }
+#endif
+    }
 }
 __device__ __forceinline__ void umma_commit(uint64_t* b) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(b)) : "memory");
@@ -79,27 +95,43 @@ template <> struct TmemLd<32> {
     }
 };
 
-// bytes of dynamic shared memory, and the carve-up (all offsets multiples of 128)
+__device__ __forceinline__ void mbar_arrive(uint64_t* b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+
+// nu = k * (c_hi + c_lo) as floor + fraction, fp32 FMAs only (k exact, |k| < 2^13): the product's
+// rounding error is recovered exactly by an FMA, so fl + frac = nu to ~1e-11 cells.
+__device__ __forceinline__ void nu_split(float k, float c_hi, float c_lo, float& fl, float& frac) {
+    const float p = k * c_hi;
+    const float e = fmaf(k, c_hi, -p);
+    const float t = fmaf(k, c_lo, e);
+    fl = floorf(p);
+    frac = (p - fl) + t;
+    if (frac < 0.f) { fl -= 1.f; frac += 1.f; }
+    else if (frac >= 1.f) { fl += 1.f; frac -= 1.f; }
+}
+
+// dynamic shared memory carve-up
 template <int MH, int NN>
 struct MmaSmem {
     static constexpr int KL = chord_len(MH);
     static constexpr int NSLOT = MPB * KL;
     static constexpr int GW = NN * 2 / 16;                   // uint4 per sample (B row)
     static constexpr int B_LBO = (NN / 8) * 128;
-    static constexpr int offA = 0;                           // [NST][KC/8][16][8][8] half
-    static constexpr int offB = offA + NST * KC * 256;       // [NST][KC/8][NN/8][8][8] half
-    static constexpr int offMeta = offB + NST * KC * NN * 2; // [NSLOT] float4
+    static constexpr int B_STAGE = SC * NN * 2;
+    static constexpr int offA = 0;                           // [NST] A stages
+    static constexpr int offB = offA + NST * A_STAGE;        // [NST] B stages
+    static constexpr int offMeta = offB + NST * B_STAGE;     // [NSLOT] float4: first tap x, d0x, first tap y, d0y
     static constexpr int offG = offMeta + NSLOT * 16;        // [NSLOT][GW] uint4
-    static constexpr int offWx = offG + NSLOT * GW * 16;     // [2][KC] uint4 (lx 0..7 | 8..15)
-    static constexpr int offWy = offWx + 2 * KC * 16;        // [KC] uint4 (ly 0..7)
-    static constexpr int offCol = offWy + KC * 16;           // [COLMAX] uint16
+    static constexpr int offWs = offG + NSLOT * GW * 16;     // [NPROD][3][32] uint4: wx lo, wx hi, wy per lane
+    static constexpr int offCol = offWs + NPROD * 3 * 32 * 16;   // [COLMAX] uint16
     static constexpr int offRec = offCol + COLMAX * 2;       // [MPB] ChordRec
-    static constexpr int offRecj = offRec + MPB * 16;        // [MPB] int
+    static constexpr int offRecj = offRec + MPB * 16;        // [MPB] int (padded to 64 B)
     static constexpr int offHits = offRecj + 64;             // [NTHR] int2
-    static constexpr int offRun = offHits + NTHR * 8;        // [NSUB][MPB] int (start | len << 16), then pre[NSUB][MPB] int
-    static constexpr int offMisc = offRun + 2 * NSUB * MPB * 4;   // wcount[9], seg[9], flags
-    static constexpr int offBar = offMisc + 128;             // mbarriers: free[NST], done
-    static constexpr int total = offBar + 64;
+    static constexpr int offRun = offHits + NTHR * 8;        // run[NSUB][MPB], pre[NSUB][MPB] int
+    static constexpr int offMisc = offRun + 2 * NSUB * MPB * 4;   // wcount[9], seg[9], tmem base, started
+    static constexpr int offBar = offMisc + 128;             // mbarriers: full[NST], empty[NST], done
+    static constexpr int total = offBar + 128;
 };
 
 // ---------------------------------------------------------------------------------------
@@ -107,15 +139,13 @@ struct MmaSmem {
 template <int MH, int NN>
 __global__ void __launch_bounds__(NTHR, 2)
     grid_mma_kernel(const __half2* __restrict__ spec, __half2* __restrict__ grid, float2* __restrict__ partial,
-                    const double2* __restrict__ trig, const int2* __restrict__ plan, const int4* __restrict__ items,
-                    int nproj, int M, int npair, float alpha2) {
+                    const double2* __restrict__ trig, const float4* __restrict__ trigf, const int2* __restrict__ plan,
+                    const int4* __restrict__ items, int nproj, int M, int npair, float alpha2) {
     using L = MmaSmem<MH, NN>;
     constexpr int KL = L::KL, GW = L::GW, NPG = NN / 2;
     extern __shared__ __align__(128) unsigned char smem[];
     float4* meta = reinterpret_cast<float4*>(smem + L::offMeta);
     uint4* gs = reinterpret_cast<uint4*>(smem + L::offG);
-    uint4* wxs = reinterpret_cast<uint4*>(smem + L::offWx);
-    uint4* wys = reinterpret_cast<uint4*>(smem + L::offWy);
     unsigned short* colslot = reinterpret_cast<unsigned short*>(smem + L::offCol);
     ChordRec* rec = reinterpret_cast<ChordRec*>(smem + L::offRec);
     int* recj = reinterpret_cast<int*>(smem + L::offRecj);
@@ -124,9 +154,11 @@ __global__ void __launch_bounds__(NTHR, 2)
     int* pre = run + NSUB * MPB;                                      // [NSUB][MPB] offset inside the segment
     int* wcount = reinterpret_cast<int*>(smem + L::offMisc);          // [9]
     int* seg = wcount + 9;                                            // [9] segment starts (columns), seg[8] = total
-    uint32_t* shared_u32 = reinterpret_cast<uint32_t*>(seg + 9);      // [0] tmem base, [1] started mask
-    uint64_t* bar_free = reinterpret_cast<uint64_t*>(smem + L::offBar);
-    uint64_t* bar_done = bar_free + NST;
+    uint32_t* shared_u32 = reinterpret_cast<uint32_t*>(seg + 9);      // [0] tmem base, [1] started mask, [2] completed passes
+    volatile uint32_t* prog = shared_u32 + 2;
+    uint64_t* bar_full = reinterpret_cast<uint64_t*>(smem + L::offBar);
+    uint64_t* bar_empty = bar_full + NST;
+    uint64_t* bar_done = bar_empty + NST;
 
     const int n = M >> 1, tiles = M / TS;
     const int4 item = items[blockIdx.x];
@@ -136,10 +168,11 @@ __global__ void __launch_bounds__(NTHR, 2)
     const int TX0 = (tile % tiles) * TS, TY0 = (tile / tiles) * TS;
 
     if (tid == 0) {
-        for (int s = 0; s < NST; ++s) mbar_init(&bar_free[s], 1);
+        for (int s = 0; s < NST; ++s) { mbar_init(&bar_full[s], 1); mbar_init(&bar_empty[s], 1); }
         mbar_init(bar_done, 1);
         asm volatile("fence.mbarrier_init.release.cluster;");
         shared_u32[1] = 0;
+        shared_u32[2] = 0;
     }
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&shared_u32[0])), "n"(NSUB * NN));
@@ -151,8 +184,8 @@ __global__ void __launch_bounds__(NTHR, 2)
     const uint32_t tmem = shared_u32[0];
     // instruction descriptor: D fp32, A/B fp16, both MN-major, N = NN, M = 128
     constexpr uint32_t IDESC = (1u << 4) | (1u << 15) | (1u << 16) | ((uint32_t)(NN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-    uint32_t started = 0;          // thread 0: sub-tiles whose accumulator has been written
-    uint32_t nfill = 0;            // stage fills so far (uniform)
+    uint32_t started = 0;          // issuer: sub-tiles whose accumulator has been written
+    uint32_t gpass = 0;            // stages filled so far in this item (uniform)
 
     for (int img = 0; img < 4; ++img) {
         const int2 win = plan[tile * 4 + img];
@@ -173,8 +206,8 @@ __global__ void __launch_bounds__(NTHR, 2)
             if (i < i_hi) {
                 j = win.x + i;
                 if (j >= nproj) j -= nproj;
-                const double2 cs = trig[j];
-                hit = chord_range((float)cs.x, (float)cs.y, bax, bbx, bay, bby, (float)(n - 1), kmin, kmax);
+                const float4 cs = trigf[j];
+                hit = chord_range(cs.x, cs.z, bax, bbx, bay, bby, (float)(n - 1), kmin, kmax);
             }
             const unsigned bal = __ballot_sync(0xffffffffu, hit);
             if (lane == 0) wcount[warp] = __popc(bal);
@@ -197,40 +230,39 @@ __global__ void __launch_bounds__(NTHR, 2)
                 const int nb = min(MPB, nhit - b0);
                 if (tid < nb) {
                     const int2 h = hits[b0 + tid];
-                    const double2 cs = trig[h.x];
+                    const float4 cs = trigf[h.x];
                     ChordRec r;
-                    r.c = (float)cs.x;
-                    r.s = (float)cs.y;
+                    r.c = cs.x;
+                    r.s = cs.z;
                     r.inv = 0.f;
                     r.pack = h.y;
                     rec[tid] = r;
                     recj[tid] = h.x;
                 }
                 __syncthreads();
-                // ---- stage the chords: one B row (NN halves) + the first tap and its distance per sample
+                // ---- stage the chords: one B row (NN halves) + the first tap and its distance per sample.
+                // taps l = floor(nu) - m + 1 + t, t = 0..2m-1, distance d_t = l - nu = d_0 + t; the open box
+                // |l - nu| < m keeps t iff d_t < m (d_0 > -m always), and d_0 = -m+1 exactly iff nu is an integer
                 for (int idx = tid; idx < nb * KL; idx += NTHR) {
                     const int r = idx / KL, kl = idx - r * KL;
                     const int pk = rec[r].pack;
                     if (kl >= ((pk >> 16) & 0xff)) continue;
                     const int k = (int)(short)(pk & 0xffff) + kl;
                     const int jj = recj[r];
-                    const double2 cs = trig[jj];
-                    const double nu1 = (double)k * cs.x, nu2 = (double)k * cs.y;
-                    // taps l = floor(nu) - m + 1 + t, t = 0..2m-1, distance d_t = l - nu; the open box
-                    // |l - nu| < m keeps t iff d_t < m (d_0 > -m always).  d_0 is rounded to fp32 so that
-                    // this test still decides as in fp64: exactly -m+1 only when nu is an integer.
-                    const double f1 = floor(nu1) - (double)(MH - 1), f2 = floor(nu2) - (double)(MH - 1);
-                    float d1 = (float)(f1 - nu1), d2 = (float)(f2 - nu2);
+                    const float4 cs = trigf[jj];
+                    float f1, r1, f2, r2;
+                    nu_split((float)k, cs.x, cs.y, f1, r1);
+                    nu_split((float)k, cs.z, cs.w, f2, r2);
                     const float dint = -(float)(MH - 1);
-                    if (d1 >= dint && (f1 - nu1) < (double)dint) d1 = __uint_as_float(__float_as_uint(dint) + 1u);   // next below
-                    if (d2 >= dint && (f2 - nu2) < (double)dint) d2 = __uint_as_float(__float_as_uint(dint) + 1u);
-                    meta[idx] = make_float4((float)(f1 - (double)X0), d1, (float)(f2 - (double)Y0), d2);
+                    float d1 = dint - r1, d2 = dint - r2;
+                    if (r1 > 0.f && d1 >= dint) d1 = __uint_as_float(__float_as_uint(dint) + 1u);   // next below -m+1
+                    if (r2 > 0.f && d2 >= dint) d2 = __uint_as_float(__float_as_uint(dint) + 1u);
+                    meta[idx] = make_float4(f1 + dint - (float)X0, d1, f2 + dint - (float)Y0, d2);
+                    const __half2* src = spec + ((size_t)(pg * NPG) * nproj + jj) * M + (size_t)(k & (M - 1));
+                    const size_t pstride = (size_t)nproj * M;
                     alignas(16) __half2 v[NPG];
 #pragma unroll
-                    for (int p = 0; p < NPG; ++p) {
-                        const int pair = pg * NPG + p;
-                        v[p] = (pair < npair) ? spec[((size_t)pair * nproj + jj) * M + (size_t)(k & (M - 1))] : czero<__half2>();
-                    }
+                    for (int p = 0; p < NPG; ++p) v[p] = (pg * NPG + p < npair) ? src[p * pstride] : czero<__half2>();
                     const uint4* vv = reinterpret_cast<const uint4*>(v);
 #pragma unroll
                     for (int q = 0; q < GW; ++q) gs[(size_t)idx * GW + q] = vv[q];
@@ -268,129 +300,141 @@ __global__ void __launch_bounds__(NTHR, 2)
                     for (int b = 0; b < NSUB; ++b) {
                         if (tid == 0) seg[b] = s0;
                         const int len = wcount[b];
-                        // fill: run slots, then padding up to a multiple of 16 columns
+                        // run slots, then padding up to a multiple of 16 columns (one MMA K step = one sub-tile)
                         if (tid < nb * NSUB && (tid - (tid / NSUB) * NSUB) == b) {
                             const int r = tid / NSUB, rv = run[b * MPB + r], st = rv & 0xffff, ln = rv >> 16;
                             unsigned short* dst = colslot + s0 + pre[b * MPB + r];
                             for (int q = 0; q < ln; ++q) dst[q] = (unsigned short)(st + q);
                         }
                         const int padded = (len + 15) & ~15;
-                        if (tid >= NTHR - 16 && s0 + len + (tid - (NTHR - 16)) < s0 + padded) colslot[s0 + len + (tid - (NTHR - 16))] = 0xffffu;
+                        if (tid >= NTHR - 16 && len + (tid - (NTHR - 16)) < padded) colslot[s0 + len + (tid - (NTHR - 16))] = 0xffffu;
                         s0 += padded;
                     }
                     if (tid == 0) seg[NSUB] = s0;
                 }
                 __syncthreads();
                 const int ncols = seg[NSUB];
-                // ---- 64 columns at a time: weights -> A stage, spectra -> B stage, MMAs
-                for (int c0 = 0; c0 < ncols; c0 += KC) {
-                    const int st = nfill & (NST - 1);
-                    if (nfill >= NST) mbar_wait(&bar_free[st], ((nfill / NST) - 1) & 1);   // MMAs that read this stage are done
-                    unsigned char* As = smem + L::offA + st * (KC * 256);
-                    unsigned char* Bs = smem + L::offB + st * (KC * NN * 2);
-                    // phase 1: thread = (column, part); part 0: x taps, 1: y taps, 2..3: B row
-                    {
-                        const int cl = tid & (KC - 1), part = tid >> 6, col = c0 + cl;
+                const int npass = (ncols + SC - 1) / SC;
+                if (warp < NPROD) {
+                    // ======== producers: one warp = one 32-column stage, one lane = one column ========
+                    uint4* ws = reinterpret_cast<uint4*>(smem + L::offWs) + warp * 3 * 32;   // wx lo | wx hi | wy, [32 lanes]
+                    for (int p = warp; p < npass; p += NPROD) {
+                        const uint32_t gp = gpass + (uint32_t)p, st = gp % NST;
+                        // the MMAs of pass gp - NST (same stage) must be complete.  An mbarrier wait only tells odd
+                        // from even phases and producers of different rounds of a stage are different warps, so
+                        // they follow the issuer's published count of completed passes instead
+                        if (gp >= NST) {
+#ifdef TCP_MBAR_WATCHDOG
+                            unsigned spins = 0;
+#endif
+                            while (*prog + NST <= gp) {
+#ifdef TCP_MBAR_WATCHDOG
+                                if (++spins > (1u << 24)) { if (lane == 0) printf("prog stuck: block %d warp %d gp %u prog %u\n", blockIdx.x, warp, gp, *prog); __trap(); }
+#endif
+                            }
+                            __threadfence_block();
+                        }
+                        unsigned char* As = smem + L::offA + st * A_STAGE;
+                        unsigned char* Bs = smem + L::offB + st * L::B_STAGE;
+                        const int col = p * SC + lane;
                         const int slot = (col < ncols) ? (int)colslot[col] : 0xffff;
                         int b = 0;
 #pragma unroll
                         for (int q = 1; q < NSUB; ++q) b += (col >= seg[q]);
-                        if (part == 0) {
-                            wxs[cl] = make_uint4(0, 0, 0, 0);
-                            wxs[KC + cl] = make_uint4(0, 0, 0, 0);
-                            if (slot != 0xffff) {
-                                const float4 mt = meta[slot];
-                                const int l0 = (int)mt.x - (b & 1) * SUBX;
-                                __half* w = reinterpret_cast<__half*>(wxs);
+                        ws[lane] = make_uint4(0, 0, 0, 0);
+                        ws[32 + lane] = make_uint4(0, 0, 0, 0);
+                        ws[64 + lane] = make_uint4(0, 0, 0, 0);
+                        unsigned char* brow = Bs + (lane >> 3) * L::B_LBO + (lane & 7) * 16;
+                        if (slot != 0xffff) {
+                            const float4 mt = meta[slot];
+                            __half* wh = reinterpret_cast<__half*>(ws);
+                            const int lx0 = (int)mt.x - (b & 1) * SUBX, ly0 = (int)mt.z - (b >> 1) * SUBY;
 #pragma unroll
-                                for (int t = 0; t < 2 * MH; ++t) {
-                                    const float d = mt.y + (float)t;
-                                    const int lx = l0 + t;
-                                    if ((unsigned)lx < (unsigned)SUBX && d < (float)MH)
-                                        w[((lx >> 3) * KC + cl) * 8 + (lx & 7)] = __float2half_rn(ex2_approx(-alpha2 * d * d));
-                                }
+                            for (int t = 0; t < 2 * MH; ++t) {
+                                const float dx = mt.y + (float)t, dy = mt.w + (float)t;
+                                const int lx = lx0 + t, ly = ly0 + t;
+                                if ((unsigned)lx < (unsigned)SUBX && dx < (float)MH)
+                                    wh[((lx >> 3) * 32 + lane) * 8 + (lx & 7)] = __float2half_rn(ex2_approx(-alpha2 * dx * dx));
+                                if ((unsigned)ly < (unsigned)SUBY && dy < (float)MH)
+                                    wh[(64 + lane) * 8 + ly] = __float2half_rn(ex2_approx(-alpha2 * dy * dy));
                             }
-                        } else if (part == 1) {
-                            wys[cl] = make_uint4(0, 0, 0, 0);
-                            if (slot != 0xffff) {
-                                const float4 mt = meta[slot];
-                                const int l0 = (int)mt.z - (b >> 1) * SUBY;
-                                __half* w = reinterpret_cast<__half*>(wys);
 #pragma unroll
-                                for (int t = 0; t < 2 * MH; ++t) {
-                                    const float d = mt.w + (float)t;
-                                    const int ly = l0 + t;
-                                    if ((unsigned)ly < (unsigned)SUBY && d < (float)MH)
-                                        w[cl * 8 + ly] = __float2half_rn(ex2_approx(-alpha2 * d * d));
-                                }
-                            }
+                            for (int q = 0; q < GW; ++q) *reinterpret_cast<uint4*>(brow + q * 128) = gs[(size_t)slot * GW + q];
                         } else {
-                            // B row: n-block q of column cl at (cl / 8) * B_LBO + q * 128 + (cl % 8) * 16
 #pragma unroll
-                            for (int q = (part - 2) * (GW / 2); q < (part - 1) * (GW / 2); ++q) {
-                                const uint4 v = (slot != 0xffff) ? gs[(size_t)slot * GW + q] : make_uint4(0, 0, 0, 0);
-                                *reinterpret_cast<uint4*>(Bs + (cl >> 3) * L::B_LBO + q * 128 + (cl & 7) * 16) = v;
+                            for (int q = 0; q < GW; ++q) *reinterpret_cast<uint4*>(brow + q * 128) = make_uint4(0, 0, 0, 0);
+                        }
+                        // A[m = ly * 16 + lx][column] = wy[ly] * wx[lx]; MN-major: 8 cells of a column = 16 B
+                        const uint4 xa = ws[lane], xc = ws[32 + lane], yv = ws[64 + lane];
+                        const unsigned yw[4] = {yv.x, yv.y, yv.z, yv.w};
+                        unsigned char* arow = As + (lane >> 3) * A_LBO + (lane & 7) * 16;
+#pragma unroll
+                        for (int ly = 0; ly < SUBY; ++ly) {
+                            const unsigned yb = (ly & 1) ? (yw[ly >> 1] >> 16) : (yw[ly >> 1] & 0xffffu);
+                            uint4 lo = make_uint4(0, 0, 0, 0), hi = lo;
+                            if (__any_sync(0xffffffffu, yb != 0)) {
+                                const unsigned y2 = yb | (yb << 16);
+                                auto mul = [&](unsigned x) {
+                                    const __half2 pr = __hmul2(*reinterpret_cast<const __half2*>(&x), *reinterpret_cast<const __half2*>(&y2));
+                                    return *reinterpret_cast<const unsigned*>(&pr);
+                                };
+                                lo = make_uint4(mul(xa.x), mul(xa.y), mul(xa.z), mul(xa.w));
+                                hi = make_uint4(mul(xc.x), mul(xc.y), mul(xc.z), mul(xc.w));
+                            }
+                            *reinterpret_cast<uint4*>(arow + (2 * ly) * 128) = lo;
+                            *reinterpret_cast<uint4*>(arow + (2 * ly + 1) * 128) = hi;
+                        }
+                        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(&bar_full[st]);
+                    }
+                } else {
+                    // ======== issuer: stages in column order ========
+                    for (int p = 0; p < npass; ++p) {
+                        const uint32_t gp = gpass + (uint32_t)p, st = gp % NST, round = gp / NST;
+                        mbar_wait(&bar_full[st], round & 1, 2, (int)gp);
+                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                        if (lane == 0) {
+                            const int nk = (min(SC, ncols - p * SC) + 15) >> 4;
+                            const uint32_t a0 = smem_u32(smem + L::offA + st * A_STAGE), b0a = smem_u32(smem + L::offB + st * L::B_STAGE);
+                            for (int kk = 0; kk < nk; ++kk) {
+                                const int col = p * SC + kk * 16;
+                                int b = 0;
+#pragma unroll
+                                for (int q = 1; q < NSUB; ++q) b += (col >= seg[q]);
+                                umma_f16(tmem + (uint32_t)(b * NN), umma_desc(a0 + kk * 2 * A_LBO, A_LBO, 128),
+                                         umma_desc(b0a + kk * 2 * L::B_LBO, L::B_LBO, 128), IDESC, (started >> b) & 1u);
+                                started |= 1u << b;
+                            }
+                            umma_commit(&bar_empty[st]);
+                            // observe the previous pass's completion (in order: no parity aliasing) and publish it
+                            if (gp > 0) {
+                                mbar_wait(&bar_empty[(gp - 1) % NST], ((gp - 1) / NST) & 1, 1, (int)gp);
+                                *prog = gp;
                             }
                         }
+                        __syncwarp();
                     }
-                    __syncthreads();
-                    // phase 2: A[m = ly * 16 + lx][column] = wy[ly] * wx[lx], MN-major: 8 cells = 16 B
-#pragma unroll
-                    for (int u = tid; u < KC * SUBY; u += NTHR) {
-                        const int cl = u & (KC - 1), ly = u >> 6;
-                        const unsigned short wyb = reinterpret_cast<const unsigned short*>(wys)[cl * 8 + ly];
-                        uint4 lo = make_uint4(0, 0, 0, 0), hi = lo;
-                        if (wyb != 0) {
-                            const __half wyh = __ushort_as_half(wyb);
-                            const __half2 wy2 = __halves2half2(wyh, wyh);
-                            const uint4 a = wxs[cl], c = wxs[KC + cl];
-                            auto mul = [&](unsigned x) {
-                                const __half2 p = __hmul2(*reinterpret_cast<const __half2*>(&x), wy2);
-                                return *reinterpret_cast<const unsigned*>(&p);
-                            };
-                            lo = make_uint4(mul(a.x), mul(a.y), mul(a.z), mul(a.w));
-                            hi = make_uint4(mul(c.x), mul(c.y), mul(c.z), mul(c.w));
-                        }
-                        unsigned char* dst = As + (cl >> 3) * A_LBO + (2 * ly) * 128 + (cl & 7) * 16;
-                        *reinterpret_cast<uint4*>(dst) = lo;
-                        *reinterpret_cast<uint4*>(dst + 128) = hi;
-                    }
-                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                    __syncthreads();
-                    if (tid == 0) {
-                        asm volatile("tcgen05.fence::after_thread_sync;");
-                        const int nk = (min(KC, ncols - c0) + 15) >> 4;
-                        const uint32_t a0 = smem_u32(As), b0a = smem_u32(Bs);
-                        for (int kk = 0; kk < nk; ++kk) {
-                            const int col = c0 + kk * 16;
-                            int b = 0;
-#pragma unroll
-                            for (int q = 1; q < NSUB; ++q) b += (col >= seg[q]);
-                            umma_f16(tmem + (uint32_t)(b * NN), umma_desc(a0 + kk * 2 * A_LBO, A_LBO, 128),
-                                     umma_desc(b0a + kk * 2 * L::B_LBO, L::B_LBO, 128), IDESC, (started >> b) & 1u);
-                            started |= 1u << b;
-                        }
-                        umma_commit(&bar_free[st]);
-                    }
-                    ++nfill;
                 }
+                gpass += (uint32_t)npass;
                 __syncthreads();                      // staging buffers, runs and column list are reused
             }
         }
     }
 
     // ---- epilogue: wait for the MMAs, TMEM -> registers -> grid (or partial tile)
-    if (tid == 0) {
+    if (tid == NPROD * 32) {
         shared_u32[1] = started;
         if (started) umma_commit(bar_done);
     }
     __syncthreads();
     const uint32_t started_all = shared_u32[1];
-    if (started_all) mbar_wait(bar_done, 0);
-    asm volatile("tcgen05.fence::after_thread_sync;");
+    if (started_all) mbar_wait(bar_done, 0, 3, 0);
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     {
         const int q = warp & 3, hsel = warp >> 2;
         const int mrow = q * 32 + lane, ly = mrow >> 4, lx = mrow & 15;
+        const size_t pstride = (size_t)M * M;
 #pragma unroll 1
         for (int bb = 0; bb < NSUB / 2; ++bb) {
             const int b = hsel * (NSUB / 2) + bb;
@@ -404,24 +448,19 @@ __global__ void __launch_bounds__(NTHR, 2)
             }
             const int ry = (b >> 1) * SUBY + ly, rx = (b & 1) * SUBX + lx;      // region-relative cell
             if (item.z < 0) {
+                __half2* dst = grid + ((size_t)(pg * NPG) * M + TY0 + ry) * M + TX0 + rx;
 #pragma unroll
-                for (int p = 0; p < NPG; ++p) {
-                    const int pair = pg * NPG + p;
-                    if (pair < npair)
-                        grid[((size_t)pair * M + TY0 + ry) * M + TX0 + rx] = __floats2half2_rn(__uint_as_float(r[2 * p]), __uint_as_float(r[2 * p + 1]));
-                }
+                for (int p = 0; p < NPG; ++p)
+                    if (pg * NPG + p < npair) dst[p * pstride] = __floats2half2_rn(__uint_as_float(r[2 * p]), __uint_as_float(r[2 * p + 1]));
             } else {
+                float2* dst = partial + (((size_t)(item.z + split) * npair + pg * NPG) * TS + ry) * TS + rx;
 #pragma unroll
-                for (int p = 0; p < NPG; ++p) {
-                    const int pair = pg * NPG + p;
-                    if (pair < npair)
-                        partial[(((size_t)(item.z + split) * npair + pair) * TS + ry) * TS + rx] =
-                            make_float2(__uint_as_float(r[2 * p]), __uint_as_float(r[2 * p + 1]));
-                }
+                for (int p = 0; p < NPG; ++p)
+                    if (pg * NPG + p < npair) dst[p * (TS * TS)] = make_float2(__uint_as_float(r[2 * p]), __uint_as_float(r[2 * p + 1]));
             }
         }
     }
-    asm volatile("tcgen05.fence::before_thread_sync;");
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(NSUB * NN));
 }
@@ -434,14 +473,14 @@ static int launch_mma_t(const tcp_ctx* c, cudaStream_t st) {
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L::total));
     const double alpha = 3.14159265358979323846 / (1.4142135623730951 * MH);
     dim3 grid(c->g_nitems, (c->npair + NN / 2 - 1) / (NN / 2));
-    kern<<<grid, NTHR, L::total, st>>>((const __half2*)c->spec, (__half2*)c->grid, c->g_partial, c->trig, c->g_plan, c->g_items,
-                                       c->nproj, c->M, c->npair, (float)(alpha * 1.4426950408889634));
+    kern<<<grid, NTHR, L::total, st>>>((const __half2*)c->spec, (__half2*)c->grid, c->g_partial, c->trig, c->trigf, c->g_plan,
+                                       c->g_items, c->nproj, c->M, c->npair, (float)(alpha * 1.4426950408889634));
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }
 
 // Enqueue the tensor-core gridding of the spectrum into the grid (fp16 storage only); the plan
-// kernel and the split-tile reduce are launched by launch_grid_tile's caller.
+// kernel and the split-tile reduce are launched by launch_grid_tile.
 int launch_grid_mma_main(const tcp_ctx* c, cudaStream_t st) {
     if (!c->half_store) return set_error(TCP_EUNSUPPORTED, "tensor-core gridding needs fp16 storage");
     const bool wide = c->npair > 8;

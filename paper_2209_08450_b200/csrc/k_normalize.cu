@@ -102,16 +102,21 @@ int launch_mean_frames(const uint16_t* frames, int nframes, int nz, int n, float
 
 // cos/sin of the float32 angles in fp64: k*cos(theta) with
 // k up to 4096 must be good to ~1e-6 grid cells for the 1e-5 fp32 gate.
-__global__ void trig_kernel(const float* __restrict__ theta, int nproj, double2* __restrict__ trig) {
+__global__ void trig_kernel(const float* __restrict__ theta, int nproj, double2* __restrict__ trig, float4* __restrict__ trigf) {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j < nproj) {
         double t = (double)theta[j];
-        trig[j] = make_double2(cos(t), sin(t));
+        const double c = cos(t), s = sin(t);
+        trig[j] = make_double2(c, s);
+        // float-float split (hi + lo = the fp64 value to 2^-48): lets the fp16 gridding kernel form
+        // k*cos, k*sin to ~1e-11 cells with fp32 FMAs only
+        const float ch = (float)c, sh = (float)s;
+        trigf[j] = make_float4(ch, (float)(c - (double)ch), sh, (float)(s - (double)sh));
     }
 }
 
 int launch_trig(const tcp_ctx* c, const float* theta, cudaStream_t st) {
-    trig_kernel<<<(c->nproj + 127) / 128, 128, 0, st>>>(theta, c->nproj, c->trig);
+    trig_kernel<<<(c->nproj + 127) / 128, 128, 0, st>>>(theta, c->nproj, c->trig, c->trigf);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }

@@ -81,6 +81,7 @@ static int build_context(tcp_ctx* c) {
     if ((rc = dev_alloc(&c->grid, (size_t)c->npair * M * M * cb, &c->bytes))) return rc;
     if ((rc = dev_alloc(&c->pass1, (size_t)c->npair * n * M * cb, &c->bytes))) return rc;
     if ((rc = dev_alloc((void**)&c->trig, (size_t)c->nproj * sizeof(double2), &c->bytes))) return rc;
+    if ((rc = dev_alloc((void**)&c->trigf, (size_t)c->nproj * sizeof(float4), &c->bytes))) return rc;
 
     std::vector<float2> tw(M);
     for (int t = 0; t < M; ++t) {
@@ -197,7 +198,7 @@ void tcp_destroy(tcp_ctx* c) {
         for (int i = 0; i < kProfileRing * (TCP_NSTAGES + 1); ++i) cudaEventDestroy(c->pev[i]);
         free(c->pev);
     }
-    cudaFree(c->sino); cudaFree(c->spec); cudaFree(c->grid); cudaFree(c->pass1); cudaFree(c->trig);
+    cudaFree(c->sino); cudaFree(c->spec); cudaFree(c->grid); cudaFree(c->pass1); cudaFree(c->trig); cudaFree(c->trigf);
     cudaFree(c->tw); cudaFree(c->hfilt); cudaFree(c->ptab); cudaFree(c->deax); cudaFree(c->deay);
     cudaFree(c->tile_order);
     grid_tile_free(c);

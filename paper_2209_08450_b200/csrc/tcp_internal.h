@@ -21,6 +21,7 @@ struct tcp_ctx {
     void* grid;           // [npair][M][M]       float2 | half2   (row = l2, FFT order)
     void* pass1;          // [npair][n][M]       float2 | half2   (row = iy, col = l1)
     double2* trig;        // [nproj] (cos, sin) of theta, fp64
+    float4* trigf;        // [nproj] (cos hi, cos lo, sin hi, sin lo): float-float split of trig
     // tables (device), built in fp64 on the host at create
     float2* tw;           // [M] e^{-2 pi i t / M}
     float* hfilt;         // [M] H[k] / M
