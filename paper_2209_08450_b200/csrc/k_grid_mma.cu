@@ -118,7 +118,7 @@ struct MmaSmem {
     static constexpr int B_STAGE = SC * NN * 2;
     static constexpr int offA = 0;                           // [NSUB][NST] A stages
     static constexpr int offB = offA + NSUB * NST * A_STAGE; // [NSUB][NST] B stages
-    static constexpr int offWs = offB + NSUB * NST * B_STAGE;    // [NSUB][3][16] uint4: wx 0..7 | wx 8..15 | wy, per column
+    static constexpr int offWs = offB + NSUB * NST * B_STAGE;    // [NSUB]: wx[16 columns][16] half (32 B rows), wy[16 columns][8] half
     static constexpr int offBar = offWs + NSUB * 3 * SC * 16;    // [NSUB][NST] mbarriers
     static constexpr int offMisc = offBar + NSUB * NST * 8;  // tmem base, started[NSUB]
     static constexpr int total = offMisc + 64;
@@ -165,9 +165,14 @@ __global__ void __launch_bounds__(NTHR, 2)
     unsigned char* Bw = smem + L::offB + warp * NST * L::B_STAGE;
     uint4* ws = reinterpret_cast<uint4*>(smem + L::offWs) + warp * 3 * SC;
     const uint64_t adesc0 = umma_desc(smem_u32(Aw), A_LBO, 128), bdesc0 = umma_desc(smem_u32(Bw), L::B_LBO, 128);
+    const uint64_t adesc1 = adesc0 + (uint64_t)(A_STAGE >> 4), bdesc1 = bdesc0 + (uint64_t)(L::B_STAGE >> 4);
+    static_assert(NST == 2, "two descriptors per operand");
     const uint32_t acc = tmem + (uint32_t)(sub * NN);
     const int cl = lane & 15, part = lane >> 4;              // column of the step; 0: x axis, 1: y axis
     uint32_t nstep = 0;                                      // K steps issued by this warp
+    const size_t pstride = (size_t)nproj * M;                // elements between slice-pair planes of the spectrum
+    const __half2* plane0 = spec + (size_t)(pg * NPG + part * HP) * pstride;      // first plane this lane gathers
+    const int nvalid = min(HP, npair - (pg * NPG + part * HP));                   // planes that exist (<= 0: none)
 
     for (int img = 0; img < 4; ++img) {
         const int2 win = plan[tile * 4 + img];
@@ -225,52 +230,45 @@ __global__ void __launch_bounds__(NTHR, 2)
                 const float hx = __shfl_sync(0xffffffffu, cs.x, h), lx_ = __shfl_sync(0xffffffffu, cs.y, h);
                 const float hy = __shfl_sync(0xffffffffu, cs.z, h), ly_ = __shfl_sync(0xffffffffu, cs.w, h);
                 const float c_hi = part ? hy : hx, c_lo = part ? ly_ : lx_;
-                // ---- phase 1: taps of this axis into a zeroed row; half of the B row
-                if (part == 0) {
-                    ws[cl] = make_uint4(0, 0, 0, 0);
-                    ws[SC + cl] = make_uint4(0, 0, 0, 0);
-                } else {
-                    ws[2 * SC + cl] = make_uint4(0, 0, 0, 0);
-                }
+                // ---- phase 1: taps of this axis into a zeroed row; half of the B row.
+                // x rows: 16 halves (32 B) per column at ws; y rows: 8 halves (16 B) per column behind them
+                unsigned char* wrow = reinterpret_cast<unsigned char*>(ws) + (part ? (SC * 32 + cl * 16) : cl * 32);
+                *reinterpret_cast<uint4*>(wrow) = make_uint4(0, 0, 0, 0);
+                if (part == 0) *reinterpret_cast<uint4*>(wrow + 16) = make_uint4(0, 0, 0, 0);
                 unsigned char* brow = Bs + (cl >> 3) * L::B_LBO + (cl & 7) * 16 + part * (GW / 2) * 128;
-                if (valid) {
-                    // taps l = floor(nu) - m + 1 + t, t = 0..2m-1, distance d_t = l - nu = d_0 + t; the open box
-                    // |l - nu| < m keeps t iff d_t < m (d_0 > -m always); d_0 = -m+1 exactly iff nu is an integer
-                    float fl, fr;
-                    nu_split((float)k, c_hi, c_lo, fl, fr);
-                    const float dint = -(float)(MH - 1);
-                    float d0 = dint - fr;
-                    if (fr > 0.f && d0 >= dint) d0 = __uint_as_float(__float_as_uint(dint) + 1u);   // next below -m+1
-                    const int l0 = (int)(fl + dint - org);
-                    __half* wh = reinterpret_cast<__half*>(ws);
+                // taps l = floor(nu) - m + 1 + t, t = 0..2m-1, distance d_t = l - nu = d_0 + t; the open box
+                // |l - nu| < m keeps t iff d_t < m (d_0 > -m always); d_0 = -m+1 exactly iff nu is an integer
+                float fl, fr;
+                nu_split((float)k, c_hi, c_lo, fl, fr);
+                const float dint = -(float)(MH - 1);
+                float d0 = dint - fr;
+                if (fr > 0.f && d0 >= dint) d0 = __uint_as_float(__float_as_uint(dint) + 1u);   // next below -m+1
+                const int l0 = valid ? (int)(fl + dint - org) : 64;                                // 64: every tap out of range
+                const unsigned lim = part ? (unsigned)SUBY : (unsigned)SUBX;
+                __half* wtap = reinterpret_cast<__half*>(wrow) + l0;
 #pragma unroll
-                    for (int t = 0; t < 2 * MH; ++t) {
-                        const float d = d0 + (float)t;
-                        const int l = l0 + t;
-                        const __half wv = __float2half_rn(ex2_approx(-alpha2 * d * d));
-                        if (part == 0) {
-                            if ((unsigned)l < (unsigned)SUBX && d < (float)MH) wh[((l >> 3) * SC + cl) * 8 + (l & 7)] = wv;
-                        } else {
-                            if ((unsigned)l < (unsigned)SUBY && d < (float)MH) wh[(2 * SC + cl) * 8 + l] = wv;
-                        }
-                    }
-                    const __half2* src = spec + ((size_t)(pg * NPG + part * HP) * nproj + jj) * M + (size_t)(k & (M - 1));
-                    const size_t pstride = (size_t)nproj * M;
+                for (int t = 0; t < 2 * MH; ++t) {
+                    const float d = d0 + (float)t;
+                    const __half wv = __float2half_rn(ex2_approx(-alpha2 * d * d));
+                    if ((unsigned)(l0 + t) < lim && d < (float)MH) wtap[t] = wv;
+                }
+                {
+                    const __half2* a = plane0 + ((size_t)jj * M + (size_t)(k & (M - 1)));
                     alignas(16) __half2 v[HP];
 #pragma unroll
-                    for (int p = 0; p < HP; ++p) v[p] = (pg * NPG + part * HP + p < npair) ? src[p * pstride] : czero<__half2>();
+                    for (int p = 0; p < HP; ++p) {
+                        v[p] = (valid && p < nvalid) ? __ldg(a) : czero<__half2>();
+                        a += pstride;
+                    }
                     const uint4* vv = reinterpret_cast<const uint4*>(v);
 #pragma unroll
                     for (int q = 0; q < GW / 2; ++q) *reinterpret_cast<uint4*>(brow + q * 128) = vv[q];
-                } else {
-#pragma unroll
-                    for (int q = 0; q < GW / 2; ++q) *reinterpret_cast<uint4*>(brow + q * 128) = make_uint4(0, 0, 0, 0);
                 }
                 __syncwarp();
                 // ---- phase 2: A[m = ly * 16 + lx][column] = wy[ly] * wx[lx]; MN-major: 8 cells of a column = 16 B.
                 // lane -> column cl, rows 4 * part .. 4 * part + 3
                 {
-                    const uint4 xa = ws[cl], xc = ws[SC + cl], yv = ws[2 * SC + cl];
+                    const uint4 xa = ws[2 * cl], xc = ws[2 * cl + 1], yv = ws[2 * SC + cl];
                     const unsigned y01 = part ? yv.z : yv.x, y23 = part ? yv.w : yv.y;
                     unsigned char* arow = As + (cl >> 3) * A_LBO + (cl & 7) * 16 + part * (8 * 128);
 #pragma unroll
@@ -295,7 +293,7 @@ __global__ void __launch_bounds__(NTHR, 2)
                 __syncwarp();
                 if (lane == 0) {
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    umma_f16(acc, adesc0 + (uint64_t)((st * A_STAGE) >> 4), bdesc0 + (uint64_t)((st * L::B_STAGE) >> 4), IDESC, nstep > 0 ? 1u : 0u);
+                    umma_f16(acc, st ? adesc1 : adesc0, st ? bdesc1 : bdesc0, IDESC, nstep > 0 ? 1u : 0u);
                     umma_commit(&bar[st]);
                 }
                 ++nstep;
