@@ -24,6 +24,13 @@ __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 
+// Two complex values that share every twiddle: two adjacent columns of the grid in the column pass
+// of the 2D transform (one 8-byte global access, one 16-byte shared-memory access per element).
+struct alignas(16) cpair { float2 a, b; };
+__device__ __forceinline__ cpair cmul(cpair x, float2 w) { return cpair{cmul(x.a, w), cmul(x.b, w)}; }
+__device__ __forceinline__ cpair cadd(cpair x, cpair y) { return cpair{cadd(x.a, y.a), cadd(x.b, y.b)}; }
+__device__ __forceinline__ cpair csub(cpair x, cpair y) { return cpair{csub(x.a, y.a), csub(x.b, y.b)}; }
+
 __host__ __device__ constexpr int pad_idx(int i) { return i + (i >> 4); }
 __host__ __device__ constexpr int padded_len(int N) { return N + (N >> 4); }
 
@@ -32,17 +39,21 @@ template <bool INV>
 __device__ __forceinline__ float2 mul_mi(float2 a) {
     return INV ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
 }
+template <bool INV>
+__device__ __forceinline__ cpair mul_mi(cpair x) { return cpair{mul_mi<INV>(x.a), mul_mi<INV>(x.b)}; }
 // multiply by e^{-/+ i phi} given (cos phi, sin phi)
 template <bool INV>
 __device__ __forceinline__ float2 mul_w(float2 a, float c, float s) {
     return INV ? make_float2(fmaf(-a.y, s, a.x * c), fmaf(a.x, s, a.y * c))
                : make_float2(fmaf(a.y, s, a.x * c), fmaf(-a.x, s, a.y * c));
 }
-
 template <bool INV>
-__device__ __forceinline__ void dft4(float2& a0, float2& a1, float2& a2, float2& a3) {
-    float2 s02 = cadd(a0, a2), d02 = csub(a0, a2), s13 = cadd(a1, a3), d13 = csub(a1, a3);
-    float2 jd = mul_mi<INV>(d13);
+__device__ __forceinline__ cpair mul_w(cpair x, float c, float s) { return cpair{mul_w<INV>(x.a, c, s), mul_w<INV>(x.b, c, s)}; }
+
+template <bool INV, class T>
+__device__ __forceinline__ void dft4(T& a0, T& a1, T& a2, T& a3) {
+    T s02 = cadd(a0, a2), d02 = csub(a0, a2), s13 = cadd(a1, a3), d13 = csub(a1, a3);
+    T jd = mul_mi<INV>(d13);
     a0 = cadd(s02, s13);
     a2 = csub(s02, s13);
     a1 = cadd(d02, jd);
@@ -54,26 +65,29 @@ struct Bfly;
 
 template <bool INV>
 struct Bfly<2, INV> {
-    static __device__ __forceinline__ void run(float2* v) {
-        float2 t = v[0];
+    template <class T>
+    static __device__ __forceinline__ void run(T* v) {
+        T t = v[0];
         v[0] = cadd(t, v[1]);
         v[1] = csub(t, v[1]);
     }
 };
 template <bool INV>
 struct Bfly<4, INV> {
-    static __device__ __forceinline__ void run(float2* v) { dft4<INV>(v[0], v[1], v[2], v[3]); }
+    template <class T>
+    static __device__ __forceinline__ void run(T* v) { dft4<INV>(v[0], v[1], v[2], v[3]); }
 };
 template <bool INV>
 struct Bfly<8, INV> {
-    static __device__ __forceinline__ void run(float2* v) {
+    template <class T>
+    static __device__ __forceinline__ void run(T* v) {
         const float c = 0.70710678118654752440f;
         dft4<INV>(v[0], v[2], v[4], v[6]);   // E0..E3 in v0,v2,v4,v6
         dft4<INV>(v[1], v[3], v[5], v[7]);   // O0..O3 in v1,v3,v5,v7
-        float2 o1 = mul_w<INV>(v[3], c, c);
-        float2 o2 = mul_mi<INV>(v[5]);
-        float2 o3 = mul_w<INV>(v[7], -c, c);
-        float2 e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1];
+        T o1 = mul_w<INV>(v[3], c, c);
+        T o2 = mul_mi<INV>(v[5]);
+        T o3 = mul_w<INV>(v[7], -c, c);
+        T e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1];
         v[0] = cadd(e0, o0); v[4] = csub(e0, o0);
         v[1] = cadd(e1, o1); v[5] = csub(e1, o1);
         v[2] = cadd(e2, o2); v[6] = csub(e2, o2);
@@ -82,7 +96,8 @@ struct Bfly<8, INV> {
 };
 template <bool INV>
 struct Bfly<16, INV> {
-    static __device__ __forceinline__ void run(float2* v) {
+    template <class T>
+    static __device__ __forceinline__ void run(T* v) {
         const float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f;  // cos, sin(pi/8)
         const float c2 = 0.70710678118654752440f;
         // step 1: for i0: A_i0[k1] = DFT4 over i1 of v[i0 + 4 i1]  (in place: v[i0 + 4 k1])
@@ -106,7 +121,7 @@ struct Bfly<16, INV> {
         for (int a = 0; a < 4; ++a)
 #pragma unroll
             for (int b = a + 1; b < 4; ++b) {
-                float2 t = v[4 * a + b];
+                T t = v[4 * a + b];
                 v[4 * a + b] = v[4 * b + a];
                 v[4 * b + a] = t;
             }
@@ -130,11 +145,11 @@ __device__ __forceinline__ void twiddle_powers(float2 w1, float2* w) {
 //   tw: table e^{-2 pi i t / N}, t in [0, N) (conjugated here for INV)
 //   FIRST: inputs come from ld(index); else from s[pad_idx(index)]
 //   LAST:  outputs go to st(index, value); else to s[pad_idx(index)]
-template <int N, int R, int NS, bool INV, bool FIRST, bool LAST, class Load, class Store>
-__device__ __forceinline__ void fft_pass(float2* s, int tid, const float2* __restrict__ tw, Load ld, Store st) {
+template <int N, int R, int NS, bool INV, bool FIRST, bool LAST, class T, class Load, class Store>
+__device__ __forceinline__ void fft_pass(T* s, int tid, const float2* __restrict__ tw, Load ld, Store st) {
     constexpr int TG = N / 16;
     constexpr int NB = 16 / R;          // butterflies per thread
-    float2 v[16];
+    T v[16];
 #pragma unroll
     for (int q = 0; q < NB; ++q) {
         const int b = tid + q * TG;
@@ -175,10 +190,10 @@ __device__ __forceinline__ void fft_pass(float2* s, int tid, const float2* __res
 // calling group's own padded line of padded_len(N) float2.
 // NOTE: when the loader reads shared memory that the storer of a previous transform
 // wrote, the caller must __syncthreads() between the two calls.
-template <int N, bool INV, class Load, class Store>
-__device__ __forceinline__ void fft_line(float2* s, int tid, const float2* __restrict__ tw, Load ld, Store st) {
-    auto nold = [](int) { return make_float2(0.f, 0.f); };
-    auto nost = [](int, float2) {};
+template <int N, bool INV, class T, class Load, class Store>
+__device__ __forceinline__ void fft_line(T* s, int tid, const float2* __restrict__ tw, Load ld, Store st) {
+    auto nold = [](int) { return T(); };
+    auto nost = [](int, T) {};
     if constexpr (N == 128) {
         fft_pass<N, 16, 1, INV, true, false>(s, tid, tw, ld, nost);
         fft_pass<N, 8, 16, INV, false, true>(s, tid, tw, nold, st);

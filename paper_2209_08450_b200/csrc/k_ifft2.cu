@@ -14,30 +14,56 @@
 
 namespace tcpk {
 
-__host__ __device__ constexpr int cols_w(int M) { return (16384 / M) < 32 ? (16384 / M) : 32; }
-__host__ __device__ constexpr int cols_stride(int M) {   // float2 units; stride = 16/W (mod 16)
-    return padded_len(M) + (cols_w(M) >= 16 ? 1 : 16 / cols_w(M));
+__host__ __device__ constexpr int cols_w(int M) { return (16384 / M) < 32 ? (16384 / M) : 32; }   // columns per CTA
+__host__ __device__ constexpr int cols_wp(int M) { return cols_w(M) / 2; }                          // column pairs per CTA
+// stride between the pair-lines of a CTA, in cpair (16 B) units: a quarter-warp (8 lanes = one
+// 128-byte shared-memory wavefront of 16-byte accesses) holds min(WP, 8) lines x 8 / min(WP, 8)
+// consecutive elements, so lines must be 8 / min(WP, 8) elements apart modulo 8
+__host__ __device__ constexpr int cols_stride(int M) {
+    const int wp = cols_wp(M) < 8 ? cols_wp(M) : 8;
+    const int want = (8 / wp) % 8;
+    return padded_len(M) + (want - padded_len(M) % 8 + 8) % 8;
 }
 
+__device__ __forceinline__ cpair ld_c2(const float2* p, size_t i) {
+    const float4 v = *reinterpret_cast<const float4*>(p + i);
+    return cpair{make_float2(v.x, v.y), make_float2(v.z, v.w)};
+}
+__device__ __forceinline__ cpair ld_c2(const __half2* p, size_t i) {
+    const uint2 v = *reinterpret_cast<const uint2*>(p + i);
+    return cpair{__half22float2(*reinterpret_cast<const __half2*>(&v.x)), __half22float2(*reinterpret_cast<const __half2*>(&v.y))};
+}
+__device__ __forceinline__ void st_c2(float2* p, size_t i, cpair v) {
+    *reinterpret_cast<float4*>(p + i) = make_float4(v.a.x, v.a.y, v.b.x, v.b.y);
+}
+__device__ __forceinline__ void st_c2(__half2* p, size_t i, cpair v) {
+    const __half2 a = __float22half2_rn(v.a), b = __float22half2_rn(v.b);
+    *reinterpret_cast<uint2*>(p + i) = make_uint2(*reinterpret_cast<const unsigned*>(&a), *reinterpret_cast<const unsigned*>(&b));
+}
+
+// A thread owns one butterfly position of TWO adjacent columns (one 8- or 16-byte global access per
+// row, one 16-byte shared-memory access per element): half the memory instructions of a
+// column-per-thread layout and two independent dependency chains per thread.
 template <int M, class TC>
-__global__ void __launch_bounds__(cols_w(M) * M / 16) ifft_cols_kernel(const TC* __restrict__ grid,
-                                                                       TC* __restrict__ pass1,
-                                                                       const float2* __restrict__ tw) {
-    constexpr int n = M / 2, W = cols_w(M), LS = cols_stride(M);
-    extern __shared__ float2 smem[];
-    const int w = threadIdx.x % W;            // column inside the CTA's strip (fastest: coalescing)
-    const int tid = threadIdx.x / W;          // thread inside the column's FFT group
-    float2* s = smem + (size_t)w * LS;
+__global__ void __launch_bounds__(cols_wp(M) * M / 16) ifft_cols_kernel(const TC* __restrict__ grid,
+                                                                        TC* __restrict__ pass1,
+                                                                        const float2* __restrict__ tw) {
+    constexpr int n = M / 2, W = cols_w(M), WP = cols_wp(M), LS = cols_stride(M);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cpair* smem = reinterpret_cast<cpair*>(smem_raw);
+    const int wp = threadIdx.x % WP;          // column pair inside the CTA's strip (fastest: coalescing)
+    const int tid = threadIdx.x / WP;         // thread inside the pair's FFT group
+    cpair* s = smem + (size_t)wp * LS;
     const int pair = blockIdx.y;
-    const int l1 = blockIdx.x * W + w;
+    const int l1 = blockIdx.x * W + 2 * wp;
     const TC* src = grid + (size_t)pair * M * M + l1;
     TC* dst = pass1 + (size_t)pair * n * M + l1;
     fft_line<M, true>(
-        s, tid, tw, [&](int l2) { return ld_c(src, (size_t)l2 * M); },
-        [&](int x2, float2 v) {
+        s, tid, tw, [&](int l2) { return ld_c2(src, (size_t)l2 * M); },
+        [&](int x2, cpair v) {
             // signed x2 in [-n/2, n/2)  <->  FFT index x2 mod M
-            if (x2 < n / 2) st_c(dst, (size_t)(x2 + n / 2) * M, v);
-            else if (x2 >= M - n / 2) st_c(dst, (size_t)(x2 - (M - n / 2)) * M, v);
+            if (x2 < n / 2) st_c2(dst, (size_t)(x2 + n / 2) * M, v);
+            else if (x2 >= M - n / 2) st_c2(dst, (size_t)(x2 - (M - n / 2)) * M, v);
         });
 }
 
@@ -74,12 +100,12 @@ __global__ void __launch_bounds__(ROWS* M / 16) ifft_rows_kernel(const TC* __res
 
 template <int M, class TC>
 static int launch_cols_t(const tcp_ctx* c, cudaStream_t st) {
-    constexpr int W = cols_w(M);
-    const size_t smem = (size_t)W * cols_stride(M) * sizeof(float2);
+    constexpr int W = cols_w(M), WP = cols_wp(M);
+    const size_t smem = (size_t)WP * cols_stride(M) * sizeof(cpair);
     auto kern = ifft_cols_kernel<M, TC>;
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid(M / W, c->npair);
-    kern<<<grid, W * M / 16, smem, st>>>((const TC*)c->grid, (TC*)c->pass1, c->tw);
+    kern<<<grid, WP * M / 16, smem, st>>>((const TC*)c->grid, (TC*)c->pass1, c->tw);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }

@@ -7,6 +7,8 @@
 // reused by all nproj projections) and one (half) or two (float) 128-bit stores.  The
 // projection-major -> slice-major transpose only permutes whole rows, so both sides stay
 // fully coalesced.
+#include <algorithm>
+
 #include "tcp_internal.h"
 
 namespace tcpk {
@@ -49,35 +51,81 @@ __global__ void __launch_bounds__(256) normalize_kernel(const uint4* __restrict_
         p[6] = neglog1((float)(r.w & 0xffffu), f1.z, d1.z);
         p[7] = neglog1((float)(r.w >> 16), f1.w, d1.w);
         const size_t o = (((size_t)z * nproj + j) * n8 + i8) * 8;   // element offset in sino
-        if constexpr (sizeof(TS) == 4) {
-            float4* dst = reinterpret_cast<float4*>(sino + o);
-            dst[0] = make_float4(p[0], p[1], p[2], p[3]);
-            dst[1] = make_float4(p[4], p[5], p[6], p[7]);
-        } else {
-            __half2 h0 = __floats2half2_rn(p[0], p[1]), h1 = __floats2half2_rn(p[2], p[3]);
-            __half2 h2 = __floats2half2_rn(p[4], p[5]), h3 = __floats2half2_rn(p[6], p[7]);
-            uint4 w;
-            w.x = *reinterpret_cast<unsigned*>(&h0);
-            w.y = *reinterpret_cast<unsigned*>(&h1);
-            w.z = *reinterpret_cast<unsigned*>(&h2);
-            w.w = *reinterpret_cast<unsigned*>(&h3);
-            *reinterpret_cast<uint4*>(sino + o) = w;
+        float4* dst = reinterpret_cast<float4*>(sino + o);
+        dst[0] = make_float4(p[0], p[1], p[2], p[3]);
+        dst[1] = make_float4(p[4], p[5], p[6], p[7]);
+    }
+}
+
+// fp16 storage: the result is rounded to half (2^-11 relative), so the hardware approximations
+// (rcp.approx, lg2.approx: ~2^-22) are exact for the purpose and the kernel stays HBM-bound instead of
+// ALU-bound.  A thread keeps 1 / (flat - dark) and dark of its 8 pixels in registers and walks JP
+// projections of the same detector row, so the flat/dark loads and the reciprocals are amortised.
+__device__ __forceinline__ float fast_rcp(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float fast_lg2(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+// uint16 -> float without the conversion pipe: 0x4B000000 | u is 2^23 + u exactly
+__device__ __forceinline__ float u16f(unsigned u) { return __uint_as_float(0x4B000000u | u) - 8388608.f; }
+
+constexpr int JP = 4;
+__global__ void __launch_bounds__(256) normalize_half_kernel(const uint4* __restrict__ raw, const float4* __restrict__ flat,
+                                                             const float4* __restrict__ dark, __half* __restrict__ sino,
+                                                             int nproj, int nz, int n8) {
+    const float eps_d = 1e-3f, t_min = 1e-6f, mln2 = -0.69314718055994531f;
+    const int jgroups = (nproj + JP - 1) / JP;
+    const size_t total = (size_t)jgroups * nz * n8;             // index space [jgroup][nz][n8]
+    for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < total; v += (size_t)gridDim.x * blockDim.x) {
+        const int i8 = (int)(v % n8);
+        const size_t row = v / n8;
+        const int z = (int)(row % nz);
+        const int j0 = (int)(row / nz) * JP;
+        const size_t fo = ((size_t)z * n8 + i8) * 2;
+        const float4 f0 = __ldg(&flat[fo]), f1 = __ldg(&flat[fo + 1]);
+        const float4 d0 = __ldg(&dark[fo]), d1 = __ldg(&dark[fo + 1]);
+        const float dk[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+        const float fl[8] = {f0.x, f0.y, f0.z, f0.w, f1.x, f1.y, f1.z, f1.w};
+        float inv[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) inv[e] = fast_rcp(fmaxf(fl[e] - dk[e], eps_d));
+        uint4 r[JP];
+#pragma unroll
+        for (int q = 0; q < JP; ++q)
+            if (j0 + q < nproj) r[q] = __ldcs(&raw[((size_t)(j0 + q) * nz + z) * n8 + i8]);
+#pragma unroll
+        for (int q = 0; q < JP; ++q) {
+            if (j0 + q >= nproj) break;
+            const unsigned w[4] = {r[q].x, r[q].y, r[q].z, r[q].w};
+            float p[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                const unsigned u = (e & 1) ? (w[e >> 1] >> 16) : (w[e >> 1] & 0xffffu);
+                p[e] = mln2 * fast_lg2(fmaxf((u16f(u) - dk[e]) * inv[e], t_min));
+            }
+            const __half2 h0 = __floats2half2_rn(p[0], p[1]), h1 = __floats2half2_rn(p[2], p[3]);
+            const __half2 h2 = __floats2half2_rn(p[4], p[5]), h3 = __floats2half2_rn(p[6], p[7]);
+            uint4 o4;
+            o4.x = *reinterpret_cast<const unsigned*>(&h0);
+            o4.y = *reinterpret_cast<const unsigned*>(&h1);
+            o4.z = *reinterpret_cast<const unsigned*>(&h2);
+            o4.w = *reinterpret_cast<const unsigned*>(&h3);
+            *reinterpret_cast<uint4*>(sino + (((size_t)z * nproj + (j0 + q)) * n8 + i8) * 8) = o4;
         }
     }
 }
 
 int launch_normalize(const tcp_ctx* c, const uint16_t* raw, const float* flat, const float* dark, cudaStream_t st) {
     const int n8 = c->n / 8;
-    const size_t total = (size_t)c->nproj * c->nz * n8;
-    int blocks = (int)((total + 255) / 256);
     const int cap = 148 * 8 * 4;                  // a few waves of 8 resident CTAs per SM
-    if (blocks > cap) blocks = cap;
-    if (c->half_store)
-        normalize_kernel<__half><<<blocks, 256, 0, st>>>((const uint4*)raw, (const float4*)flat, (const float4*)dark,
-                                                         (__half*)c->sino, c->nproj, c->nz, n8);
-    else
+    if (c->half_store) {
+        const size_t total = (size_t)((c->nproj + JP - 1) / JP) * c->nz * n8;
+        int blocks = (int)std::min<size_t>((total + 255) / 256, (size_t)cap);
+        normalize_half_kernel<<<blocks, 256, 0, st>>>((const uint4*)raw, (const float4*)flat, (const float4*)dark,
+                                                      (__half*)c->sino, c->nproj, c->nz, n8);
+    } else {
+        const size_t total = (size_t)c->nproj * c->nz * n8;
+        int blocks = (int)std::min<size_t>((total + 255) / 256, (size_t)cap);
         normalize_kernel<float><<<blocks, 256, 0, st>>>((const uint4*)raw, (const float4*)flat, (const float4*)dark,
                                                         (float*)c->sino, c->nproj, c->nz, n8);
+    }
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }
