@@ -159,6 +159,24 @@ def cpu_baseline(w, made, m, cores_hint=None):
             "slices_per_s": ns / dt}, ref, (z0, ns)
 
 
+def max_over_ranks(value, world, device=None):
+    """Whole-job time = the slowest rank's (device-timed) value; no data-path collective exists (replicas)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_slices(nz_total, nz_chunk, world):
+    """Replicas only: every rank reconstructs one full volume of nz_total slices
+    (rounded down to whole chunks); the job's voxel count is world times that."""
+    nz = nz_total - nz_total % nz_chunk
+    return nz, world * nz
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -218,10 +236,7 @@ def run_ours(args, rank, world, local_rank):
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.stop()
     r.set_profile(False)
-    if world > 1:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, world, dev)
     ms_step = ms_total / args.steps
     voxels = float(nz_total) * n * n
     value = world * voxels / (ms_step * 1e-3) / 1e9
@@ -250,10 +265,7 @@ def run_ours(args, rank, world, local_rank):
             dev_ms += ms
         barrier()
         wall = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([wall], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            wall = float(t.item())
+        wall = max_over_ranks(wall, world, dev)
         e2e = {"value": world * args.steps * float(nz_e) * n * n / wall / 1e9, "unit": "GVoxel/s",
                "h2d_bytes_per_step": int(raw_h.numel() * 2 + flat_h.numel() * 8 + w.nproj * 4),
                "d2h_bytes_per_step": int(out_h.numel() * out_h.element_size()),
@@ -274,10 +286,12 @@ def run_ours(args, rank, world, local_rank):
                       "GBps": model[k]["bytes"] / t / 1e9 if t > 0 else None,
                       "TFLOPps": model[k]["flops"] / t / 1e12 if t > 0 else None}
     dom = max(model, key=lambda k: stage_ms[k])
-    traffic = None
+    traffic = None           # DRAM bytes per launch of the dominant kernel from the committed ncu capture
     try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
-            traffic = json.load(f).get(dom)
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
+            for ln in f.read().splitlines()[1:]:
+                if ln.split(",")[0] == dom:
+                    traffic = int(ln.split(",")[1])
     except Exception:
         pass
     if dom == "grid":
