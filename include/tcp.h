@@ -99,6 +99,9 @@ int tcp_workspace(tcp_ctx* ctx, int which, void** ptr, size_t* bytes);
 /* Copy an intermediate into the caller's device buffer dst (>= the size tcp_workspace reports),
  * asynchronously on `stream` (tests only). */
 int tcp_read_workspace(tcp_ctx* ctx, int which, void* dst, size_t dst_bytes, tcp_stream_t stream);
+/* Layout of TCP_WS_GRID: 0 = [npair][M l2][M l1]; W > 0 = strip-major [npair][M/W][M l2][W l1] (the
+ * tensor-core gridding writes strips of W columns so that the column pass of S6 reads contiguously). */
+int tcp_grid_strip(const tcp_ctx* ctx);
 /* Power-of-two factor by which SPECTRUM/GRID/PASS1 are scaled relative to S4's G (1 in fp32). */
 double tcp_scale(const tcp_ctx* ctx);
 /* Total device bytes the context allocated; kernels launched by one tcp_recon. */

@@ -18,7 +18,7 @@ GRID_IMPLS = {"gather": 0, "scatter": 1, "tile": 2, "mma": 3}
 # every symbol include/tcp.h declares (tests check the library exports them all)
 EXPORTS = [
     "tcp_create", "tcp_create_ex", "tcp_recon", "tcp_destroy", "tcp_last_error",
-    "tcp_mean_frames_u16", "tcp_normalize", "tcp_workspace", "tcp_read_workspace", "tcp_scale",
+    "tcp_mean_frames_u16", "tcp_normalize", "tcp_workspace", "tcp_read_workspace", "tcp_scale", "tcp_grid_strip",
     "tcp_workspace_bytes", "tcp_launches_per_recon", "tcp_set_option", "tcp_profile_collect",
     "tcp_recon_volume_host",
 ]
@@ -64,6 +64,8 @@ def lib():
     L.tcp_read_workspace.argtypes = [vp, ci, vp, C.c_size_t, vp]
     L.tcp_scale.restype = C.c_double
     L.tcp_scale.argtypes = [vp]
+    L.tcp_grid_strip.restype = C.c_int
+    L.tcp_grid_strip.argtypes = [vp]
     L.tcp_workspace_bytes.restype = C.c_size_t
     L.tcp_workspace_bytes.argtypes = [vp]
     L.tcp_launches_per_recon.restype = ci
@@ -195,6 +197,10 @@ class Recon:
         return int(lib().tcp_launches_per_recon(self.h))
 
     @property
+    def grid_strip(self) -> int:
+        return int(lib().tcp_grid_strip(self.h))
+
+    @property
     def workspace_bytes(self) -> int:
         return int(lib().tcp_workspace_bytes(self.h))
 
@@ -230,6 +236,10 @@ class Recon:
             return buf.view(self.store_dtype).view(self.nz, self.nproj, self.n)
         shape = {"spectrum": (npair, self.nproj, M), "grid": (npair, M, M), "pass1": (npair, self.n, M)}[name]
         v = buf.view(self.store_dtype).view(*shape, 2).float()
+        if name == "grid":
+            w = int(lib().tcp_grid_strip(self.h))
+            if w:       # strip-major [npair][M/w][M l2][w l1] -> [npair][M l2][M l1]
+                v = v.view(npair, M // w, M, w, 2).permute(0, 2, 1, 3, 4).reshape(npair, M, M, 2)
         return torch.complex(v[..., 0], v[..., 1])
 
     def recon_volume_host(self, raw_host, flat_host, dark_host, theta_host, out_host=None, nbuf=3):

@@ -317,7 +317,7 @@ __global__ void __launch_bounds__(NTHR, 2)
 // red: x = tile, y = first slot, z = S.  One CTA per (split tile, pair); a thread sums 4 cells.
 template <class TC>
 __global__ void __launch_bounds__(NTHR) grid_reduce_kernel(const float2* __restrict__ partial, TC* __restrict__ grid,
-                                                           const int4* __restrict__ red, int M, int npair) {
+                                                           const int4* __restrict__ red, int M, int npair, int strip) {
     const int4 r = red[blockIdx.x];
     const int pair = blockIdx.y, tiles = M / TS;
     const int row = threadIdx.x >> 3, col = (threadIdx.x & 7) * 4;
@@ -330,9 +330,13 @@ __global__ void __launch_bounds__(NTHR) grid_reduce_kernel(const float2* __restr
         a[0].x += u.x; a[0].y += u.y; a[1].x += u.z; a[1].y += u.w;
         a[2].x += v.x; a[2].y += v.y; a[3].x += v.z; a[3].y += v.w;
     }
-    TC* g = grid + ((size_t)pair * M + (r.x / tiles) * TS + row) * M + (r.x % tiles) * TS + col;
+    const int gr = (r.x / tiles) * TS + row, gc = (r.x % tiles) * TS + col;     // col is a multiple of 4
+    TC* g = grid + (size_t)pair * M * M;
 #pragma unroll
-    for (int e = 0; e < 4; ++e) st_c(g, (size_t)e, a[e]);
+    for (int e = 0; e < 4; ++e) {
+        const int c1 = gc + e;
+        st_c(g, strip ? ((size_t)(c1 / strip) * M + gr) * strip + (c1 % strip) : (size_t)gr * M + c1, a[e]);
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -430,9 +434,9 @@ int launch_grid_tile(const tcp_ctx* c, const float* theta, cudaStream_t st) {
     if (rc) return rc;
     if (c->g_nred) {
         if (c->half_store)
-            grid_reduce_kernel<__half2><<<dim3(c->g_nred, c->npair), NTHR, 0, st>>>(c->g_partial, (__half2*)c->grid, c->g_red, c->M, c->npair);
+            grid_reduce_kernel<__half2><<<dim3(c->g_nred, c->npair), NTHR, 0, st>>>(c->g_partial, (__half2*)c->grid, c->g_red, c->M, c->npair, c->grid_strip);
         else
-            grid_reduce_kernel<float2><<<dim3(c->g_nred, c->npair), NTHR, 0, st>>>(c->g_partial, (float2*)c->grid, c->g_red, c->M, c->npair);
+            grid_reduce_kernel<float2><<<dim3(c->g_nred, c->npair), NTHR, 0, st>>>(c->g_partial, (float2*)c->grid, c->g_red, c->M, c->npair, c->grid_strip);
         TCP_CUDA_CHECK(cudaGetLastError());
     }
     return TCP_OK;

@@ -47,7 +47,7 @@ __device__ __forceinline__ void st_c2(__half2* p, size_t i, cpair v) {
 template <int M, class TC>
 __global__ void __launch_bounds__(cols_wp(M) * M / 16) ifft_cols_kernel(const TC* __restrict__ grid,
                                                                         TC* __restrict__ pass1,
-                                                                        const float2* __restrict__ tw) {
+                                                                        const float2* __restrict__ tw, int strip) {
     constexpr int n = M / 2, W = cols_w(M), WP = cols_wp(M), LS = cols_stride(M);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cpair* smem = reinterpret_cast<cpair*>(smem_raw);
@@ -56,10 +56,12 @@ __global__ void __launch_bounds__(cols_wp(M) * M / 16) ifft_cols_kernel(const TC
     cpair* s = smem + (size_t)wp * LS;
     const int pair = blockIdx.y;
     const int l1 = blockIdx.x * W + 2 * wp;
-    const TC* src = grid + (size_t)pair * M * M + l1;
+    // strip-major grid: the CTA's W columns are one contiguous block of M rows x W
+    const TC* src = grid + (size_t)pair * M * M + (strip ? (size_t)blockIdx.x * M * W + 2 * wp : (size_t)l1);
+    const size_t rstride = strip ? (size_t)W : (size_t)M;
     TC* dst = pass1 + (size_t)pair * n * M + l1;
     fft_line<M, true>(
-        s, tid, tw, [&](int l2) { return ld_c2(src, (size_t)l2 * M); },
+        s, tid, tw, [&](int l2) { return ld_c2(src, (size_t)l2 * rstride); },
         [&](int x2, cpair v) {
             // signed x2 in [-n/2, n/2)  <->  FFT index x2 mod M
             if (x2 < n / 2) st_c2(dst, (size_t)(x2 + n / 2) * M, v);
@@ -105,7 +107,7 @@ static int launch_cols_t(const tcp_ctx* c, cudaStream_t st) {
     auto kern = ifft_cols_kernel<M, TC>;
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid(M / W, c->npair);
-    kern<<<grid, WP * M / 16, smem, st>>>((const TC*)c->grid, (TC*)c->pass1, c->tw);
+    kern<<<grid, WP * M / 16, smem, st>>>((const TC*)c->grid, (TC*)c->pass1, c->tw, c->grid_strip);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }
@@ -132,6 +134,8 @@ static int rows_m(const tcp_ctx* c, void* out, cudaStream_t st) {
     if (!c->half_store) return launch_rows_t<M, float2, float>(c, out, st);
     return c->half_out ? launch_rows_t<M, __half2, __half>(c, out, st) : launch_rows_t<M, __half2, float>(c, out, st);
 }
+
+int cols_strip_width(int M) { return cols_w(M); }
 
 int launch_ifft_cols(const tcp_ctx* c, cudaStream_t st) {
     switch (c->M) {

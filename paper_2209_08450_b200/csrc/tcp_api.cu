@@ -176,6 +176,7 @@ tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, 
     // noise-level spectrum samples above the half subnormal range
     c->scale = c->half_store ? 8192.0 : 1.0;
     c->grid_impl = c->half_store ? TCP_GRID_MMA : TCP_GRID_TILE;
+    c->grid_strip = (c->grid_impl == TCP_GRID_MMA) ? cols_strip_width(c->M) : 0;
     cudaGetDevice(&c->device);
     if (build_context(c) != TCP_OK || setup_kernel_attributes(c) != TCP_OK) {
         char keep[512];
@@ -294,6 +295,7 @@ int tcp_read_workspace(tcp_ctx* c, int which, void* dst, size_t dst_bytes, tcp_s
 }
 
 double tcp_scale(const tcp_ctx* c) { return c ? c->scale : 0.0; }
+int tcp_grid_strip(const tcp_ctx* c) { return c ? c->grid_strip : 0; }
 size_t tcp_workspace_bytes(const tcp_ctx* c) { return c ? c->bytes : 0; }
 
 int tcp_set_option(tcp_ctx* c, int option, int value) {
@@ -303,6 +305,7 @@ int tcp_set_option(tcp_ctx* c, int option, int value) {
         if (value == TCP_GRID_SCATTER_ATOMIC && c->half_store) return set_error(TCP_EUNSUPPORTED, "scatter gridding supports TCP_F32 only");
         if (value == TCP_GRID_MMA && !c->half_store) return set_error(TCP_EUNSUPPORTED, "tensor-core gridding needs fp16 storage");
         c->grid_impl = value;
+        c->grid_strip = (value == TCP_GRID_MMA) ? cols_strip_width(c->M) : 0;
         return TCP_OK;
     }
     if (option == TCP_OPT_PROFILE) {

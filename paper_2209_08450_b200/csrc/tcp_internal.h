@@ -14,6 +14,7 @@ struct tcp_ctx {
     bool half_out;        // out in half (TCP_F16)
     double scale;         // power-of-two scale S of SPECTRUM / GRID / PASS1 (1 in fp32)
     int grid_impl;
+    int grid_strip;       // 0: grid rows are contiguous; W > 0: strip-major [pair][M/W][M l2][W l1] (tcgen05 gridding)
     int device;
     // workspaces (device)
     void* sino;           // [nz][nproj][n]      float | half
@@ -68,6 +69,7 @@ int launch_grid_mma_main(const tcp_ctx* c, cudaStream_t st);
 int grid_tile_setup(tcp_ctx* c);
 void grid_tile_free(tcp_ctx* c);
 int launch_ifft_cols(const tcp_ctx* c, cudaStream_t st);
+int cols_strip_width(int M);
 int launch_ifft_rows(const tcp_ctx* c, void* out, cudaStream_t st);
 int launch_mean_frames(const uint16_t* frames, int nframes, int nz, int n, float* mean, cudaStream_t st);
 int setup_kernel_attributes(const tcp_ctx* c);

@@ -131,6 +131,25 @@ def test_limited_and_uneven_angles():
         assert rl2(out[z], ref[z]) < FP32_GATE
 
 
+def test_c1_fp16_grid_stage_strip_layout():
+    """fp16 storage: the tcgen05 gridding writes the grid strip-major (tcp_grid_strip); read back in
+    row-major order it must equal the oracle's gridding of the oracle's spectrum to fp16 accuracy."""
+    w = sg.make_workload("C1")
+    rows = list(range(w.nz_total))
+    out, r, (raw, flat, dark, theta) = _gpu_recon(w, rows, "f16", keep=True)
+    assert r.grid_strip > 0
+    p = orc.neglog(raw, flat, dark)
+    for pair in (0, 2):
+        GA = orc.spectrum(orc.filter_rows(p[2 * pair], w.filter), w.center)
+        GB = orc.spectrum(orc.filter_rows(p[2 * pair + 1], w.filter), w.center)
+        Fo = orc.grid(GA + 1j * GB, theta, w.n, 3)
+        got = r.workspace("grid").cpu().numpy()[pair] / r.scale
+        assert rl2(got, Fo) < 2e-3
+    r.set_grid_impl("tile")
+    assert r.grid_strip == 0
+    r.close()
+
+
 @pytest.mark.parametrize("dtype", ["f16", "f16_out32"])
 def test_c1_fp16(dtype):
     w = sg.make_workload("C1")
