@@ -235,3 +235,35 @@ def test_pipeline_host_matches_direct():
     for z in range(2):
         assert rl2(out_h[20 + z], ref[z]) < FP32_GATE
     r.close()
+
+
+# ------------------------------------------------------------------ BASELINE full sizes, bench launch configuration
+@pytest.mark.parametrize("cfg,nz", [("C4", 32), ("C5", 4)])
+def test_full_size_chunk_sampled_against_oracle(cfg, nz):
+    """C4 (2048^2, 2048 projections, fp16, one 32-slice chunk exactly as bench.py launches it: tcgen05
+    gridding with 16 pairs per accumulator group) and C5 (4096^2, 4000 projections, M = 8192, off-centre,
+    fp16 -> fp32 output).  Inputs are manufactured on the GPU (synthgen.make_counts_torch, frame averaging
+    through tcp_mean_frames_u16) and the SAME arrays go to the oracle, which reconstructs a sample of the
+    chunk's slices one by one."""
+    tcp = _tcp()
+    w = sg.make_workload(cfg)
+    z0 = w.nz_total // 2 - nz // 2
+    rows = list(range(z0, z0 + nz))
+    raw_d, ff, df = sg.make_counts_torch(w, rows, device="cuda")
+    flat_d = torch.empty((nz, w.n), dtype=torch.float32, device="cuda")
+    dark_d = torch.empty_like(flat_d)
+    tcp.tcp_mean_frames_u16(ff.contiguous(), flat_d)
+    tcp.tcp_mean_frames_u16(df.contiguous(), dark_d)
+    theta = w.theta
+    r = tcp.Recon(w.n, w.nproj, nz, w.center, w.dtype, w.filter, 3)
+    out = r.recon(raw_d.contiguous(), flat_d, dark_d, torch.from_numpy(theta).cuda())
+    torch.cuda.synchronize()
+    out = out.float().cpu().numpy()
+    r.close()
+    sample = sorted({0, 1, nz // 2, nz - 1})
+    raw_h = raw_d.view(torch.int16)[:, sample].contiguous().cpu().numpy().view(np.uint16)
+    ref = orc.recon(raw_h, flat_d[sample].cpu().numpy(), dark_d[sample].cpu().numpy(), theta, w.center, w.filter, 3, "grid")
+    scale = np.abs(ref).max()
+    for i, z in enumerate(sample):
+        assert rl2(out[z], ref[i]) < FP16_GATE_L2, (cfg, z, rl2(out[z], ref[i]))
+        assert np.abs(out[z] - ref[i]).max() / scale < FP16_GATE_MAX
