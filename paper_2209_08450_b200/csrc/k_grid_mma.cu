@@ -17,12 +17,12 @@
 // Every WARP owns one sub-tile and runs on its own, with no block barrier inside the loop:
 //   * 32 lanes test 32 projections of the region's window against the sub-tile's sample box; a chord
 //     crosses the box in one run of consecutive k; a warp scan lays the runs end to end as columns;
-//   * 16 columns at a time (one MMA K step): lanes 0-15 take the x axis of a column, lanes 16-31 the
-//     y axis: floor/fraction of k cos, k sin by float-float FMAs, the 2m Gaussian taps scattered into
-//     a zeroed 16- or 8-entry row (phase 1), and half of the column's B row (its NN spectrum values)
-//     gathered from global memory; then the outer products wy x wx are written as the MN-major A
-//     stage (phase 2) and lane 0 issues the MMA and commits it to the stage's mbarrier; two stages
-//     per warp, so the weights of the next 16 samples are generated while the MMA runs.
+//   * 32 columns at a time (two MMA K steps), one lane per column: floor/fraction of k cos, k sin by
+//     float-float FMAs, the 2m Gaussian taps of each axis scattered into a zeroed 16- / 8-entry row
+//     (phase 1) and the column's B row (its NN spectrum values) gathered from global memory; then,
+//     once the warp's previous MMAs have released the stage, the outer products wy x wx are written
+//     as the MN-major A stage (phase 2) and lane 0 issues the two MMAs and commits them to the warp's
+//     mbarrier: the MMAs of one step run under phase 1 of the next.
 // Fixed summation order per accumulator, no atomics => bitwise reproducible.
 #include <math.h>
 #include <stdio.h>
@@ -34,8 +34,8 @@
 namespace tcpk {
 
 constexpr int SUBX = 16, SUBY = 8, NSUB = 8;      // sub-tile = 128 cells; 2 x 4 sub-tiles per region
-constexpr int SC = 16;                            // columns (samples) per A/B stage = one MMA K step
-constexpr int NST = 2;                            // stages per warp
+constexpr int SC = 32;                            // columns (samples) per A/B stage = one lane each = two MMA K steps
+constexpr int NST = 1;                            // stages per warp
 constexpr int RUNMAX = 32;                        // >= samples of one chord inside a sub-tile's sample box
 constexpr int A_LBO = (128 / 8) * 128;            // bytes between k-blocks of 8 columns in an A stage
 constexpr int A_STAGE = SC * 256;                 // bytes of one A stage: [SC/8][16][8 columns][8 cells] half
@@ -118,7 +118,7 @@ struct MmaSmem {
     static constexpr int B_STAGE = SC * NN * 2;
     static constexpr int offA = 0;                           // [NSUB][NST] A stages
     static constexpr int offB = offA + NSUB * NST * A_STAGE; // [NSUB][NST] B stages
-    static constexpr int offWs = offB + NSUB * NST * B_STAGE;    // [NSUB]: wx[16 columns][16] half (32 B rows), wy[16 columns][8] half
+    static constexpr int offWs = offB + NSUB * NST * B_STAGE;    // [NSUB]: wx[32 columns][16] half (32 B rows), wy[32 columns][8] half
     static constexpr int offBar = offWs + NSUB * 3 * SC * 16;    // [NSUB][NST] mbarriers
     static constexpr int offMisc = offBar + NSUB * NST * 8;  // tmem base, started[NSUB]
     static constexpr int total = offMisc + 64;
@@ -132,7 +132,7 @@ __global__ void __launch_bounds__(NTHR, 2)
                     const float4* __restrict__ trigf, const int2* __restrict__ plan, const int4* __restrict__ items,
                     int nproj, int M, int npair, float alpha2, int strip) {
     using L = MmaSmem<NN>;
-    constexpr int GW = L::GW, NPG = NN / 2, HP = NPG / 2;     // HP: pairs gathered per lane (half a B row)
+    constexpr int GW = L::GW, NPG = NN / 2;
     extern __shared__ __align__(128) unsigned char smem[];
     uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L::offMisc);
 
@@ -161,18 +161,18 @@ __global__ void __launch_bounds__(NTHR, 2)
 
     // ---- this warp's sub-tile
     const int sub = warp;
-    unsigned char* Aw = smem + L::offA + warp * NST * A_STAGE;
+    unsigned char* Aw = smem + L::offA + warp * NST * A_STAGE;      // this warp's single 32-column stage
     unsigned char* Bw = smem + L::offB + warp * NST * L::B_STAGE;
     uint4* ws = reinterpret_cast<uint4*>(smem + L::offWs) + warp * 3 * SC;
     const uint64_t adesc0 = umma_desc(smem_u32(Aw), A_LBO, 128), bdesc0 = umma_desc(smem_u32(Bw), L::B_LBO, 128);
-    const uint64_t adesc1 = adesc0 + (uint64_t)(A_STAGE >> 4), bdesc1 = bdesc0 + (uint64_t)(L::B_STAGE >> 4);
-    static_assert(NST == 2, "two descriptors per operand");
+    const uint64_t adesc1 = adesc0 + (uint64_t)((2 * A_LBO) >> 4), bdesc1 = bdesc0 + (uint64_t)((2 * L::B_LBO) >> 4);   // second K step
+    static_assert(NST == 1 && SC == 32, "one 32-column stage per warp");
     const uint32_t acc = tmem + (uint32_t)(sub * NN);
-    const int cl = lane & 15, part = lane >> 4;              // column of the step; 0: x axis, 1: y axis
+    const int cl = lane;                                     // column of the step
     uint32_t nstep = 0;                                      // K steps issued by this warp
     const size_t pstride = (size_t)nproj * M;                // elements between slice-pair planes of the spectrum
-    const __half2* plane0 = spec + (size_t)(pg * NPG + part * HP) * pstride;      // first plane this lane gathers
-    const int nvalid = min(HP, npair - (pg * NPG + part * HP));                   // planes that exist (<= 0: none)
+    const __half2* plane0 = spec + (size_t)(pg * NPG) * pstride;                  // first plane of this pair group
+    const int nvalid = min(NPG, npair - pg * NPG);                                // planes that exist
 
     for (int img = 0; img < 4; ++img) {
         const int2 win = plan[tile * 4 + img];
@@ -184,7 +184,6 @@ __global__ void __launch_bounds__(NTHR, 2)
         const float hw = (float)MH + 0.02f;
         const float bax = (float)SX - hw, bbx = (float)(SX + SUBX - 1) + hw;
         const float bay = (float)SY - hw, bby = (float)(SY + SUBY - 1) + hw;
-        const float org = part ? (float)SY : (float)SX;
         const int i_lo = (int)(((long long)win.y * split) / nsplit), i_hi = (int)(((long long)win.y * (split + 1)) / nsplit);
 
         for (int i0 = i_lo; i0 < i_hi; i0 += 32) {
@@ -209,10 +208,6 @@ __global__ void __launch_bounds__(NTHR, 2)
             const int off = incl - cnt;
 
             for (int c0 = 0; c0 < total; c0 += SC) {
-                const int st = nstep & (NST - 1);
-                if (nstep >= NST) mbar_wait(&bar[st], ((nstep / NST) - 1) & 1);     // this warp's MMA that read the stage is done
-                unsigned char* As = Aw + st * A_STAGE;
-                unsigned char* Bs = Bw + st * L::B_STAGE;
                 const int col = c0 + cl;
                 const bool valid = col < total;
                 // source lane: first h with incl_h > col
@@ -226,55 +221,65 @@ __global__ void __launch_bounds__(NTHR, 2)
                 const int h = min(lo, 31);
                 const int jj = __shfl_sync(0xffffffffu, j, h);
                 const int k = __shfl_sync(0xffffffffu, kmin, h) + (col - __shfl_sync(0xffffffffu, off, h));
-                // float-float trig of the source projection, this lane's axis
-                const float hx = __shfl_sync(0xffffffffu, cs.x, h), lx_ = __shfl_sync(0xffffffffu, cs.y, h);
-                const float hy = __shfl_sync(0xffffffffu, cs.z, h), ly_ = __shfl_sync(0xffffffffu, cs.w, h);
-                const float c_hi = part ? hy : hx, c_lo = part ? ly_ : lx_;
-                // ---- phase 1: taps of this axis into a zeroed row; half of the B row.
-                // x rows: 16 halves (32 B) per column at ws; y rows: 8 halves (16 B) per column behind them
-                unsigned char* wrow = reinterpret_cast<unsigned char*>(ws) + (part ? (SC * 32 + cl * 16) : cl * 32);
-                *reinterpret_cast<uint4*>(wrow) = make_uint4(0, 0, 0, 0);
-                if (part == 0) *reinterpret_cast<uint4*>(wrow + 16) = make_uint4(0, 0, 0, 0);
-                unsigned char* brow = Bs + (cl >> 3) * L::B_LBO + (cl & 7) * 16 + part * (GW / 2) * 128;
-                // taps l = floor(nu) - m + 1 + t, t = 0..2m-1, distance d_t = l - nu = d_0 + t; the open box
-                // |l - nu| < m keeps t iff d_t < m (d_0 > -m always); d_0 = -m+1 exactly iff nu is an integer
-                float fl, fr;
-                nu_split((float)k, c_hi, c_lo, fl, fr);
-                const float dint = -(float)(MH - 1);
-                float d0 = dint - fr;
-                if (fr > 0.f && d0 >= dint) d0 = __uint_as_float(__float_as_uint(dint) + 1u);   // next below -m+1
-                const int l0 = valid ? (int)(fl + dint - org) : 64;                                // 64: every tap out of range
-                const unsigned lim = part ? (unsigned)SUBY : (unsigned)SUBX;
-                __half* wtap = reinterpret_cast<__half*>(wrow) + l0;
-#pragma unroll
-                for (int t = 0; t < 2 * MH; ++t) {
-                    const float d = d0 + (float)t;
-                    const __half wv = __float2half_rn(ex2_approx(-alpha2 * d * d));
-                    if ((unsigned)(l0 + t) < lim && d < (float)MH) wtap[t] = wv;
-                }
+                // float-float trig of the source projection
+                const float cxh = __shfl_sync(0xffffffffu, cs.x, h), cxl = __shfl_sync(0xffffffffu, cs.y, h);
+                const float cyh = __shfl_sync(0xffffffffu, cs.z, h), cyl = __shfl_sync(0xffffffffu, cs.w, h);
+                // the column's B row: gather now, store after the previous MMAs released the stage
+                alignas(16) __half2 bv[NPG];
                 {
                     const __half2* a = plane0 + ((size_t)jj * M + (size_t)(k & (M - 1)));
-                    alignas(16) __half2 v[HP];
 #pragma unroll
-                    for (int p = 0; p < HP; ++p) {
-                        v[p] = (valid && p < nvalid) ? __ldg(a) : czero<__half2>();
+                    for (int p = 0; p < NPG; ++p) {
+                        bv[p] = (valid && p < nvalid) ? __ldg(a) : czero<__half2>();
                         a += pstride;
                     }
-                    const uint4* vv = reinterpret_cast<const uint4*>(v);
-#pragma unroll
-                    for (int q = 0; q < GW / 2; ++q) *reinterpret_cast<uint4*>(brow + q * 128) = vv[q];
                 }
-                __syncwarp();
-                // ---- phase 2: A[m = ly * 16 + lx][column] = wy[ly] * wx[lx]; MN-major: 8 cells of a column = 16 B.
-                // lane -> column cl, rows 4 * part .. 4 * part + 3
+                // ---- phase 1: taps of both axes into zeroed rows (x: 16 halves = 32 B, y: 8 halves = 16 B per column).
+                // taps l = floor(nu) - m + 1 + t, t = 0..2m-1, distance d_t = l - nu = d_0 + t; the open box
+                // |l - nu| < m keeps t iff d_t < m (d_0 > -m always); d_0 = -m+1 exactly iff nu is an integer
+                unsigned char* wxrow = reinterpret_cast<unsigned char*>(ws) + cl * 32;
+                unsigned char* wyrow = reinterpret_cast<unsigned char*>(ws) + SC * 32 + cl * 16;
+                *reinterpret_cast<uint4*>(wxrow) = make_uint4(0, 0, 0, 0);
+                *reinterpret_cast<uint4*>(wxrow + 16) = make_uint4(0, 0, 0, 0);
+                *reinterpret_cast<uint4*>(wyrow) = make_uint4(0, 0, 0, 0);
                 {
-                    const uint4 xa = ws[2 * cl], xc = ws[2 * cl + 1], yv = ws[2 * SC + cl];
-                    const unsigned y01 = part ? yv.z : yv.x, y23 = part ? yv.w : yv.y;
-                    unsigned char* arow = As + (cl >> 3) * A_LBO + (cl & 7) * 16 + part * (8 * 128);
+                    const float dint = -(float)(MH - 1);
+                    float flx, frx, fly, fry;
+                    nu_split((float)k, cxh, cxl, flx, frx);
+                    nu_split((float)k, cyh, cyl, fly, fry);
+                    float dx0 = dint - frx, dy0 = dint - fry;
+                    if (frx > 0.f && dx0 >= dint) dx0 = __uint_as_float(__float_as_uint(dint) + 1u);   // next below -m+1
+                    if (fry > 0.f && dy0 >= dint) dy0 = __uint_as_float(__float_as_uint(dint) + 1u);
+                    const int lx0 = valid ? (int)(flx + dint - (float)SX) : 64;                       // 64: every tap out of range
+                    const int ly0 = valid ? (int)(fly + dint - (float)SY) : 64;
+                    __half* wxt = reinterpret_cast<__half*>(wxrow) + lx0;
+                    __half* wyt = reinterpret_cast<__half*>(wyrow) + ly0;
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) {
-                        const unsigned yw = (r < 2) ? y01 : y23;
-                        const unsigned yb = (r & 1) ? (yw >> 16) : (yw & 0xffffu);
+                    for (int t = 0; t < 2 * MH; ++t) {
+                        const float dx = dx0 + (float)t, dy = dy0 + (float)t;
+                        const __half wxv = __float2half_rn(ex2_approx(-alpha2 * dx * dx));
+                        const __half wyv = __float2half_rn(ex2_approx(-alpha2 * dy * dy));
+                        if ((unsigned)(lx0 + t) < (unsigned)SUBX && dx < (float)MH) wxt[t] = wxv;
+                        if ((unsigned)(ly0 + t) < (unsigned)SUBY && dy < (float)MH) wyt[t] = wyv;
+                    }
+                }
+                // the warp's previous MMAs must have read the stage before it is overwritten
+                if (nstep > 0) mbar_wait(bar, (nstep - 1) & 1);
+                {
+                    unsigned char* brow = Bw + (cl >> 3) * L::B_LBO + (cl & 7) * 16;
+                    const uint4* vv = reinterpret_cast<const uint4*>(bv);
+#pragma unroll
+                    for (int q = 0; q < GW; ++q) *reinterpret_cast<uint4*>(brow + q * 128) = vv[q];
+                }
+                // ---- phase 2: A[m = ly * 16 + lx][column] = wy[ly] * wx[lx]; MN-major: 8 cells of a column = 16 B
+                {
+                    const uint4 xa = *reinterpret_cast<const uint4*>(wxrow), xc = *reinterpret_cast<const uint4*>(wxrow + 16);
+                    const uint4 yv = *reinterpret_cast<const uint4*>(wyrow);
+                    const unsigned yw[4] = {yv.x, yv.y, yv.z, yv.w};
+                    unsigned char* arow = Aw + (cl >> 3) * A_LBO + (cl & 7) * 16;
+#pragma unroll
+                    for (int r = 0; r < SUBY; ++r) {
+                        const unsigned yb = (r & 1) ? (yw[r >> 1] >> 16) : (yw[r >> 1] & 0xffffu);
                         uint4 lo4 = make_uint4(0, 0, 0, 0), hi4 = lo4;
                         if (yb != 0) {
                             const unsigned y2 = yb | (yb << 16);
@@ -293,8 +298,9 @@ __global__ void __launch_bounds__(NTHR, 2)
                 __syncwarp();
                 if (lane == 0) {
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    umma_f16(acc, st ? adesc1 : adesc0, st ? bdesc1 : bdesc0, IDESC, nstep > 0 ? 1u : 0u);
-                    umma_commit(&bar[st]);
+                    umma_f16(acc, adesc0, bdesc0, IDESC, nstep > 0 ? 1u : 0u);
+                    if (total - c0 > 16) umma_f16(acc, adesc1, bdesc1, IDESC, 1u);
+                    umma_commit(bar);
                 }
                 ++nstep;
                 __syncwarp();
@@ -302,7 +308,7 @@ __global__ void __launch_bounds__(NTHR, 2)
         }
     }
     // ---- this warp's MMAs complete (commits complete in order: wait for the last one)
-    if (nstep > 0) mbar_wait(&bar[(nstep - 1) & (NST - 1)], ((nstep - 1) / NST) & 1);
+    if (nstep > 0) mbar_wait(bar, (nstep - 1) & 1);
     if (lane == 0) misc[1 + warp] = nstep;
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
