@@ -130,7 +130,7 @@ template <int MH, int NN>
 __global__ void __launch_bounds__(NTHR, 2)
     grid_mma_kernel(const __half2* __restrict__ spec, __half2* __restrict__ grid, float2* __restrict__ partial,
                     const float4* __restrict__ trigf, const int2* __restrict__ plan, const int4* __restrict__ items,
-                    int nproj, int M, int npair, float alpha2, int strip) {
+                    int nproj, int M, int npair, float alpha2, int strip_log2) {
     using L = MmaSmem<NN>;
     constexpr int GW = L::GW, NPG = NN / 2;
     extern __shared__ __align__(128) unsigned char smem[];
@@ -334,7 +334,9 @@ __global__ void __launch_bounds__(NTHR, 2)
             const int ry = (b >> 1) * SUBY + ly, rx = (b & 1) * SUBX + lx;      // region-relative cell
             if (item.z < 0) {
                 const int gr = TY0 + ry, gc = TX0 + rx;
-                const size_t cell = strip ? ((size_t)(gc / strip) * M + gr) * strip + (gc % strip) : (size_t)gr * M + gc;
+                // strip-major grid (strip width 2^strip_log2 columns) or row-major (strip_log2 < 0)
+                const size_t cell = strip_log2 >= 0 ? ((((size_t)(gc >> strip_log2) * M + gr) << strip_log2) + (gc & ((1 << strip_log2) - 1)))
+                                                    : (size_t)gr * M + gc;
                 __half2* dst = grid + (size_t)(pg * NPG) * pstride + cell;
 #pragma unroll
                 for (int p = 0; p < NPG; ++p)
@@ -361,7 +363,7 @@ static int launch_mma_t(const tcp_ctx* c, cudaStream_t st) {
     const double alpha = 3.14159265358979323846 / (1.4142135623730951 * MH);
     dim3 grid(c->g_nitems, (c->npair + NN / 2 - 1) / (NN / 2));
     kern<<<grid, NTHR, L::total, st>>>((const __half2*)c->spec, (__half2*)c->grid, c->g_partial, c->trigf, c->g_plan, c->g_items,
-                                       c->nproj, c->M, c->npair, (float)(alpha * 1.4426950408889634), c->grid_strip);
+                                       c->nproj, c->M, c->npair, (float)(alpha * 1.4426950408889634), c->grid_strip ? (int)log2((double)c->grid_strip) : -1);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }
