@@ -29,6 +29,7 @@
 #include <stdlib.h>
 
 #include "grid_common.cuh"
+#include "umma.cuh"
 #include "tcp_internal.h"
 
 namespace tcpk {
@@ -39,64 +40,6 @@ constexpr int NST = 1;                            // stages per warp
 constexpr int RUNMAX = 32;                        // >= samples of one chord inside a sub-tile's sample box
 constexpr int A_LBO = (128 / 8) * 128;            // bytes between k-blocks of 8 columns in an A stage
 constexpr int A_STAGE = SC * 256;                 // bytes of one A stage: [SC/8][16][8 columns][8 cells] half
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-// shared-memory matrix descriptor, no swizzle: start >> 4, leading (k-block) and stride (mn-block) byte offsets >> 4
-__device__ __forceinline__ uint64_t umma_desc(uint32_t addr, uint32_t lbo, uint32_t sbo) {
-    return (uint64_t)((addr >> 4) & 0x3fffu) | ((uint64_t)((lbo >> 4) & 0x3fffu) << 16) |
-           ((uint64_t)((sbo >> 4) & 0x3fffu) << 32) | ((uint64_t)1 << 46);
-}
-__device__ __forceinline__ void mbar_init(uint64_t* b, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count));
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity, int tag = 0, int info = 0) {
-    uint32_t done = 0;
-#ifdef TCP_MBAR_WATCHDOG
-    unsigned spins = 0;
-#endif
-    while (!done) {
-        asm volatile("{.reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p;}"
-                     : "=r"(done)
-                     : "r"(smem_u32(b)), "r"(parity)
-                     : "memory");
-#ifdef TCP_MBAR_WATCHDOG
-        if (!done && ++spins > (1u << 22)) {
-            if ((threadIdx.x & 31) == 0)
-                printf("mbar stuck: block %d,%d warp %d tag %d parity %u info %d\n", blockIdx.x, blockIdx.y, threadIdx.x >> 5, tag, parity, info);
-            __trap();
-        }
-#endif
-    }
-}
-__device__ __forceinline__ void umma_commit(uint64_t* b) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(b)) : "memory");
-}
-__device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
-    asm volatile("{.reg .pred p; setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;}" ::"r"(tmem_d),
-                 "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
-                 : "memory");
-}
-
-template <int NN> struct TmemLd;
-template <> struct TmemLd<16> {
-    static __device__ __forceinline__ void run(uint32_t taddr, uint32_t* r) {
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
-                       "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-                     : "r"(taddr));
-    }
-};
-template <> struct TmemLd<32> {
-    static __device__ __forceinline__ void run(uint32_t taddr, uint32_t* r) {
-        TmemLd<16>::run(taddr, r);
-        TmemLd<16>::run(taddr + 16, r + 16);
-    }
-};
-
-__device__ __forceinline__ void mbar_arrive(uint64_t* b) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
-}
 
 // nu = k * (c_hi + c_lo) as floor + fraction, fp32 FMAs only (k exact, |k| < 2^13): the product's
 // rounding error is recovered exactly by an FMA, so fl + frac = nu to ~1e-11 cells.
