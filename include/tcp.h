@@ -50,7 +50,11 @@ enum { TCP_WS_SINOGRAM = 0, TCP_WS_SPECTRUM = 1, TCP_WS_GRID = 2, TCP_WS_PASS1 =
  * default for TCP_F16 / TCP_F16_OUT32); GATHER: per-cell gather (atomics-free, slow; cross-check);
  * SCATTER_ATOMIC: fp32 atomics (TCP_F32 only; cross-check) */
 enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1, TCP_GRID_TILE = 2, TCP_GRID_MMA = 3 };
-enum { TCP_OPT_GRID_IMPL = 0, TCP_OPT_PROFILE = 1 };
+/* TCP_OPT_TCFFT: bit mask of the transforms run as DFT-as-GEMM on the tensor cores (fp16 storage and
+ * M = 4096 only; elsewhere the option must be 0): 1 = detector-row kernel (S3 + S4), 2 = column pass,
+ * 4 = row pass of the inverse 2D transform.  Default: all that apply. */
+enum { TCP_OPT_GRID_IMPL = 0, TCP_OPT_PROFILE = 1, TCP_OPT_TCFFT = 2 };
+enum { TCP_TCFFT_ROWS = 1, TCP_TCFFT_COLS = 2, TCP_TCFFT_IROWS = 4 };
 /* stages timed when TCP_OPT_PROFILE is on, in launch order */
 enum { TCP_ST_TRIG = 0, TCP_ST_NORMALIZE = 1, TCP_ST_ROWS = 2, TCP_ST_GRID = 3, TCP_ST_IFFT_COLS = 4,
        TCP_ST_IFFT_ROWS = 5, TCP_NSTAGES = 6 };

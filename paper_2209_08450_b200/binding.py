@@ -176,6 +176,10 @@ class Recon:
     def set_grid_impl(self, name: str):
         _check(lib().tcp_set_option(self.h, 0, GRID_IMPLS[name]))
 
+    def set_tcfft(self, mask: int):
+        """TCP_OPT_TCFFT: which transforms run on the tensor cores (1 rows, 2 column pass, 4 row pass)."""
+        _check(lib().tcp_set_option(self.h, 2, int(mask)))
+
     STAGES = ("trig", "normalize", "rows", "grid", "ifft_cols", "ifft_rows")
 
     def set_profile(self, on: bool):

@@ -14,7 +14,10 @@
 
 namespace tcpk {
 
-__host__ __device__ constexpr int cols_w(int M) { return (16384 / M) < 32 ? (16384 / M) : 32; }   // columns per CTA
+#ifndef COLS_BUDGET
+#define COLS_BUDGET 16384
+#endif
+__host__ __device__ constexpr int cols_w(int M) { return (COLS_BUDGET / M) < 2 ? 2 : (COLS_BUDGET / M) < 32 ? (COLS_BUDGET / M) : 32; }   // columns per CTA
 __host__ __device__ constexpr int cols_wp(int M) { return cols_w(M) / 2; }                          // column pairs per CTA
 // stride between the pair-lines of a CTA, in cpair (16 B) units: a quarter-warp (8 lanes = one
 // 128-byte shared-memory wavefront of 16-byte accesses) holds min(WP, 8) lines x 8 / min(WP, 8)

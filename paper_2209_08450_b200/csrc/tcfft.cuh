@@ -43,7 +43,6 @@ namespace tcpk {
 namespace tcfft {
 
 constexpr int A_BYTES = 128 * 128 * 2;      // the DFT-64 matrix, K-major blocks [mb 16][kb 16][8 m][8 k] half
-constexpr int TW_BYTES = 32 * 64 * 16;      // twiddles: float4 (cos, sin, cos, sin)(k1; i2 = 2p, 2p + 1) at [p][k1]
 constexpr int A_LBO = 128, A_SBO = 16 * 128;
 
 template <int NB>
@@ -55,7 +54,6 @@ struct Group {
     uint32_t tmem;                                  // TMEM address of D (lane 0, first column)
     uint32_t a_addr, b_addr;                        // shared-memory addresses of A and of this group's B buffer
     unsigned char* bbuf;
-    const float4* tw;                               // twiddle table in shared memory
     uint64_t* bar;
     uint32_t phase;                                 // parity of the next completion of bar
     int t, q, lane, j, c, barid;                    // thread in group, lane quarter, lane, row in half-quarter, re|im half
@@ -120,25 +118,48 @@ __device__ __forceinline__ uint32_t pack_half2(float a, float b) {
 
 // between the stages: D = Y (row (k1, c), column (line, i2)) -> Y' = Y W4096^(k1 i2) -> B of stage C.
 // (Yr + i Yi)(C - i S): the c = 0 lane holds Yr and wants Yr C + Yi S, the c = 1 lane holds Yi and wants
-// Yi C - Yr S; the partner value comes by SHFL from 16 lanes away.
+// Yi C - Yr S; the partner value comes by SHFL from 16 lanes away.  The twiddles are NOT read from a
+// table: the kernels are bound by the shared-memory / TMEM / shuffle data path (profiles/), the FMA pipe
+// idles, so each thread steps (C, +-S)(k1, i2) along i2 by complex multiplication with its own
+// w1 = e^{2 pi i k1/4096} (sign of S folded in), restarted every 16 points from w16^m: chains of 16
+// fp32 products, error ~1e-6, far below the fp16 operand rounding.
+struct Twid { float c1, s1, c16, s16; };
 template <int NB>
-__device__ __forceinline__ void twiddle_step(const Group<NB>& g) {
+__device__ __forceinline__ Twid make_twid(const Group<NB>& g) {
     const int k1 = 16 * g.q + g.j;
-    const uint32_t sgn = g.c ? 0x80000000u : 0u;
+    Twid t;
+    sincospif((float)k1 * (1.f / 2048.f), &t.s1, &t.c1);
+    sincospif((float)((16 * k1) & 4095) * (1.f / 2048.f), &t.s16, &t.c16);
+    if (g.c) { t.s1 = -t.s1; t.s16 = -t.s16; }
+    return t;
+}
+template <int NB>
+__device__ __forceinline__ void twiddle_step(const Group<NB>& g, const Twid& tw) {
+    const int k1 = 16 * g.q + g.j;
 #pragma unroll 1
     for (int line = 0; line < NB; ++line) {
+        float bc = 1.f, bs = 0.f;                   // w16^m, m = i2 / 16
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             uint32_t r[32];
             ld_d(g, line, h, r);
             uint32_t pk[16];
 #pragma unroll
-            for (int p = 0; p < 16; ++p) {
-                const float4 w = g.tw[(h * 16 + p) * 64 + k1];
-                const float own0 = __uint_as_float(r[2 * p]), own1 = __uint_as_float(r[2 * p + 1]);
-                const float oth0 = __uint_as_float(__shfl_xor_sync(0xffffffffu, r[2 * p], 16) ^ sgn);
-                const float oth1 = __uint_as_float(__shfl_xor_sync(0xffffffffu, r[2 * p + 1], 16) ^ sgn);
-                pk[p] = pack_half2(fmaf(oth0, w.y, own0 * w.x), fmaf(oth1, w.w, own1 * w.z));
+            for (int m = 0; m < 2; ++m) {
+                float tc = bc, ts = bs;
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    const int i = 16 * m + e;
+                    const float own = __uint_as_float(r[i]);
+                    const float oth = __uint_as_float(__shfl_xor_sync(0xffffffffu, r[i], 16));
+                    const float o = fmaf(oth, ts, own * tc);
+                    if (e & 1) pk[i >> 1] = pack_half2(__uint_as_float(pk[i >> 1]), o);
+                    else pk[i >> 1] = __float_as_uint(o);
+                    const float nc = fmaf(-ts, tw.s1, tc * tw.c1), ns = fmaf(tc, tw.s1, ts * tw.c1);
+                    tc = nc; ts = ns;
+                }
+                const float nc = fmaf(-bs, tw.s16, bc * tw.c16), ns = fmaf(bc, tw.s16, bs * tw.c16);
+                bc = nc; bs = ns;
             }
             const int n = line * 64 + k1;
 #pragma unroll
@@ -148,16 +169,30 @@ __device__ __forceinline__ void twiddle_step(const Group<NB>& g) {
     }
 }
 
-// natural-order complex line (4096 half2, 16-byte aligned) -> B of stage A.  A lane takes 8 consecutive
+// natural-order complex line (4096 half2, 16-byte aligned) -> B of stage A, in two steps so that the
+// global loads of the next line fly while the current one is transformed.  A lane takes 8 consecutive
 // points (32 bytes); lanes 0-7 take 8 consecutive i1 (consecutive 16-byte chunks of one block: no bank
 // conflicts), the lane's upper bits walk the n blocks so that 4 lanes consume a whole 128-byte line.
-template <int NB, bool SWAP>
-__device__ __forceinline__ void load_line_c(const Group<NB>& g, int line, const __half2* __restrict__ src) {
+struct LineRegs { uint4 v[8]; };
+template <int NB>
+__device__ __forceinline__ void fetch_line_c(const Group<NB>& g, const __half2* __restrict__ src, LineRegs& r) {
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
         const int combo = g.q * 4 + u, i1 = 8 * (combo >> 1) + (g.lane & 7), nb = 4 * (combo & 1) + (g.lane >> 3);
         const uint4* p = reinterpret_cast<const uint4*>(src + 64 * i1 + 8 * nb);
-        const uint4 v0 = __ldg(p), v1 = __ldg(p + 1);
+        // one 32-byte load: a lane's two 16-byte halves share a sector
+        asm volatile("ld.global.nc.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                     : "=r"(r.v[2 * u].x), "=r"(r.v[2 * u].y), "=r"(r.v[2 * u].z), "=r"(r.v[2 * u].w), "=r"(r.v[2 * u + 1].x),
+                       "=r"(r.v[2 * u + 1].y), "=r"(r.v[2 * u + 1].z), "=r"(r.v[2 * u + 1].w)
+                     : "l"(p));
+    }
+}
+template <int NB, bool SWAP>
+__device__ __forceinline__ void put_line_c(const Group<NB>& g, int line, const LineRegs& r) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int combo = g.q * 4 + u, i1 = 8 * (combo >> 1) + (g.lane & 7), nb = 4 * (combo & 1) + (g.lane >> 3);
+        const uint4 v0 = r.v[2 * u], v1 = r.v[2 * u + 1];
         const uint4 re = make_uint4(__byte_perm(v0.x, v0.y, 0x5410), __byte_perm(v0.z, v0.w, 0x5410), __byte_perm(v1.x, v1.y, 0x5410),
                                     __byte_perm(v1.z, v1.w, 0x5410));
         const uint4 im = make_uint4(__byte_perm(v0.x, v0.y, 0x7632), __byte_perm(v0.z, v0.w, 0x7632), __byte_perm(v1.x, v1.y, 0x7632),
@@ -166,54 +201,59 @@ __device__ __forceinline__ void load_line_c(const Group<NB>& g, int line, const 
         *b1_chunk(g, (SWAP ? 0 : 64) + i1, line, nb) = im;
     }
 }
+template <int NB, bool SWAP>
+__device__ __forceinline__ void load_line_c(const Group<NB>& g, int line, const __half2* __restrict__ src) {
+    LineRegs r;
+    fetch_line_c(g, src, r);
+    put_line_c<NB, SWAP>(g, line, r);
+}
 
 // CTA prologue: tables into shared memory, one mbarrier and one TMEM accumulator per group.
-// Shared memory: [A 32 KB][twiddles 32 KB][NG x B][NG mbarriers][NG TMEM slots]; 128 NG threads.
+// Shared memory: [A 32 KB][NG x B][NG mbarriers][TMEM slot]; 128 NG threads.
 template <int NB, int NG>
 struct Cta {
-    static constexpr int offA = 0, offTw = A_BYTES, offB = offTw + TW_BYTES, offBar = offB + NG * Group<NB>::B_BYTES;
+    static constexpr int offA = 0, offB = A_BYTES, offBar = offB + NG * Group<NB>::B_BYTES;
     static constexpr int offSlot = offBar + 8 * NG, total = offSlot + 4 * NG + 12;
     static constexpr int threads = 128 * NG;
     static_assert(NG * 64 * NB <= 512, "TMEM has 512 columns");
+    static constexpr int tmem_cols = NG * 64 * NB <= 32 ? 32 : NG * 64 * NB <= 64 ? 64 : NG * 64 * NB <= 128 ? 128 : NG * 64 * NB <= 256 ? 256 : 512;
 
-    static __device__ __forceinline__ Group<NB> setup(unsigned char* smem, const uint4* __restrict__ amat, const uint4* __restrict__ twtab) {
+    static __device__ __forceinline__ Group<NB> setup(unsigned char* smem, const uint4* __restrict__ amat) {
         const int tid = threadIdx.x;
         for (int i = tid; i < A_BYTES / 16; i += threads) reinterpret_cast<uint4*>(smem + offA)[i] = __ldg(amat + i);
-        for (int i = tid; i < TW_BYTES / 16; i += threads) reinterpret_cast<uint4*>(smem + offTw)[i] = __ldg(twtab + i);
         Group<NB> g;
         const int grp = tid >> 7;
         g.t = tid & 127; g.q = g.t >> 5; g.lane = tid & 31; g.j = g.lane & 15; g.c = g.lane >> 4; g.barid = 1 + grp;
         g.bbuf = smem + offB + grp * Group<NB>::B_BYTES;
         g.a_addr = smem_u32(smem + offA);
         g.b_addr = smem_u32(g.bbuf);
-        g.tw = reinterpret_cast<const float4*>(smem + offTw);
         g.bar = reinterpret_cast<uint64_t*>(smem + offBar) + grp;
         g.phase = 0;
-        uint32_t* slot = reinterpret_cast<uint32_t*>(smem + offSlot) + grp;
+        uint32_t* slot = reinterpret_cast<uint32_t*>(smem + offSlot);       // one allocation per CTA, 64 NB columns per group
         if (g.t == 0) {
             mbar_init(g.bar, 1);
             asm volatile("fence.mbarrier_init.release.cluster;");
         }
-        if (g.q == 0) {
-            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slot)), "n"(64 * NB));
+        if (tid < 32) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slot)), "n"(tmem_cols));
             asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // A was written through the generic proxy
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        g.tmem = *slot;
+        g.tmem = *slot + (uint32_t)(grp * 64 * NB);
         return g;
     }
     static __device__ __forceinline__ void teardown(const Group<NB>& g) {
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
-        if (g.q == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(g.tmem), "n"(64 * NB));
+        if (threadIdx.x < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(g.tmem), "n"(tmem_cols));
     }
 };
 
-// host: the two tables, in the byte order the kernels copy into shared memory
-inline void build_tables(std::vector<__half>& amat, std::vector<float4>& tw) {
+// host: the DFT-64 matrix in the byte order the kernels copy into shared memory
+inline void build_tables(std::vector<__half>& amat) {
     const double pi = 3.14159265358979323846264338327950288;
     amat.assign(128 * 128, __float2half(0.f));
     for (int rho = 0; rho < 128; ++rho)
@@ -222,12 +262,6 @@ inline void build_tables(std::vector<__half>& amat, std::vector<float4>& tw) {
             const double th = 2.0 * pi * (double)((k * i) & 63) / 64.0;
             const double v = (c == cp) ? cos(th) : (c == 0 ? sin(th) : -sin(th));
             amat[(size_t)(((rho >> 3) * 16 + (kap >> 3)) * 64 + (rho & 7) * 8 + (kap & 7))] = __float2half((float)v);
-        }
-    tw.resize(32 * 64);
-    for (int p = 0; p < 32; ++p)
-        for (int k1 = 0; k1 < 64; ++k1) {
-            const double a0 = 2.0 * pi * (double)(k1 * (2 * p)) / 4096.0, a1 = 2.0 * pi * (double)(k1 * (2 * p + 1)) / 4096.0;
-            tw[p * 64 + k1] = make_float4((float)cos(a0), (float)sin(a0), (float)cos(a1), (float)sin(a1));
         }
 }
 

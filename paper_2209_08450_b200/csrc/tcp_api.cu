@@ -9,6 +9,7 @@
 #include <algorithm>
 #include <vector>
 
+#include "tcfft.cuh"
 #include "tcp_internal.h"
 
 namespace tcpk {
@@ -116,6 +117,22 @@ static int build_context(tcp_ctx* c) {
     if ((rc = upload(&c->deax, dx, &c->bytes))) return rc;
     if ((rc = upload(&c->deay, dy, &c->bytes))) return rc;
 
+    if (c->tcfft_ok) {
+        std::vector<__half> am;
+        tcfft::build_tables(am);
+        __half* dam = nullptr;
+        if ((rc = upload(&dam, am, &c->bytes))) return rc;
+        c->tc_amat = dam;
+        std::vector<float> hs(M);
+        std::vector<float2> ps(M);
+        for (int k = 0; k < M; ++k) {
+            hs[k] = hf[k] * 64.f;
+            ps[k] = make_float2(pt[k].x / 64.f, pt[k].y / 64.f);
+        }
+        if ((rc = upload(&c->tc_hfilt, hs, &c->bytes))) return rc;
+        if ((rc = upload(&c->tc_ptab, ps, &c->bytes))) return rc;
+    }
+
     // gather tiles, heaviest (closest to DC) first: sample density falls as 1/radius
     const int T = 16, tx = M / T;
     std::vector<std::pair<long long, int>> key;
@@ -178,6 +195,9 @@ tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, 
     c->grid_impl = c->half_store ? TCP_GRID_MMA : TCP_GRID_TILE;
     c->grid_strip = (c->grid_impl == TCP_GRID_MMA) ? cols_strip_width(c->M) : 0;
     cudaGetDevice(&c->device);
+    cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, c->device);
+    c->tcfft_ok = (c->half_store && c->M == 4096) ? TCP_TCFFT_IROWS : 0;
+    c->tcfft = 0;   // measured slower than the CUDA-core transforms: opt-in through TCP_OPT_TCFFT
     if (build_context(c) != TCP_OK || setup_kernel_attributes(c) != TCP_OK) {
         char keep[512];
         strncpy(keep, g_err, sizeof(keep));
@@ -202,6 +222,7 @@ void tcp_destroy(tcp_ctx* c) {
     cudaFree(c->sino); cudaFree(c->spec); cudaFree(c->grid); cudaFree(c->pass1); cudaFree(c->trig); cudaFree(c->trigf);
     cudaFree(c->tw); cudaFree(c->hfilt); cudaFree(c->ptab); cudaFree(c->deax); cudaFree(c->deay);
     cudaFree(c->tile_order);
+    cudaFree(c->tc_amat); cudaFree(c->tc_hfilt); cudaFree(c->tc_ptab);
     grid_tile_free(c);
     free(c);
 }
@@ -237,7 +258,7 @@ int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* d
     TCP_MARK(4);
     if ((rc = launch_ifft_cols(c, st))) return rc;
     TCP_MARK(5);
-    if ((rc = launch_ifft_rows(c, out, st))) return rc;
+    if ((rc = (c->tcfft & TCP_TCFFT_IROWS) ? launch_ifft_rows_tc(c, out, st) : launch_ifft_rows(c, out, st))) return rc;
     TCP_MARK(6);
 #undef TCP_MARK
     return TCP_OK;
@@ -306,6 +327,11 @@ int tcp_set_option(tcp_ctx* c, int option, int value) {
         if (value == TCP_GRID_MMA && !c->half_store) return set_error(TCP_EUNSUPPORTED, "tensor-core gridding needs fp16 storage");
         c->grid_impl = value;
         c->grid_strip = (value == TCP_GRID_MMA) ? cols_strip_width(c->M) : 0;
+        return TCP_OK;
+    }
+    if (option == TCP_OPT_TCFFT) {
+        if (value & ~c->tcfft_ok) return set_error(TCP_EUNSUPPORTED, "tensor-core transforms %d not available here (mask %d)", value, c->tcfft_ok);
+        c->tcfft = value;
         return TCP_OK;
     }
     if (option == TCP_OPT_PROFILE) {

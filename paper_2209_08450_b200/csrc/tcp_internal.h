@@ -15,7 +15,9 @@ struct tcp_ctx {
     double scale;         // power-of-two scale S of SPECTRUM / GRID / PASS1 (1 in fp32)
     int grid_impl;
     int grid_strip;       // 0: grid rows are contiguous; W > 0: strip-major [pair][M/W][M l2][W l1] (tcgen05 gridding)
-    int device;
+    int device, nsm;      // CUDA device and its SM count
+    int tcfft;            // TCP_TCFFT_* mask of transforms on the tensor cores (k_tcfft.cu)
+    int tcfft_ok;         // the mask this context supports
     // workspaces (device)
     void* sino;           // [nz][nproj][n]      float | half
     void* spec;           // [npair][nproj][M]   float2 | half2   (S * G of stage S4, FFT order)
@@ -29,6 +31,9 @@ struct tcp_ctx {
     float2* ptab;         // [M] S * C * e^{+2 pi i k c / M}, k signed; 0 at k = M/2
     float* deax;          // [n] 1 / (S * Phi(x))
     float* deay;          // [n] 1 / Phi(y)
+    void* tc_amat;        // tcfft.cuh: DFT-64 matrix, 128 x 128 half in operand block order
+    float* tc_hfilt;      // [M] 2^6 H[k] / M   (the filtered row rides fp16 operands: keep it off the subnormals)
+    float2* tc_ptab;      // [M] ptab / 2^6
     int* tile_order;      // gather gridding: tiles sorted by decreasing work
     int ntiles;
     // tile gridding (k_grid_tile.cu): work items, split-tile reduce list, partial tiles, per-call plan
@@ -71,6 +76,7 @@ void grid_tile_free(tcp_ctx* c);
 int launch_ifft_cols(const tcp_ctx* c, cudaStream_t st);
 int cols_strip_width(int M);
 int launch_ifft_rows(const tcp_ctx* c, void* out, cudaStream_t st);
+int launch_ifft_rows_tc(const tcp_ctx* c, void* out, cudaStream_t st);
 int launch_mean_frames(const uint16_t* frames, int nframes, int nz, int n, float* mean, cudaStream_t st);
 int setup_kernel_attributes(const tcp_ctx* c);
 void pipe_destroy(tcp_ctx* c);

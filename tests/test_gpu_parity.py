@@ -238,13 +238,14 @@ def test_pipeline_host_matches_direct():
 
 
 # ------------------------------------------------------------------ BASELINE full sizes, bench launch configuration
-@pytest.mark.parametrize("cfg,nz", [("C4", 32), ("C5", 4)])
-def test_full_size_chunk_sampled_against_oracle(cfg, nz):
+@pytest.mark.parametrize("cfg,nz,tcfft", [("C4", 32, 0), ("C4", 32, 4), ("C5", 4, 0)])
+def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft):
     """C4 (2048^2, 2048 projections, fp16, one 32-slice chunk exactly as bench.py launches it: tcgen05
     gridding with 16 pairs per accumulator group) and C5 (4096^2, 4000 projections, M = 8192, off-centre,
     fp16 -> fp32 output).  Inputs are manufactured on the GPU (synthgen.make_counts_torch, frame averaging
     through tcp_mean_frames_u16) and the SAME arrays go to the oracle, which reconstructs a sample of the
-    chunk's slices one by one."""
+    chunk's slices one by one.  tcfft = 4 additionally runs the row pass of the inverse 2D transform as
+    DFT-as-GEMM on the tensor cores (opt-in, TCP_OPT_TCFFT; same gates)."""
     tcp = _tcp()
     w = sg.make_workload(cfg)
     z0 = w.nz_total // 2 - nz // 2
@@ -256,6 +257,8 @@ def test_full_size_chunk_sampled_against_oracle(cfg, nz):
     tcp.tcp_mean_frames_u16(df.contiguous(), dark_d)
     theta = w.theta
     r = tcp.Recon(w.n, w.nproj, nz, w.center, w.dtype, w.filter, 3)
+    if tcfft:
+        r.set_tcfft(tcfft)
     out = r.recon(raw_d.contiguous(), flat_d, dark_d, torch.from_numpy(theta).cuda())
     torch.cuda.synchronize()
     out = out.float().cpu().numpy()
