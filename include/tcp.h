@@ -113,6 +113,18 @@ size_t tcp_workspace_bytes(const tcp_ctx* ctx);
 int tcp_launches_per_recon(const tcp_ctx* ctx);
 int tcp_set_option(tcp_ctx* ctx, int option, int value);
 
+/* Rotation-centre "try" mode ("--reconstruction-type try": one slice reconstructed for a
+ * set of candidate centres, for visual choice).  raw_u16 [nproj][1][n], flat / dark [n], theta [nproj] are
+ * DEVICE pointers as in tcp_recon; centers is a HOST array of ncenter rotation centres, each in [0, n-1],
+ * 1 <= ncenter <= nz_chunk; out (DEVICE) [ncenter][n][n] receives the reconstruction for centers[i] at
+ * index i, identical (to rounding) to tcp_recon on a context created with that centre.  The slice is
+ * normalised and filtered once; candidate centres differ only in the phase table of stage S4, two centres
+ * riding one complex transform.  Enqueues on stream; the phase tables are built on the host and copied
+ * from pageable memory, so the call may block until earlier work on stream has finished.
+ * Errors: TCP_EINVAL (NULL, ncenter or a centre out of range), TCP_ENOMEM, TCP_ECUDA. */
+int tcp_recon_try(tcp_ctx* ctx, const uint16_t* raw_u16, const float* flat, const float* dark, const float* theta,
+                  const float* centers, int ncenter, void* out, tcp_stream_t stream);
+
 /* Per-kernel device times.  With tcp_set_option(ctx, TCP_OPT_PROFILE, 1) every tcp_recon records
  * CUDA events around each of its kernels on the caller's stream (no host synchronisation; a ring
  * of 512 calls).  tcp_profile_collect synchronises on those events, adds the elapsed

@@ -20,7 +20,7 @@ EXPORTS = [
     "tcp_create", "tcp_create_ex", "tcp_recon", "tcp_destroy", "tcp_last_error",
     "tcp_mean_frames_u16", "tcp_normalize", "tcp_workspace", "tcp_read_workspace", "tcp_scale", "tcp_grid_strip",
     "tcp_workspace_bytes", "tcp_launches_per_recon", "tcp_set_option", "tcp_profile_collect",
-    "tcp_recon_volume_host",
+    "tcp_recon_volume_host", "tcp_recon_try",
 ]
 
 
@@ -76,6 +76,8 @@ def lib():
     L.tcp_profile_collect.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(ci)]
     L.tcp_recon_volume_host.restype = ci
     L.tcp_recon_volume_host.argtypes = [vp, vp, vp, vp, vp, vp, ci, ci, C.POINTER(cf)]
+    L.tcp_recon_try.restype = ci
+    L.tcp_recon_try.argtypes = [vp, vp, vp, vp, vp, C.POINTER(cf), ci, vp, vp]
     _lib = L
     return L
 
@@ -218,6 +220,23 @@ class Recon:
             out = torch.empty((self.nz, self.n, self.n), dtype=self.out_dtype, device=raw_u16.device)
         _dev(out, self.out_dtype, (self.nz, self.n, self.n))
         tcp_recon(self.h, raw_u16, flat, dark, theta, out, stream)
+        return out
+
+    def recon_try(self, raw_u16, flat, dark, theta, centers, out=None, stream=None):
+        """tcp_recon_try: one slice (raw [nproj][1][n], flat / dark [n] or [1][n]) for every centre in `centers`."""
+        raw_u16 = _as_u16(raw_u16)
+        _dev(raw_u16, torch.uint16, (self.nproj, 1, self.n))
+        flat, dark = flat.reshape(1, self.n), dark.reshape(1, self.n)
+        _dev(flat, torch.float32, (1, self.n))
+        _dev(dark, torch.float32, (1, self.n))
+        _dev(theta, torch.float32, (self.nproj,))
+        cs = [float(c) for c in centers]
+        if out is None:
+            out = torch.empty((len(cs), self.n, self.n), dtype=self.out_dtype, device=raw_u16.device)
+        _dev(out, self.out_dtype, (len(cs), self.n, self.n))
+        arr = (C.c_float * len(cs))(*cs)
+        _check(lib().tcp_recon_try(self.h, raw_u16.data_ptr(), flat.data_ptr(), dark.data_ptr(), theta.data_ptr(), arr, len(cs),
+                                   out.data_ptr(), _stream(stream)))
         return out
 
     def normalize(self, raw_u16, flat, dark, stream=None):

@@ -13,7 +13,7 @@ template <int M, int ROWS, class TS, class TC>
 __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict__ sino, TC* __restrict__ spec,
                                                             const float2* __restrict__ tw,
                                                             const float* __restrict__ hfilt,
-                                                            const float2* __restrict__ ptab, int nproj, int nz) {
+                                                            const float2* __restrict__ ptab, int nproj, int nz, int try_mode) {
     constexpr int n = M / 2;
     constexpr int TG = M / 16;
     extern __shared__ float2 smem[];
@@ -24,10 +24,13 @@ __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict
     const bool live = j < nproj;
     if (!live) j = nproj - 1;             // keep the group in the barriers; its stores are masked
     const int pair = blockIdx.y;
-    const int zA = 2 * pair, zB = 2 * pair + 1;
+    // try mode (tcp_recon_try): every pair transforms slice 0 alone and carries the phases of two candidate
+    // centres in its own table ptab[pair][M] = S C (e^{2 pi i k c1/M} + i e^{2 pi i k c2/M})
+    const int zA = try_mode ? 0 : 2 * pair, zB = try_mode ? nz : 2 * pair + 1;
     const TS* pA = sino + ((size_t)zA * nproj + j) * n;
     const TS* pB = sino + ((size_t)(zB < nz ? zB : zA) * nproj + j) * n;
     const bool hasB = zB < nz;
+    if (try_mode) ptab += (size_t)pair * M;
 
     // FFT #1: zero-padded load, filter on store
     fft_line<M, false>(
@@ -63,7 +66,8 @@ static int launch_rows_t(const tcp_ctx* c, cudaStream_t st) {
     auto kern = rows_kernel<M, ROWS, TS, TC>;
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid((c->nproj + ROWS - 1) / ROWS, c->npair);
-    kern<<<grid, ROWS * TG, smem, st>>>((const TS*)c->sino, (TC*)c->spec, c->tw, c->hfilt, c->ptab, c->nproj, c->nz);
+    kern<<<grid, ROWS * TG, smem, st>>>((const TS*)c->sino, (TC*)c->spec, c->tw, c->hfilt, c->try_ptab ? c->try_ptab : c->ptab, c->nproj, c->nz,
+                                       c->try_ptab ? 1 : 0);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }

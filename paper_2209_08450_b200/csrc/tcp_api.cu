@@ -222,6 +222,7 @@ void tcp_destroy(tcp_ctx* c) {
     cudaFree(c->sino); cudaFree(c->spec); cudaFree(c->grid); cudaFree(c->pass1); cudaFree(c->trig); cudaFree(c->trigf);
     cudaFree(c->tw); cudaFree(c->hfilt); cudaFree(c->ptab); cudaFree(c->deax); cudaFree(c->deay);
     cudaFree(c->tile_order);
+    cudaFree(c->try_buf);
     cudaFree(c->tc_amat); cudaFree(c->tc_hfilt); cudaFree(c->tc_ptab);
     grid_tile_free(c);
     free(c);
@@ -262,6 +263,52 @@ int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* d
     TCP_MARK(6);
 #undef TCP_MARK
     return TCP_OK;
+}
+
+int tcp_recon_try(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* dark, const float* theta,
+                  const float* centers, int ncenter, void* out, tcp_stream_t stream) {
+    if (!c || !raw || !flat || !dark || !theta || !centers || !out) return set_error(TCP_EINVAL, "NULL argument");
+    if (ncenter < 1 || ncenter > c->nz) return set_error(TCP_EINVAL, "ncenter=%d outside [1, nz_chunk=%d]", ncenter, c->nz);
+    for (int i = 0; i < ncenter; ++i)
+        if (!(centers[i] >= 0.f && centers[i] <= (float)(c->n - 1)))
+            return set_error(TCP_EINVAL, "centers[%d]=%g outside [0, n-1]", i, (double)centers[i]);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int M = c->M, npair = (ncenter + 1) / 2;
+    if (!c->try_buf) {
+        int rc = dev_alloc((void**)&c->try_buf, (size_t)c->npair * M * sizeof(float2), &c->bytes);
+        if (rc) return rc;
+    }
+    // ptab[pair][k] = S C (e^{+2 pi i k c1/M} + i e^{+2 pi i k c2/M}), k signed, 0 at k = M/2 (build_context's table twice)
+    const double C = kPi / ((double)c->nproj * (double)M);
+    std::vector<float2> pt((size_t)npair * M);
+    for (int p = 0; p < npair; ++p)
+        for (int k = 0; k < M; ++k) {
+            const int ks = (k < M / 2) ? k : k - M;
+            double re = 0.0, im = 0.0;
+            for (int h = 0; h < 2 && 2 * p + h < ncenter; ++h) {
+                const double fr = fmod((double)ks * (double)centers[2 * p + h], (double)M) / (double)M;
+                const double a = 2.0 * kPi * fr, cr = c->scale * C * cos(a), ci = c->scale * C * sin(a);
+                if (h == 0) { re += cr; im += ci; }      // slice A: real part
+                else { re -= ci; im += cr; }             // slice B: times i
+            }
+            pt[(size_t)p * M + k] = (k == M / 2) ? make_float2(0.f, 0.f) : make_float2((float)re, (float)im);
+        }
+    TCP_CUDA_CHECK(cudaMemcpyAsync(c->try_buf, pt.data(), pt.size() * sizeof(float2), cudaMemcpyHostToDevice, st));
+    int rc;
+    tcp_ctx one = *c;                 // the single input slice
+    one.nz = 1; one.npair = 1;
+    if ((rc = launch_trig(c, theta, st))) return rc;
+    if ((rc = launch_normalize(&one, raw, flat, dark, st))) return rc;
+    tcp_ctx t = *c;                   // ncenter output "slices"
+    t.nz = ncenter; t.npair = npair; t.try_ptab = c->try_buf;
+    t.tcfft = 0;
+    if ((rc = launch_rows(&t, st))) return rc;
+    if (c->grid_impl == TCP_GRID_SCATTER_ATOMIC) rc = launch_grid_scatter(&t, st);
+    else if (c->grid_impl == TCP_GRID_GATHER) rc = launch_grid_gather(&t, theta, st);
+    else rc = launch_grid_tile(&t, theta, st);
+    if (rc) return rc;
+    if ((rc = launch_ifft_cols(&t, st))) return rc;
+    return launch_ifft_rows(&t, out, st);
 }
 
 int tcp_profile_collect(tcp_ctx* c, double* ms_sum, int* ncalls) {

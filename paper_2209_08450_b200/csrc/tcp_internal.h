@@ -29,6 +29,8 @@ struct tcp_ctx {
     float2* tw;           // [M] e^{-2 pi i t / M}
     float* hfilt;         // [M] H[k] / M
     float2* ptab;         // [M] S * C * e^{+2 pi i k c / M}, k signed; 0 at k = M/2
+    float2* try_ptab;     // tcp_recon_try: [npair][M] two-centre phase tables (NULL outside a try call's context copy)
+    float2* try_buf;      // its device storage, [ceil(nz/2)][M], allocated on first use
     float* deax;          // [n] 1 / (S * Phi(x))
     float* deay;          // [n] 1 / Phi(y)
     void* tc_amat;        // tcfft.cuh: DFT-64 matrix, 128 x 128 half in operand block order

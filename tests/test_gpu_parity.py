@@ -196,6 +196,40 @@ def test_filters_and_offcentre(filt):
         assert rl2(out[z], ref[z]) < FP32_GATE
 
 
+@pytest.mark.parametrize("dtype", ["f32", "f16"])
+def test_centre_try_mode(dtype):
+    """tcp_recon_try: one slice, several candidate centres in one call.  Entry i must equal the
+    oracle's reconstruction of that slice with centre centers[i] (odd count: the last pair carries one
+    centre; non-integer centres included), and an out-of-range centre or count is refused."""
+    tcp = _tcp()
+    w = sg.make_workload("C1")
+    raw, flat, dark, theta = _inputs(w, [4])
+    centers = [61.0, 64.0, 66.5, 63.25, 70.0]
+    r = tcp.Recon(w.n, w.nproj, 8, w.center, dtype, w.filter, 3)
+    d = _to_dev(raw, flat, dark, theta)
+    out = r.recon_try(d[0], d[1], d[2], d[3], centers)
+    torch.cuda.synchronize()
+    out = out.float().cpu().numpy()
+    assert out.shape == (len(centers), w.n, w.n)
+    for i, c in enumerate(centers):
+        ref = orc.recon(raw, flat, dark, theta, c, w.filter, 3, "grid")[0]
+        if dtype == "f32":
+            assert rl2(out[i], ref) < FP32_GATE, (c, rl2(out[i], ref))
+        else:
+            assert rl2(out[i], ref) < FP16_GATE_L2, (c, rl2(out[i], ref))
+            assert np.abs(out[i] - ref).max() / np.abs(ref).max() < FP16_GATE_MAX
+    # the context still reconstructs chunks afterwards (the try tables are per call)
+    raw8, flat8, dark8, _ = _inputs(w, list(range(8)))
+    full = r.recon(*_to_dev(raw8, flat8, dark8, theta)).float().cpu().numpy()
+    ref8 = orc.recon(raw8[:, 4:5], flat8[4:5], dark8[4:5], theta, w.center, w.filter, 3, "grid")[0]
+    assert rl2(full[4], ref8) < (FP32_GATE if dtype == "f32" else FP16_GATE_L2)
+    with pytest.raises(tcp.TcpError):
+        r.recon_try(d[0], d[1], d[2], d[3], [float(w.n)])
+    with pytest.raises(tcp.TcpError):
+        r.recon_try(d[0], d[1], d[2], d[3], [64.0] * 9)
+    r.close()
+
+
 def test_mean_frames_and_errors():
     tcp = _tcp()
     rng = np.random.default_rng(0)
