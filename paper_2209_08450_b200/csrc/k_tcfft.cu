@@ -1,11 +1,8 @@
-// k_tcfft.cu -- the three transform kernels of the fp16-storage path at M = 4096 (config C4) on the
-// tensor cores (tcfft.cuh): same stages, inputs, outputs and layouts as k_rows.cu / k_ifft2.cu, which
-// stay the path for every other size and for fp32 storage.
-//   rows_tc_kernel       S3 + S4: zero-pad, FFT, x H/M, IFFT, crop, zero-pad, FFT, x S C e^{2 pi i k c/M}
-//   ifft_cols_tc_kernel  S6 pass 1 over the strip-major grid, pruned to the central n rows
-//   ifft_rows_tc_kernel  S6 pass 2 + S7: pruned to the central n columns, deapodise, crop, cast
-// (PAPER.md:57-61, :173, :300).  CTAs are persistent (the 64 KB of tables are loaded once per CTA);
-// every group of 128 threads walks batches of NB lines.
+// k_tcfft.cu -- row pass of the inverse 2D transform (S6 pass 2 + S7) for fp16 storage at M = 4096
+// (config C4) as DFT-as-GEMM on the tensor cores (tcfft.cuh): same input, output and layout as
+// ifft_rows_kernel (k_ifft2.cu).  Opt-in through TCP_OPT_TCFFT: it is parity-green but measured slower
+// than the Stockham kernel (profiles/r1_tcfft.md).  (PAPER.md:61, :173, :300.)
+// CTAs are persistent (the 32 KB matrix is loaded once per CTA); every group of 128 threads walks lines.
 #include "tcfft.cuh"
 #include "tcp_internal.h"
 
