@@ -53,7 +53,13 @@ enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1, TCP_GRID_TILE = 2, TCP_
 /* TCP_OPT_TCFFT: bit mask of the transforms run as DFT-as-GEMM on the tensor cores (fp16 storage and
  * M = 4096 only; elsewhere the option must be 0): 1 = detector-row kernel (S3 + S4), 2 = column pass,
  * 4 = row pass of the inverse 2D transform.  Default: all that apply. */
-enum { TCP_OPT_GRID_IMPL = 0, TCP_OPT_PROFILE = 1, TCP_OPT_TCFFT = 2 };
+/* TCP_OPT_ALGORITHM ("--reconstruction-algorithm"): TCP_ALG_FOURIER = FourierRec, the
+ * gridding path this library is about (default); TCP_ALG_LINE = LineRec, direct line summation with linear
+ * interpolation (O(N^4)): S1-S3 as before, then the backprojection sum per pixel.
+ * After a LINE reconstruction TCP_WS_SINOGRAM holds the FILTERED sinogram.  tcp_recon and
+ * tcp_recon_volume_host follow the option; tcp_recon_try is FourierRec only. */
+enum { TCP_OPT_GRID_IMPL = 0, TCP_OPT_PROFILE = 1, TCP_OPT_TCFFT = 2, TCP_OPT_ALGORITHM = 3 };
+enum { TCP_ALG_FOURIER = 0, TCP_ALG_LINE = 1 };
 enum { TCP_TCFFT_ROWS = 1, TCP_TCFFT_COLS = 2, TCP_TCFFT_IROWS = 4 };
 /* stages timed when TCP_OPT_PROFILE is on, in launch order */
 enum { TCP_ST_TRIG = 0, TCP_ST_NORMALIZE = 1, TCP_ST_ROWS = 2, TCP_ST_GRID = 3, TCP_ST_IFFT_COLS = 4,

@@ -58,6 +58,78 @@ __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict
         });
 }
 
+// S3 alone, for the line-summation operator (k_line.cu): the same two transforms, the cropped filtered
+// rows written back over the two sinogram rows they came from (each CTA reads its rows completely before
+// the first pass ends and writes them in the last pass of the inverse transform).
+template <int M, int ROWS, class TS>
+__global__ void __launch_bounds__(ROWS* M / 16) filter_kernel(TS* __restrict__ sino, const float2* __restrict__ tw,
+                                                              const float* __restrict__ hfilt, int nproj, int nz) {
+    constexpr int n = M / 2;
+    constexpr int TG = M / 16;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / TG;
+    const int tid = threadIdx.x % TG;
+    float2* s = smem + (size_t)g * padded_len(M);
+    int j = blockIdx.x * ROWS + g;
+    const bool live = j < nproj;
+    if (!live) j = nproj - 1;
+    const int pair = blockIdx.y;
+    const int zA = 2 * pair, zB = 2 * pair + 1;
+    const bool hasB = zB < nz;
+    TS* pA = sino + ((size_t)zA * nproj + j) * n;
+    TS* pB = sino + ((size_t)(hasB ? zB : zA) * nproj + j) * n;
+    fft_line<M, false>(
+        s, tid, tw,
+        [&](int i) {
+            if (i < n) return make_float2(ld_r(pA, i), hasB ? ld_r(pB, i) : 0.f);
+            return make_float2(0.f, 0.f);
+        },
+        [&](int k, float2 v) {
+            const float h = __ldg(&hfilt[k]);
+            s[pad_idx(k)] = make_float2(v.x * h, v.y * h);
+        });
+    __syncthreads();
+    fft_line<M, true>(
+        s, tid, tw, [&](int i) { return s[pad_idx(i)]; },
+        [&](int i, float2 v) {
+            if (live && i < n) {
+                st_r(pA, i, v.x);
+                if (hasB) st_r(pB, i, v.y);
+            }
+        });
+}
+
+template <int M, class TS>
+static int launch_filter_t(const tcp_ctx* c, cudaStream_t st) {
+    constexpr int TG = M / 16;
+    constexpr int ROWS = (TG >= 128) ? 1 : 128 / TG;
+    const size_t smem = (size_t)ROWS * padded_len(M) * sizeof(float2);
+    auto kern = filter_kernel<M, ROWS, TS>;
+    TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    dim3 grid((c->nproj + ROWS - 1) / ROWS, c->npair);
+    kern<<<grid, ROWS * TG, smem, st>>>((TS*)c->sino, c->tw, c->hfilt, c->nproj, c->nz);
+    TCP_CUDA_CHECK(cudaGetLastError());
+    return TCP_OK;
+}
+
+template <int M>
+static int launch_filter_m(const tcp_ctx* c, cudaStream_t st) {
+    return c->half_store ? launch_filter_t<M, __half>(c, st) : launch_filter_t<M, float>(c, st);
+}
+
+int launch_filter(const tcp_ctx* c, cudaStream_t st) {
+    switch (c->M) {
+        case 128: return launch_filter_m<128>(c, st);
+        case 256: return launch_filter_m<256>(c, st);
+        case 512: return launch_filter_m<512>(c, st);
+        case 1024: return launch_filter_m<1024>(c, st);
+        case 2048: return launch_filter_m<2048>(c, st);
+        case 4096: return launch_filter_m<4096>(c, st);
+        case 8192: return launch_filter_m<8192>(c, st);
+    }
+    return set_error(TCP_EUNSUPPORTED, "unsupported M=%d", c->M);
+}
+
 template <int M, class TS, class TC>
 static int launch_rows_t(const tcp_ctx* c, cudaStream_t st) {
     constexpr int TG = M / 16;

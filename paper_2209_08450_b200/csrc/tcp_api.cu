@@ -250,6 +250,15 @@ int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* d
     TCP_MARK(1);
     if ((rc = launch_normalize(c, raw, flat, dark, st))) return rc;
     TCP_MARK(2);
+    if (c->algorithm == TCP_ALG_LINE) {       // LineRec: filter (timed as "rows"), backprojection (timed as "grid")
+        if ((rc = launch_filter(c, st))) return rc;
+        TCP_MARK(3);
+        if ((rc = launch_line_bp(c, out, st))) return rc;
+        TCP_MARK(4);
+        TCP_MARK(5);
+        TCP_MARK(6);
+        return TCP_OK;
+    }
     if ((rc = launch_rows(c, st))) return rc;
     TCP_MARK(3);
     if (c->grid_impl == TCP_GRID_SCATTER_ATOMIC) rc = launch_grid_scatter(c, st);
@@ -268,6 +277,7 @@ int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* d
 int tcp_recon_try(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* dark, const float* theta,
                   const float* centers, int ncenter, void* out, tcp_stream_t stream) {
     if (!c || !raw || !flat || !dark || !theta || !centers || !out) return set_error(TCP_EINVAL, "NULL argument");
+    if (c->algorithm != TCP_ALG_FOURIER) return set_error(TCP_EUNSUPPORTED, "tcp_recon_try is FourierRec only");
     if (ncenter < 1 || ncenter > c->nz) return set_error(TCP_EINVAL, "ncenter=%d outside [1, nz_chunk=%d]", ncenter, c->nz);
     for (int i = 0; i < ncenter; ++i)
         if (!(centers[i] >= 0.f && centers[i] <= (float)(c->n - 1)))
@@ -330,6 +340,7 @@ int tcp_profile_collect(tcp_ctx* c, double* ms_sum, int* ncalls) {
 
 int tcp_launches_per_recon(const tcp_ctx* c) {
     if (!c) return 0;
+    if (c->algorithm == TCP_ALG_LINE) return 4;                          // trig, normalise, filter, backprojection
     if (c->grid_impl == TCP_GRID_TILE || c->grid_impl == TCP_GRID_MMA) return 7 + (c->g_nred ? 1 : 0);   // + plan (+ reduce)
     return c->grid_impl == TCP_GRID_SCATTER_ATOMIC ? 6 : 6;              // (scatter adds a memset, not a kernel)
 }
@@ -374,6 +385,11 @@ int tcp_set_option(tcp_ctx* c, int option, int value) {
         if (value == TCP_GRID_MMA && !c->half_store) return set_error(TCP_EUNSUPPORTED, "tensor-core gridding needs fp16 storage");
         c->grid_impl = value;
         c->grid_strip = (value == TCP_GRID_MMA) ? cols_strip_width(c->M) : 0;
+        return TCP_OK;
+    }
+    if (option == TCP_OPT_ALGORITHM) {
+        if (value != TCP_ALG_FOURIER && value != TCP_ALG_LINE) return set_error(TCP_EINVAL, "unknown algorithm %d", value);
+        c->algorithm = value;
         return TCP_OK;
     }
     if (option == TCP_OPT_TCFFT) {

@@ -14,6 +14,7 @@ struct tcp_ctx {
     bool half_out;        // out in half (TCP_F16)
     double scale;         // power-of-two scale S of SPECTRUM / GRID / PASS1 (1 in fp32)
     int grid_impl;
+    int algorithm;        // TCP_ALG_FOURIER (gridding, default) | TCP_ALG_LINE (direct line summation)
     int grid_strip;       // 0: grid rows are contiguous; W > 0: strip-major [pair][M/W][M l2][W l1] (tcgen05 gridding)
     int device, nsm;      // CUDA device and its SM count
     int tcfft;            // TCP_TCFFT_* mask of transforms on the tensor cores (k_tcfft.cu)
@@ -69,6 +70,8 @@ int launch_trig(const tcp_ctx* c, const float* theta, cudaStream_t st);
 int launch_normalize(const tcp_ctx* c, const uint16_t* raw, const float* flat, const float* dark,
                      cudaStream_t st);
 int launch_rows(const tcp_ctx* c, cudaStream_t st);
+int launch_filter(const tcp_ctx* c, cudaStream_t st);
+int launch_line_bp(const tcp_ctx* c, void* out, cudaStream_t st);
 int launch_grid_scatter(const tcp_ctx* c, cudaStream_t st);
 int launch_grid_gather(const tcp_ctx* c, const float* theta, cudaStream_t st);
 int launch_grid_tile(const tcp_ctx* c, const float* theta, cudaStream_t st);
