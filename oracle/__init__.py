@@ -103,12 +103,15 @@ def filter_table(M, filt="ramp"):
     return H
 
 
-def filter_rows(p, filt="ramp"):
-    """p [rows][n] -> q [rows][n]  (S3)."""
+PADS = {"zero": 0, "edge": 1}
+
+
+def filter_rows(p, filt="ramp", pad="zero"):
+    """p [rows][n] -> q [rows][n]  (S3); pad: "zero" (default) or "edge"."""
     p = _f64(p)
     rows, n = p.shape
     q = np.empty_like(p)
-    lib().orc_filter_rows(_p(p), C.c_int(rows), C.c_int(n), C.c_int(FILTERS[filt]), _p(q))
+    lib().orc_filter_rows_pad(_p(p), C.c_int(rows), C.c_int(n), C.c_int(FILTERS[filt]), C.c_int(PADS[pad]), _p(q))
     return q
 
 
@@ -204,26 +207,26 @@ def deapod_crop_adjoint(f, n, m=DEFAULT_M):
     return g
 
 
-def fbp_from_sino(p, theta, center, filt="ramp", m=DEFAULT_M, method="grid", return_q=False):
+def fbp_from_sino(p, theta, center, filt="ramp", m=DEFAULT_M, method="grid", return_q=False, pad="zero"):
     """p f64 [nz][nproj][n] -> out f64 [nz][n][n] (S3..S7 or the two definitions)."""
     p = _f64(p)
     theta = _f32(theta)
     nz, nproj, n = p.shape
     out = np.empty((nz, n, n))
     q = np.empty_like(p) if return_q else None
-    lib().orc_fbp_from_sino(_p(p), _p(theta), C.c_int(nproj), C.c_int(nz), C.c_int(n),
-                            C.c_double(center), C.c_int(FILTERS[filt]), C.c_int(m),
+    lib().orc_fbp_from_sino_pad(_p(p), _p(theta), C.c_int(nproj), C.c_int(nz), C.c_int(n),
+                            C.c_double(center), C.c_int(FILTERS[filt]), C.c_int(PADS[pad]), C.c_int(m),
                             C.c_int(METHODS[method]), _p(out), _p(q) if return_q else None)
     return (out, q) if return_q else out
 
 
-def recon(raw, flat, dark, theta, center, filt="ramp", m=DEFAULT_M, method="grid"):
+def recon(raw, flat, dark, theta, center, filt="ramp", m=DEFAULT_M, method="grid", pad="zero"):
     """uint16 counts -> reconstruction, S1..S7.  raw [nproj][nz][n] -> out [nz][n][n]."""
     raw = np.ascontiguousarray(raw, dtype=np.uint16)
     nproj, nz, n = raw.shape
     flat, dark, theta = _f32(flat), _f32(dark), _f32(theta)
     out = np.empty((nz, n, n))
-    lib().orc_recon(_p(raw), _p(flat), _p(dark), _p(theta), C.c_int(nproj), C.c_int(nz), C.c_int(n),
-                    C.c_double(center), C.c_int(FILTERS[filt]), C.c_int(m), C.c_int(METHODS[method]),
+    lib().orc_recon_pad(_p(raw), _p(flat), _p(dark), _p(theta), C.c_int(nproj), C.c_int(nz), C.c_int(n),
+                    C.c_double(center), C.c_int(FILTERS[filt]), C.c_int(PADS[pad]), C.c_int(m), C.c_int(METHODS[method]),
                     _p(out))
     return out

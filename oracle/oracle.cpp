@@ -147,8 +147,15 @@ void orc_filter(int M, int filter, double* H) {
 // M = 2n ("one-dimensional filtering"; padding PAPER.md:59, :173).
 //   a = [p, 0];  P = FFT(a);  Q = P H;  q = IFFT(Q)/M, kept for 0 <= i < n.
 // p, q: [rows][n].
+// pad = 1 ("edge"; padding for "samples not fitting into the detector field
+// of view"): the n padding samples repeat the nearest detector edge of the periodic length-M row,
+//   a[i] = p[n-1] for n <= i < n + n/2,  a[i] = p[0] for n + n/2 <= i < M   (pad = 0: zeros, the default).
 // ---------------------------------------------------------------------------
+void orc_filter_rows_pad(const double* p, int rows, int n, int filter, int pad, double* q);
 void orc_filter_rows(const double* p, int rows, int n, int filter, double* q) {
+    orc_filter_rows_pad(p, rows, n, filter, 0, q);
+}
+void orc_filter_rows_pad(const double* p, int rows, int n, int filter, int pad, double* q) {
     const int M = 2 * n;
     std::vector<double> H(M);
     orc_filter(M, filter, H.data());
@@ -157,7 +164,8 @@ void orc_filter_rows(const double* p, int rows, int n, int filter, double* q) {
         std::vector<cplx> a(M), P(M), b(M);
 #pragma omp for schedule(static)
         for (int r = 0; r < rows; ++r) {
-            for (int i = 0; i < M; ++i) a[i] = (i < n) ? p[(size_t)r * n + i] : 0.0;
+            const double* pr = p + (size_t)r * n;
+            for (int i = 0; i < M; ++i) a[i] = (i < n) ? pr[i] : (pad == 0 ? 0.0 : (i < n + n / 2 ? pr[n - 1] : pr[0]));
             orc_fft(a.data(), P.data(), M, -1);
             for (int k = 0; k < M; ++k) P[k] *= H[k];
             orc_fft(P.data(), b.data(), M, +1);

@@ -23,6 +23,7 @@ extern "C" {
 void orc_fft(const cplx* x, cplx* X, int N, int sign);
 void orc_neglog(const uint16_t*, const float*, const float*, int, int, int, double*);
 void orc_filter_rows(const double*, int, int, int, double*);
+void orc_filter_rows_pad(const double*, int, int, int, int, double*);
 void orc_spectrum(const double*, int, int, double, cplx*);
 
 // Gaussian gridding kernel phi(t) = exp(-alpha t^2), alpha = pi / (sqrt(2) m)   (reading Q7),
@@ -236,14 +237,21 @@ void orc_backproject_grid(const cplx* G, const float* theta, int nproj, int n, i
 // p[nz][nproj][n] (sinogram after -log) -> out[nz][n][n];  q_out (filtered sinogram,
 // [nz][nproj][n]) is written when not NULL.  Slices are independent.
 // ---------------------------------------------------------------------------
+void orc_fbp_from_sino_pad(const double* p, const float* theta, int nproj, int nz, int n, double center, int filter,
+                           int pad, int m, int method, double* out, double* q_out);
 void orc_fbp_from_sino(const double* p, const float* theta, int nproj, int nz, int n,
                        double center, int filter, int m, int method, double* out, double* q_out) {
+    orc_fbp_from_sino_pad(p, theta, nproj, nz, n, center, filter, 0, m, method, out, q_out);
+}
+// pad: padding of the filter stage (orc_filter_rows_pad): 0 zeros, 1 edge values
+void orc_fbp_from_sino_pad(const double* p, const float* theta, int nproj, int nz, int n, double center, int filter,
+                           int pad, int m, int method, double* out, double* q_out) {
     const int M = 2 * n;
     // nested parallelism is off by default, so the inner pragmas run serially here
 #pragma omp parallel for schedule(dynamic, 1) if (method != 1)
     for (int z = 0; z < nz; ++z) {
         std::vector<double> q((size_t)nproj * n);
-        orc_filter_rows(p + (size_t)z * nproj * n, nproj, n, filter, q.data());
+        orc_filter_rows_pad(p + (size_t)z * nproj * n, nproj, n, filter, pad, q.data());
         if (q_out) std::memcpy(q_out + (size_t)z * nproj * n, q.data(), sizeof(double) * q.size());
         double* f = out + (size_t)z * n * n;
         if (method == 2) {
@@ -263,6 +271,12 @@ void orc_recon(const uint16_t* raw, const float* flat, const float* dark, const 
     std::vector<double> p((size_t)nz * nproj * n);
     orc_neglog(raw, flat, dark, nproj, nz, n, p.data());
     orc_fbp_from_sino(p.data(), theta, nproj, nz, n, center, filter, m, method, out, nullptr);
+}
+void orc_recon_pad(const uint16_t* raw, const float* flat, const float* dark, const float* theta, int nproj, int nz, int n,
+                   double center, int filter, int pad, int m, int method, double* out) {
+    std::vector<double> p((size_t)nz * nproj * n);
+    orc_neglog(raw, flat, dark, nproj, nz, n, p.data());
+    orc_fbp_from_sino_pad(p.data(), theta, nproj, nz, n, center, filter, pad, m, method, out, nullptr);
 }
 
 }  // extern "C"

@@ -117,6 +117,58 @@ def test_p3_filter_rows_is_linear_convolution_with_kernel():
             assert q[r, i] == pytest.approx(ref, abs=1e-13)
 
 
+def test_p3_edge_padding_constant_row_and_convolution():
+    """Edge padding.  (a) A constant row becomes a constant periodic signal, so
+    only the DC bin survives: q = c R[0] with R[0] = 1/4 - 2 sum_{odd i < M/2} 1/(pi^2 i^2) (the kernel's sum,
+    written out here; it is the tail 2 sum_{odd i > M/2} 1/(pi^2 i^2) > 0 because the full odd series is 1/4).
+    With zero padding the same row rings at the detector edges.  (b) In general the filtered row is the
+    circular convolution of the closed-form kernel with the edge-extended row."""
+    n, M = 32, 64
+    c = 2.5
+    q = orc.filter_rows(np.full((1, n), c), "ramp", pad="edge")[0]
+    r0 = 0.25 - 2.0 * sum(1.0 / (np.pi ** 2 * i * i) for i in range(1, M // 2, 2))
+    assert 0 < r0 < 1.0 / M
+    assert np.abs(q - c * r0).max() < 1e-14
+    qz = orc.filter_rows(np.full((1, n), c), "ramp", pad="zero")[0]
+    assert qz[0] > 10 * c * r0 and qz[n // 2] < qz[0]               # zero padding: truncation edge response
+    # (b) brute force with the closed-form kernel h[0] = 1/4, h[d] = -1/(pi^2 d^2) for odd d, 0 for even d
+    rng = np.random.default_rng(11)
+    p = rng.standard_normal((2, n))
+    q = orc.filter_rows(p, "ramp", pad="edge")
+    # minus the zeroed Nyquist bin (reading Q4): R[M/2] (-1)^d / M with R[M/2] = sum_d h[d] (-1)^d
+    r_nyq = 0.25 + 2.0 * sum(1.0 / (np.pi ** 2 * i * i) for i in range(1, M // 2, 2))
+    def h(d):
+        d = abs(((d + M // 2) % M) - M // 2)                        # wrapped distance, |d| <= M/2
+        k = 0.25 if d == 0 else (-1.0 / (np.pi ** 2 * d * d) if d % 2 == 1 else 0.0)
+        return k - r_nyq * (-1.0) ** d / M
+    for r in range(2):
+        a = np.concatenate([p[r], np.full(n // 2, p[r, -1]), np.full(n // 2, p[r, 0])])
+        for i in (0, 5, n - 1):
+            ref = sum(a[j] * h(i - j) for j in range(M))
+            assert q[r, i] == pytest.approx(ref, abs=1e-13)
+    # zero padding is unchanged by the new argument
+    assert np.array_equal(orc.filter_rows(p, "ramp"), orc.filter_rows(p, "ramp", pad="zero"))
+
+
+def test_p5_edge_padding_object_outside_field_of_view():
+    """What edge padding is for: a disc wider than the detector.  Inside the field of view the
+    zero-padded reconstruction shows the well-known bright rim ("cupping") towards the detector edge; edge
+    padding, which continues the row at its edge value instead of dropping it to zero, at least halves it
+    (it over-corrects slightly: the true profile keeps falling beyond the edge)."""
+    n, nproj, mu = 64, 96, 0.01
+    theta = sg.make_theta(nproj)
+    s = np.arange(n) - n / 2
+    p = np.tile((2 * mu * np.sqrt(np.maximum(48.0 ** 2 - s ** 2, 0.0)))[None, None, :], (1, nproj, 1))   # radius 48 > n/2
+    fz = orc.fbp_from_sino(p, theta, n / 2, "ramp", 4, "exact", pad="zero")[0]
+    fe = orc.fbp_from_sino(p, theta, n / 2, "ramp", 4, "exact", pad="edge")[0]
+    xs = np.arange(n) - n // 2
+    X, Y = np.meshgrid(xs, xs)
+    inner, rim = (X ** 2 + Y ** 2) < 10 ** 2, ((X ** 2 + Y ** 2) > 24 ** 2) & ((X ** 2 + Y ** 2) < 28 ** 2)
+    cup_z, cup_e = fz[rim].mean() - fz[inner].mean(), fe[rim].mean() - fe[inner].mean()
+    assert cup_z > 0.2 * mu                 # zero padding: rim brighter than the centre by a good fraction of mu
+    assert abs(cup_e) < 0.5 * cup_z         # edge padding: less than half of it left (measured 0.45)
+
+
 # ---------------------------------------------------------------- P4: plane wave
 @pytest.mark.parametrize("m", [3, 4, 5])
 def test_p4_plane_wave(m):
