@@ -58,7 +58,12 @@ enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1, TCP_GRID_TILE = 2, TCP_
  * interpolation (O(N^4)): S1-S3 as before, then the backprojection sum per pixel.
  * After a LINE reconstruction TCP_WS_SINOGRAM holds the FILTERED sinogram.  tcp_recon and
  * tcp_recon_volume_host follow the option; tcp_recon_try is FourierRec only. */
-enum { TCP_OPT_GRID_IMPL = 0, TCP_OPT_PROFILE = 1, TCP_OPT_TCFFT = 2, TCP_OPT_ALGORITHM = 3 };
+/* TCP_OPT_PAD: the n padding samples of the filter stage S3 (the padding "allows for
+ * suppressing artifacts when processing samples not fitting into the detector field of view"):
+ * TCP_PAD_ZERO (default, the reading of north_star) or TCP_PAD_EDGE = the nearest detector edge value of
+ * the periodic length-2n row (p[n-1] for n <= i < 3n/2, p[0] after).  Stage S4 always zero-pads. */
+enum { TCP_OPT_GRID_IMPL = 0, TCP_OPT_PROFILE = 1, TCP_OPT_TCFFT = 2, TCP_OPT_ALGORITHM = 3, TCP_OPT_PAD = 4 };
+enum { TCP_PAD_ZERO = 0, TCP_PAD_EDGE = 1 };
 enum { TCP_ALG_FOURIER = 0, TCP_ALG_LINE = 1 };
 enum { TCP_TCFFT_ROWS = 1, TCP_TCFFT_COLS = 2, TCP_TCFFT_IROWS = 4 };
 /* stages timed when TCP_OPT_PROFILE is on, in launch order */

@@ -178,6 +178,10 @@ class Recon:
     def set_grid_impl(self, name: str):
         _check(lib().tcp_set_option(self.h, 0, GRID_IMPLS[name]))
 
+    def set_pad(self, name: str):
+        """TCP_OPT_PAD: "zero" (default) or "edge" padding of the filter stage."""
+        _check(lib().tcp_set_option(self.h, 4, {"zero": 0, "edge": 1}[name]))
+
     def set_algorithm(self, name: str):
         """TCP_OPT_ALGORITHM: "fourier" (FourierRec, default) or "line" (LineRec, direct line summation)."""
         _check(lib().tcp_set_option(self.h, 3, {"fourier": 0, "line": 1}[name]))

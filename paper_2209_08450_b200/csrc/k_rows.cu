@@ -13,7 +13,7 @@ template <int M, int ROWS, class TS, class TC>
 __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict__ sino, TC* __restrict__ spec,
                                                             const float2* __restrict__ tw,
                                                             const float* __restrict__ hfilt,
-                                                            const float2* __restrict__ ptab, int nproj, int nz, int try_mode) {
+                                                            const float2* __restrict__ ptab, int nproj, int nz, int try_mode, int pad_edge) {
     constexpr int n = M / 2;
     constexpr int TG = M / 16;
     extern __shared__ float2 smem[];
@@ -36,8 +36,12 @@ __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict
     fft_line<M, false>(
         s, tid, tw,
         [&](int i) {
-            if (i < n) return make_float2(ld_r(pA, i), hasB ? ld_r(pB, i) : 0.f);
-            return make_float2(0.f, 0.f);
+            // padding samples: zeros, or (TCP_OPT_PAD = TCP_PAD_EDGE) the nearest edge of the periodic row
+            if (i >= n) {
+                if (!pad_edge) return make_float2(0.f, 0.f);
+                i = (i < n + n / 2) ? n - 1 : 0;
+            }
+            return make_float2(ld_r(pA, i), hasB ? ld_r(pB, i) : 0.f);
         },
         [&](int k, float2 v) {
             const float h = __ldg(&hfilt[k]);
@@ -63,7 +67,7 @@ __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict
 // the first pass ends and writes them in the last pass of the inverse transform).
 template <int M, int ROWS, class TS>
 __global__ void __launch_bounds__(ROWS* M / 16) filter_kernel(TS* __restrict__ sino, const float2* __restrict__ tw,
-                                                              const float* __restrict__ hfilt, int nproj, int nz) {
+                                                              const float* __restrict__ hfilt, int nproj, int nz, int pad_edge) {
     constexpr int n = M / 2;
     constexpr int TG = M / 16;
     extern __shared__ float2 smem[];
@@ -81,8 +85,12 @@ __global__ void __launch_bounds__(ROWS* M / 16) filter_kernel(TS* __restrict__ s
     fft_line<M, false>(
         s, tid, tw,
         [&](int i) {
-            if (i < n) return make_float2(ld_r(pA, i), hasB ? ld_r(pB, i) : 0.f);
-            return make_float2(0.f, 0.f);
+            // padding samples: zeros, or (TCP_OPT_PAD = TCP_PAD_EDGE) the nearest edge of the periodic row
+            if (i >= n) {
+                if (!pad_edge) return make_float2(0.f, 0.f);
+                i = (i < n + n / 2) ? n - 1 : 0;
+            }
+            return make_float2(ld_r(pA, i), hasB ? ld_r(pB, i) : 0.f);
         },
         [&](int k, float2 v) {
             const float h = __ldg(&hfilt[k]);
@@ -107,7 +115,7 @@ static int launch_filter_t(const tcp_ctx* c, cudaStream_t st) {
     auto kern = filter_kernel<M, ROWS, TS>;
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid((c->nproj + ROWS - 1) / ROWS, c->npair);
-    kern<<<grid, ROWS * TG, smem, st>>>((TS*)c->sino, c->tw, c->hfilt, c->nproj, c->nz);
+    kern<<<grid, ROWS * TG, smem, st>>>((TS*)c->sino, c->tw, c->hfilt, c->nproj, c->nz, c->pad);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }
@@ -139,7 +147,7 @@ static int launch_rows_t(const tcp_ctx* c, cudaStream_t st) {
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid((c->nproj + ROWS - 1) / ROWS, c->npair);
     kern<<<grid, ROWS * TG, smem, st>>>((const TS*)c->sino, (TC*)c->spec, c->tw, c->hfilt, c->try_ptab ? c->try_ptab : c->ptab, c->nproj, c->nz,
-                                       c->try_ptab ? 1 : 0);
+                                       c->try_ptab ? 1 : 0, c->pad);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }

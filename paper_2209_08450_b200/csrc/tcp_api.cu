@@ -387,6 +387,11 @@ int tcp_set_option(tcp_ctx* c, int option, int value) {
         c->grid_strip = (value == TCP_GRID_MMA) ? cols_strip_width(c->M) : 0;
         return TCP_OK;
     }
+    if (option == TCP_OPT_PAD) {
+        if (value != TCP_PAD_ZERO && value != TCP_PAD_EDGE) return set_error(TCP_EINVAL, "unknown padding %d", value);
+        c->pad = value;
+        return TCP_OK;
+    }
     if (option == TCP_OPT_ALGORITHM) {
         if (value != TCP_ALG_FOURIER && value != TCP_ALG_LINE) return set_error(TCP_EINVAL, "unknown algorithm %d", value);
         c->algorithm = value;

@@ -260,6 +260,34 @@ def test_line_summation_operator(dtype, cfg, scale, nz):
     r.close()
 
 
+@pytest.mark.parametrize("dtype,alg", [("f32", "fourier"), ("f16", "fourier"), ("f32", "line")])
+def test_edge_padding(dtype, alg):
+    """TCP_OPT_PAD = edge against the oracle with pad="edge", on rows whose edge values are far
+    from zero (C1 counts with the centre pushed off so the phantom touches the detector edge), for both
+    backprojection operators; and back to zero padding on the same context."""
+    tcp = _tcp()
+    w = sg.make_workload("C1")
+    w.center = 40.0
+    raw, flat, dark, theta = _inputs(w, [2, 3, 4])
+    r = tcp.Recon(w.n, w.nproj, 3, w.center, dtype, w.filter, 3)
+    r.set_pad("edge")
+    r.set_algorithm(alg)
+    dev = _to_dev(raw, flat, dark, theta)
+    out = r.recon(*dev).float().cpu().numpy()
+    method = "grid" if alg == "fourier" else "lin"
+    ref = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, method, pad="edge")
+    refz = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, method)
+    assert rl2(ref[1], refz[1]) > 1e-2                       # the option matters on this input
+    gate = FP32_GATE if dtype == "f32" else FP16_GATE_L2
+    for z in range(3):
+        assert rl2(out[z], ref[z]) < gate, (z, rl2(out[z], ref[z]))
+    r.set_pad("zero")
+    outz = r.recon(*dev).float().cpu().numpy()
+    for z in range(3):
+        assert rl2(outz[z], refz[z]) < gate
+    r.close()
+
+
 def test_mean_frames_and_errors():
     tcp = _tcp()
     rng = np.random.default_rng(0)
