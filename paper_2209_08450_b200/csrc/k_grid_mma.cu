@@ -114,6 +114,7 @@ __global__ void __launch_bounds__(NTHR, 2)
     const int cl = lane;                                     // column of the step
     uint32_t nstep = 0;                                      // K steps issued by this warp
     const size_t pstride = (size_t)nproj * M;                // elements between slice-pair planes of the spectrum
+    const size_t pstride_b = pstride * sizeof(__half2);
     const __half2* plane0 = spec + (size_t)(pg * NPG) * pstride;                  // first plane of this pair group
     const int nvalid = min(NPG, npair - pg * NPG);                                // planes that exist
 
@@ -167,14 +168,26 @@ __global__ void __launch_bounds__(NTHR, 2)
                 // float-float trig of the source projection
                 const float cxh = __shfl_sync(0xffffffffu, cs.x, h), cxl = __shfl_sync(0xffffffffu, cs.y, h);
                 const float cyh = __shfl_sync(0xffffffffu, cs.z, h), cyl = __shfl_sync(0xffffffffu, cs.w, h);
-                // the column's B row: gather now, store after the previous MMAs released the stage
+                // the column's B row: gather now, store after the previous MMAs released the stage.  Loads are
+                // unconditional (no predicate, no zeroing after the load to wait on): a column past the end of
+                // the step re-reads a valid sample and carries all-zero weights (0 x finite = 0), a plane past
+                // the last pair re-reads the last plane and is dropped by the epilogue.  Byte pointers keep the
+                // per-plane address arithmetic at one 64-bit add.
                 alignas(16) __half2 bv[NPG];
                 {
-                    const __half2* a = plane0 + ((size_t)jj * M + (size_t)(k & (M - 1)));
+                    const unsigned char* a = reinterpret_cast<const unsigned char*>(plane0 + ((size_t)jj * M + (size_t)(k & (M - 1))));
+                    if (nvalid == NPG) {
 #pragma unroll
-                    for (int p = 0; p < NPG; ++p) {
-                        bv[p] = (valid && p < nvalid) ? __ldg(a) : czero<__half2>();
-                        a += pstride;
+                        for (int p = 0; p < NPG; ++p) {
+                            bv[p] = __ldg(reinterpret_cast<const __half2*>(a));
+                            a += pstride_b;
+                        }
+                    } else {
+#pragma unroll
+                        for (int p = 0; p < NPG; ++p) {
+                            bv[p] = __ldg(reinterpret_cast<const __half2*>(a));
+                            if (p + 1 < nvalid) a += pstride_b;
+                        }
                     }
                 }
                 // ---- phase 1: taps of both axes into zeroed rows (x: 16 halves = 32 B, y: 8 halves = 16 B per column).

@@ -74,7 +74,7 @@ def make_workload(name: str, scale: int = 1, dtype: str | None = None) -> Worklo
         "C2": (512, 720, 512, 32, 0.0, 40, (0.02, 0.12), "f32", 30000.0, "poisson", 1),
         "C3": (1024, 1500, 1024, 16, 3.5, 200, (0.01, 0.08), "f16", 30000.0, "gauss0.5%", 1),
         "C4": (2048, 2048, 2048, 32, 0.0, 500, (0.005, 0.06), "f16", 3500.0, "poisson", 10),
-        "C5": (4096, 4000, 256, 4, 17.5, 300, (0.005, 0.06), "f16_out32", 3500.0, "poisson", 10),
+        "C5": (4096, 4000, 256, 32, 17.5, 300, (0.005, 0.06), "f16_out32", 3500.0, "poisson", 10),
     }[name]
     n, nproj, nzt, nzc, coff, cnt, axes, dt, flat, noise, frames = spec
     n, nproj, nzt = n // scale, max(8, nproj // scale), max(2, nzt // scale)

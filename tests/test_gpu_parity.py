@@ -330,7 +330,7 @@ def test_pipeline_host_matches_direct():
 
 
 # ------------------------------------------------------------------ BASELINE full sizes, bench launch configuration
-@pytest.mark.parametrize("cfg,nz,tcfft", [("C4", 32, 0), ("C4", 32, 4), ("C5", 4, 0)])
+@pytest.mark.parametrize("cfg,nz,tcfft", [("C4", 32, 0), ("C4", 32, 4), ("C5", 32, 0)])
 def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft):
     """C4 (2048^2, 2048 projections, fp16, one 32-slice chunk exactly as bench.py launches it: tcgen05
     gridding with 16 pairs per accumulator group) and C5 (4096^2, 4000 projections, M = 8192, off-centre,
