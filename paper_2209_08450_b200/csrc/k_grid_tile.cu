@@ -68,14 +68,17 @@ __global__ void grid_plan_kernel(const float* __restrict__ theta, int nproj, int
                         const int mid = (lo + hi) >> 1;
                         if (theta[mid] - t0 < a) lo = mid + 1; else hi = mid;
                     }
-                    int cnt = 0;
-                    for (; cnt < nproj; ++cnt) {
-                        int j = lo + cnt;
+                    // window length: first cnt whose projection (theta increasing, + pi after the wrap) leaves
+                    // [a, a + 2 delta]; monotone in cnt, so a second binary search
+                    int clo = 0, chi = nproj;
+                    while (clo < chi) {
+                        const int mid = (clo + chi) >> 1;
+                        int j = lo + mid;
                         float wrapped = 0.f;
                         if (j >= nproj) { j -= nproj; wrapped = PI_F; }
-                        if ((theta[j] - t0) + wrapped - a > 2.f * delta) break;
+                        if ((theta[j] - t0) + wrapped - a > 2.f * delta) chi = mid; else clo = mid + 1;
                     }
-                    out = make_int2(lo % nproj, cnt);
+                    out = make_int2(lo % nproj, clo);
                 }
             }
         }
