@@ -9,11 +9,12 @@
 
 namespace tcpk {
 
-template <int M, int ROWS, class TS, class TC>
+template <int M, int ROWS, bool PAD_EDGE, class TS, class TC>
 __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict__ sino, TC* __restrict__ spec,
                                                             const float2* __restrict__ tw,
                                                             const float* __restrict__ hfilt,
-                                                            const float2* __restrict__ ptab, int nproj, int nz, int try_mode, int pad_edge) {
+                                                            const float2* __restrict__ ptab, int nproj, int nz, int try_mode) {
+    constexpr bool pad_edge = PAD_EDGE;
     constexpr int n = M / 2;
     constexpr int TG = M / 16;
     extern __shared__ float2 smem[];
@@ -143,11 +144,11 @@ static int launch_rows_t(const tcp_ctx* c, cudaStream_t st) {
     constexpr int TG = M / 16;
     constexpr int ROWS = (TG >= 128) ? 1 : 128 / TG;
     const size_t smem = (size_t)ROWS * padded_len(M) * sizeof(float2);
-    auto kern = rows_kernel<M, ROWS, TS, TC>;
+    auto kern = c->pad ? rows_kernel<M, ROWS, true, TS, TC> : rows_kernel<M, ROWS, false, TS, TC>;
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid((c->nproj + ROWS - 1) / ROWS, c->npair);
     kern<<<grid, ROWS * TG, smem, st>>>((const TS*)c->sino, (TC*)c->spec, c->tw, c->hfilt, c->try_ptab ? c->try_ptab : c->ptab, c->nproj, c->nz,
-                                       c->try_ptab ? 1 : 0, c->pad);
+                                       c->try_ptab ? 1 : 0);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }
