@@ -109,7 +109,9 @@ int tcp_normalize(tcp_ctx* ctx, const uint16_t* raw_u16, const float* flat, cons
 
 /* Device pointer and byte size of an intermediate left by the last tcp_recon (tests only):
  *   TCP_WS_SINOGRAM [nz][nproj][n] real; TCP_WS_SPECTRUM [npair][nproj][M] complex (FFT order,
- *   scaled by tcp_scale()); TCP_WS_GRID [npair][M l2][M l1] complex; TCP_WS_TRIG [nproj] double2. */
+ *   scaled by tcp_scale()); TCP_WS_GRID [npair][M l2][M l1] complex (or strip-major, tcp_grid_strip); TCP_WS_PASS1
+ *   [npair][M/W][n iy][W l1] complex, W = min(32, max(2, 16384/M)) (the column pass works on strips of W
+ *   columns and stores them contiguously); TCP_WS_TRIG [nproj] double2. */
 int tcp_workspace(tcp_ctx* ctx, int which, void** ptr, size_t* bytes);
 /* Copy an intermediate into the caller's device buffer dst (>= the size tcp_workspace reports),
  * asynchronously on `stream` (tests only). */

@@ -271,6 +271,9 @@ class Recon:
             w = int(lib().tcp_grid_strip(self.h))
             if w:       # strip-major [npair][M/w][M l2][w l1] -> [npair][M l2][M l1]
                 v = v.view(npair, M // w, M, w, 2).permute(0, 2, 1, 3, 4).reshape(npair, M, M, 2)
+        if name == "pass1":     # strip-major [npair][M/w][n iy][w l1] -> [npair][n iy][M l1]
+            w = min(32, max(2, 16384 // M))
+            v = v.view(npair, M // w, self.n, w, 2).permute(0, 2, 1, 3, 4).reshape(npair, self.n, M, 2)
         return torch.complex(v[..., 0], v[..., 1])
 
     def recon_volume_host(self, raw_host, flat_host, dark_host, theta_host, out_host=None, nbuf=3):

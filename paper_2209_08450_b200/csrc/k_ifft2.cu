@@ -62,13 +62,15 @@ __global__ void __launch_bounds__(cols_wp(M) * M / 16) ifft_cols_kernel(const TC
     // strip-major grid: the CTA's W columns are one contiguous block of M rows x W
     const TC* src = grid + (size_t)pair * M * M + (strip ? (size_t)blockIdx.x * M * W + 2 * wp : (size_t)l1);
     const size_t rstride = strip ? (size_t)W : (size_t)M;
-    TC* dst = pass1 + (size_t)pair * n * M + l1;
+    // pass-1 array, strip-major like the grid: [pair][M/W][n iy][W l1], so that consecutive iy of the CTA's
+    // W columns are contiguous (a warp stores 256 contiguous bytes instead of 16-byte pieces 4 M bytes apart)
+    TC* dst = pass1 + (size_t)pair * n * M + (size_t)blockIdx.x * n * W + 2 * wp;
     fft_line<M, true>(
         s, tid, tw, [&](int l2) { return ld_c2(src, (size_t)l2 * rstride); },
         [&](int x2, cpair v) {
             // signed x2 in [-n/2, n/2)  <->  FFT index x2 mod M
-            if (x2 < n / 2) st_c2(dst, (size_t)(x2 + n / 2) * M, v);
-            else if (x2 >= M - n / 2) st_c2(dst, (size_t)(x2 - (M - n / 2)) * M, v);
+            if (x2 < n / 2) st_c2(dst, (size_t)(x2 + n / 2) * W, v);
+            else if (x2 >= M - n / 2) st_c2(dst, (size_t)(x2 - (M - n / 2)) * W, v);
         });
 }
 
@@ -83,14 +85,15 @@ __global__ void __launch_bounds__(ROWS* M / 16) ifft_rows_kernel(const TC* __res
     float2* s = smem + (size_t)g * padded_len(M);
     const int pair = blockIdx.y;
     const int iy = blockIdx.x * ROWS + g;     // n is a multiple of ROWS
-    const TC* src = pass1 + ((size_t)pair * n + iy) * M;
+    constexpr int W = cols_w(M);              // strip width of the pass-1 array (ifft_cols_kernel)
+    const TC* src = pass1 + (size_t)pair * n * M + (size_t)iy * W;
     const float dy = __ldg(&deay[iy]);
     const int zA = 2 * pair, zB = 2 * pair + 1;
     TO* oA = out + ((size_t)zA * n + iy) * n;
     TO* oB = out + ((size_t)zB * n + iy) * n;
     const bool hasB = zB < nz;
     fft_line<M, true>(
-        s, tid, tw, [&](int l1) { return ld_c(src, (size_t)l1); },
+        s, tid, tw, [&](int l1) { return ld_c(src, (size_t)(l1 / W) * n * W + (size_t)(l1 % W)); },
         [&](int x1, float2 v) {
             int ix = -1;
             if (x1 < n / 2) ix = x1 + n / 2;

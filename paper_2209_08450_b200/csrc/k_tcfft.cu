@@ -38,11 +38,13 @@ __global__ void __launch_bounds__(128 * NG, 1) ifft_rows_tc_kernel(const __half2
     const int nlines = npair * TC_N, step = gridDim.x * NG;
     int ln = blockIdx.x * NG + grp;
     LineRegs pf;
-    if (ln < nlines) fetch_line_c(g, pass1 + (size_t)ln * TC_M, pf);
+    // pass-1 array: [pair][M/4][n iy][4 l1] (k_ifft2.cu)
+    auto line_base = [&](int l) { return pass1 + (size_t)(l / TC_N) * TC_N * TC_M + (size_t)(l % TC_N) * 4; };
+    if (ln < nlines) fetch_line_strip4(g, line_base(ln), (size_t)TC_N * 4, pf);
     for (; ln < nlines; ln += step) {
         const int pair = ln / TC_N, iy = ln % TC_N;
         put_line_c<1, true>(g, 0, pf);
-        if (ln + step < nlines) fetch_line_c(g, pass1 + (size_t)(ln + step) * TC_M, pf);
+        if (ln + step < nlines) fetch_line_strip4(g, line_base(ln + step), (size_t)TC_N * 4, pf);
         stage_mma<1, false>(g, 0xffu);
         twiddle_step(g, tw);
         stage_mma<1, true>(g, 0xffu);

@@ -187,6 +187,18 @@ __device__ __forceinline__ void fetch_line_c(const Group<NB>& g, const __half2* 
                      : "l"(p));
     }
 }
+// the same line held strip-major with strips of 4 points: point l at base[(l / 4) * strip_stride + l % 4]
+// (the pass-1 array of the inverse 2D transform): a lane's 8 points are two 16-byte pieces
+template <int NB>
+__device__ __forceinline__ void fetch_line_strip4(const Group<NB>& g, const __half2* __restrict__ base, size_t strip_stride, LineRegs& r) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int combo = g.q * 4 + u, i1 = 8 * (combo >> 1) + (g.lane & 7), nb = 4 * (combo & 1) + (g.lane >> 3);
+        const __half2* p = base + (size_t)((64 * i1 + 8 * nb) >> 2) * strip_stride;
+        r.v[2 * u] = __ldg(reinterpret_cast<const uint4*>(p));
+        r.v[2 * u + 1] = __ldg(reinterpret_cast<const uint4*>(p + strip_stride));
+    }
+}
 template <int NB, bool SWAP>
 __device__ __forceinline__ void put_line_c(const Group<NB>& g, int line, const LineRegs& r) {
 #pragma unroll

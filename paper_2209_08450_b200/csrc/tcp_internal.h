@@ -24,7 +24,7 @@ struct tcp_ctx {
     void* sino;           // [nz][nproj][n]      float | half
     void* spec;           // [npair][nproj][M]   float2 | half2   (S * G of stage S4, FFT order)
     void* grid;           // [npair][M][M]       float2 | half2   (row = l2, FFT order)
-    void* pass1;          // [npair][n][M]       float2 | half2   (row = iy, col = l1)
+    void* pass1;          // [npair][M/W][n][W]  float2 | half2   (strip of W = cols_strip_width(M) columns l1, row = iy)
     double2* trig;        // [nproj] (cos, sin) of theta, fp64
     float4* trigf;        // [nproj] (cos hi, cos lo, sin hi, sin lo): float-float split of trig
     // tables (device), built in fp64 on the host at create
