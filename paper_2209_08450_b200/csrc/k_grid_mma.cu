@@ -61,8 +61,7 @@ struct MmaSmem {
     static constexpr int B_STAGE = SC * NN * 2;
     static constexpr int offA = 0;                           // [NSUB][NST] A stages
     static constexpr int offB = offA + NSUB * NST * A_STAGE; // [NSUB][NST] B stages
-    static constexpr int offWs = offB + NSUB * NST * B_STAGE;    // [NSUB]: wx[32 columns][16] half (32 B rows), wy[32 columns][8] half
-    static constexpr int offBar = offWs + NSUB * 3 * SC * 16;    // [NSUB][NST] mbarriers
+    static constexpr int offBar = offB + NSUB * NST * B_STAGE;   // [NSUB][NST] mbarriers
     static constexpr int offMisc = offBar + NSUB * NST * 8;  // tmem base, started[NSUB]
     static constexpr int total = offMisc + 64;
 };
@@ -106,7 +105,6 @@ __global__ void __launch_bounds__(NTHR, 2)
     const int sub = warp;
     unsigned char* Aw = smem + L::offA + warp * NST * A_STAGE;      // this warp's single 32-column stage
     unsigned char* Bw = smem + L::offB + warp * NST * L::B_STAGE;
-    uint4* ws = reinterpret_cast<uint4*>(smem + L::offWs) + warp * 3 * SC;
     const uint64_t adesc0 = umma_desc(smem_u32(Aw), A_LBO, 128), bdesc0 = umma_desc(smem_u32(Bw), L::B_LBO, 128);
     const uint64_t adesc1 = adesc0 + (uint64_t)((2 * A_LBO) >> 4), bdesc1 = bdesc0 + (uint64_t)((2 * L::B_LBO) >> 4);   // second K step
     static_assert(NST == 1 && SC == 32, "one 32-column stage per warp");
@@ -190,34 +188,39 @@ __global__ void __launch_bounds__(NTHR, 2)
                         }
                     }
                 }
-                // ---- phase 1: taps of both axes into zeroed rows (x: 16 halves = 32 B, y: 8 halves = 16 B per column).
-                // taps l = floor(nu) - m + 1 + t, t = 0..2m-1, distance d_t = l - nu = d_0 + t; the open box
-                // |l - nu| < m keeps t iff d_t < m (d_0 > -m always); d_0 = -m+1 exactly iff nu is an integer
-                unsigned char* wxrow = reinterpret_cast<unsigned char*>(ws) + cl * 32;
-                unsigned char* wyrow = reinterpret_cast<unsigned char*>(ws) + SC * 32 + cl * 16;
-                *reinterpret_cast<uint4*>(wxrow) = make_uint4(0, 0, 0, 0);
-                *reinterpret_cast<uint4*>(wxrow + 16) = make_uint4(0, 0, 0, 0);
-                *reinterpret_cast<uint4*>(wyrow) = make_uint4(0, 0, 0, 0);
+                // ---- phase 1: the weights of both axes, per CELL POSITION of the sub-tile and in registers (no
+                // scatter through shared memory: the kernel is bound by the L1 data pipe, the MUFU and FMA
+                // pipes idle).  Cell X = SX + lx is tap a = X - floor(nu) of the sample (an exact small integer),
+                // at distance d = a - frac; the open box |l - nu| < m keeps a in [-m+1, m] for a fractional nu
+                // and [-m+1, m-1] when nu is an integer.
+                uint4 xa, xc, yv;
                 {
-                    const float dint = -(float)(MH - 1);
                     float flx, frx, fly, fry;
                     nu_split((float)k, cxh, cxl, flx, frx);
                     nu_split((float)k, cyh, cyl, fly, fry);
-                    float dx0 = dint - frx, dy0 = dint - fry;
-                    if (frx > 0.f && dx0 >= dint) dx0 = __uint_as_float(__float_as_uint(dint) + 1u);   // next below -m+1
-                    if (fry > 0.f && dy0 >= dint) dy0 = __uint_as_float(__float_as_uint(dint) + 1u);
-                    const int lx0 = valid ? (int)(flx + dint - (float)SX) : 64;                       // 64: every tap out of range
-                    const int ly0 = valid ? (int)(fly + dint - (float)SY) : 64;
-                    __half* wxt = reinterpret_cast<__half*>(wxrow) + lx0;
-                    __half* wyt = reinterpret_cast<__half*>(wyrow) + ly0;
+                    const float lo = -(float)(MH - 1);
+                    const float hix = valid ? (frx > 0.f ? (float)MH : (float)(MH - 1)) : -64.f;      // -64: no tap in range
+                    const float hiy = valid ? (fry > 0.f ? (float)MH : (float)(MH - 1)) : -64.f;
+                    const float ax0 = (float)SX - flx, ay0 = (float)SY - fly;
+                    auto wgt = [&](float a, float frac, float hi) {
+                        const float d = a - frac;
+                        const float w = ex2_approx(-alpha2 * d * d);
+                        return (a >= lo && a <= hi) ? w : 0.f;
+                    };
+                    unsigned wx[SUBX / 2], wy[SUBY / 2];
 #pragma unroll
-                    for (int t = 0; t < 2 * MH; ++t) {
-                        const float dx = dx0 + (float)t, dy = dy0 + (float)t;
-                        const __half wxv = __float2half_rn(ex2_approx(-alpha2 * dx * dx));
-                        const __half wyv = __float2half_rn(ex2_approx(-alpha2 * dy * dy));
-                        if ((unsigned)(lx0 + t) < (unsigned)SUBX && dx < (float)MH) wxt[t] = wxv;
-                        if ((unsigned)(ly0 + t) < (unsigned)SUBY && dy < (float)MH) wyt[t] = wyv;
+                    for (int e = 0; e < SUBX / 2; ++e) {
+                        const __half2 h = __floats2half2_rn(wgt(ax0 + (float)(2 * e), frx, hix), wgt(ax0 + (float)(2 * e + 1), frx, hix));
+                        wx[e] = *reinterpret_cast<const unsigned*>(&h);
                     }
+#pragma unroll
+                    for (int e = 0; e < SUBY / 2; ++e) {
+                        const __half2 h = __floats2half2_rn(wgt(ay0 + (float)(2 * e), fry, hiy), wgt(ay0 + (float)(2 * e + 1), fry, hiy));
+                        wy[e] = *reinterpret_cast<const unsigned*>(&h);
+                    }
+                    xa = make_uint4(wx[0], wx[1], wx[2], wx[3]);
+                    xc = make_uint4(wx[4], wx[5], wx[6], wx[7]);
+                    yv = make_uint4(wy[0], wy[1], wy[2], wy[3]);
                 }
                 // the warp's previous MMAs must have read the stage before it is overwritten
                 if (nstep > 0) mbar_wait(bar, (nstep - 1) & 1);
@@ -229,8 +232,6 @@ __global__ void __launch_bounds__(NTHR, 2)
                 }
                 // ---- phase 2: A[m = ly * 16 + lx][column] = wy[ly] * wx[lx]; MN-major: 8 cells of a column = 16 B
                 {
-                    const uint4 xa = *reinterpret_cast<const uint4*>(wxrow), xc = *reinterpret_cast<const uint4*>(wxrow + 16);
-                    const uint4 yv = *reinterpret_cast<const uint4*>(wyrow);
                     const unsigned yw[4] = {yv.x, yv.y, yv.z, yv.w};
                     unsigned char* arow = Aw + (cl >> 3) * A_LBO + (cl & 7) * 16;
 #pragma unroll
