@@ -207,7 +207,7 @@ def deapod_crop_adjoint(f, n, m=DEFAULT_M):
     return g
 
 
-def fbp_from_sino(p, theta, center, filt="ramp", m=DEFAULT_M, method="grid", return_q=False, pad="zero"):
+def fbp_from_sino(p, theta, center, filt="ramp", m=DEFAULT_M, method="grid", return_q=False, pad="zero", fused=False):
     """p f64 [nz][nproj][n] -> out f64 [nz][n][n] (S3..S7 or the two definitions)."""
     p = _f64(p)
     theta = _f32(theta)
@@ -215,18 +215,18 @@ def fbp_from_sino(p, theta, center, filt="ramp", m=DEFAULT_M, method="grid", ret
     out = np.empty((nz, n, n))
     q = np.empty_like(p) if return_q else None
     lib().orc_fbp_from_sino_pad(_p(p), _p(theta), C.c_int(nproj), C.c_int(nz), C.c_int(n),
-                            C.c_double(center), C.c_int(FILTERS[filt]), C.c_int(PADS[pad]), C.c_int(m),
+                            C.c_double(center), C.c_int(FILTERS[filt]), C.c_int(PADS[pad] | (2 if fused else 0)), C.c_int(m),
                             C.c_int(METHODS[method]), _p(out), _p(q) if return_q else None)
     return (out, q) if return_q else out
 
 
-def recon(raw, flat, dark, theta, center, filt="ramp", m=DEFAULT_M, method="grid", pad="zero"):
+def recon(raw, flat, dark, theta, center, filt="ramp", m=DEFAULT_M, method="grid", pad="zero", fused=False):
     """uint16 counts -> reconstruction, S1..S7.  raw [nproj][nz][n] -> out [nz][n][n]."""
     raw = np.ascontiguousarray(raw, dtype=np.uint16)
     nproj, nz, n = raw.shape
     flat, dark, theta = _f32(flat), _f32(dark), _f32(theta)
     out = np.empty((nz, n, n))
     lib().orc_recon_pad(_p(raw), _p(flat), _p(dark), _p(theta), C.c_int(nproj), C.c_int(nz), C.c_int(n),
-                    C.c_double(center), C.c_int(FILTERS[filt]), C.c_int(PADS[pad]), C.c_int(m), C.c_int(METHODS[method]),
+                    C.c_double(center), C.c_int(FILTERS[filt]), C.c_int(PADS[pad] | (2 if fused else 0)), C.c_int(m), C.c_int(METHODS[method]),
                     _p(out))
     return out

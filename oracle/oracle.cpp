@@ -197,4 +197,31 @@ void orc_spectrum(const double* q, int nproj, int n, double center, cplx* G) {
     }
 }
 
+
+// ---------------------------------------------------------------------------
+// S3 + S4 fused, WITHOUT the crop between them (SURVEY 8(c) "literal vs fused reading", Q6; an option of
+// SURVEY 8(f-2), not the default): the filter and the spectrum have the same length M, so
+//   G[j][k] = C H[k] P_j[k] e^{+2 pi i k c / M},   P_j = FFT_M(padded row),   G[j][-M/2] = 0.
+// It backprojects the UNCROPPED periodic filtered row (tails outside the detector included).
+// p[nproj][n] -> G[nproj][M], FFT order; pad as in orc_filter_rows_pad.
+// ---------------------------------------------------------------------------
+void orc_spectrum_fused(const double* p, int nproj, int n, double center, int filter, int pad, cplx* G) {
+    const int M = 2 * n;
+    const double C = PI / ((double)nproj * (double)M);
+    std::vector<double> H(M);
+    orc_filter(M, filter, H.data());
+    std::vector<cplx> a(M), P(M);
+    for (int j = 0; j < nproj; ++j) {
+        const double* pr = p + (size_t)j * n;
+        for (int i = 0; i < M; ++i) a[i] = (i < n) ? pr[i] : (pad == 0 ? 0.0 : (i < n + n / 2 ? pr[n - 1] : pr[0]));
+        orc_fft(a.data(), P.data(), M, -1);
+        for (int k = 0; k < M; ++k) {
+            int ks = (k < M / 2) ? k : k - M;
+            double ph = 2.0 * PI * (double)ks * center / (double)M;
+            G[(size_t)j * M + k] = C * H[k] * P[k] * cplx(std::cos(ph), std::sin(ph));
+        }
+        G[(size_t)j * M + M / 2] = 0.0;
+    }
+}
+
 }  // extern "C"

@@ -25,6 +25,7 @@ void orc_neglog(const uint16_t*, const float*, const float*, int, int, int, doub
 void orc_filter_rows(const double*, int, int, int, double*);
 void orc_filter_rows_pad(const double*, int, int, int, int, double*);
 void orc_spectrum(const double*, int, int, double, cplx*);
+void orc_spectrum_fused(const double*, int, int, double, int, int, cplx*);
 
 // Gaussian gridding kernel phi(t) = exp(-alpha t^2), alpha = pi / (sqrt(2) m)   (reading Q7),
 // and its continuous transform  Phi^(x) = sqrt(pi/alpha) exp(-pi^2 x^2 / (alpha M^2))  (Q8).
@@ -243,7 +244,8 @@ void orc_fbp_from_sino(const double* p, const float* theta, int nproj, int nz, i
                        double center, int filter, int m, int method, double* out, double* q_out) {
     orc_fbp_from_sino_pad(p, theta, nproj, nz, n, center, filter, 0, m, method, out, q_out);
 }
-// pad: padding of the filter stage (orc_filter_rows_pad): 0 zeros, 1 edge values
+// pad: bit 0 = padding of the filter stage (orc_filter_rows_pad): 0 zeros, 1 edge values;
+//      bit 1 = S3 + S4 fused without the crop (orc_spectrum_fused; gridding / exact backprojection only)
 void orc_fbp_from_sino_pad(const double* p, const float* theta, int nproj, int nz, int n, double center, int filter,
                            int pad, int m, int method, double* out, double* q_out) {
     const int M = 2 * n;
@@ -251,14 +253,15 @@ void orc_fbp_from_sino_pad(const double* p, const float* theta, int nproj, int n
 #pragma omp parallel for schedule(dynamic, 1) if (method != 1)
     for (int z = 0; z < nz; ++z) {
         std::vector<double> q((size_t)nproj * n);
-        orc_filter_rows_pad(p + (size_t)z * nproj * n, nproj, n, filter, pad, q.data());
+        orc_filter_rows_pad(p + (size_t)z * nproj * n, nproj, n, filter, pad & 1, q.data());
         if (q_out) std::memcpy(q_out + (size_t)z * nproj * n, q.data(), sizeof(double) * q.size());
         double* f = out + (size_t)z * n * n;
         if (method == 2) {
             orc_backproject_lin(q.data(), theta, nproj, n, center, f);
         } else {
             std::vector<cplx> G((size_t)nproj * M);
-            orc_spectrum(q.data(), nproj, n, center, G.data());
+            if (pad & 2) orc_spectrum_fused(p + (size_t)z * nproj * n, nproj, n, center, filter, pad & 1, G.data());
+            else orc_spectrum(q.data(), nproj, n, center, G.data());
             if (method == 0) orc_backproject_grid(G.data(), theta, nproj, n, m, f, nullptr);
             else orc_backproject_exact(G.data(), theta, nproj, n, f, nullptr);
         }

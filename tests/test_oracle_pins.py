@@ -169,6 +169,35 @@ def test_p5_edge_padding_object_outside_field_of_view():
     assert abs(cup_e) < 0.5 * cup_z         # edge padding: less than half of it left (measured 0.45)
 
 
+def test_p3_fused_filter_equals_literal_plus_backprojected_tails():
+    """The fused (uncropped) S3 + S4 option differs from the literal chain exactly by
+    the backprojection of what the crop removes: with q_full = IFFT(H FFT(pad p)) the uncropped periodic
+    filtered row (numpy.fft here, not the oracle's transforms), linearity gives
+        recon_fused(p) = recon_literal(p) + B_exact(spectrum of the tail rows q_full[n:M] placed at [n, M)).
+    A sign, scale, phase or index slip in the fused path breaks the identity; it also shows that the two
+    readings are NOT the same image (the tails of a ramp-filtered row decay only like 1/i^2)."""
+    n, M, nproj, c = 16, 32, 12, 7.25
+    theta = sg.make_theta(nproj)
+    rng = np.random.default_rng(21)
+    p = rng.standard_normal((1, nproj, n))
+    lit = orc.fbp_from_sino(p, theta, c, "shepp", 4, "exact")[0]
+    fus = orc.fbp_from_sino(p, theta, c, "shepp", 4, "exact", fused=True)[0]
+    H = orc.filter_table(M, "shepp")
+    a = np.concatenate([p[0], np.zeros((nproj, n))], axis=1)
+    q_full = np.fft.ifft(np.fft.fft(a, axis=1) * H[None, :], axis=1).real
+    tail = q_full.copy()
+    tail[:, :n] = 0.0
+    ks = np.where(np.arange(M) < M // 2, np.arange(M), np.arange(M) - M)
+    G = (np.pi / (nproj * M)) * np.fft.fft(tail, axis=1) * np.exp(2j * np.pi * ks * c / M)[None, :]
+    G[:, M // 2] = 0.0
+    extra = orc.backproject_exact(G, theta, n).real
+    assert np.abs(fus - (lit + extra)).max() < 1e-12 * max(1.0, np.abs(lit).max())
+    assert rl2(fus, lit) > 1e-3
+    # gridding follows the same spectrum
+    fg = orc.fbp_from_sino(p, theta, c, "shepp", 4, "grid", fused=True)[0]
+    assert rl2(fg, fus) < 2e-3
+
+
 # ---------------------------------------------------------------- P4: plane wave
 @pytest.mark.parametrize("m", [3, 4, 5])
 def test_p4_plane_wave(m):
