@@ -62,7 +62,13 @@ enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1, TCP_GRID_TILE = 2, TCP_
  * suppressing artifacts when processing samples not fitting into the detector field of view"):
  * TCP_PAD_ZERO (default, the reading of north_star) or TCP_PAD_EDGE = the nearest detector edge value of
  * the periodic length-2n row (p[n-1] for n <= i < 3n/2, p[0] after).  Stage S4 always zero-pads. */
-enum { TCP_OPT_GRID_IMPL = 0, TCP_OPT_PROFILE = 1, TCP_OPT_TCFFT = 2, TCP_OPT_ALGORITHM = 3, TCP_OPT_PAD = 4 };
+/* TCP_OPT_FILTER_FUSED (0 default | 1): the second reading of "filter, then Fourier backprojection" (DESIGN.md
+ * Q6): filter and spectrum have the same length M = 2n, so S3 + S4 collapse to G = C H FFT_M(padded row) x phase
+ * with NO crop of the filtered row in between: one transform per row instead of three, and a slightly different
+ * image (the tails of the filtered row outside the detector are backprojected too).  FourierRec, tcp_recon and
+ * tcp_recon_volume_host only; tcp_recon_try keeps the default chain. */
+enum { TCP_OPT_GRID_IMPL = 0, TCP_OPT_PROFILE = 1, TCP_OPT_TCFFT = 2, TCP_OPT_ALGORITHM = 3, TCP_OPT_PAD = 4,
+       TCP_OPT_FILTER_FUSED = 5 };
 enum { TCP_PAD_ZERO = 0, TCP_PAD_EDGE = 1 };
 enum { TCP_ALG_FOURIER = 0, TCP_ALG_LINE = 1 };
 enum { TCP_TCFFT_ROWS = 1, TCP_TCFFT_COLS = 2, TCP_TCFFT_IROWS = 4 };

@@ -63,6 +63,41 @@ __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict
         });
 }
 
+// S3 + S4 fused without the crop (TCP_OPT_FILTER_FUSED; SURVEY 8(c) Q6's second reading, an option): one
+// transform, G = FFT_M(padded row) x (H x S C e^{+2 pi i k c/M}); the table carries the whole product.
+template <int M, int ROWS, bool PAD_EDGE, class TS, class TC>
+__global__ void __launch_bounds__(ROWS* M / 16) rows_fused_kernel(const TS* __restrict__ sino, TC* __restrict__ spec,
+                                                                  const float2* __restrict__ tw,
+                                                                  const float2* __restrict__ ftab, int nproj, int nz) {
+    constexpr int n = M / 2;
+    constexpr int TG = M / 16;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / TG;
+    const int tid = threadIdx.x % TG;
+    float2* s = smem + (size_t)g * padded_len(M);
+    int j = blockIdx.x * ROWS + g;
+    const bool live = j < nproj;
+    if (!live) j = nproj - 1;
+    const int pair = blockIdx.y;
+    const int zA = 2 * pair, zB = 2 * pair + 1;
+    const bool hasB = zB < nz;
+    const TS* pA = sino + ((size_t)zA * nproj + j) * n;
+    const TS* pB = sino + ((size_t)(hasB ? zB : zA) * nproj + j) * n;
+    TC* out = spec + ((size_t)pair * nproj + j) * M;
+    fft_line<M, false>(
+        s, tid, tw,
+        [&](int i) {
+            if (i >= n) {
+                if (!PAD_EDGE) return make_float2(0.f, 0.f);
+                i = (i < n + n / 2) ? n - 1 : 0;
+            }
+            return make_float2(ld_r(pA, i), hasB ? ld_r(pB, i) : 0.f);
+        },
+        [&](int k, float2 v) {
+            if (live) st_c(out, k, cmul(v, __ldg(&ftab[k])));
+        });
+}
+
 // S3 alone, for the line-summation operator (k_line.cu): the same two transforms, the cropped filtered
 // rows written back over the two sinogram rows they came from (each CTA reads its rows completely before
 // the first pass ends and writes them in the last pass of the inverse transform).
@@ -144,6 +179,14 @@ static int launch_rows_t(const tcp_ctx* c, cudaStream_t st) {
     constexpr int TG = M / 16;
     constexpr int ROWS = (TG >= 128) ? 1 : 128 / TG;
     const size_t smem = (size_t)ROWS * padded_len(M) * sizeof(float2);
+    if (c->filter_fused && !c->try_ptab) {
+        auto kf = c->pad ? rows_fused_kernel<M, ROWS, true, TS, TC> : rows_fused_kernel<M, ROWS, false, TS, TC>;
+        TCP_CUDA_CHECK(cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kf<<<dim3((c->nproj + ROWS - 1) / ROWS, c->npair), ROWS * TG, smem, st>>>((const TS*)c->sino, (TC*)c->spec, c->tw, c->ftab, c->nproj,
+                                                                                   c->nz);
+        TCP_CUDA_CHECK(cudaGetLastError());
+        return TCP_OK;
+    }
     auto kern = c->pad ? rows_kernel<M, ROWS, true, TS, TC> : rows_kernel<M, ROWS, false, TS, TC>;
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid((c->nproj + ROWS - 1) / ROWS, c->npair);

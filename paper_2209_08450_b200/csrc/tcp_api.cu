@@ -105,6 +105,14 @@ static int build_context(tcp_ctx* c) {
     }
     pt[M / 2] = make_float2(0.f, 0.f);
     if ((rc = upload(&c->ptab, pt, &c->bytes))) return rc;
+    {   // fused path: (H[k]/M) M x ptab[k]
+        std::vector<float2> ft(M);
+        for (int k = 0; k < M; ++k) {
+            const double h = (double)hf[k] * (double)M;
+            ft[k] = make_float2((float)(h * (double)pt[k].x), (float)(h * (double)pt[k].y));
+        }
+        if ((rc = upload(&c->ftab, ft, &c->bytes))) return rc;
+    }
 
     const double alpha = kPi / (sqrt(2.0) * (double)m);
     std::vector<float> dx(n), dy(n);
@@ -220,7 +228,7 @@ void tcp_destroy(tcp_ctx* c) {
         free(c->pev);
     }
     cudaFree(c->sino); cudaFree(c->spec); cudaFree(c->grid); cudaFree(c->pass1); cudaFree(c->trig); cudaFree(c->trigf);
-    cudaFree(c->tw); cudaFree(c->hfilt); cudaFree(c->ptab); cudaFree(c->deax); cudaFree(c->deay);
+    cudaFree(c->tw); cudaFree(c->hfilt); cudaFree(c->ptab); cudaFree(c->ftab); cudaFree(c->deax); cudaFree(c->deay);
     cudaFree(c->tile_order);
     cudaFree(c->try_buf);
     cudaFree(c->tc_amat); cudaFree(c->tc_hfilt); cudaFree(c->tc_ptab);
@@ -385,6 +393,10 @@ int tcp_set_option(tcp_ctx* c, int option, int value) {
         if (value == TCP_GRID_MMA && !c->half_store) return set_error(TCP_EUNSUPPORTED, "tensor-core gridding needs fp16 storage");
         c->grid_impl = value;
         c->grid_strip = (value == TCP_GRID_MMA) ? cols_strip_width(c->M) : 0;
+        return TCP_OK;
+    }
+    if (option == TCP_OPT_FILTER_FUSED) {
+        c->filter_fused = value != 0;
         return TCP_OK;
     }
     if (option == TCP_OPT_PAD) {

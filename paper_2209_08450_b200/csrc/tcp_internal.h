@@ -14,6 +14,8 @@ struct tcp_ctx {
     bool half_out;        // out in half (TCP_F16)
     double scale;         // power-of-two scale S of SPECTRUM / GRID / PASS1 (1 in fp32)
     int grid_impl;
+    int filter_fused;     // TCP_OPT_FILTER_FUSED: S3 + S4 as one transform, no crop (FourierRec only)
+    float2* ftab;         // [M] H[k] x ptab[k]: the fused path's table
     int pad;              // TCP_PAD_ZERO | TCP_PAD_EDGE: padding samples of the filter stage S3
     int algorithm;        // TCP_ALG_FOURIER (gridding, default) | TCP_ALG_LINE (direct line summation)
     int grid_strip;       // 0: grid rows are contiguous; W > 0: strip-major [pair][M/W][M l2][W l1] (tcgen05 gridding)

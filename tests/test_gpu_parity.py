@@ -318,6 +318,33 @@ def test_recon_under_cuda_graph_capture(dtype):
     r.close()
 
 
+@pytest.mark.parametrize("dtype,pad", [("f32", "zero"), ("f32", "edge"), ("f16", "zero")])
+def test_fused_filter_option(dtype, pad):
+    """TCP_OPT_FILTER_FUSED (the uncropped reading of S3 + S4, one transform per row) against the oracle with
+    fused=True; it is a different image from the default chain, which the same context still produces after
+    the option is switched off."""
+    tcp = _tcp()
+    w = sg.make_workload("C1")
+    w.center = 58.5
+    raw, flat, dark, theta = _inputs(w, [1, 2, 3, 4, 5])
+    r = tcp.Recon(w.n, w.nproj, 5, w.center, dtype, w.filter, 3)
+    r.set_filter_fused(True)
+    r.set_pad(pad)
+    dev = _to_dev(raw, flat, dark, theta)
+    out = r.recon(*dev).float().cpu().numpy()
+    ref = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, "grid", pad=pad, fused=True)
+    lit = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, "grid", pad=pad)
+    gate = FP32_GATE if dtype == "f32" else FP16_GATE_L2
+    assert rl2(ref[2], lit[2]) > 10 * gate or dtype == "f16"
+    for z in range(5):
+        assert rl2(out[z], ref[z]) < gate, (z, rl2(out[z], ref[z]))
+    r.set_filter_fused(False)
+    out2 = r.recon(*dev).float().cpu().numpy()
+    for z in range(5):
+        assert rl2(out2[z], lit[z]) < gate
+    r.close()
+
+
 def test_mean_frames_and_errors():
     tcp = _tcp()
     rng = np.random.default_rng(0)
