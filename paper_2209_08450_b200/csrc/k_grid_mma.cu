@@ -35,6 +35,10 @@
 namespace tcpk {
 
 constexpr int SUBX = 16, SUBY = 8, NSUB = 8;      // sub-tile = 128 cells; 2 x 4 sub-tiles per region
+#ifndef GRID_CW
+#define GRID_CW 8
+#endif
+constexpr int CW = GRID_CW;                       // warps (= sub-tiles) per CTA; a region is NSUB / CW CTAs (blockIdx.z)
 constexpr int SC = 32;                            // columns (samples) per A/B stage = one lane each = two MMA K steps
 constexpr int NST = 1;                            // stages per warp
 constexpr int RUNMAX = 32;                        // >= samples of one chord inside a sub-tile's sample box
@@ -59,17 +63,17 @@ struct MmaSmem {
     static constexpr int GW = NN * 2 / 16;                   // uint4 per sample (B row)
     static constexpr int B_LBO = (NN / 8) * 128;
     static constexpr int B_STAGE = SC * NN * 2;
-    static constexpr int offA = 0;                           // [NSUB][NST] A stages
-    static constexpr int offB = offA + NSUB * NST * A_STAGE; // [NSUB][NST] B stages
-    static constexpr int offBar = offB + NSUB * NST * B_STAGE;   // [NSUB][NST] mbarriers
-    static constexpr int offMisc = offBar + NSUB * NST * 8;  // tmem base, started[NSUB]
+    static constexpr int offA = 0;                           // [CW][NST] A stages
+    static constexpr int offB = offA + CW * NST * A_STAGE;   // [CW][NST] B stages
+    static constexpr int offBar = offB + CW * NST * B_STAGE;     // [CW][NST] mbarriers
+    static constexpr int offMisc = offBar + CW * NST * 8;    // tmem base, started[CW]
     static constexpr int total = offMisc + 64;
 };
 
 // ---------------------------------------------------------------------------------------
 // item: x = region (32 x 32 tile) index, y = split s | nsplit S << 16, z = first partial slot (-1: write the grid)
 template <int MH, int NN>
-__global__ void __launch_bounds__(NTHR, 2)
+__global__ void __launch_bounds__(32 * CW, 16 / CW)
     grid_mma_kernel(const __half2* __restrict__ spec, __half2* __restrict__ grid, float2* __restrict__ partial,
                     const float4* __restrict__ trigf, const int2* __restrict__ plan, const int4* __restrict__ items,
                     int nproj, int M, int npair, float alpha2, int strip_log2) {
@@ -91,7 +95,7 @@ __global__ void __launch_bounds__(NTHR, 2)
         asm volatile("fence.mbarrier_init.release.cluster;");
     }
     if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&misc[0])), "n"(NSUB * NN));
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&misc[0])), "n"(CW * NN));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
@@ -102,13 +106,13 @@ __global__ void __launch_bounds__(NTHR, 2)
     constexpr uint32_t IDESC = (1u << 4) | (1u << 15) | (1u << 16) | ((uint32_t)(NN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
 
     // ---- this warp's sub-tile
-    const int sub = warp;
+    const int sub = (int)blockIdx.z * CW + warp;
     unsigned char* Aw = smem + L::offA + warp * NST * A_STAGE;      // this warp's single 32-column stage
     unsigned char* Bw = smem + L::offB + warp * NST * L::B_STAGE;
     const uint64_t adesc0 = umma_desc(smem_u32(Aw), A_LBO, 128), bdesc0 = umma_desc(smem_u32(Bw), L::B_LBO, 128);
     const uint64_t adesc1 = adesc0 + (uint64_t)((2 * A_LBO) >> 4), bdesc1 = bdesc0 + (uint64_t)((2 * L::B_LBO) >> 4);   // second K step
     static_assert(NST == 1 && SC == 32, "one 32-column stage per warp");
-    const uint32_t acc = tmem + (uint32_t)(sub * NN);
+    const uint32_t acc = tmem + (uint32_t)(warp * NN);
     const int cl = lane;                                     // column of the step
     uint32_t nstep = 0;                                      // K steps issued by this warp
     const size_t pstride = (size_t)nproj * M;                // elements between slice-pair planes of the spectrum
@@ -272,14 +276,16 @@ __global__ void __launch_bounds__(NTHR, 2)
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 
     // ---- epilogue: TMEM -> registers -> grid (or partial tile).  A warp can read only its own lane
-    // quarter of TMEM: warp w takes rows 32 (w & 3) .. +31 of the four sub-tiles of half (w >> 2)
+    // quarter of TMEM: warp w takes rows 32 (w & 3) .. +31 of CW / (CW / 4) of the CTA's sub-tiles
     {
         const int q = warp & 3, hsel = warp >> 2;
+        constexpr int PER = CW / (CW / 4);                     // sub-tiles per epilogue warp (4)
         const int mrow = q * 32 + lane, ly = mrow >> 4, lx = mrow & 15;
         const size_t pstride = (size_t)M * M;
 #pragma unroll 1
-        for (int bb = 0; bb < NSUB / 2; ++bb) {
-            const int b = hsel * (NSUB / 2) + bb;
+        for (int bb = 0; bb < PER; ++bb) {
+            const int b = hsel * PER + bb;                      // accumulator inside the CTA
+            const int gb = (int)blockIdx.z * CW + b;            // sub-tile inside the region
             uint32_t r[NN];
             if (misc[1 + b] != 0) {
                 TmemLd<NN>::run(tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(b * NN), r);
@@ -288,7 +294,7 @@ __global__ void __launch_bounds__(NTHR, 2)
 #pragma unroll
                 for (int e = 0; e < NN; ++e) r[e] = 0u;
             }
-            const int ry = (b >> 1) * SUBY + ly, rx = (b & 1) * SUBX + lx;      // region-relative cell
+            const int ry = (gb >> 1) * SUBY + ly, rx = (gb & 1) * SUBX + lx;    // region-relative cell
             if (item.z < 0) {
                 const int gr = TY0 + ry, gc = TX0 + rx;
                 // strip-major grid (strip width 2^strip_log2 columns) or row-major (strip_log2 < 0)
@@ -308,7 +314,7 @@ __global__ void __launch_bounds__(NTHR, 2)
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(NSUB * NN));
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(CW * NN));
 }
 
 // ---------------------------------------------------------------------------------------
@@ -318,8 +324,8 @@ static int launch_mma_t(const tcp_ctx* c, cudaStream_t st) {
     auto kern = grid_mma_kernel<MH, NN>;
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L::total));
     const double alpha = 3.14159265358979323846 / (1.4142135623730951 * MH);
-    dim3 grid(c->g_nitems, (c->npair + NN / 2 - 1) / (NN / 2));
-    kern<<<grid, NTHR, L::total, st>>>((const __half2*)c->spec, (__half2*)c->grid, c->g_partial, c->trigf, c->g_plan, c->g_items,
+    dim3 grid(c->g_nitems, (c->npair + NN / 2 - 1) / (NN / 2), NSUB / CW);
+    kern<<<grid, 32 * CW, L::total, st>>>((const __half2*)c->spec, (__half2*)c->grid, c->g_partial, c->trigf, c->g_plan, c->g_items,
                                        c->nproj, c->M, c->npair, (float)(alpha * 1.4426950408889634), c->grid_strip ? (int)log2((double)c->grid_strip) : -1);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
