@@ -76,18 +76,15 @@ template <int MH, int NN>
 __global__ void __launch_bounds__(32 * CW, 16 / CW)
     grid_mma_kernel(const __half2* __restrict__ spec, __half2* __restrict__ grid, float2* __restrict__ partial,
                     const float4* __restrict__ trigf, const int2* __restrict__ plan, const int4* __restrict__ items,
-                    int nproj, int M, int npair, float alpha2, int strip_log2) {
+                    int nproj, int M, int npair, float alpha2, int strip_log2, int nitems, int* __restrict__ counter) {
     using L = MmaSmem<NN>;
     constexpr int GW = L::GW, NPG = NN / 2;
     extern __shared__ __align__(128) unsigned char smem[];
     uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L::offMisc);
 
     const int n = M >> 1, tiles = M / TS;
-    const int4 item = items[blockIdx.x];
-    const int tile = item.x, split = item.y & 0xffff, nsplit = item.y >> 16;
     const int pg = blockIdx.y;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int TX0 = (tile % tiles) * TS, TY0 = (tile / tiles) * TS;
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L::offBar) + warp * NST;
 
     if (lane == 0) {
@@ -114,12 +111,25 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
     static_assert(NST == 1 && SC == 32, "one 32-column stage per warp");
     const uint32_t acc = tmem + (uint32_t)(warp * NN);
     const int cl = lane;                                     // column of the step
-    uint32_t nstep = 0;                                      // K steps issued by this warp
+    uint32_t nstep = 0;                                      // K steps issued by this warp since the kernel started (mbarrier parity)
     const size_t pstride = (size_t)nproj * M;                // elements between slice-pair planes of the spectrum
     const size_t pstride_b = pstride * sizeof(__half2);
     const __half2* plane0 = spec + (size_t)(pg * NPG) * pstride;                  // first plane of this pair group
     const int nvalid = min(NPG, npair - pg * NPG);                                // planes that exist
 
+    // persistent CTA: items claimed from a counter, heaviest regions first (TMEM allocation, barrier set-up and
+    // launch cost once per CTA, not per item)
+    int* const ctr = counter + (blockIdx.y * gridDim.z + blockIdx.z);
+#pragma unroll 1
+    for (;;) {
+    if (tid == 0) misc[12] = (uint32_t)atomicAdd(ctr, 1);
+    __syncthreads();
+    const int it = (int)misc[12];
+    if (it >= nitems) break;
+    const int4 item = items[it];
+    const int tile = item.x, split = item.y & 0xffff, nsplit = item.y >> 16;
+    const int TX0 = (tile % tiles) * TS, TY0 = (tile / tiles) * TS;
+    uint32_t istep = 0;                                      // K steps of this item (0: the accumulator holds nothing)
     for (int img = 0; img < 4; ++img) {
         const int2 win = plan[tile * 4 + img];
         if (win.y == 0) continue;
@@ -259,18 +269,19 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                 __syncwarp();
                 if (lane == 0) {
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    umma_f16(acc, adesc0, bdesc0, IDESC, nstep > 0 ? 1u : 0u);
+                    umma_f16(acc, adesc0, bdesc0, IDESC, istep > 0 ? 1u : 0u);
                     if (total - c0 > 16) umma_f16(acc, adesc1, bdesc1, IDESC, 1u);
                     umma_commit(bar);
                 }
                 ++nstep;
+                ++istep;
                 __syncwarp();
             }
         }
     }
     // ---- this warp's MMAs complete (commits complete in order: wait for the last one)
-    if (nstep > 0) mbar_wait(bar, (nstep - 1) & 1);
-    if (lane == 0) misc[1 + warp] = nstep;
+    if (istep > 0) mbar_wait(bar, (nstep - 1) & 1);
+    if (lane == 0) misc[1 + warp] = istep;
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -312,8 +323,11 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
             }
         }
     }
+    // every warp has read the accumulators (and misc) before the next item overwrites them
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    }   // items
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(CW * NN));
 }
 
@@ -324,9 +338,14 @@ static int launch_mma_t(const tcp_ctx* c, cudaStream_t st) {
     auto kern = grid_mma_kernel<MH, NN>;
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L::total));
     const double alpha = 3.14159265358979323846 / (1.4142135623730951 * MH);
-    dim3 grid(c->g_nitems, (c->npair + NN / 2 - 1) / (NN / 2), NSUB / CW);
+    const int ny = (c->npair + NN / 2 - 1) / (NN / 2), nz = NSUB / CW;
+    int ctas = (c->nsm * (16 / CW) + ny * nz - 1) / (ny * nz);            // resident CTAs per (pair group, region part)
+    if (ctas > c->g_nitems) ctas = c->g_nitems;
+    if (ctas < 1) ctas = 1;
+    dim3 grid(ctas, ny, nz);
     kern<<<grid, 32 * CW, L::total, st>>>((const __half2*)c->spec, (__half2*)c->grid, c->g_partial, c->trigf, c->g_plan, c->g_items,
-                                       c->nproj, c->M, c->npair, (float)(alpha * 1.4426950408889634), c->grid_strip ? (int)log2((double)c->grid_strip) : -1);
+                                       c->nproj, c->M, c->npair, (float)(alpha * 1.4426950408889634), c->grid_strip ? (int)log2((double)c->grid_strip) : -1,
+                                       c->g_nitems, c->g_counter);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }

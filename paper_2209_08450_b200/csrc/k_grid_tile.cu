@@ -34,9 +34,10 @@ namespace tcpk {
 // ---------------------------------------------------------------------------------------
 // Plan: per tile and periodic image, the window [ja, ja + count) (mod nproj) of projections whose
 // ray can cross the tile.  One thread per (tile, image).
-__global__ void grid_plan_kernel(const float* __restrict__ theta, int nproj, int M, int MH, int2* __restrict__ plan) {
+__global__ void grid_plan_kernel(const float* __restrict__ theta, int nproj, int M, int MH, int2* __restrict__ plan, int* __restrict__ counter) {
     const int n = M >> 1, tiles = M / TS;
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx < 64) counter[idx] = 0;          // work counters of the persistent tcgen05 gridding CTAs
     if (idx >= tiles * tiles * 4) return;
     const int img = idx & 3, tile = idx >> 2;
     const int tx = tile % tiles, ty = tile / tiles;
@@ -396,12 +397,13 @@ int grid_tile_setup(tcp_ctx* c) {
         c->bytes += pb + red.size() * sizeof(int4);
     }
     TCP_CUDA_CHECK(cudaMalloc((void**)&c->g_plan, (size_t)tiles * tiles * 4 * sizeof(int2)));
+    TCP_CUDA_CHECK(cudaMalloc((void**)&c->g_counter, 64 * sizeof(int)));
     c->bytes += (size_t)tiles * tiles * 4 * sizeof(int2);
     return TCP_OK;
 }
 
 void grid_tile_free(tcp_ctx* c) {
-    cudaFree(c->g_items); cudaFree(c->g_red); cudaFree(c->g_partial); cudaFree(c->g_plan);
+    cudaFree(c->g_items); cudaFree(c->g_red); cudaFree(c->g_partial); cudaFree(c->g_plan); cudaFree(c->g_counter);
 }
 
 template <int MH, int NP, class TC>
@@ -428,7 +430,7 @@ static int launch_tile_np(const tcp_ctx* c, cudaStream_t st) {
 // storage) -> sum of the split near-DC tiles
 int launch_grid_tile(const tcp_ctx* c, const float* theta, cudaStream_t st) {
     const int tiles = c->M / TS, nplan = tiles * tiles * 4;
-    grid_plan_kernel<<<(nplan + 127) / 128, 128, 0, st>>>(theta, c->nproj, c->M, c->m, c->g_plan);
+    grid_plan_kernel<<<(nplan + 127) / 128, 128, 0, st>>>(theta, c->nproj, c->M, c->m, c->g_plan, c->g_counter);
     TCP_CUDA_CHECK(cudaGetLastError());
     int rc;
     if (c->grid_impl == TCP_GRID_MMA) rc = launch_grid_mma_main(c, st);

@@ -47,6 +47,7 @@ struct tcp_ctx {
     int4* g_red;
     float2* g_partial;
     int2* g_plan;
+    int* g_counter;       // [64] next-item counters of the persistent gridding CTAs, zeroed by the plan kernel
     int g_nitems, g_nred;
     size_t bytes;
     // per-kernel profiling (TCP_OPT_PROFILE): ring of event sets, TCP_NSTAGES + 1 events per call
