@@ -190,24 +190,34 @@ __device__ __forceinline__ void fft_pass(T* s, int tid, const float2* __restrict
 // calling group's own padded line of padded_len(N) float2.
 // NOTE: when the loader reads shared memory that the storer of a previous transform
 // wrote, the caller must __syncthreads() between the two calls.
-template <int N, bool INV, class T, class Load, class Store>
-__device__ __forceinline__ void fft_line(T* s, int tid, const float2* __restrict__ tw, Load ld, Store st) {
+struct NoHook {
+    __device__ __forceinline__ void operator()() const {}
+};
+
+// `hook` runs once, right after the first pass (every thread of the group has consumed the loader's
+// source by then: a caller may start refilling it).
+template <int N, bool INV, class T, class Load, class Store, class Hook = NoHook>
+__device__ __forceinline__ void fft_line(T* s, int tid, const float2* __restrict__ tw, Load ld, Store st, Hook hook = Hook()) {
     auto nold = [](int) { return T(); };
     auto nost = [](int, T) {};
     if constexpr (N == 128) {
         fft_pass<N, 16, 1, INV, true, false>(s, tid, tw, ld, nost);
+        hook();
         fft_pass<N, 8, 16, INV, false, true>(s, tid, tw, nold, st);
     } else if constexpr (N == 256) {
         fft_pass<N, 16, 1, INV, true, false>(s, tid, tw, ld, nost);
+        hook();
         fft_pass<N, 16, 16, INV, false, true>(s, tid, tw, nold, st);
     } else if constexpr (N == 8192) {
         fft_pass<N, 16, 1, INV, true, false>(s, tid, tw, ld, nost);
+        hook();
         fft_pass<N, 16, 16, INV, false, false>(s, tid, tw, nold, nost);
         fft_pass<N, 16, 256, INV, false, false>(s, tid, tw, nold, nost);
         fft_pass<N, 2, 4096, INV, false, true>(s, tid, tw, nold, st);
     } else {
         constexpr int RL = N / 256;     // 2, 4, 8 or 16
         fft_pass<N, 16, 1, INV, true, false>(s, tid, tw, ld, nost);
+        hook();
         fft_pass<N, 16, 16, INV, false, false>(s, tid, tw, nold, nost);
         fft_pass<N, RL, 256, INV, false, true>(s, tid, tw, nold, st);
     }

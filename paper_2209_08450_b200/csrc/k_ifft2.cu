@@ -74,6 +74,49 @@ __global__ void __launch_bounds__(cols_wp(M) * M / 16) ifft_cols_kernel(const TC
         });
 }
 
+// The same column pass as a persistent kernel for the strip-major grid of the fp16 path: one CTA per SM
+// (its lines fill most of the shared memory), so a CTA's global loads are not hidden by another CTA's
+// compute.  Here the next strip (a contiguous block of M x W half2) is copied into a staging buffer with
+// cp.async while the current strip is transformed, and the first pass reads its inputs from there.
+template <int M>
+__global__ void __launch_bounds__(cols_wp(M) * M / 16, 1) ifft_cols_pf_kernel(const __half2* __restrict__ grid,
+                                                                              __half2* __restrict__ pass1,
+                                                                              const float2* __restrict__ tw, int nunits) {
+    constexpr int n = M / 2, W = cols_w(M), WP = cols_wp(M), LS = cols_stride(M), NT = WP * M / 16;
+    constexpr int CHUNKS = M * W * (int)sizeof(__half2) / 16;       // 16-byte pieces of a strip
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cpair* smem = reinterpret_cast<cpair*>(smem_raw);
+    const __half2* stage = reinterpret_cast<const __half2*>(smem_raw + (size_t)WP * LS * sizeof(cpair));
+    const uint32_t stage_u32 = (uint32_t)__cvta_generic_to_shared(stage);
+    const int wp = threadIdx.x % WP, tid = threadIdx.x / WP;
+    cpair* s = smem + (size_t)wp * LS;
+    auto prefetch = [&](int unit) {                                  // unit = pair * (M / W) + strip: a contiguous block
+        if (unit < nunits) {
+            const unsigned char* g = reinterpret_cast<const unsigned char*>(grid + (size_t)unit * M * W);
+#pragma unroll
+            for (int c = threadIdx.x; c < CHUNKS; c += NT)
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(stage_u32 + c * 16), "l"(g + (size_t)c * 16) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    prefetch(blockIdx.x);
+#pragma unroll 1
+    for (int unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
+        const int pair = unit / (M / W), strip = unit % (M / W);
+        __half2* dst = pass1 + (size_t)pair * n * M + (size_t)strip * n * W + 2 * wp;
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();
+        fft_line<M, true>(
+            s, tid, tw, [&](int l2) { return ld_c2(stage, (size_t)l2 * W + 2 * wp); },
+            [&](int x2, cpair v) {
+                if (x2 < n / 2) st_c2(dst, (size_t)(x2 + n / 2) * W, v);
+                else if (x2 >= M - n / 2) st_c2(dst, (size_t)(x2 - (M - n / 2)) * W, v);
+            },
+            [&]() { prefetch(unit + gridDim.x); });
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+}
+
 template <int M, int ROWS, class TC, class TO>
 __global__ void __launch_bounds__(ROWS* M / 16) ifft_rows_kernel(const TC* __restrict__ pass1, TO* __restrict__ out,
                                                                  const float2* __restrict__ tw,
@@ -110,6 +153,17 @@ template <int M, class TC>
 static int launch_cols_t(const tcp_ctx* c, cudaStream_t st) {
     constexpr int W = cols_w(M), WP = cols_wp(M);
     const size_t smem = (size_t)WP * cols_stride(M) * sizeof(cpair);
+    if constexpr (sizeof(TC) == sizeof(__half2)) {
+        const size_t smem_pf = smem + (size_t)M * W * sizeof(__half2);
+        if (c->grid_strip == W && smem_pf <= 227 * 1024 && smem > 64 * 1024) {      // long lines, one CTA per SM
+            auto kpf = ifft_cols_pf_kernel<M>;
+            TCP_CUDA_CHECK(cudaFuncSetAttribute(kpf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_pf));
+            const int nunits = (M / W) * c->npair;
+            kpf<<<nunits < c->nsm ? nunits : c->nsm, WP * M / 16, smem_pf, st>>>((const __half2*)c->grid, (__half2*)c->pass1, c->tw, nunits);
+            TCP_CUDA_CHECK(cudaGetLastError());
+            return TCP_OK;
+        }
+    }
     auto kern = ifft_cols_kernel<M, TC>;
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid(M / W, c->npair);
