@@ -187,7 +187,7 @@ def run_ours(args, rank, world, local_rank):
         raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    w = sg.make_workload(args.workload)
+    w = sg.make_workload(args.workload, dtype=args.dtype or None)
     if args.nz_chunk:
         w.nz_chunk = args.nz_chunk
     nz_total = args.nz or w.nz_total
@@ -402,6 +402,8 @@ def main():
     ap.add_argument("--nz-chunk", type=int, default=0)
     ap.add_argument("--m", type=int, default=3, help="gridding kernel half-width")
     ap.add_argument("--e2e-nz", type=int, default=512, help="slices streamed through the host pipeline per step")
+    ap.add_argument("--dtype", default="", choices=["", "f32", "f16", "f16_out32"],
+                    help="override the workload's dtype (C2 is specified in both f32 and f16)")
     ap.add_argument("--fused-filter", action="store_true",
                     help="TCP_OPT_FILTER_FUSED: the uncropped one-transform reading of S3 + S4 (NOT the contract's default chain)")
     ap.add_argument("--algorithm", default="fourier", choices=["fourier", "line"],
