@@ -291,7 +291,11 @@ def run_ours(args, rank, world, local_rank):
         t = stage_ms[k] / max(ncalls, 1) * 1e-3               # average launch duration, s
         kernels[k] = {"ms_per_launch": t * 1e3, "share": stage_ms[k] / max(sum(stage_ms.values()), 1e-9),
                       "GBps": model[k]["bytes"] / t / 1e9 if t > 0 else None,
-                      "TFLOPps": model[k]["flops"] / t / 1e12 if t > 0 else None}
+                      "TFLOPps": model[k]["flops"] / t / 1e12 if t > 0 else None,
+                      # fractions of roofline: algorithmic bytes against the measured HBM peak, algorithmic flops
+                      # (5 N log2 N per transform, 4 per gridding tap, pair and sample) against the fp32 CUDA-core peak
+                      "hbm_frac": model[k]["bytes"] / t / 1e9 / hbm_gbs if t > 0 else None,
+                      "fp32_frac": model[k]["flops"] / t / 1e12 / alu_peak if t > 0 else None}
     dom = max(model, key=lambda k: stage_ms[k])
     traffic = None           # DRAM bytes per launch of the dominant kernel from the committed ncu capture
     try:
