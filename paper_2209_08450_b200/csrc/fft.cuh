@@ -16,6 +16,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <type_traits>
+
 namespace tcpk {
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
@@ -145,6 +147,22 @@ __device__ __forceinline__ void twiddle_powers(float2 w1, float2* w) {
 //   tw: table e^{-2 pi i t / N}, t in [0, N) (conjugated here for INV)
 //   FIRST: inputs come from ld(index); else from s[pad_idx(index)]
 //   LAST:  outputs go to st(index, value); else to s[pad_idx(index)]
+// A loader / storer may take the thread's register slot (compile-time after unrolling) as an extra
+// argument: the 16 outputs of a thread in the LAST pass of one transform and its 16 inputs in the FIRST
+// pass of the next are the same elements when both passes are radix 16 over 16 N/16-strided points
+// (tid + r N/16, slot r), so chained transforms can hand them over in registers instead of through
+// shared memory.
+template <class Load>
+__device__ __forceinline__ auto call_ld(Load& ld, int i, int slot) {
+    if constexpr (std::is_invocable_v<Load, int, int>) return ld(i, slot);
+    else return ld(i);
+}
+template <class Store, class T>
+__device__ __forceinline__ void call_st(Store& st, int i, T v, int slot) {
+    if constexpr (std::is_invocable_v<Store, int, T, int>) st(i, v, slot);
+    else st(i, v);
+}
+
 template <int N, int R, int NS, bool INV, bool FIRST, bool LAST, class T, class Load, class Store>
 __device__ __forceinline__ void fft_pass(T* s, int tid, const float2* __restrict__ tw, Load ld, Store st) {
     constexpr int TG = N / 16;
@@ -156,7 +174,7 @@ __device__ __forceinline__ void fft_pass(T* s, int tid, const float2* __restrict
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int i = b + r * (N / R);
-            if constexpr (FIRST) v[q * R + r] = ld(i);
+            if constexpr (FIRST) v[q * R + r] = call_ld(ld, i, q * R + r);
             else v[q * R + r] = s[pad_idx(i)];
         }
         if (NS > 1) {
@@ -177,11 +195,24 @@ __device__ __forceinline__ void fft_pass(T* s, int tid, const float2* __restrict
         const int o = (b / NS) * (NS * R) + (b % NS);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            if constexpr (LAST) st(o + r * NS, v[q * R + r]);
+            if constexpr (LAST) call_st(st, o + r * NS, v[q * R + r], q * R + r);
             else s[pad_idx(o + r * NS)] = v[q * R + r];
         }
     }
     if (!LAST) __syncthreads();
+}
+
+// Register hand-over between chained transforms of length N: a thread's 16 outputs of the LAST pass
+// (radix RL, 16 / RL butterflies b = tid + q N/16, outputs b + r N/RL, slot q RL + r) are the elements
+// tid + (q + (16 / RL) r) N/16, i.e. exactly its 16 inputs of the next transform's FIRST pass (radix 16,
+// input r' at tid + r' N/16, slot r') with r' = q + (16 / RL) r.
+__host__ __device__ constexpr int fft_last_radix(int N) {
+    return N == 128 ? 8 : N == 256 ? 16 : N == 8192 ? 2 : N / 256;      // plans below
+}
+template <int N>
+__host__ __device__ constexpr int fft_chain_slot(int last_slot) {
+    constexpr int RL = fft_last_radix(N);
+    return last_slot / RL + (16 / RL) * (last_slot % RL);
 }
 
 // Full transform.  Radix plans: 128: 16,8 | 256: 16,16 | 512: 16,16,2 | 1024: 16,16,4 |

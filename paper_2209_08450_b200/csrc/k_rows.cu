@@ -33,34 +33,30 @@ __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict
     const bool hasB = zB < nz;
     if (try_mode) ptab += (size_t)pair * M;
 
-    // FFT #1: zero-padded load, filter on store
-    fft_line<M, false>(
-        s, tid, tw,
-        [&](int i) {
-            // padding samples: zeros, or (TCP_OPT_PAD = TCP_PAD_EDGE) the nearest edge of the periodic row
-            if (i >= n) {
-                if (!pad_edge) return make_float2(0.f, 0.f);
-                i = (i < n + n / 2) ? n - 1 : 0;
-            }
-            return make_float2(ld_r(pA, i), hasB ? ld_r(pB, i) : 0.f);
-        },
-        [&](int k, float2 v) {
-            const float h = __ldg(&hfilt[k]);
-            s[pad_idx(k)] = make_float2(v.x * h, v.y * h);
-        });
-    __syncthreads();
-    // FFT #2 (inverse): crop to the detector on store
-    fft_line<M, true>(
-        s, tid, tw, [&](int i) { return s[pad_idx(i)]; },
-        [&](int i, float2 v) { s[pad_idx(i)] = (i < n) ? v : make_float2(0.f, 0.f); });
-    __syncthreads();
-    // FFT #3: spectrum, centre phase and scale on store
+    auto load_padded = [&](int i) {
+        // padding samples: zeros, or (TCP_OPT_PAD = TCP_PAD_EDGE) the nearest edge of the periodic row
+        if (i >= n) {
+            if (!pad_edge) return make_float2(0.f, 0.f);
+            i = (i < n + n / 2) ? n - 1 : 0;
+        }
+        return make_float2(ld_r(pA, i), hasB ? ld_r(pB, i) : 0.f);
+    };
     TC* out = spec + ((size_t)pair * nproj + j) * M;
-    fft_line<M, false>(
-        s, tid, tw, [&](int i) { return s[pad_idx(i)]; },
-        [&](int k, float2 v) {
-            if (live) st_c(out, k, cmul(v, __ldg(&ptab[k])));
-        });
+    // the three transforms hand their lines over in registers (fft_chain_slot: same elements, permuted slots):
+    // no shared-memory round trip and no barrier at the two boundaries; results are bit-identical
+    float2 keep[16];
+    // FFT #1: zero-padded load, filter on the way out
+    fft_line<M, false>(s, tid, tw, load_padded, [&](int k, float2 v, int slot) {
+        const float h = __ldg(&hfilt[k]);
+        keep[fft_chain_slot<M>(slot)] = make_float2(v.x * h, v.y * h);
+    });
+    // FFT #2 (inverse): crop to the detector on the way out
+    fft_line<M, true>(s, tid, tw, [&](int, int slot) { return keep[slot]; },
+                      [&](int i, float2 v, int slot) { keep[fft_chain_slot<M>(slot)] = (i < n) ? v : make_float2(0.f, 0.f); });
+    // FFT #3: spectrum, centre phase and scale on store
+    fft_line<M, false>(s, tid, tw, [&](int, int slot) { return keep[slot]; }, [&](int k, float2 v) {
+        if (live) st_c(out, k, cmul(v, __ldg(&ptab[k])));
+    });
 }
 
 // S3 + S4 fused without the crop (TCP_OPT_FILTER_FUSED; SURVEY 8(c) Q6's second reading, an option): one
@@ -118,6 +114,7 @@ __global__ void __launch_bounds__(ROWS* M / 16) filter_kernel(TS* __restrict__ s
     const bool hasB = zB < nz;
     TS* pA = sino + ((size_t)zA * nproj + j) * n;
     TS* pB = sino + ((size_t)(hasB ? zB : zA) * nproj + j) * n;
+    float2 keep[16];
     fft_line<M, false>(
         s, tid, tw,
         [&](int i) {
@@ -128,13 +125,12 @@ __global__ void __launch_bounds__(ROWS* M / 16) filter_kernel(TS* __restrict__ s
             }
             return make_float2(ld_r(pA, i), hasB ? ld_r(pB, i) : 0.f);
         },
-        [&](int k, float2 v) {
+        [&](int k, float2 v, int slot) {
             const float h = __ldg(&hfilt[k]);
-            s[pad_idx(k)] = make_float2(v.x * h, v.y * h);
+            keep[fft_chain_slot<M>(slot)] = make_float2(v.x * h, v.y * h);      // handed over in registers (fft.cuh)
         });
-    __syncthreads();
     fft_line<M, true>(
-        s, tid, tw, [&](int i) { return s[pad_idx(i)]; },
+        s, tid, tw, [&](int, int slot) { return keep[slot]; },
         [&](int i, float2 v) {
             if (live && i < n) {
                 st_r(pA, i, v.x);
