@@ -251,9 +251,18 @@ def run_ours(args, rank, world, local_rank):
     # ---- end to end: pinned host -> pinned host through the three-stream pipeline
     e2e = None
     if not args.no_e2e:
-        nz_e = min(nz_total, args.e2e_nz)
+        nz_e = min(nz_total, args.e2e_nz or nz_total)
         nz_e -= nz_e % nzc
-        raw_h = torch.empty((w.nproj, nz_e, n), dtype=torch.uint16).pin_memory()
+        while True:
+            try:
+                raw_h = torch.empty((w.nproj, nz_e, n), dtype=torch.uint16).pin_memory()
+                out_h = torch.empty((nz_e, n, n), dtype=out_dt).pin_memory()
+                break
+            except RuntimeError:          # not enough pinned host memory on this box: stream a shorter stack
+                raw_h = out_h = None
+                if nz_e <= 2 * nzc:
+                    raise
+                nz_e = (nz_e // 2) - (nz_e // 2) % nzc
         flat_h = torch.empty((nz_e, n), dtype=torch.float32).pin_memory()
         dark_h = torch.empty((nz_e, n), dtype=torch.float32).pin_memory()
         for ch in range(nz_e // nzc):
@@ -261,7 +270,6 @@ def run_ours(args, rank, world, local_rank):
             flat_h[ch * nzc:(ch + 1) * nzc].copy_(flat[ch])
             dark_h[ch * nzc:(ch + 1) * nzc].copy_(dark[ch])
         theta_h = torch.from_numpy(w.theta).pin_memory()
-        out_h = torch.empty((nz_e, n, n), dtype=out_dt).pin_memory()
         for _ in range(min(args.warmup, 2)):
             r.recon_volume_host(raw_h, flat_h, dark_h, theta_h, out_h, nbuf=3)
         barrier()
@@ -405,7 +413,8 @@ def main():
     ap.add_argument("--nz", type=int, default=0, help="override the number of slices in the volume")
     ap.add_argument("--nz-chunk", type=int, default=0)
     ap.add_argument("--m", type=int, default=3, help="gridding kernel half-width")
-    ap.add_argument("--e2e-nz", type=int, default=512, help="slices streamed through the host pipeline per step")
+    ap.add_argument("--e2e-nz", type=int, default=0,
+                    help="slices streamed through the host pipeline per step (0: the whole volume; halved if pinned host memory runs out)")
     ap.add_argument("--dtype", default="", choices=["", "f32", "f16", "f16_out32"],
                     help="override the workload's dtype (C2 is specified in both f32 and f16)")
     ap.add_argument("--fused-filter", action="store_true",
