@@ -13,16 +13,18 @@
 //
 // Work decomposition: an item is a 32 x 32 region of cells (or a projection sub-range of a near-DC
 // region, summed later in split order), shared with k_grid_tile.cu; the region is 8 sub-tiles of
-// 16 x 8 cells = the M = 128 rows of one TMEM accumulator each (8 x NN columns per CTA).
-// Every WARP owns one sub-tile and runs on its own, with no block barrier inside the loop:
+// 16 x 8 cells = the M = 128 rows of one TMEM accumulator each (8 x NN columns per CTA).  CTAs are
+// persistent: TMEM and barriers are set up once and items (heaviest first) are claimed from a counter
+// that the plan kernel zeroes.  Every WARP owns one sub-tile and runs on its own, with no block barrier
+// inside the loop:
 //   * 32 lanes test 32 projections of the region's window against the sub-tile's sample box; a chord
 //     crosses the box in one run of consecutive k; a warp scan lays the runs end to end as columns;
 //   * 32 columns at a time (two MMA K steps), one lane per column: floor/fraction of k cos, k sin by
-//     float-float FMAs, the 2m Gaussian taps of each axis scattered into a zeroed 16- / 8-entry row
-//     (phase 1) and the column's B row (its NN spectrum values) gathered from global memory; then,
-//     once the warp's previous MMAs have released the stage, the outer products wy x wx are written
-//     as the MN-major A stage (phase 2) and lane 0 issues the two MMAs and commits them to the warp's
-//     mbarrier: the MMAs of one step run under phase 1 of the next.
+//     float-float FMAs, the column's B row (its NN spectrum values) gathered from global memory, and
+//     the Gaussian weights of both axes per CELL POSITION of the sub-tile (16 + 8 values, zero outside
+//     the open box) in registers (phase 1); then, once the warp's previous MMAs have released the stage,
+//     the outer products wy x wx are written as the MN-major A stage (phase 2) and lane 0 issues the two
+//     MMAs and commits them to the warp's mbarrier: the MMAs of one step run under phase 1 of the next.
 // Fixed summation order per accumulator, no atomics => bitwise reproducible.
 #include <math.h>
 #include <stdio.h>
