@@ -67,8 +67,12 @@ enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1, TCP_GRID_TILE = 2, TCP_
  * with NO crop of the filtered row in between: one transform per row instead of three, and a slightly different
  * image (the tails of the filtered row outside the detector are backprojected too).  FourierRec, tcp_recon and
  * tcp_recon_volume_host only; tcp_recon_try keeps the default chain. */
+/* TCP_OPT_WEIGHT_CACHE (1 default | 0): the tensor-core gridding keeps the interpolation weights of every
+ * (sub-tile, sample), which depend only on theta, n and m, in a device cache built on the first call and
+ * rebuilt (on the device, no host synchronisation) whenever the angles passed to tcp_recon change; 0 computes
+ * them in every call.  Same results bit for bit. */
 enum { TCP_OPT_GRID_IMPL = 0, TCP_OPT_PROFILE = 1, TCP_OPT_TCFFT = 2, TCP_OPT_ALGORITHM = 3, TCP_OPT_PAD = 4,
-       TCP_OPT_FILTER_FUSED = 5 };
+       TCP_OPT_FILTER_FUSED = 5, TCP_OPT_WEIGHT_CACHE = 6 };
 enum { TCP_PAD_ZERO = 0, TCP_PAD_EDGE = 1 };
 enum { TCP_ALG_FOURIER = 0, TCP_ALG_LINE = 1 };
 enum { TCP_TCFFT_ROWS = 1, TCP_TCFFT_COLS = 2, TCP_TCFFT_IROWS = 4 };

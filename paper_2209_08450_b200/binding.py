@@ -178,6 +178,10 @@ class Recon:
     def set_grid_impl(self, name: str):
         _check(lib().tcp_set_option(self.h, 0, GRID_IMPLS[name]))
 
+    def set_weight_cache(self, on: bool):
+        """TCP_OPT_WEIGHT_CACHE: reuse the gridding weights across calls with the same angles (default on)."""
+        _check(lib().tcp_set_option(self.h, 6, 1 if on else 0))
+
     def set_filter_fused(self, on: bool):
         """TCP_OPT_FILTER_FUSED: S3 + S4 as one transform without the crop (a different reading; off by default)."""
         _check(lib().tcp_set_option(self.h, 5, 1 if on else 0))

@@ -30,6 +30,8 @@
 #include <stdio.h>
 #include <stdlib.h>
 
+#include <algorithm>
+
 #include "grid_common.cuh"
 #include "umma.cuh"
 #include "tcp_internal.h"
@@ -74,11 +76,28 @@ struct MmaSmem {
 
 // ---------------------------------------------------------------------------------------
 // item: x = region (32 x 32 tile) index, y = split s | nsplit S << 16, z = first partial slot (-1: write the grid)
-template <int MH, int NN>
+//
+// MODE: the weights depend only on the geometry (theta, M, m), not on the data, so they are computed once per
+// set of angles and replayed for every chunk (WeightCache, below):
+//   GM_DIRECT  enumerate, weigh and multiply-accumulate in one go (no usable cache: too large, or disabled)
+//   GM_COUNT   enumerate only: K steps per (item, sub-tile)                       } run when the angles changed
+//   GM_FILL    enumerate and weigh: one record per step and column into the cache  }
+//   GM_CACHED  replay the records: gather, outer product, multiply-accumulate
+enum { GM_DIRECT = 0, GM_COUNT = 1, GM_FILL = 2, GM_CACHED = 3 };
+enum { WS_CHECKSUM = 0, WS_USABLE = 1, WS_REBUILD = 2, WS_ACC = 3 };       // WeightCache::state
+
+template <int MH, int NN, int MODE>
 __global__ void __launch_bounds__(32 * CW, 16 / CW)
     grid_mma_kernel(const __half2* __restrict__ spec, __half2* __restrict__ grid, float2* __restrict__ partial,
                     const float4* __restrict__ trigf, const int2* __restrict__ plan, const int4* __restrict__ items,
-                    int nproj, int M, int npair, float alpha2, int strip_log2, int nitems, int* __restrict__ counter) {
+                    int nproj, int M, int npair, float alpha2, int strip_log2, int nitems, int* __restrict__ counter,
+                    const int* __restrict__ wstate, int* __restrict__ wcount, const int* __restrict__ woff,
+                    uint4* __restrict__ wrec, unsigned* __restrict__ wsamp) {
+    if (MODE == GM_DIRECT && wstate[WS_USABLE]) return;
+    if (MODE == GM_CACHED && !wstate[WS_USABLE]) return;
+    if (MODE == GM_COUNT && !wstate[WS_REBUILD]) return;
+    if (MODE == GM_FILL && !(wstate[WS_REBUILD] && wstate[WS_USABLE])) return;
+    constexpr bool MMA = MODE == GM_DIRECT || MODE == GM_CACHED;
     using L = MmaSmem<NN>;
     constexpr int GW = L::GW, NPG = NN / 2;
     extern __shared__ __align__(128) unsigned char smem[];
@@ -89,18 +108,20 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L::offBar) + warp * NST;
 
-    if (lane == 0) {
-        for (int s = 0; s < NST; ++s) mbar_init(&bar[s], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;");
+    if (MMA) {
+        if (lane == 0) {
+            for (int s = 0; s < NST; ++s) mbar_init(&bar[s], 1);
+            asm volatile("fence.mbarrier_init.release.cluster;");
+        }
+        if (warp == 0) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&misc[0])), "n"(CW * NN));
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;");
+        __syncthreads();
+        asm volatile("tcgen05.fence::after_thread_sync;");
     }
-    if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&misc[0])), "n"(CW * NN));
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;");
-    __syncthreads();
-    asm volatile("tcgen05.fence::after_thread_sync;");
-    const uint32_t tmem = misc[0];
+    const uint32_t tmem = MMA ? misc[0] : 0u;
     // instruction descriptor: D fp32, A/B fp16, both MN-major, N = NN, M = 128
     constexpr uint32_t IDESC = (1u << 4) | (1u << 15) | (1u << 16) | ((uint32_t)(NN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
 
@@ -119,9 +140,71 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
     const __half2* plane0 = spec + (size_t)(pg * NPG) * pstride;                  // first plane of this pair group
     const int nvalid = min(NPG, npair - pg * NPG);                                // planes that exist
 
+    // the column's B row (NPG spectrum values, one per slice pair of the group) from sample offset `samp`
+    auto gather = [&](unsigned samp, __half2* bv) {
+        const unsigned char* a = reinterpret_cast<const unsigned char*>(plane0 + samp);
+        if (nvalid == NPG) {
+#pragma unroll
+            for (int p = 0; p < NPG; ++p) {
+                bv[p] = __ldg(reinterpret_cast<const __half2*>(a));
+                a += pstride_b;
+            }
+        } else {
+#pragma unroll
+            for (int p = 0; p < NPG; ++p) {
+                bv[p] = __ldg(reinterpret_cast<const __half2*>(a));
+                if (p + 1 < nvalid) a += pstride_b;
+            }
+        }
+    };
+    uint32_t istep = 0;                                      // K steps of the current item (0: the accumulator holds nothing)
+    // one stage: B rows and the A tile (outer products wy x wx) of 32 columns into shared memory, two MMAs
+    auto issue_step = [&](const uint4& xa, const uint4& xc, const uint4& yv, const __half2* bv, bool two) {
+        // the warp's previous MMAs must have read the stage before it is overwritten
+        if (nstep > 0) mbar_wait(bar, (nstep - 1) & 1);
+        {
+            unsigned char* brow = Bw + (cl >> 3) * L::B_LBO + (cl & 7) * 16;
+            const uint4* vv = reinterpret_cast<const uint4*>(bv);
+#pragma unroll
+            for (int q = 0; q < GW; ++q) *reinterpret_cast<uint4*>(brow + q * 128) = vv[q];
+        }
+        // ---- phase 2: A[m = ly * 16 + lx][column] = wy[ly] * wx[lx]; MN-major: 8 cells of a column = 16 B
+        {
+            const unsigned yw[4] = {yv.x, yv.y, yv.z, yv.w};
+            unsigned char* arow = Aw + (cl >> 3) * A_LBO + (cl & 7) * 16;
+#pragma unroll
+            for (int r = 0; r < SUBY; ++r) {
+                const unsigned yb = (r & 1) ? (yw[r >> 1] >> 16) : (yw[r >> 1] & 0xffffu);
+                uint4 lo4 = make_uint4(0, 0, 0, 0), hi4 = lo4;
+                if (yb != 0) {
+                    const unsigned y2 = yb | (yb << 16);
+                    auto mul = [&](unsigned x) {
+                        const __half2 pr = __hmul2(*reinterpret_cast<const __half2*>(&x), *reinterpret_cast<const __half2*>(&y2));
+                        return *reinterpret_cast<const unsigned*>(&pr);
+                    };
+                    lo4 = make_uint4(mul(xa.x), mul(xa.y), mul(xa.z), mul(xa.w));
+                    hi4 = make_uint4(mul(xc.x), mul(xc.y), mul(xc.z), mul(xc.w));
+                }
+                *reinterpret_cast<uint4*>(arow + (2 * r) * 128) = lo4;
+                *reinterpret_cast<uint4*>(arow + (2 * r + 1) * 128) = hi4;
+            }
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            umma_f16(acc, adesc0, bdesc0, IDESC, istep > 0 ? 1u : 0u);
+            if (two) umma_f16(acc, adesc1, bdesc1, IDESC, 1u);
+            umma_commit(bar);
+        }
+        ++nstep;
+        ++istep;
+        __syncwarp();
+    };
+
     // persistent CTA: items claimed from a counter, heaviest regions first (TMEM allocation, barrier set-up and
     // launch cost once per CTA, not per item)
-    int* const ctr = counter + (blockIdx.y * gridDim.z + blockIdx.z);
+    int* const ctr = counter + (MODE * 16 + blockIdx.y * gridDim.z + blockIdx.z);
 #pragma unroll 1
     for (;;) {
     if (tid == 0) misc[12] = (uint32_t)atomicAdd(ctr, 1);
@@ -131,7 +214,38 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
     const int4 item = items[it];
     const int tile = item.x, split = item.y & 0xffff, nsplit = item.y >> 16;
     const int TX0 = (tile % tiles) * TS, TY0 = (tile / tiles) * TS;
-    uint32_t istep = 0;                                      // K steps of this item (0: the accumulator holds nothing)
+    istep = 0;
+    const int wbase = (MODE == GM_FILL || MODE == GM_CACHED) ? woff[it * NSUB + sub] : 0;
+    if constexpr (MODE == GM_CACHED) {
+        // replay, software-pipelined two deep: the gather of step s + 1 and the sample offsets of step s + 2 are in
+        // flight while step s is staged (a step is otherwise two dependent global-load latencies with nothing to hide them)
+        const int ns = wcount[it * NSUB + sub];
+        if (ns > 0) {
+            const size_t st0 = (size_t)wbase;
+            alignas(16) __half2 bvA[NPG], bvB[NPG];
+            uint4 xaA = __ldg(&wrec[(st0 * 3 + 0) * 32 + lane]), xcA = __ldg(&wrec[(st0 * 3 + 1) * 32 + lane]);
+            uint4 yvA = __ldg(&wrec[(st0 * 3 + 2) * 32 + lane]);
+            gather(__ldg(&wsamp[st0 * 32 + lane]), bvA);
+            unsigned samp_next = ns > 1 ? __ldg(&wsamp[(st0 + 1) * 32 + lane]) : 0u;
+#pragma unroll 1
+            for (int sidx = 0; sidx < ns; ++sidx) {
+                const size_t st = st0 + sidx + 1;
+                const bool more = sidx + 1 < ns;
+                uint4 xaB = xaA, xcB = xcA, yvB = yvA;
+                if (more) {
+                    gather(samp_next, bvB);
+                    xaB = __ldg(&wrec[(st * 3 + 0) * 32 + lane]);
+                    xcB = __ldg(&wrec[(st * 3 + 1) * 32 + lane]);
+                    yvB = __ldg(&wrec[(st * 3 + 2) * 32 + lane]);
+                    if (sidx + 2 < ns) samp_next = __ldg(&wsamp[(st + 1) * 32 + lane]);
+                }
+                issue_step(xaA, xcA, yvA, bvA, true);
+                xaA = xaB; xcA = xcB; yvA = yvB;
+#pragma unroll
+                for (int p = 0; p < NPG; ++p) bvA[p] = bvB[p];
+            }
+        }
+    } else
     for (int img = 0; img < 4; ++img) {
         const int2 win = plan[tile * 4 + img];
         if (win.y == 0) continue;
@@ -165,6 +279,10 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
             const int total = __shfl_sync(0xffffffffu, incl, 31);
             const int off = incl - cnt;
 
+            if constexpr (MODE == GM_COUNT) {
+                istep += (uint32_t)((total + SC - 1) / SC);
+                continue;
+            }
             for (int c0 = 0; c0 < total; c0 += SC) {
                 const int col = c0 + cl;
                 const bool valid = col < total;
@@ -187,23 +305,9 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                 // the step re-reads a valid sample and carries all-zero weights (0 x finite = 0), a plane past
                 // the last pair re-reads the last plane and is dropped by the epilogue.  Byte pointers keep the
                 // per-plane address arithmetic at one 64-bit add.
+                const unsigned samp = (unsigned)jj * (unsigned)M + (unsigned)(k & (M - 1));
                 alignas(16) __half2 bv[NPG];
-                {
-                    const unsigned char* a = reinterpret_cast<const unsigned char*>(plane0 + ((size_t)jj * M + (size_t)(k & (M - 1))));
-                    if (nvalid == NPG) {
-#pragma unroll
-                        for (int p = 0; p < NPG; ++p) {
-                            bv[p] = __ldg(reinterpret_cast<const __half2*>(a));
-                            a += pstride_b;
-                        }
-                    } else {
-#pragma unroll
-                        for (int p = 0; p < NPG; ++p) {
-                            bv[p] = __ldg(reinterpret_cast<const __half2*>(a));
-                            if (p + 1 < nvalid) a += pstride_b;
-                        }
-                    }
-                }
+                if constexpr (MODE == GM_DIRECT) gather(samp, bv);
                 // ---- phase 1: the weights of both axes, per CELL POSITION of the sub-tile and in registers (no
                 // scatter through shared memory: the kernel is bound by the L1 data pipe, the MUFU and FMA
                 // pipes idle).  Cell X = SX + lx is tap a = X - floor(nu) of the sample (an exact small integer),
@@ -238,48 +342,24 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                     xc = make_uint4(wx[4], wx[5], wx[6], wx[7]);
                     yv = make_uint4(wy[0], wy[1], wy[2], wy[3]);
                 }
-                // the warp's previous MMAs must have read the stage before it is overwritten
-                if (nstep > 0) mbar_wait(bar, (nstep - 1) & 1);
-                {
-                    unsigned char* brow = Bw + (cl >> 3) * L::B_LBO + (cl & 7) * 16;
-                    const uint4* vv = reinterpret_cast<const uint4*>(bv);
-#pragma unroll
-                    for (int q = 0; q < GW; ++q) *reinterpret_cast<uint4*>(brow + q * 128) = vv[q];
+                if constexpr (MODE == GM_FILL) {
+                    // record of this step and column: [step][xa | xc | yv][lane] and the sample offset
+                    const size_t st = (size_t)wbase + istep;
+                    wrec[(st * 3 + 0) * 32 + lane] = xa;
+                    wrec[(st * 3 + 1) * 32 + lane] = xc;
+                    wrec[(st * 3 + 2) * 32 + lane] = yv;
+                    wsamp[st * 32 + lane] = samp;
+                    ++istep;
+                } else {
+                    issue_step(xa, xc, yv, bv, total - c0 > 16);
                 }
-                // ---- phase 2: A[m = ly * 16 + lx][column] = wy[ly] * wx[lx]; MN-major: 8 cells of a column = 16 B
-                {
-                    const unsigned yw[4] = {yv.x, yv.y, yv.z, yv.w};
-                    unsigned char* arow = Aw + (cl >> 3) * A_LBO + (cl & 7) * 16;
-#pragma unroll
-                    for (int r = 0; r < SUBY; ++r) {
-                        const unsigned yb = (r & 1) ? (yw[r >> 1] >> 16) : (yw[r >> 1] & 0xffffu);
-                        uint4 lo4 = make_uint4(0, 0, 0, 0), hi4 = lo4;
-                        if (yb != 0) {
-                            const unsigned y2 = yb | (yb << 16);
-                            auto mul = [&](unsigned x) {
-                                const __half2 pr = __hmul2(*reinterpret_cast<const __half2*>(&x), *reinterpret_cast<const __half2*>(&y2));
-                                return *reinterpret_cast<const unsigned*>(&pr);
-                            };
-                            lo4 = make_uint4(mul(xa.x), mul(xa.y), mul(xa.z), mul(xa.w));
-                            hi4 = make_uint4(mul(xc.x), mul(xc.y), mul(xc.z), mul(xc.w));
-                        }
-                        *reinterpret_cast<uint4*>(arow + (2 * r) * 128) = lo4;
-                        *reinterpret_cast<uint4*>(arow + (2 * r + 1) * 128) = hi4;
-                    }
-                }
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                __syncwarp();
-                if (lane == 0) {
-                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    umma_f16(acc, adesc0, bdesc0, IDESC, istep > 0 ? 1u : 0u);
-                    if (total - c0 > 16) umma_f16(acc, adesc1, bdesc1, IDESC, 1u);
-                    umma_commit(bar);
-                }
-                ++nstep;
-                ++istep;
-                __syncwarp();
             }
         }
+    }
+    if constexpr (!MMA) {
+        if (MODE == GM_COUNT && lane == 0) wcount[it * NSUB + sub] = (int)istep;
+        __syncthreads();                 // everyone has read misc[12] before the next claim
+        continue;
     }
     // ---- this warp's MMAs complete (commits complete in order: wait for the last one)
     if (istep > 0) mbar_wait(bar, (nstep - 1) & 1);
@@ -330,26 +410,117 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     }   // items
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(CW * NN));
+    if (MMA && warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(CW * NN));
 }
 
 // ---------------------------------------------------------------------------------------
-template <int MH, int NN>
-static int launch_mma_t(const tcp_ctx* c, cudaStream_t st) {
+// WeightCache bookkeeping (device side only: tcp_recon never synchronises with the host).
+// state[WS_ACC] collects a checksum of the angles in trig_kernel; wc_decide_kernel compares it with the one the
+// cache was built for and raises WS_REBUILD; the count / scan / fill kernels then run (they exit at once
+// otherwise) and WS_USABLE tells the multiply-accumulate kernels which of the two (cached, direct) works.
+__global__ void wc_decide_kernel(int* __restrict__ state, int enable) {
+    const int cs = state[WS_ACC];
+    state[WS_ACC] = 0;
+    if (!enable) { state[WS_USABLE] = 0; state[WS_REBUILD] = 0; return; }
+    if (!state[WS_USABLE] || cs != state[WS_CHECKSUM]) {
+        state[WS_CHECKSUM] = cs;
+        state[WS_USABLE] = 0;
+        state[WS_REBUILD] = 1;
+    } else {
+        state[WS_REBUILD] = 0;
+    }
+}
+
+// exclusive scan of the step counts (one block); the cache is usable if everything fits
+__global__ void __launch_bounds__(1024) wc_scan_kernel(const int* __restrict__ count, int* __restrict__ off, int nentries, int cap,
+                                                       int* __restrict__ state) {
+    if (!state[WS_REBUILD]) return;
+    __shared__ long long part[1024];
+    const int t = threadIdx.x, per = (nentries + 1023) / 1024;
+    const int lo = t * per, hi = min(nentries, lo + per);
+    long long sum = 0;
+    for (int i = lo; i < hi; ++i) sum += count[i];
+    part[t] = sum;
+    __syncthreads();
+    for (int d = 1; d < 1024; d <<= 1) {
+        const long long v = (t >= d) ? part[t - d] : 0;
+        __syncthreads();
+        part[t] += v;
+        __syncthreads();
+    }
+    const long long total = part[1023];
+    long long run = part[t] - sum;
+    if (total <= (long long)cap) {
+        for (int i = lo; i < hi; ++i) {
+            off[i] = (int)run;
+            run += count[i];
+        }
+    }
+    if (t == 0) state[WS_USABLE] = (total <= (long long)cap) ? 1 : 0;
+}
+
+template <int MH, int NN, int MODE>
+static int launch_mma_mode(const tcp_ctx* c, cudaStream_t st) {
     using L = MmaSmem<NN>;
-    auto kern = grid_mma_kernel<MH, NN>;
+    auto kern = grid_mma_kernel<MH, NN, MODE>;
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L::total));
     const double alpha = 3.14159265358979323846 / (1.4142135623730951 * MH);
-    const int ny = (c->npair + NN / 2 - 1) / (NN / 2), nz = NSUB / CW;
+    const bool mma = MODE == GM_DIRECT || MODE == GM_CACHED;
+    const int ny = mma ? (c->npair + NN / 2 - 1) / (NN / 2) : 1, nz = NSUB / CW;
     int ctas = (c->nsm * (16 / CW) + ny * nz - 1) / (ny * nz);            // resident CTAs per (pair group, region part)
     if (ctas > c->g_nitems) ctas = c->g_nitems;
     if (ctas < 1) ctas = 1;
     dim3 grid(ctas, ny, nz);
     kern<<<grid, 32 * CW, L::total, st>>>((const __half2*)c->spec, (__half2*)c->grid, c->g_partial, c->trigf, c->g_plan, c->g_items,
                                        c->nproj, c->M, c->npair, (float)(alpha * 1.4426950408889634), c->grid_strip ? (int)log2((double)c->grid_strip) : -1,
-                                       c->g_nitems, c->g_counter);
+                                       c->g_nitems, c->g_counter, c->w_state, c->w_count, c->w_off, c->w_rec, c->w_samp);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
+}
+
+template <int MH, int NN>
+static int launch_mma_t(const tcp_ctx* c, cudaStream_t st) {
+    int rc;
+    wc_decide_kernel<<<1, 1, 0, st>>>(c->w_state, c->w_cap > 0 && c->w_enable ? 1 : 0);
+    if (c->w_cap > 0) {
+        if ((rc = launch_mma_mode<MH, 16, GM_COUNT>(c, st))) return rc;
+        wc_scan_kernel<<<1, 1024, 0, st>>>(c->w_count, c->w_off, c->g_nitems * NSUB, c->w_cap, c->w_state);
+        if ((rc = launch_mma_mode<MH, 16, GM_FILL>(c, st))) return rc;
+        if ((rc = launch_mma_mode<MH, NN, GM_CACHED>(c, st))) return rc;
+    }
+    return launch_mma_mode<MH, NN, GM_DIRECT>(c, st);
+}
+
+// weight cache storage: called from grid_tile_setup for fp16 storage.  Capacity: every sample lands in about
+// 2.4 sub-tile boxes (halo), 32 columns per step, partially filled last steps: 1.6 x slack; beyond it the
+// direct kernel runs.
+int grid_mma_cache_setup(tcp_ctx* c) {
+    c->w_enable = 1;
+    c->w_cap = 0;
+    if (cudaMalloc((void**)&c->w_state, 4 * sizeof(int)) != cudaSuccess) { cudaGetLastError(); c->w_state = nullptr; return set_error(TCP_ENOMEM, "weight cache state"); }
+    cudaMemset(c->w_state, 0, 4 * sizeof(int));
+    c->bytes += 16;
+    const size_t nent = (size_t)c->g_nitems * NSUB;
+    const double steps = (double)c->nproj * (double)c->M * 2.4 / 32.0 * 1.6 + 4.0 * (double)nent;
+    const size_t cap = (size_t)std::min(steps, 2.0e9 / 1.0);
+    size_t freeb = 0, totalb = 0;
+    cudaMemGetInfo(&freeb, &totalb);
+    const size_t need = cap * (3 * 32 * sizeof(uint4) + 32 * sizeof(unsigned)) + 2 * nent * sizeof(int);
+    if (need > freeb / 4) return TCP_OK;                                  // leave the memory to the caller: direct kernel
+    if (cudaMalloc((void**)&c->w_count, nent * sizeof(int)) != cudaSuccess || cudaMalloc((void**)&c->w_off, nent * sizeof(int)) != cudaSuccess ||
+        cudaMalloc((void**)&c->w_rec, cap * 3 * 32 * sizeof(uint4)) != cudaSuccess || cudaMalloc((void**)&c->w_samp, cap * 32 * sizeof(unsigned)) != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(c->w_count); cudaFree(c->w_off); cudaFree(c->w_rec); cudaFree(c->w_samp);
+        c->w_count = c->w_off = nullptr; c->w_rec = nullptr; c->w_samp = nullptr;
+        return TCP_OK;
+    }
+    c->w_cap = (int)std::min<size_t>(cap, 2000000000u);
+    c->bytes += need;
+    return TCP_OK;
+}
+
+void grid_mma_cache_free(tcp_ctx* c) {
+    cudaFree(c->w_state); cudaFree(c->w_count); cudaFree(c->w_off); cudaFree(c->w_rec); cudaFree(c->w_samp);
 }
 
 // Enqueue the tensor-core gridding of the spectrum into the grid (fp16 storage only); the plan

@@ -399,11 +399,13 @@ int grid_tile_setup(tcp_ctx* c) {
     TCP_CUDA_CHECK(cudaMalloc((void**)&c->g_plan, (size_t)tiles * tiles * 4 * sizeof(int2)));
     TCP_CUDA_CHECK(cudaMalloc((void**)&c->g_counter, 64 * sizeof(int)));
     c->bytes += (size_t)tiles * tiles * 4 * sizeof(int2);
+    if (c->half_store) return grid_mma_cache_setup(c);
     return TCP_OK;
 }
 
 void grid_tile_free(tcp_ctx* c) {
     cudaFree(c->g_items); cudaFree(c->g_red); cudaFree(c->g_partial); cudaFree(c->g_plan); cudaFree(c->g_counter);
+    grid_mma_cache_free(c);
 }
 
 template <int MH, int NP, class TC>

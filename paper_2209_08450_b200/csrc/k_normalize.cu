@@ -150,9 +150,12 @@ int launch_mean_frames(const uint16_t* frames, int nframes, int nz, int n, float
 
 // cos/sin of the float32 angles in fp64: k*cos(theta) with
 // k up to 4096 must be good to ~1e-6 grid cells for the 1e-5 fp32 gate.
-__global__ void trig_kernel(const float* __restrict__ theta, int nproj, double2* __restrict__ trig, float4* __restrict__ trigf) {
+__global__ void trig_kernel(const float* __restrict__ theta, int nproj, double2* __restrict__ trig, float4* __restrict__ trigf,
+                            int* __restrict__ wstate) {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j < nproj) {
+        // order-independent checksum of the angles for the gridding weight cache (k_grid_mma.cu, state[3])
+        if (wstate) atomicAdd(&wstate[3], (int)((__float_as_uint(theta[j]) ^ 0x9e3779b9u) * (2u * (unsigned)j + 1u)));
         double t = (double)theta[j];
         const double c = cos(t), s = sin(t);
         trig[j] = make_double2(c, s);
@@ -164,7 +167,7 @@ __global__ void trig_kernel(const float* __restrict__ theta, int nproj, double2*
 }
 
 int launch_trig(const tcp_ctx* c, const float* theta, cudaStream_t st) {
-    trig_kernel<<<(c->nproj + 127) / 128, 128, 0, st>>>(theta, c->nproj, c->trig, c->trigf);
+    trig_kernel<<<(c->nproj + 127) / 128, 128, 0, st>>>(theta, c->nproj, c->trig, c->trigf, c->w_state);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }

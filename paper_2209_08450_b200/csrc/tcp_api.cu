@@ -349,7 +349,9 @@ int tcp_profile_collect(tcp_ctx* c, double* ms_sum, int* ncalls) {
 int tcp_launches_per_recon(const tcp_ctx* c) {
     if (!c) return 0;
     if (c->algorithm == TCP_ALG_LINE) return 4;                          // trig, normalise, filter, backprojection
-    if (c->grid_impl == TCP_GRID_TILE || c->grid_impl == TCP_GRID_MMA) return 7 + (c->g_nred ? 1 : 0);   // + plan (+ reduce)
+    if (c->grid_impl == TCP_GRID_MMA)       // + plan, cache decide (+ count, scan, fill, cached kernel: most exit at once) (+ reduce)
+        return 8 + (c->w_cap > 0 ? 4 : 0) + (c->g_nred ? 1 : 0);
+    if (c->grid_impl == TCP_GRID_TILE) return 7 + (c->g_nred ? 1 : 0);   // + plan (+ reduce)
     return c->grid_impl == TCP_GRID_SCATTER_ATOMIC ? 6 : 6;              // (scatter adds a memset, not a kernel)
 }
 
@@ -393,6 +395,10 @@ int tcp_set_option(tcp_ctx* c, int option, int value) {
         if (value == TCP_GRID_MMA && !c->half_store) return set_error(TCP_EUNSUPPORTED, "tensor-core gridding needs fp16 storage");
         c->grid_impl = value;
         c->grid_strip = (value == TCP_GRID_MMA) ? cols_strip_width(c->M) : 0;
+        return TCP_OK;
+    }
+    if (option == TCP_OPT_WEIGHT_CACHE) {
+        c->w_enable = value != 0;
         return TCP_OK;
     }
     if (option == TCP_OPT_FILTER_FUSED) {

@@ -47,6 +47,8 @@ struct tcp_ctx {
     int4* g_red;
     float2* g_partial;
     int2* g_plan;
+    // weight cache of the tcgen05 gridding (k_grid_mma.cu): per-step records, built on the device when theta changes
+    int* w_state; int* w_count; int* w_off; uint4* w_rec; unsigned* w_samp; int w_cap, w_enable;
     int* g_counter;       // [64] next-item counters of the persistent gridding CTAs, zeroed by the plan kernel
     int g_nitems, g_nred;
     size_t bytes;
@@ -80,6 +82,8 @@ int launch_grid_scatter(const tcp_ctx* c, cudaStream_t st);
 int launch_grid_gather(const tcp_ctx* c, const float* theta, cudaStream_t st);
 int launch_grid_tile(const tcp_ctx* c, const float* theta, cudaStream_t st);
 int launch_grid_mma_main(const tcp_ctx* c, cudaStream_t st);
+int grid_mma_cache_setup(tcp_ctx* c);
+void grid_mma_cache_free(tcp_ctx* c);
 int grid_tile_setup(tcp_ctx* c);
 void grid_tile_free(tcp_ctx* c);
 int launch_ifft_cols(const tcp_ctx* c, cudaStream_t st);

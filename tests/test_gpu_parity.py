@@ -345,6 +345,35 @@ def test_fused_filter_option(dtype, pad):
     r.close()
 
 
+def test_gridding_weight_cache():
+    """TCP_OPT_WEIGHT_CACHE: the cached replay equals the direct kernel bit for bit; the cache follows a change of
+    the angles between calls (rebuilt on the device) and of nothing else."""
+    tcp = _tcp()
+    w = sg.make_workload("C1")
+    raw, flat, dark, theta = _inputs(w, list(range(8)))
+    d = _to_dev(raw, flat, dark, theta)
+    r = tcp.Recon(w.n, w.nproj, 8, w.center, "f16", w.filter, 3)
+    r.set_weight_cache(False)
+    direct = r.recon(*d).clone()
+    r.set_weight_cache(True)
+    first = r.recon(*d).clone()          # builds the cache
+    second = r.recon(*d).clone()         # replays it
+    assert torch.equal(first, direct) and torch.equal(second, direct)
+    # other angles: uneven, limited range
+    th2 = np.sort((w.theta * 0.8 + 0.05 + 0.002 * np.sin(np.arange(w.nproj))).astype(np.float32))
+    d2 = (d[0], d[1], d[2], torch.from_numpy(th2).cuda())
+    a = r.recon(*d2).clone()
+    r.set_weight_cache(False)
+    b = r.recon(*d2).clone()
+    assert torch.equal(a, b)
+    ref = orc.recon(raw[:, 3:4], flat[3:4], dark[3:4], th2, w.center, w.filter, 3, "grid")[0]
+    assert rl2(a[3].float().cpu().numpy(), ref) < FP16_GATE_L2
+    # back to the first angles
+    r.set_weight_cache(True)
+    assert torch.equal(r.recon(*d), direct)
+    r.close()
+
+
 def test_mean_frames_and_errors():
     tcp = _tcp()
     rng = np.random.default_rng(0)
