@@ -230,3 +230,29 @@ def recon(raw, flat, dark, theta, center, filt="ramp", m=DEFAULT_M, method="grid
                     C.c_double(center), C.c_int(FILTERS[filt]), C.c_int(PADS[pad] | (2 if fused else 0)), C.c_int(m), C.c_int(METHODS[method]),
                     _p(out))
     return out
+
+
+def padded_size(ndet: int) -> tuple[int, int]:
+    """Detector of any width ndet -> (n, pad_l): n = the power of two >= max(ndet, 64) the FFTs run on
+    (PAPER.md:57-59: "16-bit data are additionally padded/unpadded to the power of 2 sizes"; DESIGN.md
+    reading Q19 applies it to fp32 too), pad_l = ceil((n - ndet)/2) air samples (p = 0) on the left, so
+    that output pixel ix sits at x = ix - floor(ndet/2)."""
+    n = 64
+    while n < ndet:
+        n *= 2
+    return n, (n - ndet + 1) // 2
+
+
+def recon_padded(raw, flat, dark, theta, center, filt="ramp", m=DEFAULT_M, method="grid", pad="zero"):
+    """Detector width ndet not a power of two: S1+S2 on the ndet samples,
+    every sinogram row embedded at offset pad_l in a row of n zeros ("padded"), the rotation centre moved
+    with it, S3..S7 (or a definition) at size n, and the central ndet x ndet pixels cut out ("unpadded").
+    raw [nproj][nz][ndet] -> out [nz][ndet][ndet]."""
+    raw = np.ascontiguousarray(raw, dtype=np.uint16)
+    nproj, nz, ndet = raw.shape
+    n, pad_l = padded_size(ndet)
+    p = neglog(raw, flat, dark)                                   # [nz][nproj][ndet]
+    pp = np.zeros((nz, nproj, n))
+    pp[:, :, pad_l:pad_l + ndet] = p
+    out = fbp_from_sino(pp, theta, float(center) + pad_l, filt=filt, m=m, method=method, pad=pad)
+    return np.ascontiguousarray(out[:, pad_l:pad_l + ndet, pad_l:pad_l + ndet])

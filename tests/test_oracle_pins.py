@@ -392,3 +392,78 @@ def test_brute_force_python_gridding_tiny():
                         continue
                     F[l2 % M, l1 % M] += G[j, k] * np.exp(-alpha * (l1 - n1) ** 2) * np.exp(-alpha * (l2 - n2) ** 2)
     assert np.abs(orc.grid(G, theta, n, m) - F).max() < 1e-13
+
+
+# ---------------------------------------------------------------- P10: detector width not a power of two
+def _textbook_fbp(raw, flat, dark, theta, center, M):
+    """FBP written out from the textbook on the UNPADDED detector (no FFT, no padding anywhere):
+    p = -ln((raw - dark)/(flat - dark)); q = p * h as a direct sum with the closed-form band-limited
+    ramp kernel h[0] = 1/4, h[i] = -1/(pi^2 i^2) for odd i, 0 for even i; f(x, y) = pi/nproj sum_j of the
+    linear interpolation of q_j at s = x cos + y sin + c, zero outside the detector; x = ix - floor(ndet/2).
+    Reading Q4 zeroes the Nyquist bin of the length-M filter: in closed form that subtracts
+    (-1)^i R[M/2]/M from the kernel, R[M/2] = sum_i (-1)^i h[i] = 1/4 + 2 sum_{odd i < M/2} 1/(pi^2 i^2)."""
+    nproj, nz, ndet = raw.shape
+    lag = np.arange(-(ndet - 1), ndet)
+    h = np.where(lag == 0, 0.25, np.where(lag % 2 != 0, -1.0 / (np.pi ** 2 * np.maximum(lag * lag, 1)), 0.0))
+    r_nyq = 0.25 + 2.0 * sum(1.0 / (np.pi ** 2 * i * i) for i in range(1, M // 2, 2))
+    h = h - np.where(lag % 2 != 0, -1.0, 1.0) * r_nyq / M
+    xs = np.arange(ndet) - ndet // 2
+    X, Y = np.meshgrid(xs, xs)                                     # [iy][ix]
+    out = np.zeros((nz, ndet, ndet))
+    for z in range(nz):
+        p = -np.log((raw[:, z, :].astype(np.float64) - dark[z]) / (flat[z].astype(np.float64) - dark[z]))
+        for j in range(nproj):
+            q = np.array([sum(h[(i - i2) + ndet - 1] * p[j, i2] for i2 in range(ndet)) for i in range(ndet)])
+            t = float(theta[j])
+            s = X * np.cos(t) + Y * np.sin(t) + center
+            i0 = np.floor(s).astype(int)
+            w = s - i0
+            qz = np.concatenate([q, [0.0, 0.0]])                   # q[-1] and q[ndet] read as 0
+            a = np.where((i0 >= 0) & (i0 < ndet), qz[np.clip(i0, -1, ndet)], 0.0)
+            b = np.where((i0 + 1 >= 0) & (i0 + 1 < ndet), qz[np.clip(i0 + 1, -1, ndet)], 0.0)
+            out[z] += (1 - w) * a + w * b
+    return out * np.pi / nproj, X, Y
+
+
+@pytest.mark.parametrize("ndet,center", [(50, 25.0), (45, 20.75), (90, 47.5)])
+def test_p10_padded_detector_equals_textbook_fbp_on_the_unpadded_detector(ndet, center):
+    """Padding the detector to a power of two, moving the centre with it and cutting the image back
+     must not change the textbook reconstruction wherever every ray through the pixel
+    hits the real detector: catches a wrong pad offset, centre shift, crop offset or odd-width rounding."""
+    rng = np.random.default_rng(11)
+    nproj, nz = 24, 2
+    theta = sg.make_theta(nproj)
+    flat = rng.uniform(20000, 30000, (nz, ndet)).astype(np.float32)
+    dark = rng.uniform(90, 110, (nz, ndet)).astype(np.float32)
+    p_true = rng.uniform(0.0, 2.0, (nproj, nz, ndet))
+    raw = np.rint((flat - dark)[None] * np.exp(-p_true) + dark[None]).astype(np.uint16)
+    n, pad_l = orc.padded_size(ndet)
+    assert n == (64 if ndet <= 64 else 128) and pad_l == (n - ndet + 1) // 2
+    ref, X, Y = _textbook_fbp(raw, flat, dark, theta, center, 2 * n)
+    got = orc.recon_padded(raw, flat, dark, theta, center, filt="ramp", method="lin")
+    assert got.shape == (nz, ndet, ndet)
+    inside = np.hypot(X, Y) <= min(center, ndet - 1 - center) - 1e-9
+    assert inside.sum() > ndet * ndet // 3
+    assert np.abs(got - ref)[:, inside].max() < 1e-12 * np.abs(ref).max() + 1e-13
+    # outside that disc the padded detector sees the filter's tails where the textbook sees nothing
+    assert np.abs(got - ref)[:, ~inside].max() > 1e-6
+
+
+def test_p10_padded_detector_is_the_identity_for_powers_of_two_and_consistent_across_methods():
+    w = sg.make_workload("C1")
+    raw, _ = sg.make_counts(w, [3, 4])
+    flat, dark, _, _ = sg.make_flat_dark(w, [3, 4])
+    a = orc.recon(raw, flat, dark, w.theta, w.center, filt="shepp", m=3)
+    b = orc.recon_padded(raw, flat, dark, w.theta, w.center, filt="shepp", m=3)
+    assert np.array_equal(a, b)
+    # a cut-down detector (100 of the 128 columns, phantom still inside): gridding vs the exact sum, 2e-3 gate
+    cut = slice(14, 114)
+    g = orc.recon_padded(raw[:, :, cut], flat[:, cut], dark[:, cut], w.theta, w.center - 14, filt="shepp", m=3)
+    e = orc.recon_padded(raw[:, :, cut], flat[:, cut], dark[:, cut], w.theta, w.center - 14, filt="shepp", m=3,
+                         method="exact")
+    assert g.shape == (2, 100, 100)
+    assert max(rl2(g[z], e[z]) for z in range(2)) < 2e-3
+    # and the cut-down reconstruction shows the same object as the full one (same pixels, x = ix - 50 vs ix - 64)
+    full = a[:, 14:114, 14:114]
+    disc = np.hypot(*np.meshgrid(np.arange(100) - 50, np.arange(100) - 50)) < 40
+    assert np.abs(g - full)[:, disc].max() < 0.15 * np.abs(full).max()      # count noise of the dropped air columns
