@@ -96,6 +96,21 @@ tcp_ctx* tcp_create(int n, int nproj, int nz_chunk, float center, int dtype, int
  * 0 = default 3, which meets the 2e-3 gridding-vs-exact gate with 3x margin). */
 tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, int filter, int m);
 
+/* Detector width that is not a power of two ("16-bit data are additionally padded/unpadded to
+ * the power of 2 sizes"; applied to FP32 as well, reading Q19).  ndet in [8, 4096] is the detector
+ * width and the image side of every array the caller passes to tcp_recon / tcp_recon_try / tcp_normalize /
+ * tcp_recon_volume_host (raw [nproj][nz][ndet], flat / dark [nz][ndet], out [nz][ndet][ndet]); center is in
+ * the caller's detector pixels, 0 <= c <= ndet-1.  Inside, S1+S2 write every row at offset
+ * pad_l = ceil((n - ndet)/2) of a row of n = the power of two >= max(ndet, 64), the other samples being air
+ * (p = 0); S3..S7 run at size n with the centre c + pad_l; the central ndet x ndet pixels are copied out, so
+ * pixel ix sits at x = ix - floor(ndet/2).  Wherever every ray through a pixel hits the real detector the
+ * result is that of the unpadded textbook sum; elsewhere the padded air columns carry the filter's tails.
+ * The workspaces tcp_workspace reports keep the padded size n = tcp_padded_n(ctx).  When ndet is itself a
+ * power of two >= 64 this is tcp_create_ex.  m as in tcp_create_ex.  NULL on error. */
+tcp_ctx* tcp_create_det(int ndet, int nproj, int nz_chunk, float center, int dtype, int filter, int m);
+/* The power of two the context's transforms run on (= n of tcp_create / tcp_create_ex). */
+int tcp_padded_n(const tcp_ctx* ctx);
+
 /* Reconstruct one chunk, S1..S7, asynchronously on `stream` (no host synchronisation).
  *   raw_u16 [nproj][nz_chunk][n] uint16 counts, projection-major as a detector delivers them
  *   flat, dark [nz_chunk][n] float32, already averaged over frames

@@ -12,6 +12,8 @@ from .binding import (  # noqa: F401
     lib_path,
     tcp_create,
     tcp_create_ex,
+    tcp_create_det,
+    tcp_padded_n,
     tcp_destroy,
     tcp_recon,
     tcp_normalize,

@@ -20,7 +20,7 @@ EXPORTS = [
     "tcp_create", "tcp_create_ex", "tcp_recon", "tcp_destroy", "tcp_last_error",
     "tcp_mean_frames_u16", "tcp_normalize", "tcp_workspace", "tcp_read_workspace", "tcp_scale", "tcp_grid_strip",
     "tcp_workspace_bytes", "tcp_launches_per_recon", "tcp_set_option", "tcp_profile_collect",
-    "tcp_recon_volume_host", "tcp_recon_try",
+    "tcp_recon_volume_host", "tcp_recon_try", "tcp_create_det", "tcp_padded_n",
 ]
 
 
@@ -49,6 +49,10 @@ def lib():
     L.tcp_create.argtypes = [ci, ci, ci, cf, ci, ci]
     L.tcp_create_ex.restype = vp
     L.tcp_create_ex.argtypes = [ci, ci, ci, cf, ci, ci, ci]
+    L.tcp_create_det.restype = vp
+    L.tcp_create_det.argtypes = [ci, ci, ci, cf, ci, ci, ci]
+    L.tcp_padded_n.restype = ci
+    L.tcp_padded_n.argtypes = [vp]
     L.tcp_recon.restype = ci
     L.tcp_recon.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     L.tcp_destroy.restype = None
@@ -120,6 +124,18 @@ def tcp_create_ex(n, nproj, nz_chunk, center, dtype, filter, m):
     return h
 
 
+def tcp_create_det(ndet, nproj, nz_chunk, center, dtype, filter, m=0):
+    h = lib().tcp_create_det(ndet, nproj, nz_chunk, float(center), DTYPES.get(dtype, dtype),
+                             FILTERS.get(filter, filter), int(m))
+    if not h:
+        raise TcpError("tcp_create_det failed: " + tcp_last_error())
+    return h
+
+
+def tcp_padded_n(h) -> int:
+    return int(lib().tcp_padded_n(h))
+
+
 def tcp_destroy(h):
     lib().tcp_destroy(h)
 
@@ -164,7 +180,9 @@ class Recon:
             raise TcpError("no CUDA device: this library has no CPU fallback")
         self.n, self.nproj, self.nz, self.center = n, nproj, nz_chunk, float(center)
         self.dtype, self.filter = dtype, filter
-        self.h = tcp_create_ex(n, nproj, nz_chunk, center, dtype, filter, m)
+        # n is the caller's detector width / image side; the library pads it to a power of two if it must
+        self.h = tcp_create_det(n, nproj, nz_chunk, center, dtype, filter, m)
+        self.npad = tcp_padded_n(self.h)
         self.out_dtype = torch.float16 if dtype == "f16" else torch.float32
         self.store_dtype = torch.float32 if dtype == "f32" else torch.float16
 
@@ -265,15 +283,15 @@ class Recon:
         """Copy of an intermediate of the last recon, as a torch tensor (tests only)."""
         ptr, nbytes = C.c_void_p(), C.c_size_t()
         _check(lib().tcp_workspace(self.h, WS[name], C.byref(ptr), C.byref(nbytes)))
-        npair, M = (self.nz + 1) // 2, 2 * self.n
+        npair, M, n = (self.nz + 1) // 2, 2 * self.npad, self.npad
         buf = torch.empty(nbytes.value, dtype=torch.uint8, device="cuda")
         _check(lib().tcp_read_workspace(self.h, WS[name], buf.data_ptr(), nbytes.value, _stream(None)))
         torch.cuda.synchronize()
         if name == "trig":
             return buf.view(torch.float64).view(self.nproj, 2)
         if name == "sinogram":
-            return buf.view(self.store_dtype).view(self.nz, self.nproj, self.n)
-        shape = {"spectrum": (npair, self.nproj, M), "grid": (npair, M, M), "pass1": (npair, self.n, M)}[name]
+            return buf.view(self.store_dtype).view(self.nz, self.nproj, n)
+        shape = {"spectrum": (npair, self.nproj, M), "grid": (npair, M, M), "pass1": (npair, n, M)}[name]
         v = buf.view(self.store_dtype).view(*shape, 2).float()
         if name == "grid":
             w = int(lib().tcp_grid_strip(self.h))
@@ -281,7 +299,7 @@ class Recon:
                 v = v.view(npair, M // w, M, w, 2).permute(0, 2, 1, 3, 4).reshape(npair, M, M, 2)
         if name == "pass1":     # strip-major [npair][M/w][n iy][w l1] -> [npair][n iy][M l1]
             w = min(32, max(2, 16384 // M))
-            v = v.view(npair, M // w, self.n, w, 2).permute(0, 2, 1, 3, 4).reshape(npair, self.n, M, 2)
+            v = v.view(npair, M // w, n, w, 2).permute(0, 2, 1, 3, 4).reshape(npair, n, M, 2)
         return torch.complex(v[..., 0], v[..., 1])
 
     def recon_volume_host(self, raw_host, flat_host, dark_host, theta_host, out_host=None, nbuf=3):

@@ -112,7 +112,64 @@ __global__ void __launch_bounds__(256) normalize_half_kernel(const uint4* __rest
     }
 }
 
+// Detector width ndet not a power of two (tcp_create_det; "padded/unpadded to the power of 2
+// sizes"): sample i of the caller's row lands at i + pad_l of a row of n, the rest is air (p = 0).  Scalar
+// loads: ndet may be odd.  Same arithmetic as normalize_kernel, one rounding to the storage type.
+template <class TS>
+__global__ void __launch_bounds__(256) normalize_pad_kernel(const uint16_t* __restrict__ raw, const float* __restrict__ flat,
+                                                            const float* __restrict__ dark, TS* __restrict__ sino, int nproj,
+                                                            int nz, int n, int ndet, int pad_l) {
+    const size_t total = (size_t)nproj * nz * n;                // index space [nproj][nz][n] (padded rows, raw order)
+    for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < total; v += (size_t)gridDim.x * blockDim.x) {
+        const int ip = (int)(v % n);
+        const size_t row = v / n;
+        const int z = (int)(row % nz);
+        const int j = (int)(row / nz);
+        const int i = ip - pad_l;
+        float p = 0.f;
+        if (i >= 0 && i < ndet)
+            p = neglog1((float)raw[((size_t)j * nz + z) * ndet + i], __ldg(&flat[(size_t)z * ndet + i]),
+                        __ldg(&dark[(size_t)z * ndet + i]));
+        st_r(sino, ((size_t)z * nproj + j) * n + ip, p);
+    }
+}
+
+// the central ndet x ndet pixels of the padded image [nslices][n][n] -> out [nslices][ndet][ndet]
+template <class TO>
+__global__ void __launch_bounds__(256) crop_out_kernel(const TO* __restrict__ src, TO* __restrict__ dst, int nslices, int n,
+                                                       int ndet, int pad_l) {
+    const size_t total = (size_t)nslices * ndet * ndet;
+    for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < total; v += (size_t)gridDim.x * blockDim.x) {
+        const int ix = (int)(v % ndet);
+        const size_t r = v / ndet;
+        const int iy = (int)(r % ndet);
+        const size_t z = r / ndet;
+        dst[v] = src[(z * n + (iy + pad_l)) * n + (ix + pad_l)];
+    }
+}
+
+int launch_crop_out(const tcp_ctx* c, int nslices, void* out, cudaStream_t st) {
+    const size_t total = (size_t)nslices * c->ndet * c->ndet;
+    const int blocks = (int)std::min<size_t>((total + 255) / 256, (size_t)148 * 8 * 4);
+    if (c->half_out)
+        crop_out_kernel<__half><<<blocks, 256, 0, st>>>((const __half*)c->out_pad, (__half*)out, nslices, c->n, c->ndet, c->pad_l);
+    else
+        crop_out_kernel<float><<<blocks, 256, 0, st>>>((const float*)c->out_pad, (float*)out, nslices, c->n, c->ndet, c->pad_l);
+    TCP_CUDA_CHECK(cudaGetLastError());
+    return TCP_OK;
+}
+
 int launch_normalize(const tcp_ctx* c, const uint16_t* raw, const float* flat, const float* dark, cudaStream_t st) {
+    if (c->ndet != c->n) {
+        const size_t total = (size_t)c->nproj * c->nz * c->n;
+        const int blocks = (int)std::min<size_t>((total + 255) / 256, (size_t)148 * 8 * 4);
+        if (c->half_store)
+            normalize_pad_kernel<__half><<<blocks, 256, 0, st>>>(raw, flat, dark, (__half*)c->sino, c->nproj, c->nz, c->n, c->ndet, c->pad_l);
+        else
+            normalize_pad_kernel<float><<<blocks, 256, 0, st>>>(raw, flat, dark, (float*)c->sino, c->nproj, c->nz, c->n, c->ndet, c->pad_l);
+        TCP_CUDA_CHECK(cudaGetLastError());
+        return TCP_OK;
+    }
     const int n8 = c->n / 8;
     const int cap = 148 * 8 * 4;                  // a few waves of 8 resident CTAs per SM
     if (c->half_store) {

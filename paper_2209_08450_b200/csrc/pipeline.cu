@@ -45,6 +45,7 @@ static int pipe_create(tcp_ctx* c, int nbuf) {
     c->pipe = p;
     p->nbuf = nbuf;
     const size_t ob = c->half_out ? 2 : 4;
+    const int n = c->ndet;                    // width of the caller's rows and side of the caller's images
     TCP_CUDA_CHECK(cudaStreamCreateWithFlags(&p->s_h2d, cudaStreamNonBlocking));
     TCP_CUDA_CHECK(cudaStreamCreateWithFlags(&p->s_comp, cudaStreamNonBlocking));
     TCP_CUDA_CHECK(cudaStreamCreateWithFlags(&p->s_d2h, cudaStreamNonBlocking));
@@ -52,14 +53,14 @@ static int pipe_create(tcp_ctx* c, int nbuf) {
     TCP_CUDA_CHECK(cudaEventCreate(&p->ev_stop));
     TCP_CUDA_CHECK(cudaMalloc((void**)&p->theta, (size_t)c->nproj * sizeof(float)));
     for (int b = 0; b < nbuf; ++b) {
-        TCP_CUDA_CHECK(cudaMalloc((void**)&p->raw[b], (size_t)c->nproj * c->nz * c->n * 2));
-        TCP_CUDA_CHECK(cudaMalloc((void**)&p->flat[b], (size_t)c->nz * c->n * 4));
-        TCP_CUDA_CHECK(cudaMalloc((void**)&p->dark[b], (size_t)c->nz * c->n * 4));
-        TCP_CUDA_CHECK(cudaMalloc(&p->out[b], (size_t)c->nz * c->n * c->n * ob));
+        TCP_CUDA_CHECK(cudaMalloc((void**)&p->raw[b], (size_t)c->nproj * c->nz * n * 2));
+        TCP_CUDA_CHECK(cudaMalloc((void**)&p->flat[b], (size_t)c->nz * n * 4));
+        TCP_CUDA_CHECK(cudaMalloc((void**)&p->dark[b], (size_t)c->nz * n * 4));
+        TCP_CUDA_CHECK(cudaMalloc(&p->out[b], (size_t)c->nz * n * n * ob));
         // a partial last chunk leaves rows unwritten: keep them finite
-        TCP_CUDA_CHECK(cudaMemset(p->raw[b], 0, (size_t)c->nproj * c->nz * c->n * 2));
-        TCP_CUDA_CHECK(cudaMemset(p->flat[b], 0, (size_t)c->nz * c->n * 4));
-        TCP_CUDA_CHECK(cudaMemset(p->dark[b], 0, (size_t)c->nz * c->n * 4));
+        TCP_CUDA_CHECK(cudaMemset(p->raw[b], 0, (size_t)c->nproj * c->nz * n * 2));
+        TCP_CUDA_CHECK(cudaMemset(p->flat[b], 0, (size_t)c->nz * n * 4));
+        TCP_CUDA_CHECK(cudaMemset(p->dark[b], 0, (size_t)c->nz * n * 4));
         TCP_CUDA_CHECK(cudaEventCreateWithFlags(&p->ev_h2d[b], cudaEventDisableTiming));
         TCP_CUDA_CHECK(cudaEventCreateWithFlags(&p->ev_comp[b], cudaEventDisableTiming));
         TCP_CUDA_CHECK(cudaEventCreateWithFlags(&p->ev_d2h[b], cudaEventDisableTiming));
@@ -82,7 +83,7 @@ extern "C" int tcp_recon_volume_host(tcp_ctx* c, const uint16_t* raw_host, const
     int rc;
     if ((rc = pipe_create(c, nbuf))) return rc;
     Pipe* p = c->pipe;
-    const int n = c->n, nz = c->nz;
+    const int n = c->ndet, nz = c->nz;
     const size_t ob = c->half_out ? 2 : 4;
     const int nchunks = (nz_total + nz - 1) / nz;
 

@@ -173,7 +173,8 @@ extern "C" {
 
 const char* tcp_last_error(void) { return g_err; }
 
-tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, int filter, int m) {
+// n: the power of two the transforms run on; ndet <= n: the caller's detector width (tcp_create_det), embedded at pad_l
+static tcp_ctx* create_impl(int n, int ndet, int pad_l, int nproj, int nz_chunk, float center, int dtype, int filter, int m) {
     g_err[0] = 0;
     if (m == 0) m = 3;
     if (n < 64 || n > 4096 || (n & (n - 1)) != 0) {
@@ -181,7 +182,8 @@ tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, 
         return nullptr;
     }
     if (nproj < 1 || nz_chunk < 1) { set_error(TCP_EINVAL, "nproj=%d and nz_chunk=%d must be >= 1", nproj, nz_chunk); return nullptr; }
-    if (!(center >= 0.f && center <= (float)(n - 1))) { set_error(TCP_EINVAL, "center=%g outside [0, n-1]", (double)center); return nullptr; }
+    if (!(center >= 0.f && center <= (float)(ndet - 1))) { set_error(TCP_EINVAL, "center=%g outside [0, n-1]", (double)center); return nullptr; }
+    center += (float)pad_l;
     if (dtype < TCP_F32 || dtype > TCP_F16_OUT32) { set_error(TCP_EINVAL, "unknown dtype %d", dtype); return nullptr; }
     if (filter < TCP_FILTER_RAMP || filter > TCP_FILTER_PARZEN) { set_error(TCP_EINVAL, "unknown filter %d", filter); return nullptr; }
     if (m != 3 && m != 4) { set_error(TCP_EINVAL, "kernel half-width m=%d must be 3 or 4", m); return nullptr; }
@@ -195,6 +197,7 @@ tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, 
     if (!c) { set_error(TCP_ENOMEM, "out of host memory"); return nullptr; }
     c->n = n; c->M = 2 * n; c->nproj = nproj; c->nz = nz_chunk; c->npair = (nz_chunk + 1) / 2;
     c->dtype = dtype; c->filter = filter; c->m = m; c->center = center;
+    c->ndet = ndet; c->pad_l = pad_l;
     c->half_store = dtype != TCP_F32;
     c->half_out = dtype == TCP_F16;
     // fp16 storage: S = 2^13 puts |f| Phi^2 S <= 65504 for |f| < 1.9 per pixel while keeping
@@ -206,7 +209,9 @@ tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, 
     cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, c->device);
     c->tcfft_ok = (c->half_store && c->M == 4096) ? TCP_TCFFT_IROWS : 0;
     c->tcfft = 0;   // measured slower than the CUDA-core transforms: opt-in through TCP_OPT_TCFFT
-    if (build_context(c) != TCP_OK || setup_kernel_attributes(c) != TCP_OK) {
+    int rc_pad = TCP_OK;
+    if (ndet != n) rc_pad = dev_alloc(&c->out_pad, (size_t)nz_chunk * n * n * (c->half_out ? 2 : 4), &c->bytes);
+    if (rc_pad != TCP_OK || build_context(c) != TCP_OK || setup_kernel_attributes(c) != TCP_OK) {
         char keep[512];
         strncpy(keep, g_err, sizeof(keep));
         tcp_destroy(c);
@@ -215,6 +220,23 @@ tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, 
     }
     return c;
 }
+
+tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, int filter, int m) {
+    return create_impl(n, n, 0, nproj, nz_chunk, center, dtype, filter, m);
+}
+
+tcp_ctx* tcp_create_det(int ndet, int nproj, int nz_chunk, float center, int dtype, int filter, int m) {
+    if (ndet < 8 || ndet > 4096) {
+        g_err[0] = 0;
+        set_error(TCP_EINVAL, "ndet=%d must be in [8, 4096]", ndet);
+        return nullptr;
+    }
+    int n = 64;
+    while (n < ndet) n *= 2;
+    return create_impl(n, ndet, (n - ndet + 1) / 2, nproj, nz_chunk, center, dtype, filter, m);
+}
+
+int tcp_padded_n(const tcp_ctx* c) { return c ? c->n : 0; }
 
 tcp_ctx* tcp_create(int n, int nproj, int nz_chunk, float center, int dtype, int filter) {
     return tcp_create_ex(n, nproj, nz_chunk, center, dtype, filter, 0);
@@ -231,6 +253,7 @@ void tcp_destroy(tcp_ctx* c) {
     cudaFree(c->tw); cudaFree(c->hfilt); cudaFree(c->ptab); cudaFree(c->ftab); cudaFree(c->deax); cudaFree(c->deay);
     cudaFree(c->tile_order);
     cudaFree(c->try_buf);
+    cudaFree(c->out_pad);
     cudaFree(c->tc_amat); cudaFree(c->tc_hfilt); cudaFree(c->tc_ptab);
     grid_tile_free(c);
     free(c);
@@ -246,6 +269,8 @@ int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* d
     if (!c || !raw || !flat || !dark || !theta || !out) return set_error(TCP_EINVAL, "NULL argument");
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
+    void* const user_out = out;
+    if (c->out_pad) out = c->out_pad;         // tcp_create_det: reconstruct at n, then cut the ndet x ndet image out
     cudaEvent_t* ev = nullptr;
     if (c->profile) {
         if (c->pcalls >= kProfileRing) return set_error(TCP_EINVAL, "profile ring full: call tcp_profile_collect");
@@ -262,6 +287,7 @@ int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* d
         if ((rc = launch_filter(c, st))) return rc;
         TCP_MARK(3);
         if ((rc = launch_line_bp(c, out, st))) return rc;
+        if (c->out_pad && (rc = launch_crop_out(c, c->nz, user_out, st))) return rc;
         TCP_MARK(4);
         TCP_MARK(5);
         TCP_MARK(6);
@@ -277,6 +303,7 @@ int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* d
     if ((rc = launch_ifft_cols(c, st))) return rc;
     TCP_MARK(5);
     if ((rc = (c->tcfft & TCP_TCFFT_IROWS) ? launch_ifft_rows_tc(c, out, st) : launch_ifft_rows(c, out, st))) return rc;
+    if (c->out_pad && (rc = launch_crop_out(c, c->nz, user_out, st))) return rc;
     TCP_MARK(6);
 #undef TCP_MARK
     return TCP_OK;
@@ -288,7 +315,7 @@ int tcp_recon_try(tcp_ctx* c, const uint16_t* raw, const float* flat, const floa
     if (c->algorithm != TCP_ALG_FOURIER) return set_error(TCP_EUNSUPPORTED, "tcp_recon_try is FourierRec only");
     if (ncenter < 1 || ncenter > c->nz) return set_error(TCP_EINVAL, "ncenter=%d outside [1, nz_chunk=%d]", ncenter, c->nz);
     for (int i = 0; i < ncenter; ++i)
-        if (!(centers[i] >= 0.f && centers[i] <= (float)(c->n - 1)))
+        if (!(centers[i] >= 0.f && centers[i] <= (float)(c->ndet - 1)))
             return set_error(TCP_EINVAL, "centers[%d]=%g outside [0, n-1]", i, (double)centers[i]);
     cudaStream_t st = (cudaStream_t)stream;
     const int M = c->M, npair = (ncenter + 1) / 2;
@@ -304,7 +331,7 @@ int tcp_recon_try(tcp_ctx* c, const uint16_t* raw, const float* flat, const floa
             const int ks = (k < M / 2) ? k : k - M;
             double re = 0.0, im = 0.0;
             for (int h = 0; h < 2 && 2 * p + h < ncenter; ++h) {
-                const double fr = fmod((double)ks * (double)centers[2 * p + h], (double)M) / (double)M;
+                const double fr = fmod((double)ks * ((double)centers[2 * p + h] + (double)c->pad_l), (double)M) / (double)M;
                 const double a = 2.0 * kPi * fr, cr = c->scale * C * cos(a), ci = c->scale * C * sin(a);
                 if (h == 0) { re += cr; im += ci; }      // slice A: real part
                 else { re -= ci; im += cr; }             // slice B: times i
@@ -326,7 +353,8 @@ int tcp_recon_try(tcp_ctx* c, const uint16_t* raw, const float* flat, const floa
     else rc = launch_grid_tile(&t, theta, st);
     if (rc) return rc;
     if ((rc = launch_ifft_cols(&t, st))) return rc;
-    return launch_ifft_rows(&t, out, st);
+    if ((rc = launch_ifft_rows(&t, c->out_pad ? c->out_pad : out, st))) return rc;
+    return c->out_pad ? launch_crop_out(c, ncenter, out, st) : TCP_OK;
 }
 
 int tcp_profile_collect(tcp_ctx* c, double* ms_sum, int* ncalls) {
@@ -348,11 +376,12 @@ int tcp_profile_collect(tcp_ctx* c, double* ms_sum, int* ncalls) {
 
 int tcp_launches_per_recon(const tcp_ctx* c) {
     if (!c) return 0;
-    if (c->algorithm == TCP_ALG_LINE) return 4;                          // trig, normalise, filter, backprojection
+    const int crop = c->out_pad ? 1 : 0;                                 // tcp_create_det: + the cut-out copy
+    if (c->algorithm == TCP_ALG_LINE) return 4 + crop;                   // trig, normalise, filter, backprojection
     if (c->grid_impl == TCP_GRID_MMA)       // + plan, cache decide (+ count, scan, fill, cached kernel: most exit at once) (+ reduce)
-        return 8 + (c->w_cap > 0 ? 4 : 0) + (c->g_nred ? 1 : 0);
-    if (c->grid_impl == TCP_GRID_TILE) return 7 + (c->g_nred ? 1 : 0);   // + plan (+ reduce)
-    return c->grid_impl == TCP_GRID_SCATTER_ATOMIC ? 6 : 6;              // (scatter adds a memset, not a kernel)
+        return 8 + (c->w_cap > 0 ? 4 : 0) + (c->g_nred ? 1 : 0) + crop;
+    if (c->grid_impl == TCP_GRID_TILE) return 7 + (c->g_nred ? 1 : 0) + crop;   // + plan (+ reduce)
+    return 6 + crop;                                                     // (scatter adds a memset, not a kernel)
 }
 
 int tcp_mean_frames_u16(const uint16_t* frames, int nframes, int nz, int n, float* mean, tcp_stream_t stream) {

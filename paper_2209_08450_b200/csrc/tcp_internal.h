@@ -9,7 +9,9 @@
 
 struct tcp_ctx {
     int n, M, nproj, nz, npair, dtype, filter, m;
-    float center;
+    float center;         // rotation centre in the padded row (caller's centre + pad_l)
+    int ndet, pad_l;      // tcp_create_det: caller's detector width / image side, air samples left of it (ndet == n, 0 otherwise)
+    void* out_pad;        // [nz][n][n] in the output dtype when ndet != n (the central ndet x ndet pixels are then copied out)
     bool half_store;      // intermediates in half / half2 (TCP_F16, TCP_F16_OUT32)
     bool half_out;        // out in half (TCP_F16)
     double scale;         // power-of-two scale S of SPECTRUM / GRID / PASS1 (1 in fp32)
@@ -90,6 +92,7 @@ int launch_ifft_cols(const tcp_ctx* c, cudaStream_t st);
 int cols_strip_width(int M);
 int launch_ifft_rows(const tcp_ctx* c, void* out, cudaStream_t st);
 int launch_ifft_rows_tc(const tcp_ctx* c, void* out, cudaStream_t st);
+int launch_crop_out(const tcp_ctx* c, int nslices, void* out, cudaStream_t st);
 int launch_mean_frames(const uint16_t* frames, int nframes, int nz, int n, float* mean, cudaStream_t st);
 int setup_kernel_attributes(const tcp_ctx* c);
 void pipe_destroy(tcp_ctx* c);

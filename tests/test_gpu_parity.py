@@ -415,6 +415,101 @@ def test_pipeline_host_matches_direct():
     r.close()
 
 
+# ------------------------------------------------------------------ detector width not a power of two (8(f-2))
+def _cut(w, rows, lo, hi):
+    """Columns lo..hi of a workload's detector: a narrower (possibly odd, possibly truncating) detector."""
+    raw, flat, dark, theta = _inputs(w, rows)
+    return (np.ascontiguousarray(raw[:, :, lo:hi]), np.ascontiguousarray(flat[:, lo:hi]),
+            np.ascontiguousarray(dark[:, lo:hi]), theta, w.center - lo)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f16", "f16_out32"])
+@pytest.mark.parametrize("cfg,scale,lo,hi", [("C1", 1, 14, 114), ("C1", 1, 14, 113), ("C2", 2, 60, 190), ("C2", 4, 38, 100)])
+def test_detector_width_not_a_power_of_two(dtype, cfg, scale, lo, hi):
+    """tcp_create_det: widths 100, 99 (odd), 130 (just above a power of two, object truncated)
+    and 62 (below the smallest transform) against the oracle's recon_padded, whose padding, centre shift and
+    cut-out pin P10 fixes; 5 slices = an odd chunk."""
+    tcp = _tcp()
+    w = sg.make_workload(cfg, scale=scale)
+    rows = list(range(w.nz_total // 2 - 2, w.nz_total // 2 + 3))
+    raw, flat, dark, theta, c = _cut(w, rows, lo, hi)
+    ndet = hi - lo
+    r = tcp.Recon(ndet, w.nproj, len(rows), c, dtype, w.filter, 3)
+    assert r.npad == orc.padded_size(ndet)[0] and r.npad != ndet
+    out = r.recon(*_to_dev(raw, flat, dark, theta))
+    torch.cuda.synchronize()
+    assert out.shape == (len(rows), ndet, ndet)
+    out = out.float().cpu().numpy()
+    ref = orc.recon_padded(raw, flat, dark, theta, c, w.filter, 3, "grid")
+    scale_v = np.abs(ref).max()
+    for z in range(len(rows)):
+        if dtype == "f32":
+            assert rl2(out[z], ref[z]) < FP32_GATE, (z, rl2(out[z], ref[z]))
+        else:
+            assert rl2(out[z], ref[z]) < FP16_GATE_L2, (z, rl2(out[z], ref[z]))
+            assert np.abs(out[z] - ref[z]).max() / scale_v < FP16_GATE_MAX
+    # the padded sinogram workspace: air outside the detector, S1+S2 inside
+    sino = r.workspace("sinogram").float().cpu().numpy()
+    pad_l = orc.padded_size(ndet)[1]
+    assert sino.shape == (len(rows), w.nproj, r.npad)
+    assert not sino[:, :, :pad_l].any() and not sino[:, :, pad_l + ndet:].any()
+    p = orc.neglog(raw, flat, dark)
+    assert np.abs(sino[:, :, pad_l:pad_l + ndet] - p).max() < (2e-6 if dtype == "f32" else 2e-3) * max(1.0, np.abs(p).max())
+    r.close()
+
+
+def test_detector_width_variants_pipeline_try_line_and_errors():
+    """The other entry points on a padded context: LineRec, the rotation-centre try mode, the host pipeline with
+    a partial last chunk; tcp_create_det on a power of two is tcp_create_ex bit for bit; argument errors."""
+    tcp = _tcp()
+    w = sg.make_workload("C1")
+    rows = list(range(8))
+    raw, flat, dark, theta, c = _cut(w, rows, 14, 113)            # ndet = 99
+    ndet = 99
+    r = tcp.Recon(ndet, w.nproj, 4, c, "f32", w.filter, 3)
+    # host pipeline: 2 chunks of 4 ... of a 7-slice stack (partial last chunk)
+    raw_h = torch.from_numpy(np.ascontiguousarray(raw[:, :7]).view(np.int16)).view(torch.uint16).pin_memory()
+    out_h, ms = r.recon_volume_host(raw_h, torch.from_numpy(flat[:7].copy()).pin_memory(),
+                                    torch.from_numpy(dark[:7].copy()).pin_memory(), torch.from_numpy(theta).pin_memory(), nbuf=2)
+    ref = orc.recon_padded(raw[:, :7], flat[:7], dark[:7], theta, c, w.filter, 3, "grid")
+    assert out_h.shape == (7, ndet, ndet)
+    for z in range(7):
+        assert rl2(out_h[z].numpy(), ref[z]) < FP32_GATE
+    # try mode
+    centers = [c - 2.0, c, c + 1.5]
+    d = _to_dev(np.ascontiguousarray(raw[:, 3:4]), flat[3:4], dark[3:4], theta)
+    t = r.recon_try(d[0], d[1], d[2], d[3], centers).cpu().numpy()
+    assert t.shape == (3, ndet, ndet)
+    for i, ci in enumerate(centers):
+        ri = orc.recon_padded(raw[:, 3:4], flat[3:4], dark[3:4], theta, ci, w.filter, 3, "grid")[0]
+        assert rl2(t[i], ri) < FP32_GATE, (ci, rl2(t[i], ri))
+    with pytest.raises(tcp.TcpError):
+        r.recon_try(d[0], d[1], d[2], d[3], [float(ndet)])        # centre range is the caller's detector
+    # LineRec
+    r.set_algorithm("line")
+    o = r.recon(*_to_dev(np.ascontiguousarray(raw[:, :4]), flat[:4], dark[:4], theta)).cpu().numpy()
+    rl = orc.recon_padded(raw[:, :4], flat[:4], dark[:4], theta, c, w.filter, 3, "lin")
+    for z in range(4):
+        assert rl2(o[z], rl[z]) < FP32_GATE
+    r.close()
+    # a power of two: tcp_create_det == tcp_create_ex
+    raw8, flat8, dark8, _ = _inputs(w, rows)
+    dev = _to_dev(raw8, flat8, dark8, theta)
+    outs = []
+    for create in (tcp.tcp_create_det, tcp.tcp_create_ex):
+        h = create(w.n, w.nproj, 8, w.center, "f16", w.filter, 3)
+        assert tcp.tcp_padded_n(h) == w.n
+        o = torch.empty((8, w.n, w.n), dtype=torch.float16, device="cuda")
+        tcp.tcp_recon(h, *dev, o)
+        torch.cuda.synchronize()
+        outs.append(o.cpu())
+        tcp.tcp_destroy(h)
+    assert torch.equal(outs[0], outs[1])
+    for bad in [(7, 10, 2, 3.0), (4097, 10, 2, 50.0), (100, 10, 2, 99.5), (100, 10, 2, -1.0), (100, 0, 2, 50.0)]:
+        with pytest.raises(tcp.TcpError):
+            tcp.tcp_create_det(bad[0], bad[1], bad[2], bad[3], "f32", "ramp", 0)
+
+
 # ------------------------------------------------------------------ BASELINE full sizes, bench launch configuration
 @pytest.mark.parametrize("cfg,nz,tcfft", [("C4", 32, 0), ("C4", 32, 4), ("C5", 32, 0)])
 def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft):
