@@ -20,7 +20,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liboracle.so")
 _SRC = [os.path.join(_HERE, "oracle.cpp"), os.path.join(_HERE, "oracle_bp.cpp")]
 
-FILTERS = {"ramp": 0, "shepp": 1, "parzen": 2}
+FILTERS = {"ramp": 0, "shepp": 1, "parzen": 2, "cosine": 3, "hann": 4, "hamming": 5}
 METHODS = {"grid": 0, "exact": 1, "lin": 2}
 DEFAULT_M = 4
 

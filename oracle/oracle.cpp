@@ -115,7 +115,10 @@ void orc_neglog(const uint16_t* raw, const float* flat, const float* dark,
 //       h[0] = 1/4, h[i] = -1/(pi^2 i^2) for odd i, 0 for even i != 0   (i signed, wrapped)
 //   W: ramp 1; shepp sin(pi k/M)/(pi k/M); parzen with u = |k|/(M/2):
 //       1 - 6u^2(1-u) for u <= 1/2, 2(1-u)^3 for u > 1/2.     H[M/2] := 0.
-// filter: 0 ramp, 1 shepp, 2 parzen ("Shepp-Logan, Parzen or other filter").
+//   "or other filter": the textbook apodisation windows on the same u,
+//       cosine cos(pi u/2), Hann (1 + cos(pi u))/2, Hamming 0.54 + 0.46 cos(pi u).
+// filter: 0 ramp, 1 shepp, 2 parzen ("Shepp-Logan, Parzen or other filter"),
+//         3 cosine, 4 hann, 5 hamming.
 // ---------------------------------------------------------------------------
 void orc_filter(int M, int filter, double* H) {
     std::vector<cplx> h(M), R(M);
@@ -136,6 +139,11 @@ void orc_filter(int M, int filter, double* H) {
         } else if (filter == 2) {
             double u = std::fabs((double)ks) / (double)(M / 2);
             W = (u <= 0.5) ? 1.0 - 6.0 * u * u * (1.0 - u) : 2.0 * (1.0 - u) * (1.0 - u) * (1.0 - u);
+        } else if (filter >= 3) {
+            double u = std::fabs((double)ks) / (double)(M / 2);
+            if (filter == 3) W = std::cos(0.5 * PI * u);
+            else if (filter == 4) W = 0.5 * (1.0 + std::cos(PI * u));
+            else W = 0.54 + 0.46 * std::cos(PI * u);
         }
         H[k] = R[k].real() * W;
     }

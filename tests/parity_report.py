@@ -25,8 +25,11 @@ def rl2(a, b):
     return float(np.linalg.norm(a - b) / np.linalg.norm(b))
 
 
-def case(label, w, rows, dtype, method="grid", alg="fourier", pad="zero", tcfft=0, gpu_inputs=False):
+def case(label, w, rows, dtype, method="grid", alg="fourier", pad="zero", tcfft=0, gpu_inputs=False, cut=None):
+    """cut = (lo, hi): only detector columns lo..hi are passed on (a width that is not a power of two, tcp_create_det)."""
     nz = len(rows)
+    lo, hi = cut if cut else (0, w.n)
+    ndet, center = hi - lo, w.center - lo
     if gpu_inputs:
         raw_d, ff, df = sg.make_counts_torch(w, rows, device="cuda")
         flat_d = torch.empty((nz, w.n), dtype=torch.float32, device="cuda")
@@ -40,7 +43,10 @@ def case(label, w, rows, dtype, method="grid", alg="fourier", pad="zero", tcfft=
         flat, dark, _, _ = sg.make_flat_dark(w, rows)
         raw_d = torch.from_numpy(raw.view(np.int16)).cuda().view(torch.uint16)
         flat_d, dark_d, theta_d = torch.from_numpy(flat).cuda(), torch.from_numpy(dark).cuda(), torch.from_numpy(w.theta).cuda()
-    r = tcp.Recon(w.n, w.nproj, nz, w.center, dtype, w.filter, 3)
+    if cut:
+        raw_d = raw_d[:, :, lo:hi].contiguous()
+        flat_d, dark_d = flat_d[:, lo:hi].contiguous(), dark_d[:, lo:hi].contiguous()
+    r = tcp.Recon(ndet, w.nproj, nz, center, dtype, w.filter, 3)
     r.set_algorithm(alg)
     r.set_pad(pad)
     if tcfft:
@@ -51,11 +57,12 @@ def case(label, w, rows, dtype, method="grid", alg="fourier", pad="zero", tcfft=
     r.close()
     sample = sorted({0, 1, nz // 2, nz - 1}) if nz > 4 else list(range(nz))
     raw_h = raw_d.view(torch.int16)[:, sample].contiguous().cpu().numpy().view(np.uint16)
-    ref = orc.recon(raw_h, flat_d[sample].cpu().numpy(), dark_d[sample].cpu().numpy(), w.theta, w.center, w.filter, 3, method, pad=pad)
+    recon = orc.recon_padded if cut else orc.recon
+    ref = recon(raw_h, flat_d[sample].cpu().numpy(), dark_d[sample].cpu().numpy(), w.theta, center, w.filter, 3, method, pad=pad)
     e2 = max(rl2(out[z], ref[i]) for i, z in enumerate(sample))
     em = max(float(np.abs(out[z] - ref[i]).max()) for i, z in enumerate(sample)) / float(np.abs(ref).max())
     gate = "1e-5 / -" if dtype == "f32" else "5e-3 / 1e-2"
-    print("| %s | %d x %d^2, %d proj | %s | %d of %d | %.2e | %.2e | %s |" % (label, nz, w.n, w.nproj, dtype, len(sample), nz, e2, em, gate), flush=True)
+    print("| %s | %d x %d^2, %d proj | %s | %d of %d | %.2e | %.2e | %s |" % (label, nz, ndet, w.nproj, dtype, len(sample), nz, e2, em, gate), flush=True)
 
 
 def main():
@@ -74,6 +81,8 @@ def main():
     h = w.nz_total // 2
     case("C2 FourierRec", w, list(range(h - 4, h + 4)), "f32")
     case("C2 FourierRec", w, list(range(h - 4, h + 4)), "f16")
+    case("C2, detector cut to 500 columns (tcp_create_det, padded to 512)", w, list(range(h - 4, h + 4)), "f32", cut=(6, 506))
+    case("C2, detector cut to 333 columns (odd, object truncated)", w, list(range(h - 4, h + 4)), "f16", cut=(90, 423))
     w = sg.make_workload("C3")
     h = w.nz_total // 2
     case("C3 FourierRec (centre 515.5)", w, list(range(h - 8, h + 8)), "f16", gpu_inputs=True)

@@ -415,6 +415,61 @@ def test_pipeline_host_matches_direct():
     r.close()
 
 
+# ------------------------------------------------------------------ degenerate cases of the method
+@pytest.mark.parametrize("dtype", ["f32", "f16"])
+@pytest.mark.parametrize("case", ["one_projection", "axis_angles", "centre_at_edges", "guards"])
+def test_degenerate_cases(dtype, case):
+    """The smallest problem the ABI accepts and the method's special points: a single projection at theta = 0
+    (every sample on a grid point: 2m-1 taps, reading Q7), angles on the axes and diagonals, the rotation centre on
+    the first / last detector pixel, a single slice (paired with zeros), and (fp32) the guards of S1:
+    raw = 0, raw = 65535, raw < dark, flat = dark."""
+    tcp = _tcp()
+    n, nz = 64, 1
+    rng = np.random.default_rng(77)
+    if case == "one_projection":
+        theta, centers = np.array([0.0], np.float32), [32.0]
+    elif case == "axis_angles":
+        theta, centers = (np.arange(4) * np.float32(np.pi / 4)).astype(np.float32), [31.5]
+    elif case == "centre_at_edges":
+        theta, centers = sg.make_theta(12), [0.0, float(n - 1)]
+    else:
+        theta, centers = sg.make_theta(9), [30.25]
+    nproj = theta.size
+    flat = rng.uniform(20000, 30000, (nz, n)).astype(np.float32)
+    dark = rng.uniform(90, 110, (nz, n)).astype(np.float32)
+    raw = np.rint((flat - dark)[None] * np.exp(-rng.uniform(0.0, 1.5, (nproj, nz, n))) + dark[None]).astype(np.uint16)
+    if case == "guards":
+        if dtype != "f32":
+            pytest.skip("p = 13.8 rows leave the range the fp16 scaling is set for (DESIGN.md: |f| < 1.9 per pixel)")
+        raw[0, 0, 3], raw[1, 0, 4], raw[2, 0, 5] = 0, 65535, 50
+        flat[0, 9] = dark[0, 9]
+    for c in centers:
+        r = tcp.Recon(n, nproj, nz, c, dtype, "ramp", 3)
+        out = r.recon(*_to_dev(raw, flat, dark, theta)).float().cpu().numpy()
+        r.close()
+        ref = orc.recon(raw, flat, dark, theta, c, "ramp", 3, "grid")
+        assert np.isfinite(out).all()
+        if dtype == "f32":
+            assert rl2(out[0], ref[0]) < FP32_GATE, (case, c, rl2(out[0], ref[0]))
+        else:
+            assert rl2(out[0], ref[0]) < FP16_GATE_L2, (case, c, rl2(out[0], ref[0]))
+            assert np.abs(out[0] - ref[0]).max() / np.abs(ref).max() < FP16_GATE_MAX
+
+
+def test_empty_inputs_are_refused():
+    tcp = _tcp()
+    r = tcp.Recon(64, 4, 2, 32.0, "f32", "ramp")
+    e = torch.empty((4, 0, 64), dtype=torch.uint16)
+    f = torch.empty((0, 64), dtype=torch.float32)
+    with pytest.raises(tcp.TcpError):
+        r.recon_volume_host(e, f, f, torch.zeros(4), torch.empty((0, 64, 64)))
+    with pytest.raises(tcp.TcpError):
+        tcp.tcp_create(64, 0, 2, 32.0, "f32", "ramp")
+    with pytest.raises(tcp.TcpError):
+        tcp.tcp_create(64, 4, 0, 32.0, "f32", "ramp")
+    r.close()
+
+
 # ------------------------------------------------------------------ detector width not a power of two (8(f-2))
 def _cut(w, rows, lo, hi):
     """Columns lo..hi of a workload's detector: a narrower (possibly odd, possibly truncating) detector."""

@@ -104,6 +104,31 @@ def test_p3_filter_tables(M):
         assert Hp[(M - kk) % M] == pytest.approx(Hr[(M - kk) % M] * wv, rel=1e-12)
 
 
+@pytest.mark.parametrize("M", [64, 256])
+def test_p3_other_windows_closed_form_impulse_responses(M):
+    """cosine / Hann / Hamming ("or other filter").  A raised-cosine window a + b cos(2 pi k/M) turns
+    the impulse response into a h[i] + b/2 (h[i-1] + h[i+1]) of the closed-form ramp kernel h (periodic in M), minus
+    the zeroed Nyquist bin; the cosine window is pinned by its values (its shift is half a sample)."""
+    k = np.arange(M)
+    ks = np.where(k < M // 2, k, k - M)
+    i = ks.astype(np.float64)
+    alt = np.where(ks % 2 == 0, 1.0, -1.0)
+    href = np.where(ks == 0, 0.25, np.where(ks % 2 != 0, -1.0 / (np.pi ** 2 * np.maximum(i * i, 1)), 0.0))
+    r_nyq = np.sum(href * alt)
+    for name, a, b in (("hann", 0.5, 0.5), ("hamming", 0.54, 0.46)):
+        H = orc.filter_table(M, name)
+        assert H[M // 2] == 0.0 and np.abs(H[1:] - H[1:][::-1]).max() < 1e-14
+        expect = a * href + 0.5 * b * (np.roll(href, 1) + np.roll(href, -1)) - (a - b) * r_nyq / M * alt
+        assert np.abs(np.fft.ifft(H).real - expect).max() < 1e-14
+    Hc, Hr = orc.filter_table(M, "cosine"), orc.filter_table(M, "ramp")
+    assert Hc[M // 2] == 0.0 and np.abs(Hc[1:] - Hc[1:][::-1]).max() < 1e-14
+    for u, wv in ((0.0, 1.0), (0.5, np.sqrt(0.5)), (2.0 / 3.0, 0.5), (0.25, np.cos(np.pi / 8))):
+        kk = int(round(u * M / 2))
+        if abs(kk - u * M / 2) < 1e-12:
+            assert Hc[kk] == pytest.approx(Hr[kk] * wv, rel=1e-12)
+            assert Hc[(M - kk) % M] == pytest.approx(Hr[(M - kk) % M] * wv, rel=1e-12)
+
+
 def test_p3_filter_rows_is_linear_convolution_with_kernel():
     # zero padding to M = 2n makes the FFT product a LINEAR convolution on [0, n)
     n, M = 32, 64
