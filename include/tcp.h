@@ -39,8 +39,11 @@ typedef void* tcp_stream_t;                     /* a cudaStream_t (NULL = legacy
 /* compute/storage dtype of the intermediates and dtype of `out` (FP16 storage
  * with FP32 arithmetic where FP16 would lose accuracy).  F16_OUT32 exists for config C5. */
 enum { TCP_F32 = 0, TCP_F16 = 1, TCP_F16_OUT32 = 2 };
-/* "--fbp-filter": windows multiplying the band-limited ramp. */
-enum { TCP_FILTER_RAMP = 0, TCP_FILTER_SHEPP = 1, TCP_FILTER_PARZEN = 2 };
+/* "--fbp-filter": windows multiplying the band-limited ramp; "Shepp-Logan, Parzen or other
+ * filter": the others are the textbook apodisation windows on u = |k|/(M/2): cosine cos(pi u/2),
+ * Hann (1 + cos(pi u))/2, Hamming 0.54 + 0.46 cos(pi u). */
+enum { TCP_FILTER_RAMP = 0, TCP_FILTER_SHEPP = 1, TCP_FILTER_PARZEN = 2, TCP_FILTER_COSINE = 3, TCP_FILTER_HANN = 4,
+       TCP_FILTER_HAMMING = 5 };
 enum { TCP_OK = 0, TCP_EINVAL = -1, TCP_ENOMEM = -2, TCP_ECUDA = -3, TCP_EUNSUPPORTED = -4 };
 /* intermediates a test may inspect through tcp_workspace() */
 enum { TCP_WS_SINOGRAM = 0, TCP_WS_SPECTRUM = 1, TCP_WS_GRID = 2, TCP_WS_PASS1 = 3, TCP_WS_TRIG = 4 };

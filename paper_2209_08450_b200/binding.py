@@ -11,7 +11,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libtcp.so")
 
 DTYPES = {"f32": 0, "f16": 1, "f16_out32": 2}
-FILTERS = {"ramp": 0, "shepp": 1, "parzen": 2}
+FILTERS = {"ramp": 0, "shepp": 1, "parzen": 2, "cosine": 3, "hann": 4, "hamming": 5}
 WS = {"sinogram": 0, "spectrum": 1, "grid": 2, "pass1": 3, "trig": 4}
 GRID_IMPLS = {"gather": 0, "scatter": 1, "tile": 2, "mma": 3}
 

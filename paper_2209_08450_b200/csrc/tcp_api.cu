@@ -47,6 +47,9 @@ static void build_filter(int M, int filter, std::vector<float>& out) {
         } else if (filter == TCP_FILTER_PARZEN) {
             double u = (double)k / (double)(M / 2);
             w = (u <= 0.5) ? 1.0 - 6.0 * u * u * (1.0 - u) : 2.0 * (1.0 - u) * (1.0 - u) * (1.0 - u);
+        } else if (filter == TCP_FILTER_COSINE || filter == TCP_FILTER_HANN || filter == TCP_FILTER_HAMMING) {
+            const double u = (double)k / (double)(M / 2);       // "or other filter": textbook apodisation windows
+            w = filter == TCP_FILTER_COSINE ? cos(0.5 * kPi * u) : filter == TCP_FILTER_HANN ? 0.5 * (1.0 + cos(kPi * u)) : 0.54 + 0.46 * cos(kPi * u);
         }
         double h = (k == M / 2) ? 0.0 : r * w / (double)M;
         out[k] = (float)h;
@@ -185,7 +188,7 @@ static tcp_ctx* create_impl(int n, int ndet, int pad_l, int nproj, int nz_chunk,
     if (!(center >= 0.f && center <= (float)(ndet - 1))) { set_error(TCP_EINVAL, "center=%g outside [0, n-1]", (double)center); return nullptr; }
     center += (float)pad_l;
     if (dtype < TCP_F32 || dtype > TCP_F16_OUT32) { set_error(TCP_EINVAL, "unknown dtype %d", dtype); return nullptr; }
-    if (filter < TCP_FILTER_RAMP || filter > TCP_FILTER_PARZEN) { set_error(TCP_EINVAL, "unknown filter %d", filter); return nullptr; }
+    if (filter < TCP_FILTER_RAMP || filter > TCP_FILTER_HAMMING) { set_error(TCP_EINVAL, "unknown filter %d", filter); return nullptr; }
     if (m != 3 && m != 4) { set_error(TCP_EINVAL, "kernel half-width m=%d must be 3 or 4", m); return nullptr; }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {

@@ -185,7 +185,7 @@ def test_downscaled_configs(cfg, scale, dtype):
         assert np.abs(out - ref).max() / np.abs(ref).max() < FP16_GATE_MAX
 
 
-@pytest.mark.parametrize("filt", ["ramp", "shepp", "parzen"])
+@pytest.mark.parametrize("filt", ["ramp", "shepp", "parzen", "cosine", "hann", "hamming"])
 def test_filters_and_offcentre(filt):
     w = sg.make_workload("C1")
     w.center = 61.75
