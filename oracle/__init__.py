@@ -207,10 +207,29 @@ def deapod_crop_adjoint(f, n, m=DEFAULT_M):
     return g
 
 
-def fbp_from_sino(p, theta, center, filt="ramp", m=DEFAULT_M, method="grid", return_q=False, pad="zero", fused=False):
-    """p f64 [nz][nproj][n] -> out f64 [nz][n][n] (S3..S7 or the two definitions)."""
+def angle_weights(theta):
+    """Quadrature weights of the backprojection integral over [0, pi) for angles that are NOT equally spaced
+    (the Fourier-based method, unlike the log-polar one, applies to "non-equally spaced angles",
+    e.g. interlaced scanning; reading Q20): the trapezoid (midpoint-cell) rule on the periodic
+    angle axis, w_j = (theta_{j+1} - theta_{j-1}) / 2 with theta_nproj = theta_0 + pi and
+    theta_{-1} = theta_{nproj-1} - pi, returned RELATIVE to the constant pi/nproj the default path uses
+    (all ones for equispaced angles over a half turn).  theta float32, increasing, spanning less than pi;
+    arithmetic in double from the float32 values."""
+    t = _f32(theta).astype(np.float64)
+    nxt = np.concatenate([t[1:], [t[0] + np.pi]])
+    prv = np.concatenate([[t[-1] - np.pi], t[:-1]])
+    return 0.5 * (nxt - prv) * t.size / np.pi
+
+
+def fbp_from_sino(p, theta, center, filt="ramp", m=DEFAULT_M, method="grid", return_q=False, pad="zero", fused=False,
+                  angle_weighted=False):
+    """p f64 [nz][nproj][n] -> out f64 [nz][n][n] (S3..S7 or the two definitions).
+    angle_weighted: projection j enters with weight angle_weights(theta)[j] * pi/nproj instead of pi/nproj
+    (everything after S2 is linear in the projection, so the row of the sinogram is scaled)."""
     p = _f64(p)
     theta = _f32(theta)
+    if angle_weighted:
+        p = np.ascontiguousarray(p * angle_weights(theta)[None, :, None])
     nz, nproj, n = p.shape
     out = np.empty((nz, n, n))
     q = np.empty_like(p) if return_q else None
@@ -220,11 +239,15 @@ def fbp_from_sino(p, theta, center, filt="ramp", m=DEFAULT_M, method="grid", ret
     return (out, q) if return_q else out
 
 
-def recon(raw, flat, dark, theta, center, filt="ramp", m=DEFAULT_M, method="grid", pad="zero", fused=False):
+def recon(raw, flat, dark, theta, center, filt="ramp", m=DEFAULT_M, method="grid", pad="zero", fused=False,
+          angle_weighted=False):
     """uint16 counts -> reconstruction, S1..S7.  raw [nproj][nz][n] -> out [nz][n][n]."""
     raw = np.ascontiguousarray(raw, dtype=np.uint16)
     nproj, nz, n = raw.shape
     flat, dark, theta = _f32(flat), _f32(dark), _f32(theta)
+    if angle_weighted:
+        return fbp_from_sino(neglog(raw, flat, dark), theta, center, filt=filt, m=m, method=method, pad=pad, fused=fused,
+                             angle_weighted=True)
     out = np.empty((nz, n, n))
     lib().orc_recon_pad(_p(raw), _p(flat), _p(dark), _p(theta), C.c_int(nproj), C.c_int(nz), C.c_int(n),
                     C.c_double(center), C.c_int(FILTERS[filt]), C.c_int(PADS[pad] | (2 if fused else 0)), C.c_int(m), C.c_int(METHODS[method]),
