@@ -74,8 +74,14 @@ enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1, TCP_GRID_TILE = 2, TCP_
  * (sub-tile, sample), which depend only on theta, n and m, in a device cache built on the first call and
  * rebuilt (on the device, no host synchronisation) whenever the angles passed to tcp_recon change; 0 computes
  * them in every call.  Same results bit for bit. */
+/* TCP_OPT_ANGLE_WEIGHTS (0 default | 1): quadrature weights for angles that are not equally spaced (PAPER.md:61:
+ * unlike the log-polar method, the Fourier-based one applies to "non-equally spaced angles", e.g. interlaced
+ * scanning).  0: every projection enters with pi/nproj (equispaced half turn).  1: projection j enters with
+ * (theta[j+1] - theta[j-1]) / 2, where theta[nproj] = theta[0] + pi and theta[-1] = theta[nproj-1] - pi (trapezoid
+ * rule on the periodic angle axis; the angles must cover the half turn), computed on the device from the angles of
+ * each call.  All algorithms and tcp_recon_try. */
 enum { TCP_OPT_GRID_IMPL = 0, TCP_OPT_PROFILE = 1, TCP_OPT_TCFFT = 2, TCP_OPT_ALGORITHM = 3, TCP_OPT_PAD = 4,
-       TCP_OPT_FILTER_FUSED = 5, TCP_OPT_WEIGHT_CACHE = 6 };
+       TCP_OPT_FILTER_FUSED = 5, TCP_OPT_WEIGHT_CACHE = 6, TCP_OPT_ANGLE_WEIGHTS = 7 };
 enum { TCP_PAD_ZERO = 0, TCP_PAD_EDGE = 1 };
 enum { TCP_ALG_FOURIER = 0, TCP_ALG_LINE = 1 };
 enum { TCP_TCFFT_ROWS = 1, TCP_TCFFT_COLS = 2, TCP_TCFFT_IROWS = 4 };

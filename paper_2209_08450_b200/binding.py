@@ -200,6 +200,10 @@ class Recon:
         """TCP_OPT_WEIGHT_CACHE: reuse the gridding weights across calls with the same angles (default on)."""
         _check(lib().tcp_set_option(self.h, 6, 1 if on else 0))
 
+    def set_angle_weights(self, on: bool):
+        """TCP_OPT_ANGLE_WEIGHTS: trapezoid quadrature weights for unequally spaced angles (off by default)."""
+        _check(lib().tcp_set_option(self.h, 7, 1 if on else 0))
+
     def set_filter_fused(self, on: bool):
         """TCP_OPT_FILTER_FUSED: S3 + S4 as one transform without the crop (a different reading; off by default)."""
         _check(lib().tcp_set_option(self.h, 5, 1 if on else 0))

@@ -208,9 +208,18 @@ int launch_mean_frames(const uint16_t* frames, int nframes, int nz, int n, float
 // cos/sin of the float32 angles in fp64: k*cos(theta) with
 // k up to 4096 must be good to ~1e-6 grid cells for the 1e-5 fp32 gate.
 __global__ void trig_kernel(const float* __restrict__ theta, int nproj, double2* __restrict__ trig, float4* __restrict__ trigf,
-                            int* __restrict__ wstate) {
+                            int* __restrict__ wstate, float* __restrict__ wq) {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j < nproj) {
+        // quadrature weight for unequally spaced angles (TCP_OPT_ANGLE_WEIGHTS, reading Q20):
+        // trapezoid rule on the periodic angle axis, (theta_{j+1} - theta_{j-1}) / 2 with theta_nproj = theta_0 + pi
+        // and theta_{-1} = theta_{nproj-1} - pi, relative to pi/nproj; fp64 from the float32 angles
+        {
+            const double pi = 3.14159265358979323846264338327950288;
+            const double nxt = (j + 1 < nproj) ? (double)theta[j + 1] : (double)theta[0] + pi;
+            const double prv = (j > 0) ? (double)theta[j - 1] : (double)theta[nproj - 1] - pi;
+            wq[j] = (float)(0.5 * (nxt - prv) * (double)nproj / pi);
+        }
         // order-independent checksum of the angles for the gridding weight cache (k_grid_mma.cu, state[3])
         if (wstate) atomicAdd(&wstate[3], (int)((__float_as_uint(theta[j]) ^ 0x9e3779b9u) * (2u * (unsigned)j + 1u)));
         double t = (double)theta[j];
@@ -224,7 +233,7 @@ __global__ void trig_kernel(const float* __restrict__ theta, int nproj, double2*
 }
 
 int launch_trig(const tcp_ctx* c, const float* theta, cudaStream_t st) {
-    trig_kernel<<<(c->nproj + 127) / 128, 128, 0, st>>>(theta, c->nproj, c->trig, c->trigf, c->w_state);
+    trig_kernel<<<(c->nproj + 127) / 128, 128, 0, st>>>(theta, c->nproj, c->trig, c->trigf, c->w_state, c->wq);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }

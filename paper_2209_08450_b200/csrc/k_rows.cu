@@ -13,7 +13,8 @@ template <int M, int ROWS, bool PAD_EDGE, class TS, class TC>
 __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict__ sino, TC* __restrict__ spec,
                                                             const float2* __restrict__ tw,
                                                             const float* __restrict__ hfilt,
-                                                            const float2* __restrict__ ptab, int nproj, int nz, int try_mode) {
+                                                            const float2* __restrict__ ptab, int nproj, int nz, int try_mode,
+                                                            const float* __restrict__ wq) {
     constexpr bool pad_edge = PAD_EDGE;
     constexpr int n = M / 2;
     constexpr int TG = M / 16;
@@ -32,6 +33,7 @@ __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict
     const TS* pB = sino + ((size_t)(zB < nz ? zB : zA) * nproj + j) * n;
     const bool hasB = zB < nz;
     if (try_mode) ptab += (size_t)pair * M;
+    const float wj = wq ? __ldg(&wq[j]) : 1.f;      // TCP_OPT_ANGLE_WEIGHTS: everything after S2 is linear in the projection
 
     auto load_padded = [&](int i) {
         // padding samples: zeros, or (TCP_OPT_PAD = TCP_PAD_EDGE) the nearest edge of the periodic row
@@ -39,7 +41,7 @@ __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict
             if (!pad_edge) return make_float2(0.f, 0.f);
             i = (i < n + n / 2) ? n - 1 : 0;
         }
-        return make_float2(ld_r(pA, i), hasB ? ld_r(pB, i) : 0.f);
+        return make_float2(ld_r(pA, i) * wj, hasB ? ld_r(pB, i) * wj : 0.f);
     };
     TC* out = spec + ((size_t)pair * nproj + j) * M;
     // the three transforms hand their lines over in registers (fft_chain_slot: same elements, permuted slots):
@@ -64,7 +66,8 @@ __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict
 template <int M, int ROWS, bool PAD_EDGE, class TS, class TC>
 __global__ void __launch_bounds__(ROWS* M / 16) rows_fused_kernel(const TS* __restrict__ sino, TC* __restrict__ spec,
                                                                   const float2* __restrict__ tw,
-                                                                  const float2* __restrict__ ftab, int nproj, int nz) {
+                                                                  const float2* __restrict__ ftab, int nproj, int nz,
+                                                                  const float* __restrict__ wq) {
     constexpr int n = M / 2;
     constexpr int TG = M / 16;
     extern __shared__ float2 smem[];
@@ -80,6 +83,7 @@ __global__ void __launch_bounds__(ROWS* M / 16) rows_fused_kernel(const TS* __re
     const TS* pA = sino + ((size_t)zA * nproj + j) * n;
     const TS* pB = sino + ((size_t)(hasB ? zB : zA) * nproj + j) * n;
     TC* out = spec + ((size_t)pair * nproj + j) * M;
+    const float wj = wq ? __ldg(&wq[j]) : 1.f;
     fft_line<M, false>(
         s, tid, tw,
         [&](int i) {
@@ -87,7 +91,7 @@ __global__ void __launch_bounds__(ROWS* M / 16) rows_fused_kernel(const TS* __re
                 if (!PAD_EDGE) return make_float2(0.f, 0.f);
                 i = (i < n + n / 2) ? n - 1 : 0;
             }
-            return make_float2(ld_r(pA, i), hasB ? ld_r(pB, i) : 0.f);
+            return make_float2(ld_r(pA, i) * wj, hasB ? ld_r(pB, i) * wj : 0.f);
         },
         [&](int k, float2 v) {
             if (live) st_c(out, k, cmul(v, __ldg(&ftab[k])));
@@ -99,7 +103,8 @@ __global__ void __launch_bounds__(ROWS* M / 16) rows_fused_kernel(const TS* __re
 // the first pass ends and writes them in the last pass of the inverse transform).
 template <int M, int ROWS, class TS>
 __global__ void __launch_bounds__(ROWS* M / 16) filter_kernel(TS* __restrict__ sino, const float2* __restrict__ tw,
-                                                              const float* __restrict__ hfilt, int nproj, int nz, int pad_edge) {
+                                                              const float* __restrict__ hfilt, int nproj, int nz, int pad_edge,
+                                                              const float* __restrict__ wq) {
     constexpr int n = M / 2;
     constexpr int TG = M / 16;
     extern __shared__ float2 smem[];
@@ -114,6 +119,7 @@ __global__ void __launch_bounds__(ROWS* M / 16) filter_kernel(TS* __restrict__ s
     const bool hasB = zB < nz;
     TS* pA = sino + ((size_t)zA * nproj + j) * n;
     TS* pB = sino + ((size_t)(hasB ? zB : zA) * nproj + j) * n;
+    const float wj = wq ? __ldg(&wq[j]) : 1.f;
     float2 keep[16];
     fft_line<M, false>(
         s, tid, tw,
@@ -123,7 +129,7 @@ __global__ void __launch_bounds__(ROWS* M / 16) filter_kernel(TS* __restrict__ s
                 if (!pad_edge) return make_float2(0.f, 0.f);
                 i = (i < n + n / 2) ? n - 1 : 0;
             }
-            return make_float2(ld_r(pA, i), hasB ? ld_r(pB, i) : 0.f);
+            return make_float2(ld_r(pA, i) * wj, hasB ? ld_r(pB, i) * wj : 0.f);
         },
         [&](int k, float2 v, int slot) {
             const float h = __ldg(&hfilt[k]);
@@ -147,7 +153,7 @@ static int launch_filter_t(const tcp_ctx* c, cudaStream_t st) {
     auto kern = filter_kernel<M, ROWS, TS>;
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid((c->nproj + ROWS - 1) / ROWS, c->npair);
-    kern<<<grid, ROWS * TG, smem, st>>>((TS*)c->sino, c->tw, c->hfilt, c->nproj, c->nz, c->pad);
+    kern<<<grid, ROWS * TG, smem, st>>>((TS*)c->sino, c->tw, c->hfilt, c->nproj, c->nz, c->pad, c->angle_weights ? c->wq : nullptr);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }
@@ -179,7 +185,7 @@ static int launch_rows_t(const tcp_ctx* c, cudaStream_t st) {
         auto kf = c->pad ? rows_fused_kernel<M, ROWS, true, TS, TC> : rows_fused_kernel<M, ROWS, false, TS, TC>;
         TCP_CUDA_CHECK(cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         kf<<<dim3((c->nproj + ROWS - 1) / ROWS, c->npair), ROWS * TG, smem, st>>>((const TS*)c->sino, (TC*)c->spec, c->tw, c->ftab, c->nproj,
-                                                                                   c->nz);
+                                                                                   c->nz, c->angle_weights ? c->wq : nullptr);
         TCP_CUDA_CHECK(cudaGetLastError());
         return TCP_OK;
     }
@@ -187,7 +193,7 @@ static int launch_rows_t(const tcp_ctx* c, cudaStream_t st) {
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid((c->nproj + ROWS - 1) / ROWS, c->npair);
     kern<<<grid, ROWS * TG, smem, st>>>((const TS*)c->sino, (TC*)c->spec, c->tw, c->hfilt, c->try_ptab ? c->try_ptab : c->ptab, c->nproj, c->nz,
-                                       c->try_ptab ? 1 : 0);
+                                       c->try_ptab ? 1 : 0, c->angle_weights ? c->wq : nullptr);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }

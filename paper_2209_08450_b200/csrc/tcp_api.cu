@@ -86,6 +86,7 @@ static int build_context(tcp_ctx* c) {
     if ((rc = dev_alloc(&c->pass1, (size_t)c->npair * n * M * cb, &c->bytes))) return rc;
     if ((rc = dev_alloc((void**)&c->trig, (size_t)c->nproj * sizeof(double2), &c->bytes))) return rc;
     if ((rc = dev_alloc((void**)&c->trigf, (size_t)c->nproj * sizeof(float4), &c->bytes))) return rc;
+    if ((rc = dev_alloc((void**)&c->wq, (size_t)c->nproj * sizeof(float), &c->bytes))) return rc;
 
     std::vector<float2> tw(M);
     for (int t = 0; t < M; ++t) {
@@ -252,7 +253,7 @@ void tcp_destroy(tcp_ctx* c) {
         for (int i = 0; i < kProfileRing * (TCP_NSTAGES + 1); ++i) cudaEventDestroy(c->pev[i]);
         free(c->pev);
     }
-    cudaFree(c->sino); cudaFree(c->spec); cudaFree(c->grid); cudaFree(c->pass1); cudaFree(c->trig); cudaFree(c->trigf);
+    cudaFree(c->sino); cudaFree(c->spec); cudaFree(c->grid); cudaFree(c->pass1); cudaFree(c->trig); cudaFree(c->trigf); cudaFree(c->wq);
     cudaFree(c->tw); cudaFree(c->hfilt); cudaFree(c->ptab); cudaFree(c->ftab); cudaFree(c->deax); cudaFree(c->deay);
     cudaFree(c->tile_order);
     cudaFree(c->try_buf);
@@ -431,6 +432,10 @@ int tcp_set_option(tcp_ctx* c, int option, int value) {
     }
     if (option == TCP_OPT_WEIGHT_CACHE) {
         c->w_enable = value != 0;
+        return TCP_OK;
+    }
+    if (option == TCP_OPT_ANGLE_WEIGHTS) {
+        c->angle_weights = value != 0;
         return TCP_OK;
     }
     if (option == TCP_OPT_FILTER_FUSED) {

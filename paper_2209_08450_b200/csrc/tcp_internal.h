@@ -31,6 +31,8 @@ struct tcp_ctx {
     void* pass1;          // [npair][M/W][n][W]  float2 | half2   (strip of W = cols_strip_width(M) columns l1, row = iy)
     double2* trig;        // [nproj] (cos, sin) of theta, fp64
     float4* trigf;        // [nproj] (cos hi, cos lo, sin hi, sin lo): float-float split of trig
+    float* wq;            // [nproj] quadrature weight of every projection relative to pi/nproj (trig_kernel, every call)
+    int angle_weights;    // TCP_OPT_ANGLE_WEIGHTS: the row kernels scale projection j by wq[j] (unequally spaced angles)
     // tables (device), built in fp64 on the host at create
     float2* tw;           // [M] e^{-2 pi i t / M}
     float* hfilt;         // [M] H[k] / M

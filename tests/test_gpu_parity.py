@@ -415,6 +415,51 @@ def test_pipeline_host_matches_direct():
     r.close()
 
 
+# ------------------------------------------------------------------ unequally spaced angles
+@pytest.mark.parametrize("dtype,alg", [("f32", "fourier"), ("f16", "fourier"), ("f32", "line")])
+def test_angle_weights_for_unequally_spaced_angles(dtype, alg):
+    """TCP_OPT_ANGLE_WEIGHTS: angles in two interleaved spacings; the GPU's trapezoid weights (trig_kernel, fp64 from
+    the float32 angles) against the oracle's (pin P11); also through tcp_recon_try; with equispaced angles the
+    option changes nothing beyond rounding; switching it off restores the default bit for bit."""
+    tcp = _tcp()
+    w = sg.make_workload("C1")
+    raw, flat, dark, _ = _inputs(w, [2, 3, 4])
+    nproj = w.nproj
+    na = 2 * nproj // 3
+    theta = np.concatenate([np.arange(na) * (np.pi / 2 / na), np.pi / 2 + np.arange(nproj - na) * (np.pi / 2 / (nproj - na))]).astype(np.float32)
+    r = tcp.Recon(w.n, nproj, 3, w.center, dtype, w.filter, 3)
+    dev = _to_dev(raw, flat, dark, theta)
+    base = r.recon(*dev).float().cpu().numpy()
+    r.set_algorithm(alg)
+    r.set_angle_weights(True)
+    out = r.recon(*dev).float().cpu().numpy()
+    method = "grid" if alg == "fourier" else "lin"
+    ref = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, method, angle_weighted=True)
+    plain = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, method)
+    assert rl2(plain[0], ref[0]) > 0.05                      # the weights matter for these angles
+    for z in range(3):
+        if dtype == "f32":
+            assert rl2(out[z], ref[z]) < FP32_GATE, (z, rl2(out[z], ref[z]))
+        else:
+            assert rl2(out[z], ref[z]) < FP16_GATE_L2
+            assert np.abs(out[z] - ref[z]).max() / np.abs(ref).max() < FP16_GATE_MAX
+    if alg == "fourier":
+        t = r.recon_try(dev[0][:, 1:2].contiguous(), dev[1][1:2], dev[2][1:2], dev[3], [w.center, w.center + 1.5]).float().cpu().numpy()
+        assert rl2(t[0], ref[1]) < (FP32_GATE if dtype == "f32" else FP16_GATE_L2)
+        r.set_angle_weights(False)
+        again = r.recon(*dev).float().cpu().numpy()
+        assert np.array_equal(again, base)
+    r.close()
+    # equispaced: weights are 1 to float32 rounding of the angles
+    r = tcp.Recon(w.n, nproj, 3, w.center, "f32", w.filter, 3)
+    d2 = _to_dev(raw, flat, dark, w.theta)
+    a = r.recon(*d2).cpu().numpy()
+    r.set_angle_weights(True)
+    b = r.recon(*d2).cpu().numpy()
+    r.close()
+    assert rl2(b, a) < 2e-5
+
+
 # ------------------------------------------------------------------ degenerate cases of the method
 @pytest.mark.parametrize("dtype", ["f32", "f16"])
 @pytest.mark.parametrize("case", ["one_projection", "axis_angles", "centre_at_edges", "guards"])
