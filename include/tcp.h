@@ -192,6 +192,19 @@ int tcp_recon_volume_host(tcp_ctx* ctx, const uint16_t* raw_host, const float* f
                           const float* dark_host, const float* theta_host, void* out_host,
                           int nz_total, int nbuf, float* ms_out);
 
+/* The same pipeline on the slice range [z_begin, z_end) of a stack of nz_stack slices ("--start-row / --end-row",
+ * PAPER.md:133-135; the paper's multi-GPU recipe: one process per GPU, each on its own
+ * subset of slices, nothing exchanged).  All HOST arrays keep the full-stack shapes of tcp_recon_volume_host with
+ * nz_total = nz_stack (several processes may share them); only rows z_begin..z_end-1 are read, and only those
+ * slices of out_host are written.  TCP_EINVAL unless 0 <= z_begin < z_end <= nz_stack. */
+int tcp_recon_volume_host_rows(tcp_ctx* ctx, const uint16_t* raw_host, const float* flat_host,
+                               const float* dark_host, const float* theta_host, void* out_host,
+                               int nz_stack, int z_begin, int z_end, int nbuf, float* ms_out);
+/* HOST logic only (no CUDA call): the contiguous slice range [*z0, *z1) of process `rank` of `world` over
+ * nz_total slices; the ranges tile [0, nz_total) in rank order and differ by at most one slice (a rank may get
+ * an empty range when world > nz_total).  TCP_EINVAL on a bad argument. */
+int tcp_slice_range(int nz_total, int rank, int world, int* z0, int* z1);
+
 #ifdef __cplusplus
 }
 #endif

@@ -19,6 +19,8 @@ from .binding import (  # noqa: F401
     tcp_normalize,
     tcp_mean_frames_u16,
     tcp_recon_volume_host,
+    tcp_recon_volume_host_rows,
+    tcp_slice_range,
     tcp_last_error,
     DTYPES,
     FILTERS,

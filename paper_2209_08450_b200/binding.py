@@ -21,6 +21,7 @@ EXPORTS = [
     "tcp_mean_frames_u16", "tcp_normalize", "tcp_workspace", "tcp_read_workspace", "tcp_scale", "tcp_grid_strip",
     "tcp_workspace_bytes", "tcp_launches_per_recon", "tcp_set_option", "tcp_profile_collect",
     "tcp_recon_volume_host", "tcp_recon_try", "tcp_create_det", "tcp_padded_n",
+    "tcp_recon_volume_host_rows", "tcp_slice_range",
 ]
 
 
@@ -80,6 +81,10 @@ def lib():
     L.tcp_profile_collect.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(ci)]
     L.tcp_recon_volume_host.restype = ci
     L.tcp_recon_volume_host.argtypes = [vp, vp, vp, vp, vp, vp, ci, ci, C.POINTER(cf)]
+    L.tcp_recon_volume_host_rows.restype = ci
+    L.tcp_recon_volume_host_rows.argtypes = [vp, vp, vp, vp, vp, vp, ci, ci, ci, ci, C.POINTER(cf)]
+    L.tcp_slice_range.restype = ci
+    L.tcp_slice_range.argtypes = [ci, ci, ci, C.POINTER(ci), C.POINTER(ci)]
     L.tcp_recon_try.restype = ci
     L.tcp_recon_try.argtypes = [vp, vp, vp, vp, vp, C.POINTER(cf), ci, vp, vp]
     _lib = L
@@ -162,6 +167,22 @@ def tcp_recon_volume_host(h, raw_host, flat_host, dark_host, theta_host, out_hos
                                        theta_host.data_ptr(), out_host.data_ptr(), int(nz_total), int(nbuf),
                                        C.byref(ms)))
     return float(ms.value)
+
+
+def tcp_recon_volume_host_rows(h, raw_host, flat_host, dark_host, theta_host, out_host, nz_stack, z_begin, z_end, nbuf=3):
+    """Slices [z_begin, z_end) of full-stack host tensors; returns the device-timed milliseconds."""
+    ms = C.c_float(0.0)
+    _check(lib().tcp_recon_volume_host_rows(h, raw_host.data_ptr(), flat_host.data_ptr(), dark_host.data_ptr(),
+                                            theta_host.data_ptr(), out_host.data_ptr(), int(nz_stack), int(z_begin),
+                                            int(z_end), int(nbuf), C.byref(ms)))
+    return float(ms.value)
+
+
+def tcp_slice_range(nz_total, rank, world):
+    """(z0, z1): the slice range of process `rank` of `world` (host logic in the library, no GPU needed)."""
+    z0, z1 = C.c_int(0), C.c_int(0)
+    _check(lib().tcp_slice_range(int(nz_total), int(rank), int(world), C.byref(z0), C.byref(z1)))
+    return int(z0.value), int(z1.value)
 
 
 def _as_u16(t: torch.Tensor) -> torch.Tensor:
@@ -306,11 +327,17 @@ class Recon:
             v = v.view(npair, M // w, n, w, 2).permute(0, 2, 1, 3, 4).reshape(npair, n, M, 2)
         return torch.complex(v[..., 0], v[..., 1])
 
-    def recon_volume_host(self, raw_host, flat_host, dark_host, theta_host, out_host=None, nbuf=3):
+    def recon_volume_host(self, raw_host, flat_host, dark_host, theta_host, out_host=None, nbuf=3, rows=None):
+        """rows = (z_begin, z_end): only that slice range of the stack (tcp_recon_volume_host_rows), e.g.
+        tcp_slice_range(nz_total, rank, world) in a one-process-per-GPU job; out_host keeps the full-stack shape."""
         raw_host = _as_u16(raw_host)
         nproj, nz_total, n = raw_host.shape
         assert (nproj, n) == (self.nproj, self.n)
         if out_host is None:
             out_host = torch.empty((nz_total, n, n), dtype=self.out_dtype).pin_memory()
-        ms = tcp_recon_volume_host(self.h, raw_host, flat_host, dark_host, theta_host, out_host, nz_total, nbuf)
+        if rows is None:
+            ms = tcp_recon_volume_host(self.h, raw_host, flat_host, dark_host, theta_host, out_host, nz_total, nbuf)
+        else:
+            ms = tcp_recon_volume_host_rows(self.h, raw_host, flat_host, dark_host, theta_host, out_host, nz_total,
+                                            rows[0], rows[1], nbuf)
         return out_host, ms

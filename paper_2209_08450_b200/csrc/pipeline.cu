@@ -57,7 +57,7 @@ static int pipe_create(tcp_ctx* c, int nbuf) {
         TCP_CUDA_CHECK(cudaMalloc((void**)&p->flat[b], (size_t)c->nz * n * 4));
         TCP_CUDA_CHECK(cudaMalloc((void**)&p->dark[b], (size_t)c->nz * n * 4));
         TCP_CUDA_CHECK(cudaMalloc(&p->out[b], (size_t)c->nz * n * n * ob));
-        // a partial last chunk leaves rows unwritten: keep them finite
+        // (buffers start zeroed: nothing reads rows a call did not write, this only keeps debugging dumps clean)
         TCP_CUDA_CHECK(cudaMemset(p->raw[b], 0, (size_t)c->nproj * c->nz * n * 2));
         TCP_CUDA_CHECK(cudaMemset(p->flat[b], 0, (size_t)c->nz * n * 4));
         TCP_CUDA_CHECK(cudaMemset(p->dark[b], 0, (size_t)c->nz * n * 4));
@@ -73,31 +73,52 @@ static int pipe_create(tcp_ctx* c, int nbuf) {
 
 using namespace tcpk;
 
+// Contiguous slice range of rank `rank` of `world` (one process per GPU on a subset of the
+// slices, no exchange between them): ranges differ by at most one slice and tile [0, nz_total) in rank order.
+extern "C" int tcp_slice_range(int nz_total, int rank, int world, int* z0, int* z1) {
+    if (nz_total < 0 || world < 1 || rank < 0 || rank >= world || !z0 || !z1) return set_error(TCP_EINVAL, "bad slice-range argument");
+    const long long q = nz_total / world, r = nz_total % world;
+    *z0 = (int)(q * rank + (rank < r ? rank : r));
+    *z1 = *z0 + (int)q + (rank < r ? 1 : 0);
+    return TCP_OK;
+}
+
 extern "C" int tcp_recon_volume_host(tcp_ctx* c, const uint16_t* raw_host, const float* flat_host,
                                      const float* dark_host, const float* theta_host, void* out_host, int nz_total,
                                      int nbuf, float* ms_out) {
+    return tcp_recon_volume_host_rows(c, raw_host, flat_host, dark_host, theta_host, out_host, nz_total, 0, nz_total, nbuf, ms_out);
+}
+
+extern "C" int tcp_recon_volume_host_rows(tcp_ctx* c, const uint16_t* raw_host, const float* flat_host,
+                                          const float* dark_host, const float* theta_host, void* out_host, int nz_stack,
+                                          int z_begin, int z_end, int nbuf, float* ms_out) {
     if (!c || !raw_host || !flat_host || !dark_host || !theta_host || !out_host)
         return set_error(TCP_EINVAL, "NULL argument");
-    if (nz_total < 1) return set_error(TCP_EINVAL, "nz_total=%d must be >= 1", nz_total);
+    if (nz_stack < 1) return set_error(TCP_EINVAL, "nz_total=%d must be >= 1", nz_stack);
+    if (z_begin < 0 || z_end > nz_stack || z_begin >= z_end)
+        return set_error(TCP_EINVAL, "rows [%d, %d) must be a non-empty range inside [0, %d)", z_begin, z_end, nz_stack);
     if (nbuf != 2 && nbuf != 3) return set_error(TCP_EINVAL, "nbuf=%d must be 2 or 3", nbuf);
     int rc;
     if ((rc = pipe_create(c, nbuf))) return rc;
     Pipe* p = c->pipe;
     const int n = c->ndet, nz = c->nz;
     const size_t ob = c->half_out ? 2 : 4;
+    const int nz_total = z_end - z_begin;                  // slices of this call; the arrays hold nz_stack
     const int nchunks = (nz_total + nz - 1) / nz;
 
     TCP_CUDA_CHECK(cudaEventRecord(p->ev_start, p->s_h2d));
     TCP_CUDA_CHECK(cudaMemcpyAsync(p->theta, theta_host, (size_t)c->nproj * 4, cudaMemcpyHostToDevice, p->s_h2d));
     for (int ch = 0; ch < nchunks; ++ch) {
         const int b = ch % nbuf;
-        const int z0 = ch * nz;
-        const int nzc = (nz_total - z0 < nz) ? nz_total - z0 : nz;
+        const int z0 = z_begin + ch * nz;
+        const int nzc = (z_end - z0 < nz) ? z_end - z0 : nz;
         // H2D: raw[b] is free once the compute of chunk ch - nbuf has finished
         if (ch >= nbuf) TCP_CUDA_CHECK(cudaStreamWaitEvent(p->s_h2d, p->ev_comp[b], 0));
-        // strided gather of rows z0..z0+nzc of every projection: one 2D copy
-        TCP_CUDA_CHECK(cudaMemcpy2DAsync(p->raw[b], (size_t)nz * n * 2, raw_host + (size_t)z0 * n,
-                                         (size_t)nz_total * n * 2, (size_t)nzc * n * 2, c->nproj,
+        // strided gather of rows z0..z0+nzc of every projection: one 2D copy.  A partial last chunk is laid out and
+        // reconstructed as a chunk of nzc slices (device array [nproj][nzc][n]): its result does not depend on what
+        // an earlier chunk left in the buffers, and an odd last slice is paired with zeros
+        TCP_CUDA_CHECK(cudaMemcpy2DAsync(p->raw[b], (size_t)nzc * n * 2, raw_host + (size_t)z0 * n,
+                                         (size_t)nz_stack * n * 2, (size_t)nzc * n * 2, c->nproj,
                                          cudaMemcpyHostToDevice, p->s_h2d));
         TCP_CUDA_CHECK(cudaMemcpyAsync(p->flat[b], flat_host + (size_t)z0 * n, (size_t)nzc * n * 4,
                                        cudaMemcpyHostToDevice, p->s_h2d));
@@ -107,7 +128,16 @@ extern "C" int tcp_recon_volume_host(tcp_ctx* c, const uint16_t* raw_host, const
         // compute: needs the inputs, and out[b] drained by the D2H of chunk ch - nbuf
         TCP_CUDA_CHECK(cudaStreamWaitEvent(p->s_comp, p->ev_h2d[b], 0));
         if (ch >= nbuf) TCP_CUDA_CHECK(cudaStreamWaitEvent(p->s_comp, p->ev_d2h[b], 0));
-        if ((rc = tcp_recon(c, p->raw[b], p->flat[b], p->dark[b], p->theta, p->out[b], p->s_comp))) return rc;
+        if (nzc == nz) {
+            rc = tcp_recon(c, p->raw[b], p->flat[b], p->dark[b], p->theta, p->out[b], p->s_comp);
+        } else {
+            tcp_ctx part = *c;                 // same workspaces and tables, fewer slices (as tcp_recon_try does)
+            part.nz = nzc;
+            part.npair = (nzc + 1) / 2;
+            part.profile = false;
+            rc = tcp_recon(&part, p->raw[b], p->flat[b], p->dark[b], p->theta, p->out[b], p->s_comp);
+        }
+        if (rc) return rc;
         TCP_CUDA_CHECK(cudaEventRecord(p->ev_comp[b], p->s_comp));
         // D2H
         TCP_CUDA_CHECK(cudaStreamWaitEvent(p->s_d2h, p->ev_comp[b], 0));

@@ -67,3 +67,17 @@ def test_stage_model_matches_survey_bytes_per_voxel():
     assert per_voxel == pytest.approx(40.0, rel=1e-12)
     flops = sum(v["flops"] for v in model.values()) / (16 * 2048 * 2048)
     assert 600 < flops < 660      # ~620 flop/voxel at m = 4
+
+
+def test_slice_range_host_logic():
+    """tcp_slice_range: contiguous, in rank order, sizes differ by at most one, empty ranges when world > nz_total."""
+    import paper_2209_08450_b200 as tcp
+    for nz, world in [(2048, 1), (2048, 8), (2049, 8), (10, 3), (3, 8), (0, 2)]:
+        rs = [tcp.tcp_slice_range(nz, r, world) for r in range(world)]
+        assert rs[0][0] == 0 and rs[-1][1] == nz
+        assert all(rs[i][1] == rs[i + 1][0] for i in range(world - 1))
+        sizes = [b - a for a, b in rs]
+        assert max(sizes) - min(sizes) <= 1 and sizes == sorted(sizes, reverse=True)
+    for bad in [(10, 2, 2), (10, -1, 2), (10, 0, 0), (-1, 0, 1)]:
+        with pytest.raises(tcp.TcpError):
+            tcp.tcp_slice_range(*bad)

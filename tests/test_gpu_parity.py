@@ -413,6 +413,12 @@ def test_pipeline_host_matches_direct():
     for z in range(2):
         assert rl2(out_h[20 + z], ref[z]) < FP32_GATE
     r.close()
+    # the partial last chunk runs as a chunk of its own size: equal to a 2-slice context, bit for bit
+    r2 = tcp.Recon(w.n, w.nproj, 2, w.center, "f32", w.filter)
+    d = r2.recon(*_to_dev(np.ascontiguousarray(raw[:, 20:22]), flat[20:22], dark[20:22], theta))
+    torch.cuda.synchronize()
+    assert np.array_equal(out_h[20:22], d.cpu().numpy())
+    r2.close()
 
 
 # ------------------------------------------------------------------ unequally spaced angles
@@ -608,6 +614,38 @@ def test_detector_width_variants_pipeline_try_line_and_errors():
     for bad in [(7, 10, 2, 3.0), (4097, 10, 2, 50.0), (100, 10, 2, 99.5), (100, 10, 2, -1.0), (100, 0, 2, 50.0)]:
         with pytest.raises(tcp.TcpError):
             tcp.tcp_create_det(bad[0], bad[1], bad[2], bad[3], "f32", "ramp", 0)
+
+
+def test_pipeline_slice_ranges_equal_the_whole_volume():
+    """tcp_recon_volume_host_rows ("--start-row/--end-row"; the multi-GPU recipe of PAPER.md:145-149):
+    three "ranks" (one after the other on this GPU, each with its own context; nothing waits on anything) reconstruct
+    their tcp_slice_range of shared full-stack host arrays; the union equals the one-call volume bit for bit, rows
+    outside a rank's range are left untouched, bad ranges are refused."""
+    tcp = _tcp()
+    w = sg.make_workload("C2", scale=4)
+    nzt = 23
+    raw, flat, dark, theta = _inputs(w, list(range(nzt)))
+    raw_h = torch.from_numpy(raw.view(np.int16)).view(torch.uint16).pin_memory()
+    flat_h, dark_h, th_h = torch.from_numpy(flat).pin_memory(), torch.from_numpy(dark).pin_memory(), torch.from_numpy(theta).pin_memory()
+    r = tcp.Recon(w.n, w.nproj, 4, w.center, "f16", w.filter)
+    whole, _ = r.recon_volume_host(raw_h, flat_h, dark_h, th_h, nbuf=3)
+    whole = whole.clone()
+    r.close()
+    out = torch.full((nzt, w.n, w.n), -7.0, dtype=torch.float16).pin_memory()
+    world = 3
+    for rank in range(world):
+        z0, z1 = tcp.tcp_slice_range(nzt, rank, world)
+        rr = tcp.Recon(w.n, w.nproj, 4, w.center, "f16", w.filter)
+        before = out.clone()
+        rr.recon_volume_host(raw_h, flat_h, dark_h, th_h, out_host=out, nbuf=2, rows=(z0, z1))
+        assert torch.equal(out[:z0], before[:z0]) and torch.equal(out[z1:], before[z1:])
+        rr.close()
+    assert torch.equal(out, whole)
+    r = tcp.Recon(w.n, w.nproj, 4, w.center, "f16", w.filter)
+    for bad in [(5, 5), (-1, 3), (20, 24), (7, 3)]:
+        with pytest.raises(tcp.TcpError):
+            r.recon_volume_host(raw_h, flat_h, dark_h, th_h, out_host=out, rows=bad)
+    r.close()
 
 
 # ------------------------------------------------------------------ BASELINE full sizes, bench launch configuration
