@@ -89,9 +89,10 @@ KERNEL_NAMES = {"normalize": "normalize_half_kernel / normalize_kernel", "rows":
                 "ifft_rows": "ifft_rows_kernel"}
 
 
-def stage_model(w, nz, m, half_store, half_out):
+def stage_model(w, nz, m, half_store, half_out, fused_s12=False):
     """Algorithmic HBM bytes and flops of one tcp_recon call (one chunk of nz slices), per kernel
-    (SURVEY 8(d))."""
+    (SURVEY 8(d)).  fused_s12: S1+S2 run in the row kernel's loader
+    (TCP_OPT_FUSE_NORMALIZE): no normalise kernel, the row kernel reads the uint16 counts."""
     n, M, P = w.n, 2 * w.n, w.nproj
     npair = (nz + 1) // 2
     br = 2 if half_store else 4
@@ -99,6 +100,13 @@ def stage_model(w, nz, m, half_store, half_out):
     bo = 2 if half_out else 4
     lg = np.log2(M)
     fft = 5.0 * M * lg                      # flops of one length-M complex transform
+    if fused_s12:
+        return {
+            "rows": {"bytes": P * nz * n * 2 + npair * P * M * bc, "flops": 3 * fft * npair * P + 10.0 * P * nz * n},
+            "grid": {"bytes": npair * P * M * bc + npair * M * M * bc, "flops": 4.0 * (2 * m) ** 2 * npair * P * M},
+            "ifft_cols": {"bytes": npair * M * M * bc + npair * n * M * bc, "flops": fft * npair * M},
+            "ifft_rows": {"bytes": npair * n * M * bc + nz * n * n * bo, "flops": fft * npair * n},
+        }
     return {
         "normalize": {"bytes": P * nz * n * (2 + br), "flops": 10.0 * P * nz * n},
         "rows": {"bytes": P * nz * n * br + npair * P * M * bc, "flops": 3 * fft * npair * P},
@@ -296,7 +304,8 @@ def run_ours(args, rank, world, local_rank):
         return
     # ---- roofline of the dominant kernel
     hbm_gbs, sm_max_mhz, which = _peaks()
-    model = stage_model(w, nzc, m, half_store, half_out)
+    fused_s12 = half_store and not args.fused_filter and args.algorithm == "fourier"      # tcp.h: TCP_OPT_FUSE_NORMALIZE
+    model = stage_model(w, nzc, m, half_store, half_out, fused_s12)
     alu_peak = 148 * 128 * 2 * sm_max_mhz * 1e6 / 1e12        # fp32 FMA lanes x 2 flop x clock, TFLOP/s
     kernels = {}
     for k in model:
@@ -335,7 +344,10 @@ def run_ours(args, rank, world, local_rank):
     else:
         roof = {"kernel": KERNEL_NAMES.get(dom, dom), "bound": "hbm", "achieved": kernels[dom]["GBps"], "peak": hbm_gbs, "unit": "GB/s",
                 "frac": kernels[dom]["GBps"] / hbm_gbs, "traffic": traffic, "peak_source": "MEASURED_PEAKS.json (%s)" % which}
-    whole_bytes = sum(v["bytes"] for v in model.values()) * nchunks
+    # whole path: SURVEY 8(d)'s algorithmic figure of the method (40 B/voxel at C4), whether or not a stage is fused away
+    whole_bytes = sum(v["bytes"] for v in stage_model(w, nzc, m, half_store, half_out).values()) * nchunks
+    if fused_s12:
+        kernels["normalize"] = "fused into rows_kernel's loader (TCP_OPT_FUSE_NORMALIZE)"
     line = {
         "metric": "reconstructed GVoxel/s", "value": value, "unit": "GVoxel/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",

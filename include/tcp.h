@@ -80,8 +80,12 @@ enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1, TCP_GRID_TILE = 2, TCP_
  * (theta[j+1] - theta[j-1]) / 2, where theta[nproj] = theta[0] + pi and theta[-1] = theta[nproj-1] - pi (trapezoid
  * rule on the periodic angle axis; the angles must cover the half turn), computed on the device from the angles of
  * each call.  All algorithms and tcp_recon_try. */
+/* TCP_OPT_FUSE_NORMALIZE (1 default | 0): with fp16 storage tcp_recon runs S1+S2 inside the loader of the detector-row
+ * kernel instead of as a kernel of their own (the sinogram then never goes to HBM and TCP_WS_SINOGRAM is NOT updated by
+ * tcp_recon; tcp_normalize still fills it).  Same results bit for bit.  Applies to FourierRec's default chain on
+ * contexts whose detector width is the transform's; everywhere else the option is ignored. */
 enum { TCP_OPT_GRID_IMPL = 0, TCP_OPT_PROFILE = 1, TCP_OPT_TCFFT = 2, TCP_OPT_ALGORITHM = 3, TCP_OPT_PAD = 4,
-       TCP_OPT_FILTER_FUSED = 5, TCP_OPT_WEIGHT_CACHE = 6, TCP_OPT_ANGLE_WEIGHTS = 7 };
+       TCP_OPT_FILTER_FUSED = 5, TCP_OPT_WEIGHT_CACHE = 6, TCP_OPT_ANGLE_WEIGHTS = 7, TCP_OPT_FUSE_NORMALIZE = 8 };
 enum { TCP_PAD_ZERO = 0, TCP_PAD_EDGE = 1 };
 enum { TCP_ALG_FOURIER = 0, TCP_ALG_LINE = 1 };
 enum { TCP_TCFFT_ROWS = 1, TCP_TCFFT_COLS = 2, TCP_TCFFT_IROWS = 4 };

@@ -221,6 +221,10 @@ class Recon:
         """TCP_OPT_WEIGHT_CACHE: reuse the gridding weights across calls with the same angles (default on)."""
         _check(lib().tcp_set_option(self.h, 6, 1 if on else 0))
 
+    def set_fuse_normalize(self, on: bool):
+        """TCP_OPT_FUSE_NORMALIZE: S1+S2 inside the row kernel's loader (fp16 storage; default on; same bits)."""
+        _check(lib().tcp_set_option(self.h, 8, 1 if on else 0))
+
     def set_angle_weights(self, on: bool):
         """TCP_OPT_ANGLE_WEIGHTS: trapezoid quadrature weights for unequally spaced angles (off by default)."""
         _check(lib().tcp_set_option(self.h, 7, 1 if on else 0))

@@ -61,10 +61,7 @@ __global__ void __launch_bounds__(256) normalize_kernel(const uint4* __restrict_
 // (rcp.approx, lg2.approx: ~2^-22) are exact for the purpose and the kernel stays HBM-bound instead of
 // ALU-bound.  A thread keeps 1 / (flat - dark) and dark of its 8 pixels in registers and walks JP
 // projections of the same detector row, so the flat/dark loads and the reciprocals are amortised.
-__device__ __forceinline__ float fast_rcp(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-__device__ __forceinline__ float fast_lg2(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-// uint16 -> float without the conversion pipe: 0x4B000000 | u is 2^23 + u exactly
-__device__ __forceinline__ float u16f(unsigned u) { return __uint_as_float(0x4B000000u | u) - 8388608.f; }
+// fast_rcp, fast_lg2, u16f: tcp_internal.h (shared with the fused loader of rows_kernel)
 
 constexpr int JP = 4;
 __global__ void __launch_bounds__(256) normalize_half_kernel(const uint4* __restrict__ raw, const float4* __restrict__ flat,
@@ -208,7 +205,14 @@ int launch_mean_frames(const uint16_t* frames, int nframes, int nz, int n, float
 // cos/sin of the float32 angles in fp64: k*cos(theta) with
 // k up to 4096 must be good to ~1e-6 grid cells for the 1e-5 fp32 gate.
 __global__ void trig_kernel(const float* __restrict__ theta, int nproj, double2* __restrict__ trig, float4* __restrict__ trigf,
-                            int* __restrict__ wstate, float* __restrict__ wq) {
+                            int* __restrict__ wstate, float* __restrict__ wq, const float* __restrict__ flat,
+                            const float* __restrict__ dark, float2* __restrict__ fdtab, int nfd) {
+    // fused S1+S2 (rows_kernel's loader): per detector pixel of the chunk the reciprocal normalize_half_kernel forms, and dark
+    if (flat)
+        for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nfd; i += gridDim.x * blockDim.x) {
+            const float dk = dark[i];
+            fdtab[i] = make_float2(fast_rcp(fmaxf(flat[i] - dk, 1e-3f)), dk);
+        }
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j < nproj) {
         // quadrature weight for unequally spaced angles (TCP_OPT_ANGLE_WEIGHTS, reading Q20):
@@ -232,8 +236,10 @@ __global__ void trig_kernel(const float* __restrict__ theta, int nproj, double2*
     }
 }
 
-int launch_trig(const tcp_ctx* c, const float* theta, cudaStream_t st) {
-    trig_kernel<<<(c->nproj + 127) / 128, 128, 0, st>>>(theta, c->nproj, c->trig, c->trigf, c->w_state, c->wq);
+int launch_trig(const tcp_ctx* c, const float* theta, cudaStream_t st, const float* flat, const float* dark) {
+    const int nfd = c->nz * c->n;
+    const int blocks = flat ? std::max((c->nproj + 127) / 128, std::min((nfd + 127) / 128, 148 * 4)) : (c->nproj + 127) / 128;
+    trig_kernel<<<blocks, 128, 0, st>>>(theta, c->nproj, c->trig, c->trigf, c->w_state, c->wq, flat, dark, c->fdtab, nfd);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }

@@ -9,12 +9,17 @@
 
 namespace tcpk {
 
-template <int M, int ROWS, bool PAD_EDGE, class TS, class TC>
+// RAW: the two rows come straight from the uint16 projections raw[nproj][nz][n] with fdtab[nz][n] = (1 / max(flat - dark,
+// eps_d), dark) of this call (trig_kernel): S1+S2 run in the
+// loader with the arithmetic of normalize_half_kernel (same half value bit for bit, rounded to the storage type before
+// use), so the sinogram never goes to HBM and back (TCP_OPT_FUSE_NORMALIZE; fp16 storage only).
+template <int M, int ROWS, bool PAD_EDGE, bool RAW, class TS, class TC>
 __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict__ sino, TC* __restrict__ spec,
                                                             const float2* __restrict__ tw,
                                                             const float* __restrict__ hfilt,
                                                             const float2* __restrict__ ptab, int nproj, int nz, int try_mode,
-                                                            const float* __restrict__ wq) {
+                                                            const float* __restrict__ wq, const uint16_t* __restrict__ raw,
+                                                            const float2* __restrict__ fdtab) {
     constexpr bool pad_edge = PAD_EDGE;
     constexpr int n = M / 2;
     constexpr int TG = M / 16;
@@ -35,13 +40,20 @@ __global__ void __launch_bounds__(ROWS* M / 16) rows_kernel(const TS* __restrict
     if (try_mode) ptab += (size_t)pair * M;
     const float wj = wq ? __ldg(&wq[j]) : 1.f;      // TCP_OPT_ANGLE_WEIGHTS: everything after S2 is linear in the projection
 
+    const int zBs = hasB ? zB : zA;
+    auto neglog_raw = [&](int z, int i) {
+        const float2 fd = __ldg(&fdtab[(size_t)z * n + i]);
+        const float p = -0.69314718055994531f * fast_lg2(fmaxf((u16f(__ldg(&raw[((size_t)j * nz + z) * n + i])) - fd.y) * fd.x, 1e-6f));
+        return __half2float(__float2half_rn(p));
+    };
     auto load_padded = [&](int i) {
         // padding samples: zeros, or (TCP_OPT_PAD = TCP_PAD_EDGE) the nearest edge of the periodic row
         if (i >= n) {
             if (!pad_edge) return make_float2(0.f, 0.f);
             i = (i < n + n / 2) ? n - 1 : 0;
         }
-        return make_float2(ld_r(pA, i) * wj, hasB ? ld_r(pB, i) * wj : 0.f);
+        if constexpr (RAW) return make_float2(neglog_raw(zA, i) * wj, hasB ? neglog_raw(zBs, i) * wj : 0.f);
+        else return make_float2(ld_r(pA, i) * wj, hasB ? ld_r(pB, i) * wj : 0.f);
     };
     TC* out = spec + ((size_t)pair * nproj + j) * M;
     // the three transforms hand their lines over in registers (fft_chain_slot: same elements, permuted slots):
@@ -177,7 +189,7 @@ int launch_filter(const tcp_ctx* c, cudaStream_t st) {
 }
 
 template <int M, class TS, class TC>
-static int launch_rows_t(const tcp_ctx* c, cudaStream_t st) {
+static int launch_rows_t(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw, const float* flat, const float* dark) {
     constexpr int TG = M / 16;
     constexpr int ROWS = (TG >= 128) ? 1 : 128 / TG;
     const size_t smem = (size_t)ROWS * padded_len(M) * sizeof(float2);
@@ -189,29 +201,39 @@ static int launch_rows_t(const tcp_ctx* c, cudaStream_t st) {
         TCP_CUDA_CHECK(cudaGetLastError());
         return TCP_OK;
     }
-    auto kern = c->pad ? rows_kernel<M, ROWS, true, TS, TC> : rows_kernel<M, ROWS, false, TS, TC>;
+    auto kern = c->pad ? rows_kernel<M, ROWS, true, false, TS, TC> : rows_kernel<M, ROWS, false, false, TS, TC>;
+    if constexpr (std::is_same_v<TS, __half>) {
+        if (raw) kern = c->pad ? rows_kernel<M, ROWS, true, true, TS, TC> : rows_kernel<M, ROWS, false, true, TS, TC>;
+    }
     TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid((c->nproj + ROWS - 1) / ROWS, c->npair);
     kern<<<grid, ROWS * TG, smem, st>>>((const TS*)c->sino, (TC*)c->spec, c->tw, c->hfilt, c->try_ptab ? c->try_ptab : c->ptab, c->nproj, c->nz,
-                                       c->try_ptab ? 1 : 0, c->angle_weights ? c->wq : nullptr);
+                                       c->try_ptab ? 1 : 0, c->angle_weights ? c->wq : nullptr, raw, c->fdtab);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }
 
 template <int M>
-static int launch_rows_m(const tcp_ctx* c, cudaStream_t st) {
-    return c->half_store ? launch_rows_t<M, __half, __half2>(c, st) : launch_rows_t<M, float, float2>(c, st);
+static int launch_rows_m(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw, const float* flat, const float* dark) {
+    return c->half_store ? launch_rows_t<M, __half, __half2>(c, st, raw, flat, dark) : launch_rows_t<M, float, float2>(c, st, nullptr, nullptr, nullptr);
 }
 
-int launch_rows(const tcp_ctx* c, cudaStream_t st) {
+// S1+S2 can ride the loader of rows_kernel: fp16 storage (the fused value is the stored half, bit for bit), the default
+// chain (not the uncropped-filter option, not the try mode), the caller's rows as wide as the transform's
+bool rows_fuses_normalize(const tcp_ctx* c) {
+    return c->fuse_norm && c->half_store && c->algorithm == TCP_ALG_FOURIER && !c->filter_fused && !c->try_ptab && c->ndet == c->n;
+}
+
+int launch_rows(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw, const float* flat, const float* dark) {
+    if (raw && !rows_fuses_normalize(c)) return set_error(TCP_EINVAL, "fused S1+S2 not available on this context");
     switch (c->M) {
-        case 128: return launch_rows_m<128>(c, st);
-        case 256: return launch_rows_m<256>(c, st);
-        case 512: return launch_rows_m<512>(c, st);
-        case 1024: return launch_rows_m<1024>(c, st);
-        case 2048: return launch_rows_m<2048>(c, st);
-        case 4096: return launch_rows_m<4096>(c, st);
-        case 8192: return launch_rows_m<8192>(c, st);
+        case 128: return launch_rows_m<128>(c, st, raw, flat, dark);
+        case 256: return launch_rows_m<256>(c, st, raw, flat, dark);
+        case 512: return launch_rows_m<512>(c, st, raw, flat, dark);
+        case 1024: return launch_rows_m<1024>(c, st, raw, flat, dark);
+        case 2048: return launch_rows_m<2048>(c, st, raw, flat, dark);
+        case 4096: return launch_rows_m<4096>(c, st, raw, flat, dark);
+        case 8192: return launch_rows_m<8192>(c, st, raw, flat, dark);
     }
     return set_error(TCP_EUNSUPPORTED, "unsupported M=%d", c->M);
 }

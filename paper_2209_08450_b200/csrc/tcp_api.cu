@@ -87,6 +87,7 @@ static int build_context(tcp_ctx* c) {
     if ((rc = dev_alloc((void**)&c->trig, (size_t)c->nproj * sizeof(double2), &c->bytes))) return rc;
     if ((rc = dev_alloc((void**)&c->trigf, (size_t)c->nproj * sizeof(float4), &c->bytes))) return rc;
     if ((rc = dev_alloc((void**)&c->wq, (size_t)c->nproj * sizeof(float), &c->bytes))) return rc;
+    if (c->half_store && (rc = dev_alloc((void**)&c->fdtab, (size_t)c->nz * n * sizeof(float2), &c->bytes))) return rc;
 
     std::vector<float2> tw(M);
     for (int t = 0; t < M; ++t) {
@@ -202,6 +203,7 @@ static tcp_ctx* create_impl(int n, int ndet, int pad_l, int nproj, int nz_chunk,
     c->n = n; c->M = 2 * n; c->nproj = nproj; c->nz = nz_chunk; c->npair = (nz_chunk + 1) / 2;
     c->dtype = dtype; c->filter = filter; c->m = m; c->center = center;
     c->ndet = ndet; c->pad_l = pad_l;
+    c->fuse_norm = 1;
     c->half_store = dtype != TCP_F32;
     c->half_out = dtype == TCP_F16;
     // fp16 storage: S = 2^13 puts |f| Phi^2 S <= 65504 for |f| < 1.9 per pixel while keeping
@@ -253,7 +255,7 @@ void tcp_destroy(tcp_ctx* c) {
         for (int i = 0; i < kProfileRing * (TCP_NSTAGES + 1); ++i) cudaEventDestroy(c->pev[i]);
         free(c->pev);
     }
-    cudaFree(c->sino); cudaFree(c->spec); cudaFree(c->grid); cudaFree(c->pass1); cudaFree(c->trig); cudaFree(c->trigf); cudaFree(c->wq);
+    cudaFree(c->sino); cudaFree(c->spec); cudaFree(c->grid); cudaFree(c->pass1); cudaFree(c->trig); cudaFree(c->trigf); cudaFree(c->wq); cudaFree(c->fdtab);
     cudaFree(c->tw); cudaFree(c->hfilt); cudaFree(c->ptab); cudaFree(c->ftab); cudaFree(c->deax); cudaFree(c->deay);
     cudaFree(c->tile_order);
     cudaFree(c->try_buf);
@@ -283,9 +285,10 @@ int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* d
     }
 #define TCP_MARK(i) do { if (ev) TCP_CUDA_CHECK(cudaEventRecord(ev[i], st)); } while (0)
     TCP_MARK(0);
-    if ((rc = launch_trig(c, theta, st))) return rc;
+    const bool fused_s12 = rows_fuses_normalize(c);       // S1+S2 in the loader of rows_kernel: no sinogram round trip
+    if ((rc = fused_s12 ? launch_trig(c, theta, st, flat, dark) : launch_trig(c, theta, st))) return rc;
     TCP_MARK(1);
-    if ((rc = launch_normalize(c, raw, flat, dark, st))) return rc;
+    if (!fused_s12 && (rc = launch_normalize(c, raw, flat, dark, st))) return rc;
     TCP_MARK(2);
     if (c->algorithm == TCP_ALG_LINE) {       // LineRec: filter (timed as "rows"), backprojection (timed as "grid")
         if ((rc = launch_filter(c, st))) return rc;
@@ -297,7 +300,7 @@ int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* d
         TCP_MARK(6);
         return TCP_OK;
     }
-    if ((rc = launch_rows(c, st))) return rc;
+    if ((rc = fused_s12 ? launch_rows(c, st, raw, flat, dark) : launch_rows(c, st))) return rc;
     TCP_MARK(3);
     if (c->grid_impl == TCP_GRID_SCATTER_ATOMIC) rc = launch_grid_scatter(c, st);
     else if (c->grid_impl == TCP_GRID_GATHER) rc = launch_grid_gather(c, theta, st);
@@ -380,7 +383,7 @@ int tcp_profile_collect(tcp_ctx* c, double* ms_sum, int* ncalls) {
 
 int tcp_launches_per_recon(const tcp_ctx* c) {
     if (!c) return 0;
-    const int crop = c->out_pad ? 1 : 0;                                 // tcp_create_det: + the cut-out copy
+    const int crop = (c->out_pad ? 1 : 0) - (rows_fuses_normalize(c) ? 1 : 0);   // tcp_create_det: + the cut-out copy; fused S1+S2: - normalise
     if (c->algorithm == TCP_ALG_LINE) return 4 + crop;                   // trig, normalise, filter, backprojection
     if (c->grid_impl == TCP_GRID_MMA)       // + plan, cache decide (+ count, scan, fill, cached kernel: most exit at once) (+ reduce)
         return 8 + (c->w_cap > 0 ? 4 : 0) + (c->g_nred ? 1 : 0) + crop;
@@ -432,6 +435,10 @@ int tcp_set_option(tcp_ctx* c, int option, int value) {
     }
     if (option == TCP_OPT_WEIGHT_CACHE) {
         c->w_enable = value != 0;
+        return TCP_OK;
+    }
+    if (option == TCP_OPT_FUSE_NORMALIZE) {
+        c->fuse_norm = value != 0;
         return TCP_OK;
     }
     if (option == TCP_OPT_ANGLE_WEIGHTS) {

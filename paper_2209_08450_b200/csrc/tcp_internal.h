@@ -32,6 +32,8 @@ struct tcp_ctx {
     double2* trig;        // [nproj] (cos, sin) of theta, fp64
     float4* trigf;        // [nproj] (cos hi, cos lo, sin hi, sin lo): float-float split of trig
     float* wq;            // [nproj] quadrature weight of every projection relative to pi/nproj (trig_kernel, every call)
+    float2* fdtab;        // [nz][n] (1 / max(flat - dark, eps_d), dark) of the call, written by trig_kernel for the fused S1+S2 loader
+    int fuse_norm;        // TCP_OPT_FUSE_NORMALIZE: S1+S2 in the loader of rows_kernel where that applies (fp16 storage)
     int angle_weights;    // TCP_OPT_ANGLE_WEIGHTS: the row kernels scale projection j by wq[j] (unequally spaced angles)
     // tables (device), built in fp64 on the host at create
     float2* tw;           // [M] e^{-2 pi i t / M}
@@ -76,10 +78,14 @@ int set_error(int code, const char* fmt, ...);
     } while (0)
 
 // kernel launchers: each enqueues on `st` and returns TCP_OK or an error code
-int launch_trig(const tcp_ctx* c, const float* theta, cudaStream_t st);
+// flat != NULL: also fill c->fdtab from the call's flat / dark (fused S1+S2 loader of rows_kernel)
+int launch_trig(const tcp_ctx* c, const float* theta, cudaStream_t st, const float* flat = nullptr, const float* dark = nullptr);
 int launch_normalize(const tcp_ctx* c, const uint16_t* raw, const float* flat, const float* dark,
                      cudaStream_t st);
-int launch_rows(const tcp_ctx* c, cudaStream_t st);
+// raw != NULL: S1+S2 fused into the loader (rows_fuses_normalize(c) must hold); else the sinogram workspace is read
+int launch_rows(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw = nullptr, const float* flat = nullptr,
+                const float* dark = nullptr);
+bool rows_fuses_normalize(const tcp_ctx* c);
 int launch_filter(const tcp_ctx* c, cudaStream_t st);
 int launch_line_bp(const tcp_ctx* c, void* out, cudaStream_t st);
 int launch_grid_scatter(const tcp_ctx* c, cudaStream_t st);
@@ -108,5 +114,12 @@ __device__ __forceinline__ float ld_r(const float* p, size_t i) { return p[i]; }
 __device__ __forceinline__ float ld_r(const __half* p, size_t i) { return __half2float(p[i]); }
 __device__ __forceinline__ void st_r(float* p, size_t i, float v) { p[i] = v; }
 __device__ __forceinline__ void st_r(__half* p, size_t i, float v) { p[i] = __float2half_rn(v); }
+
+// S1+S2 for fp16 storage (normalize_half_kernel and the fused loader of rows_kernel share these, so both give the
+// same half value bit for bit): hardware approximations (~2^-22) under a rounding to 2^-11
+__device__ __forceinline__ float fast_rcp(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float fast_lg2(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+// uint16 -> float without the conversion pipe: 0x4B000000 | u is 2^23 + u exactly
+__device__ __forceinline__ float u16f(unsigned u) { return __uint_as_float(0x4B000000u | u) - 8388608.f; }
 
 }  // namespace tcpk

@@ -421,6 +421,40 @@ def test_pipeline_host_matches_direct():
     r2.close()
 
 
+# ------------------------------------------------------------------ S1+S2 fused into the row kernel's loader
+@pytest.mark.parametrize("dtype,nz,pad", [("f16", 8, "zero"), ("f16", 5, "edge"), ("f16_out32", 18, "zero")])
+def test_fused_normalize_is_bit_identical(dtype, nz, pad):
+    """TCP_OPT_FUSE_NORMALIZE (default on with fp16 storage): S1+S2 inside rows_kernel's loader give the same bits as
+    the separate normalise kernel + sinogram round trip (also on an odd chunk, with edge padding, with the angle
+    weights), one launch fewer; tcp_normalize still fills the sinogram workspace."""
+    tcp = _tcp()
+    w = sg.make_workload("C2", scale=4)
+    rows = list(range(30, 30 + nz))
+    raw, flat, dark, theta = _inputs(w, rows)
+    dev = _to_dev(raw, flat, dark, theta)
+    r = tcp.Recon(w.n, w.nproj, nz, w.center, dtype, w.filter, 3)
+    r.set_pad(pad)
+    n_fused = r.launches_per_recon
+    a = r.recon(*dev).clone()
+    r.set_angle_weights(True)
+    aw = r.recon(*dev).clone()
+    r.set_fuse_normalize(False)
+    assert r.launches_per_recon == n_fused + 1
+    bw = r.recon(*dev).clone()
+    r.set_angle_weights(False)
+    b = r.recon(*dev).clone()
+    torch.cuda.synchronize()
+    assert torch.equal(a, b) and torch.equal(aw, bw)
+    sino = r.normalize(dev[0], dev[1], dev[2]).float().cpu().numpy()
+    p = orc.neglog(raw, flat, dark)
+    assert np.abs(sino - p).max() < 2e-3 * max(1.0, np.abs(p).max())
+    r.close()
+    ref = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, "grid", pad=pad)
+    out = a.float().cpu().numpy()
+    for z in range(nz):
+        assert rl2(out[z], ref[z]) < FP16_GATE_L2
+
+
 # ------------------------------------------------------------------ unequally spaced angles (PAPER.md:61)
 @pytest.mark.parametrize("dtype,alg", [("f32", "fourier"), ("f16", "fourier"), ("f32", "line")])
 def test_angle_weights_for_unequally_spaced_angles(dtype, alg):
