@@ -204,6 +204,10 @@ int tcp_recon_volume_host(tcp_ctx* ctx, const uint16_t* raw_host, const float* f
 int tcp_recon_volume_host_rows(tcp_ctx* ctx, const uint16_t* raw_host, const float* flat_host,
                                const float* dark_host, const float* theta_host, void* out_host,
                                int nz_stack, int z_begin, int z_end, int nbuf, float* ms_out);
+/* HOST logic only (no CUDA call): TCP_OK if theta_host[nproj] is what tcp_recon accepts (finite, strictly increasing,
+ * last - first < pi), else TCP_EINVAL with the offending index in tcp_last_error().  tcp_recon cannot check its DEVICE
+ * angles without a synchronisation and does not; tcp_recon_volume_host[_rows] check their HOST angles with this. */
+int tcp_check_angles(const float* theta_host, int nproj);
 /* HOST logic only (no CUDA call): the contiguous slice range [*z0, *z1) of process `rank` of `world` over
  * nz_total slices; the ranges tile [0, nz_total) in rank order and differ by at most one slice (a rank may get
  * an empty range when world > nz_total).  TCP_EINVAL on a bad argument. */

@@ -21,6 +21,7 @@ from .binding import (  # noqa: F401
     tcp_recon_volume_host,
     tcp_recon_volume_host_rows,
     tcp_slice_range,
+    tcp_check_angles,
     tcp_last_error,
     DTYPES,
     FILTERS,

@@ -21,7 +21,7 @@ EXPORTS = [
     "tcp_mean_frames_u16", "tcp_normalize", "tcp_workspace", "tcp_read_workspace", "tcp_scale", "tcp_grid_strip",
     "tcp_workspace_bytes", "tcp_launches_per_recon", "tcp_set_option", "tcp_profile_collect",
     "tcp_recon_volume_host", "tcp_recon_try", "tcp_create_det", "tcp_padded_n",
-    "tcp_recon_volume_host_rows", "tcp_slice_range",
+    "tcp_recon_volume_host_rows", "tcp_slice_range", "tcp_check_angles",
 ]
 
 
@@ -83,6 +83,8 @@ def lib():
     L.tcp_recon_volume_host.argtypes = [vp, vp, vp, vp, vp, vp, ci, ci, C.POINTER(cf)]
     L.tcp_recon_volume_host_rows.restype = ci
     L.tcp_recon_volume_host_rows.argtypes = [vp, vp, vp, vp, vp, vp, ci, ci, ci, ci, C.POINTER(cf)]
+    L.tcp_check_angles.restype = ci
+    L.tcp_check_angles.argtypes = [vp, ci]
     L.tcp_slice_range.restype = ci
     L.tcp_slice_range.argtypes = [ci, ci, ci, C.POINTER(ci), C.POINTER(ci)]
     L.tcp_recon_try.restype = ci
@@ -176,6 +178,12 @@ def tcp_recon_volume_host_rows(h, raw_host, flat_host, dark_host, theta_host, ou
                                             theta_host.data_ptr(), out_host.data_ptr(), int(nz_stack), int(z_begin),
                                             int(z_end), int(nbuf), C.byref(ms)))
     return float(ms.value)
+
+
+def tcp_check_angles(theta_host):
+    """Raises TcpError unless the HOST float32 tensor / array of angles is finite, strictly increasing and spans < pi."""
+    t = np.ascontiguousarray(theta_host.numpy() if isinstance(theta_host, torch.Tensor) else theta_host, dtype=np.float32)
+    _check(lib().tcp_check_angles(t.ctypes.data_as(C.c_void_p), int(t.size)))
 
 
 def tcp_slice_range(nz_total, rank, world):

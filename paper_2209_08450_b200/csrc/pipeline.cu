@@ -83,6 +83,19 @@ extern "C" int tcp_slice_range(int nz_total, int rank, int world, int* z0, int* 
     return TCP_OK;
 }
 
+// HOST logic: the angles tcp_recon accepts (the projection window of a grid region is an index range of theta)
+extern "C" int tcp_check_angles(const float* theta_host, int nproj) {
+    if (!theta_host || nproj < 1) return set_error(TCP_EINVAL, "bad angle array");
+    for (int j = 0; j < nproj; ++j) {
+        if (!(theta_host[j] == theta_host[j]) || !(theta_host[j] - theta_host[j] == 0.f)) return set_error(TCP_EINVAL, "theta[%d] is not finite", j);
+        if (j > 0 && !(theta_host[j] > theta_host[j - 1]))
+            return set_error(TCP_EINVAL, "theta must be strictly increasing: theta[%d]=%g <= theta[%d]=%g", j, (double)theta_host[j], j - 1, (double)theta_host[j - 1]);
+    }
+    if (!((double)theta_host[nproj - 1] - (double)theta_host[0] < 3.14159265358979323846))
+        return set_error(TCP_EINVAL, "theta spans %g >= pi: fold a full turn onto [0, pi) first", (double)theta_host[nproj - 1] - (double)theta_host[0]);
+    return TCP_OK;
+}
+
 extern "C" int tcp_recon_volume_host(tcp_ctx* c, const uint16_t* raw_host, const float* flat_host,
                                      const float* dark_host, const float* theta_host, void* out_host, int nz_total,
                                      int nbuf, float* ms_out) {
@@ -94,7 +107,9 @@ extern "C" int tcp_recon_volume_host_rows(tcp_ctx* c, const uint16_t* raw_host, 
                                           int z_begin, int z_end, int nbuf, float* ms_out) {
     if (!c || !raw_host || !flat_host || !dark_host || !theta_host || !out_host)
         return set_error(TCP_EINVAL, "NULL argument");
+    int rc0;
     if (nz_stack < 1) return set_error(TCP_EINVAL, "nz_total=%d must be >= 1", nz_stack);
+    if ((rc0 = tcp_check_angles(theta_host, c->nproj))) return rc0;
     if (z_begin < 0 || z_end > nz_stack || z_begin >= z_end)
         return set_error(TCP_EINVAL, "rows [%d, %d) must be a non-empty range inside [0, %d)", z_begin, z_end, nz_stack);
     if (nbuf != 2 && nbuf != 3) return set_error(TCP_EINVAL, "nbuf=%d must be 2 or 3", nbuf);

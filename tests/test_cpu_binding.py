@@ -81,3 +81,15 @@ def test_slice_range_host_logic():
     for bad in [(10, 2, 2), (10, -1, 2), (10, 0, 0), (-1, 0, 1)]:
         with pytest.raises(tcp.TcpError):
             tcp.tcp_slice_range(*bad)
+
+
+def test_check_angles_host_logic():
+    import numpy as np
+    import paper_2209_08450_b200 as tcp
+    tcp.tcp_check_angles(np.linspace(0, np.pi, 180, endpoint=False).astype(np.float32))
+    tcp.tcp_check_angles(np.array([0.3], np.float32))
+    tcp.tcp_check_angles(np.linspace(-1.0, 2.0, 50).astype(np.float32))           # any start, span < pi
+    for bad in (np.linspace(0, 2 * np.pi, 360, endpoint=False), np.array([0.0, 0.2, 0.2, 0.4]), np.array([0.5, 0.4]),
+                np.array([0.0, np.nan, 1.0]), np.array([0.0, np.inf]), np.array([0.0, np.pi])):
+        with pytest.raises(tcp.TcpError):
+            tcp.tcp_check_angles(bad.astype(np.float32))

@@ -679,6 +679,8 @@ def test_pipeline_slice_ranges_equal_the_whole_volume():
     for bad in [(5, 5), (-1, 3), (20, 24), (7, 3)]:
         with pytest.raises(tcp.TcpError):
             r.recon_volume_host(raw_h, flat_h, dark_h, th_h, out_host=out, rows=bad)
+    with pytest.raises(tcp.TcpError):               # angles over a full turn: refused on the host, before any copy
+        r.recon_volume_host(raw_h, flat_h, dark_h, (th_h * 2.0).pin_memory(), out_host=out)
     r.close()
 
 
