@@ -421,6 +421,28 @@ def test_pipeline_host_matches_direct():
     r2.close()
 
 
+# ------------------------------------------------------------------ stored oracle values (tests/golden)
+@pytest.mark.parametrize("m", [3, 4])
+def test_c1_against_stored_oracle_values(m):
+    """The CUDA path against values the oracle wrote to tests/golden/c1_oracle_samples.txt (make_golden.py calls only
+    oracle/): fp32 path, sampled pixels of three C1 slices, within 1e-5 of the volume's scale."""
+    import os
+    stored = {}
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "c1_oracle_samples.txt")) as f:
+        for ln in f:
+            if ln.startswith("#") or not ln.strip():
+                continue
+            method, mm, z, iy, ix, v = ln.split()
+            if method == "grid" and int(mm) == m:
+                stored[(int(z), int(iy), int(ix))] = float(v)
+    assert len(stored) == 24
+    w = sg.make_workload("C1")
+    out, _, _ = _gpu_recon(w, list(range(w.nz_total)), "f32", m=m)
+    scale = max(abs(v) for v in stored.values())
+    for (z, iy, ix), v in stored.items():
+        assert abs(out[z, iy, ix] - v) < 1e-5 * scale, (z, iy, ix, out[z, iy, ix], v)
+
+
 # ------------------------------------------------------------------ S1+S2 fused into the row kernel's loader
 @pytest.mark.parametrize("dtype,nz,pad", [("f16", 8, "zero"), ("f16", 5, "edge"), ("f16_out32", 18, "zero")])
 def test_fused_normalize_is_bit_identical(dtype, nz, pad):

@@ -519,3 +519,28 @@ def test_p10_padded_detector_is_the_identity_for_powers_of_two_and_consistent_ac
     full = a[:, 14:114, 14:114]
     disc = np.hypot(*np.meshgrid(np.arange(100) - 50, np.arange(100) - 50)) < 40
     assert np.abs(g - full)[:, disc].max() < 0.15 * np.abs(full).max()      # count noise of the dropped air columns
+
+
+# ---------------------------------------------------------------- golden fixture (oracle drift guard)
+def test_golden_c1_oracle_samples():
+    """tests/golden/c1_oracle_samples.txt (written by tests/golden/make_golden.py from oracle/ alone; the paper prints
+    no numerical example to store): the oracle still computes what it computed when the fixture was written."""
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    now = mg.compute()
+    stored = {}
+    with open(os.path.join(here, "c1_oracle_samples.txt")) as f:
+        for ln in f:
+            if ln.startswith("#") or not ln.strip():
+                continue
+            method, m, z, iy, ix, v = ln.split()
+            stored[(method, int(m), int(z), int(iy), int(ix))] = float(v)
+    assert stored.keys() == now.keys() and len(stored) == 96
+    scale = max(abs(v) for v in stored.values())
+    assert scale > 1e-3
+    for k, v in stored.items():
+        assert abs(now[k] - v) <= 1e-12 * scale, (k, now[k], v)
