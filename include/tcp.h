@@ -73,7 +73,8 @@ enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1, TCP_GRID_TILE = 2, TCP_
 /* TCP_OPT_WEIGHT_CACHE (1 default | 0): the tensor-core gridding keeps the interpolation weights of every
  * (sub-tile, sample), which depend only on theta, n and m, in a device cache built on the first call and
  * rebuilt (on the device, no host synchronisation) whenever the angles passed to tcp_recon change; 0 computes
- * them in every call.  Same results bit for bit. */
+ * them in every call.  Same results bit for bit.  The cache is keyed by an element-by-element comparison of the call's
+ * angles with a device copy of the angles it was built for (no checksum). */
 /* TCP_OPT_ANGLE_WEIGHTS (0 default | 1): quadrature weights for angles that are not equally spaced (PAPER.md:61:
  * unlike the log-polar method, the Fourier-based one applies to "non-equally spaced angles", e.g. interlaced
  * scanning).  0: every projection enters with pi/nproj (equispaced half turn).  1: projection j enters with
@@ -170,8 +171,8 @@ int tcp_set_option(tcp_ctx* ctx, int option, int value);
  * 1 <= ncenter <= nz_chunk; out (DEVICE) [ncenter][n][n] receives the reconstruction for centers[i] at
  * index i, identical (to rounding) to tcp_recon on a context created with that centre.  The slice is
  * normalised and filtered once; candidate centres differ only in the phase table of stage S4, two centres
- * riding one complex transform.  Enqueues on stream; the phase tables are built on the host and copied
- * from pageable memory, so the call may block until earlier work on stream has finished.
+ * riding one complex transform.  Enqueues on stream only: the phase tables are built by a kernel (fp64) from the
+ * centres, which travel by value as kernel arguments, so the call never waits for earlier work on stream.
  * Errors: TCP_EINVAL (NULL, ncenter or a centre out of range), TCP_ENOMEM, TCP_ECUDA. */
 int tcp_recon_try(tcp_ctx* ctx, const uint16_t* raw_u16, const float* flat, const float* dark, const float* theta,
                   const float* centers, int ncenter, void* out, tcp_stream_t stream);

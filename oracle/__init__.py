@@ -5,8 +5,12 @@ precision, no code shared with the CUDA path).  Only tests/,
 __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference arm may
 import this package; the product package paper_2209_08450_b200 never does.
 
-Every wrapper below only marshals numpy arrays; the arithmetic is in the C++
-files, each function citing the PAPER.md passage / DESIGN.md reading it follows.
+The stage arithmetic S1..S7, the exact and linear backprojections and the adjoint
+pairs are in the C++ files; the wrappers of those only marshal numpy arrays.  Three
+small functions do their arithmetic here in numpy (double precision), each citing
+the reading it follows and pinned by its own test: `angle_weights` (trapezoid
+weights, reading Q20, pin P11), `padded_size` and `recon_padded` (detector width not
+a power of two, reading Q19, pin P10).
 """
 from __future__ import annotations
 

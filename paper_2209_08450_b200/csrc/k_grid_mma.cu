@@ -84,7 +84,7 @@ struct MmaSmem {
 //   GM_FILL    enumerate and weigh: one record per step and column into the cache  }
 //   GM_CACHED  replay the records: gather, outer product, multiply-accumulate
 enum { GM_DIRECT = 0, GM_COUNT = 1, GM_FILL = 2, GM_CACHED = 3 };
-enum { WS_CHECKSUM = 0, WS_USABLE = 1, WS_REBUILD = 2, WS_ACC = 3 };       // WeightCache::state
+enum { WS_USABLE = 1, WS_REBUILD = 2 };       // WeightCache::state
 
 template <int MH, int NN, int MODE>
 __global__ void __launch_bounds__(32 * CW, 16 / CW)
@@ -396,7 +396,7 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                 __half2* dst = grid + (size_t)(pg * NPG) * pstride + cell;
 #pragma unroll
                 for (int p = 0; p < NPG; ++p)
-                    if (pg * NPG + p < npair) dst[p * pstride] = __floats2half2_rn(__uint_as_float(r[2 * p]), __uint_as_float(r[2 * p + 1]));
+                    if (pg * NPG + p < npair) dst[p * pstride] = f2h2_sat(make_float2(__uint_as_float(r[2 * p]), __uint_as_float(r[2 * p + 1])));
             } else {
                 float2* dst = partial + (((size_t)(item.z + split) * npair + pg * NPG) * TS + ry) * TS + rx;
 #pragma unroll
@@ -415,19 +415,27 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
 
 // ---------------------------------------------------------------------------------------
 // WeightCache bookkeeping (device side only: tcp_recon never synchronises with the host).
-// state[WS_ACC] collects a checksum of the angles in trig_kernel; wc_decide_kernel compares it with the one the
-// cache was built for and raises WS_REBUILD; the count / scan / fill kernels then run (they exit at once
-// otherwise) and WS_USABLE tells the multiply-accumulate kernels which of the two (cached, direct) works.
-__global__ void wc_decide_kernel(int* __restrict__ state, int enable) {
-    const int cs = state[WS_ACC];
-    state[WS_ACC] = 0;
-    if (!enable) { state[WS_USABLE] = 0; state[WS_REBUILD] = 0; return; }
-    if (!state[WS_USABLE] || cs != state[WS_CHECKSUM]) {
-        state[WS_CHECKSUM] = cs;
-        state[WS_USABLE] = 0;
-        state[WS_REBUILD] = 1;
-    } else {
-        state[WS_REBUILD] = 0;
+// wc_decide_kernel compares the call's angles ELEMENT BY ELEMENT (bit patterns) with the copy the cache was built for
+// (w_theta, nproj floats: no checksum, nothing to collide) and, when any differs or no cache exists, stores the new
+// angles and raises WS_REBUILD; the count / scan / fill kernels then run (they exit at once otherwise) and WS_USABLE
+// tells the multiply-accumulate kernels which of the two (cached, direct) works.  One block.
+__global__ void __launch_bounds__(1024) wc_decide_kernel(int* __restrict__ state, int enable, const float* __restrict__ theta,
+                                                         float* __restrict__ w_theta, int nproj) {
+    int differ = 0;
+    if (enable)
+        for (int j = threadIdx.x; j < nproj; j += blockDim.x) differ |= __float_as_uint(theta[j]) != __float_as_uint(w_theta[j]);
+    differ = __syncthreads_or(differ);
+    if (!enable) {
+        if (threadIdx.x == 0) { state[WS_USABLE] = 0; state[WS_REBUILD] = 0; }
+        return;
+    }
+    const bool rebuild = !state[WS_USABLE] || differ;
+    __syncthreads();                                     // every thread has read the state before thread 0 changes it
+    if (rebuild)
+        for (int j = threadIdx.x; j < nproj; j += blockDim.x) w_theta[j] = theta[j];
+    if (threadIdx.x == 0) {
+        if (rebuild) state[WS_USABLE] = 0;
+        state[WS_REBUILD] = rebuild ? 1 : 0;
     }
 }
 
@@ -463,7 +471,7 @@ template <int MH, int NN, int MODE>
 static int launch_mma_mode(const tcp_ctx* c, cudaStream_t st) {
     using L = MmaSmem<NN>;
     auto kern = grid_mma_kernel<MH, NN, MODE>;
-    TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L::total));
+    TCP_SMEM(kern, L::total);
     const double alpha = 3.14159265358979323846 / (1.4142135623730951 * MH);
     const bool mma = MODE == GM_DIRECT || MODE == GM_CACHED;
     const int ny = mma ? (c->npair + NN / 2 - 1) / (NN / 2) : 1, nz = NSUB / CW;
@@ -479,9 +487,9 @@ static int launch_mma_mode(const tcp_ctx* c, cudaStream_t st) {
 }
 
 template <int MH, int NN>
-static int launch_mma_t(const tcp_ctx* c, cudaStream_t st) {
+static int launch_mma_t(const tcp_ctx* c, const float* theta, cudaStream_t st) {
     int rc;
-    wc_decide_kernel<<<1, 1, 0, st>>>(c->w_state, c->w_cap > 0 && c->w_enable ? 1 : 0);
+    wc_decide_kernel<<<1, 1024, 0, st>>>(c->w_state, c->w_cap > 0 && c->w_enable ? 1 : 0, theta, c->w_theta, c->nproj);
     if (c->w_cap > 0) {
         if ((rc = launch_mma_mode<MH, 16, GM_COUNT>(c, st))) return rc;
         wc_scan_kernel<<<1, 1024, 0, st>>>(c->w_count, c->w_off, c->g_nitems * NSUB, c->w_cap, c->w_state);
@@ -499,7 +507,9 @@ int grid_mma_cache_setup(tcp_ctx* c) {
     c->w_cap = 0;
     if (cudaMalloc((void**)&c->w_state, 4 * sizeof(int)) != cudaSuccess) { cudaGetLastError(); c->w_state = nullptr; return set_error(TCP_ENOMEM, "weight cache state"); }
     cudaMemset(c->w_state, 0, 4 * sizeof(int));
-    c->bytes += 16;
+    if (cudaMalloc((void**)&c->w_theta, (size_t)c->nproj * sizeof(float)) != cudaSuccess) { cudaGetLastError(); c->w_theta = nullptr; return set_error(TCP_ENOMEM, "weight cache angles"); }
+    cudaMemset(c->w_theta, 0xff, (size_t)c->nproj * sizeof(float));
+    c->bytes += 16 + (size_t)c->nproj * sizeof(float);
     const size_t nent = (size_t)c->g_nitems * NSUB;
     const double steps = (double)c->nproj * (double)c->M * 2.4 / 32.0 * 1.6 + 4.0 * (double)nent;
     const size_t cap = (size_t)std::min(steps, 2.0e9 / 1.0);
@@ -520,16 +530,16 @@ int grid_mma_cache_setup(tcp_ctx* c) {
 }
 
 void grid_mma_cache_free(tcp_ctx* c) {
-    cudaFree(c->w_state); cudaFree(c->w_count); cudaFree(c->w_off); cudaFree(c->w_rec); cudaFree(c->w_samp);
+    cudaFree(c->w_state); cudaFree(c->w_theta); cudaFree(c->w_count); cudaFree(c->w_off); cudaFree(c->w_rec); cudaFree(c->w_samp);
 }
 
 // Enqueue the tensor-core gridding of the spectrum into the grid (fp16 storage only); the plan
 // kernel and the split-tile reduce are launched by launch_grid_tile.
-int launch_grid_mma_main(const tcp_ctx* c, cudaStream_t st) {
+int launch_grid_mma_main(const tcp_ctx* c, const float* theta, cudaStream_t st) {
     if (!c->half_store) return set_error(TCP_EUNSUPPORTED, "tensor-core gridding needs fp16 storage");
     const bool wide = c->npair > 8;
-    if (c->m == 3) return wide ? launch_mma_t<3, 32>(c, st) : launch_mma_t<3, 16>(c, st);
-    return wide ? launch_mma_t<4, 32>(c, st) : launch_mma_t<4, 16>(c, st);
+    if (c->m == 3) return wide ? launch_mma_t<3, 32>(c, theta, st) : launch_mma_t<3, 16>(c, theta, st);
+    return wide ? launch_mma_t<4, 32>(c, theta, st) : launch_mma_t<4, 16>(c, theta, st);
 }
 
 }  // namespace tcpk

@@ -294,8 +294,8 @@ __global__ void __launch_bounds__(NTHR, 2)
             if (pair >= npair) break;
             TC* g0 = grid + ((size_t)pair * M + L2) * M + L1;
             if constexpr (sizeof(TC) == 4) {
-                const __half2 a = __floats2half2_rn(acc[0][p][0], acc[0][p][1]), b = __floats2half2_rn(acc[1][p][0], acc[1][p][1]);
-                const __half2 c = __floats2half2_rn(acc[2][p][0], acc[2][p][1]), d = __floats2half2_rn(acc[3][p][0], acc[3][p][1]);
+                const __half2 a = f2h2_sat(make_float2(acc[0][p][0], acc[0][p][1])), b = f2h2_sat(make_float2(acc[1][p][0], acc[1][p][1]));
+                const __half2 c = f2h2_sat(make_float2(acc[2][p][0], acc[2][p][1])), d = f2h2_sat(make_float2(acc[3][p][0], acc[3][p][1]));
                 *reinterpret_cast<uint2*>(g0) = make_uint2(*reinterpret_cast<const unsigned*>(&a), *reinterpret_cast<const unsigned*>(&b));
                 *reinterpret_cast<uint2*>(g0 + M) = make_uint2(*reinterpret_cast<const unsigned*>(&c), *reinterpret_cast<const unsigned*>(&d));
             } else {
@@ -414,7 +414,7 @@ static int launch_tile_t(const tcp_ctx* c, cudaStream_t st) {
     const size_t smem = (size_t)PB * KL * (16 + NP * sizeof(TC)) + (size_t)PB * (sizeof(ChordRec) + 4) + 8 +
                         NTHR * sizeof(int2) + (NTHR / 32 + 1) * sizeof(int);
     auto kern = grid_tile_kernel<MH, NP, TC>;
-    TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    TCP_SMEM(kern, (int)smem);
     const double alpha = 3.14159265358979323846 / (1.4142135623730951 * MH);
     dim3 grid(c->g_nitems, (c->npair + NP - 1) / NP);
     kern<<<grid, NTHR, smem, st>>>((const TC*)c->spec, (TC*)c->grid, c->g_partial, c->trig, c->g_plan, c->g_items, c->nproj,
@@ -435,7 +435,7 @@ int launch_grid_tile(const tcp_ctx* c, const float* theta, cudaStream_t st) {
     grid_plan_kernel<<<(nplan + 127) / 128, 128, 0, st>>>(theta, c->nproj, c->M, c->m, c->g_plan, c->g_counter);
     TCP_CUDA_CHECK(cudaGetLastError());
     int rc;
-    if (c->grid_impl == TCP_GRID_MMA) rc = launch_grid_mma_main(c, st);
+    if (c->grid_impl == TCP_GRID_MMA) rc = launch_grid_mma_main(c, theta, st);
     else if (c->m == 3) rc = c->half_store ? launch_tile_np<3, __half2>(c, st) : launch_tile_np<3, float2>(c, st);
     else rc = c->half_store ? launch_tile_np<4, __half2>(c, st) : launch_tile_np<4, float2>(c, st);
     if (rc) return rc;

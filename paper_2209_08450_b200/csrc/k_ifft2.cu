@@ -40,7 +40,7 @@ __device__ __forceinline__ void st_c2(float2* p, size_t i, cpair v) {
     *reinterpret_cast<float4*>(p + i) = make_float4(v.a.x, v.a.y, v.b.x, v.b.y);
 }
 __device__ __forceinline__ void st_c2(__half2* p, size_t i, cpair v) {
-    const __half2 a = __float22half2_rn(v.a), b = __float22half2_rn(v.b);
+    const __half2 a = f2h2_sat(v.a), b = f2h2_sat(v.b);
     *reinterpret_cast<uint2*>(p + i) = make_uint2(*reinterpret_cast<const unsigned*>(&a), *reinterpret_cast<const unsigned*>(&b));
 }
 
@@ -157,7 +157,7 @@ static int launch_cols_t(const tcp_ctx* c, cudaStream_t st) {
         const size_t smem_pf = smem + (size_t)M * W * sizeof(__half2);
         if (c->grid_strip == W && smem_pf <= 227 * 1024 && smem > 64 * 1024) {      // long lines, one CTA per SM
             auto kpf = ifft_cols_pf_kernel<M>;
-            TCP_CUDA_CHECK(cudaFuncSetAttribute(kpf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_pf));
+            TCP_SMEM(kpf, (int)smem_pf);
             const int nunits = (M / W) * c->npair;
             kpf<<<nunits < c->nsm ? nunits : c->nsm, WP * M / 16, smem_pf, st>>>((const __half2*)c->grid, (__half2*)c->pass1, c->tw, nunits);
             TCP_CUDA_CHECK(cudaGetLastError());
@@ -165,7 +165,7 @@ static int launch_cols_t(const tcp_ctx* c, cudaStream_t st) {
         }
     }
     auto kern = ifft_cols_kernel<M, TC>;
-    TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    TCP_SMEM(kern, (int)smem);
     dim3 grid(M / W, c->npair);
     kern<<<grid, WP * M / 16, smem, st>>>((const TC*)c->grid, (TC*)c->pass1, c->tw, c->grid_strip);
     TCP_CUDA_CHECK(cudaGetLastError());
@@ -178,7 +178,7 @@ static int launch_rows_t(const tcp_ctx* c, void* out, cudaStream_t st) {
     constexpr int ROWS = (TG >= 128) ? 1 : 128 / TG;
     const size_t smem = (size_t)ROWS * padded_len(M) * sizeof(float2);
     auto kern = ifft_rows_kernel<M, ROWS, TC, TO>;
-    TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    TCP_SMEM(kern, (int)smem);
     dim3 grid((M / 2) / ROWS, c->npair);
     kern<<<grid, ROWS * TG, smem, st>>>((const TC*)c->pass1, (TO*)out, c->tw, c->deax, c->deay, c->nz);
     TCP_CUDA_CHECK(cudaGetLastError());

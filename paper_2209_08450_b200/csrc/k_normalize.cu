@@ -205,7 +205,7 @@ int launch_mean_frames(const uint16_t* frames, int nframes, int nz, int n, float
 // cos/sin of the float32 angles in fp64: k*cos(theta) with
 // k up to 4096 must be good to ~1e-6 grid cells for the 1e-5 fp32 gate.
 __global__ void trig_kernel(const float* __restrict__ theta, int nproj, double2* __restrict__ trig, float4* __restrict__ trigf,
-                            int* __restrict__ wstate, float* __restrict__ wq, const float* __restrict__ flat,
+                            float* __restrict__ wq, const float* __restrict__ flat,
                             const float* __restrict__ dark, float2* __restrict__ fdtab, int nfd) {
     // fused S1+S2 (rows_kernel's loader): per detector pixel of the chunk the reciprocal normalize_half_kernel forms, and dark
     if (flat)
@@ -224,8 +224,6 @@ __global__ void trig_kernel(const float* __restrict__ theta, int nproj, double2*
             const double prv = (j > 0) ? (double)theta[j - 1] : (double)theta[nproj - 1] - pi;
             wq[j] = (float)(0.5 * (nxt - prv) * (double)nproj / pi);
         }
-        // order-independent checksum of the angles for the gridding weight cache (k_grid_mma.cu, state[3])
-        if (wstate) atomicAdd(&wstate[3], (int)((__float_as_uint(theta[j]) ^ 0x9e3779b9u) * (2u * (unsigned)j + 1u)));
         double t = (double)theta[j];
         const double c = cos(t), s = sin(t);
         trig[j] = make_double2(c, s);
@@ -239,7 +237,7 @@ __global__ void trig_kernel(const float* __restrict__ theta, int nproj, double2*
 int launch_trig(const tcp_ctx* c, const float* theta, cudaStream_t st, const float* flat, const float* dark) {
     const int nfd = c->nz * c->n;
     const int blocks = flat ? std::max((c->nproj + 127) / 128, std::min((nfd + 127) / 128, 148 * 4)) : (c->nproj + 127) / 128;
-    trig_kernel<<<blocks, 128, 0, st>>>(theta, c->nproj, c->trig, c->trigf, c->w_state, c->wq, flat, dark, c->fdtab, nfd);
+    trig_kernel<<<blocks, 128, 0, st>>>(theta, c->nproj, c->trig, c->trigf, c->wq, flat, dark, c->fdtab, nfd);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }

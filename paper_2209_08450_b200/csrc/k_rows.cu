@@ -163,7 +163,7 @@ static int launch_filter_t(const tcp_ctx* c, cudaStream_t st) {
     constexpr int ROWS = (TG >= 128) ? 1 : 128 / TG;
     const size_t smem = (size_t)ROWS * padded_len(M) * sizeof(float2);
     auto kern = filter_kernel<M, ROWS, TS>;
-    TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    TCP_SMEM(kern, (int)smem);
     dim3 grid((c->nproj + ROWS - 1) / ROWS, c->npair);
     kern<<<grid, ROWS * TG, smem, st>>>((TS*)c->sino, c->tw, c->hfilt, c->nproj, c->nz, c->pad, c->angle_weights ? c->wq : nullptr);
     TCP_CUDA_CHECK(cudaGetLastError());
@@ -195,7 +195,7 @@ static int launch_rows_t(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw,
     const size_t smem = (size_t)ROWS * padded_len(M) * sizeof(float2);
     if (c->filter_fused && !c->try_ptab) {
         auto kf = c->pad ? rows_fused_kernel<M, ROWS, true, TS, TC> : rows_fused_kernel<M, ROWS, false, TS, TC>;
-        TCP_CUDA_CHECK(cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        TCP_SMEM(kf, (int)smem);
         kf<<<dim3((c->nproj + ROWS - 1) / ROWS, c->npair), ROWS * TG, smem, st>>>((const TS*)c->sino, (TC*)c->spec, c->tw, c->ftab, c->nproj,
                                                                                    c->nz, c->angle_weights ? c->wq : nullptr);
         TCP_CUDA_CHECK(cudaGetLastError());
@@ -205,7 +205,7 @@ static int launch_rows_t(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw,
     if constexpr (std::is_same_v<TS, __half>) {
         if (raw) kern = c->pad ? rows_kernel<M, ROWS, true, true, TS, TC> : rows_kernel<M, ROWS, false, true, TS, TC>;
     }
-    TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    TCP_SMEM(kern, (int)smem);
     dim3 grid((c->nproj + ROWS - 1) / ROWS, c->npair);
     kern<<<grid, ROWS * TG, smem, st>>>((const TS*)c->sino, (TC*)c->spec, c->tw, c->hfilt, c->try_ptab ? c->try_ptab : c->ptab, c->nproj, c->nz,
                                        c->try_ptab ? 1 : 0, c->angle_weights ? c->wq : nullptr, raw, c->fdtab);

@@ -80,7 +80,7 @@ template <int NG, class TO>
 static int launch_ifft_rows_tc_t(const tcp_ctx* c, void* out, cudaStream_t st) {
     using C = Cta<1, NG>;
     auto kern = ifft_rows_tc_kernel<NG, TO>;
-    TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::total));
+    TCP_SMEM(kern, C::total);
     const int nlines = c->npair * TC_N;
     int ctas = c->nsm;
     if (ctas * NG > nlines) ctas = (nlines + NG - 1) / NG;

@@ -21,29 +21,55 @@ struct Pipe {
 
 namespace tcpk {
 
-int setup_kernel_attributes(const tcp_ctx*) { return TCP_OK; }
+// Called once from tcp_create: the device must offer the opt-in shared memory the context's transforms need (one padded
+// line of M complex values per row transform, cols_wp(M) lines + staging for the column pass: up to 227 KB); the
+// per-kernel opt-in itself is memoised at first launch (ensure_smem), not repeated per launch.
+int setup_kernel_attributes(const tcp_ctx* c) {
+    int optin = 0;
+    TCP_CUDA_CHECK(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device));
+    const int line = (c->M + c->M / 16) * 8;
+    if (optin < 2 * line || optin < 200 * 1024)
+        return set_error(TCP_EUNSUPPORTED, "device offers %d B of opt-in shared memory per block; sm_100a (227 KB) is required", optin);
+    return TCP_OK;
+}
 
 void pipe_destroy(tcp_ctx* c) {
     Pipe* p = c->pipe;
     if (!p) return;
     for (int b = 0; b < p->nbuf; ++b) {
         cudaFree(p->raw[b]); cudaFree(p->flat[b]); cudaFree(p->dark[b]); cudaFree(p->out[b]);
-        cudaEventDestroy(p->ev_h2d[b]); cudaEventDestroy(p->ev_comp[b]); cudaEventDestroy(p->ev_d2h[b]);
+        if (p->ev_h2d[b]) cudaEventDestroy(p->ev_h2d[b]);
+        if (p->ev_comp[b]) cudaEventDestroy(p->ev_comp[b]);
+        if (p->ev_d2h[b]) cudaEventDestroy(p->ev_d2h[b]);
     }
     cudaFree(p->theta);
-    cudaEventDestroy(p->ev_start); cudaEventDestroy(p->ev_stop);
-    cudaStreamDestroy(p->s_h2d); cudaStreamDestroy(p->s_comp); cudaStreamDestroy(p->s_d2h);
+    if (p->ev_start) cudaEventDestroy(p->ev_start);
+    if (p->ev_stop) cudaEventDestroy(p->ev_stop);
+    if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
+    if (p->s_comp) cudaStreamDestroy(p->s_comp);
+    if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
     free(p);
     c->pipe = nullptr;
 }
 
+static int pipe_fill(tcp_ctx* c, Pipe* p, int nbuf);
+
+// The pipe is published in the context only when every stream, buffer and event exists: a failed allocation leaves
+// c->pipe NULL (and frees what was made), so the next call starts over instead of running on NULL handles.
 static int pipe_create(tcp_ctx* c, int nbuf) {
     if (c->pipe && c->pipe->nbuf == nbuf) return TCP_OK;
     pipe_destroy(c);
     Pipe* p = (Pipe*)calloc(1, sizeof(Pipe));
     if (!p) return set_error(TCP_ENOMEM, "out of host memory");
-    c->pipe = p;
     p->nbuf = nbuf;
+    const int rc = pipe_fill(c, p, nbuf);
+    c->pipe = p;
+    if (rc != TCP_OK) pipe_destroy(c);        // cudaFree / destroy of a zero handle is a no-op or a harmless error
+    cudaGetLastError();
+    return rc;
+}
+
+static int pipe_fill(tcp_ctx* c, Pipe* p, int nbuf) {
     const size_t ob = c->half_out ? 2 : 4;
     const int n = c->ndet;                    // width of the caller's rows and side of the caller's images
     TCP_CUDA_CHECK(cudaStreamCreateWithFlags(&p->s_h2d, cudaStreamNonBlocking));
@@ -121,6 +147,9 @@ extern "C" int tcp_recon_volume_host_rows(tcp_ctx* c, const uint16_t* raw_host, 
     const int nz_total = z_end - z_begin;                  // slices of this call; the arrays hold nz_stack
     const int nchunks = (nz_total + nz - 1) / nz;
 
+    // An error inside the loop must not return while copies on the caller's pinned buffers are in flight (the caller
+    // may free or reuse them): the loop runs in a lambda and every exit path drains the three streams first.
+    auto enqueue = [&]() -> int {
     TCP_CUDA_CHECK(cudaEventRecord(p->ev_start, p->s_h2d));
     TCP_CUDA_CHECK(cudaMemcpyAsync(p->theta, theta_host, (size_t)c->nproj * 4, cudaMemcpyHostToDevice, p->s_h2d));
     for (int ch = 0; ch < nchunks; ++ch) {
@@ -161,9 +190,14 @@ extern "C" int tcp_recon_volume_host_rows(tcp_ctx* c, const uint16_t* raw_host, 
         TCP_CUDA_CHECK(cudaEventRecord(p->ev_d2h[b], p->s_d2h));
     }
     TCP_CUDA_CHECK(cudaEventRecord(p->ev_stop, p->s_d2h));
-    TCP_CUDA_CHECK(cudaStreamSynchronize(p->s_d2h));
-    TCP_CUDA_CHECK(cudaStreamSynchronize(p->s_comp));
-    TCP_CUDA_CHECK(cudaStreamSynchronize(p->s_h2d));
+    return TCP_OK;
+    };
+    rc = enqueue();
+    const cudaError_t e1 = cudaStreamSynchronize(p->s_d2h), e2 = cudaStreamSynchronize(p->s_comp), e3 = cudaStreamSynchronize(p->s_h2d);
+    if (rc) return rc;
+    TCP_CUDA_CHECK(e1);
+    TCP_CUDA_CHECK(e2);
+    TCP_CUDA_CHECK(e3);
     if (ms_out) TCP_CUDA_CHECK(cudaEventElapsedTime(ms_out, p->ev_start, p->ev_stop));
     return TCP_OK;
 }

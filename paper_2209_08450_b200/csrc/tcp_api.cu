@@ -7,6 +7,8 @@
 #include <string.h>
 
 #include <algorithm>
+#include <map>
+#include <mutex>
 #include <vector>
 
 #include "tcfft.cuh"
@@ -22,6 +24,20 @@ int set_error(int code, const char* fmt, ...) {
     vsnprintf(g_err, sizeof(g_err), fmt, ap);
     va_end(ap);
     return code;
+}
+
+// (device, kernel) -> largest dynamic shared-memory size set so far
+int ensure_smem(const void* kern, int bytes) {
+    static std::mutex mu;
+    static std::map<std::pair<int, const void*>, int> done;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    std::lock_guard<std::mutex> lk(mu);
+    int& have = done[std::make_pair(dev, kern)];
+    if (have >= bytes && have > 0) return TCP_OK;
+    if (bytes > 48 * 1024 || have > 0) TCP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    have = bytes > 0 ? bytes : 1;
+    return TCP_OK;
 }
 
 static const int kProfileRing = 512;
@@ -168,6 +184,29 @@ static int build_context(tcp_ctx* c) {
     c->ntiles = (int)order.size();
     if ((rc = upload(&c->tile_order, order, &c->bytes))) return rc;
     return grid_tile_setup(c);
+}
+
+// tcp_recon_try: candidate centres of up to kMax / 2 pairs by value (a negative entry = no slice B in the last pair)
+struct TryCentres {
+    static constexpr int kMax = 256;
+    float c[kMax];
+};
+
+__global__ void try_ptab_kernel(float2* __restrict__ ptab, TryCentres tc, int M, double SC) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x, p = blockIdx.y;
+    if (k >= M) return;
+    const int ks = (k < M / 2) ? k : k - M;
+    double re = 0.0, im = 0.0;
+    for (int h = 0; h < 2; ++h) {
+        const float ce = tc.c[2 * p + h];
+        if (ce < 0.f) continue;
+        const double fr = fmod((double)ks * (double)ce, (double)M) / (double)M;
+        double sn, cs;
+        sincospi(2.0 * fr, &sn, &cs);
+        if (h == 0) { re += SC * cs; im += SC * sn; }    // slice A: real part
+        else { re -= SC * sn; im += SC * cs; }           // slice B: times i
+    }
+    ptab[(size_t)p * M + k] = (k == M / 2) ? make_float2(0.f, 0.f) : make_float2((float)re, (float)im);
 }
 
 }  // namespace tcpk
@@ -330,22 +369,15 @@ int tcp_recon_try(tcp_ctx* c, const uint16_t* raw, const float* flat, const floa
         int rc = dev_alloc((void**)&c->try_buf, (size_t)c->npair * M * sizeof(float2), &c->bytes);
         if (rc) return rc;
     }
-    // ptab[pair][k] = S C (e^{+2 pi i k c1/M} + i e^{+2 pi i k c2/M}), k signed, 0 at k = M/2 (build_context's table twice)
-    const double C = kPi / ((double)c->nproj * (double)M);
-    std::vector<float2> pt((size_t)npair * M);
-    for (int p = 0; p < npair; ++p)
-        for (int k = 0; k < M; ++k) {
-            const int ks = (k < M / 2) ? k : k - M;
-            double re = 0.0, im = 0.0;
-            for (int h = 0; h < 2 && 2 * p + h < ncenter; ++h) {
-                const double fr = fmod((double)ks * ((double)centers[2 * p + h] + (double)c->pad_l), (double)M) / (double)M;
-                const double a = 2.0 * kPi * fr, cr = c->scale * C * cos(a), ci = c->scale * C * sin(a);
-                if (h == 0) { re += cr; im += ci; }      // slice A: real part
-                else { re -= ci; im += cr; }             // slice B: times i
-            }
-            pt[(size_t)p * M + k] = (k == M / 2) ? make_float2(0.f, 0.f) : make_float2((float)re, (float)im);
-        }
-    TCP_CUDA_CHECK(cudaMemcpyAsync(c->try_buf, pt.data(), pt.size() * sizeof(float2), cudaMemcpyHostToDevice, st));
+    // ptab[pair][k] = S C (e^{+2 pi i k c1/M} + i e^{+2 pi i k c2/M}), k signed, 0 at k = M/2 (build_context's table twice),
+    // built on the device in fp64; the centres travel by value as kernel arguments (no pageable copy, no hidden sync)
+    for (int p0 = 0; p0 < npair; p0 += TryCentres::kMax / 2) {
+        TryCentres tc;
+        const int np = std::min(npair - p0, TryCentres::kMax / 2);
+        for (int i = 0; i < 2 * np; ++i) tc.c[i] = (2 * p0 + i < ncenter) ? centers[2 * p0 + i] + (float)c->pad_l : -1.f;
+        try_ptab_kernel<<<dim3((M + 255) / 256, np), 256, 0, st>>>(c->try_buf + (size_t)p0 * M, tc, M, c->scale * kPi / ((double)c->nproj * (double)M));
+        TCP_CUDA_CHECK(cudaGetLastError());
+    }
     int rc;
     tcp_ctx one = *c;                 // the single input slice
     one.nz = 1; one.npair = 1;

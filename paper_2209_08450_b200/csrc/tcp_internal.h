@@ -55,6 +55,7 @@ struct tcp_ctx {
     int2* g_plan;
     // weight cache of the tcgen05 gridding (k_grid_mma.cu): per-step records, built on the device when theta changes
     int* w_state; int* w_count; int* w_off; uint4* w_rec; unsigned* w_samp; int w_cap, w_enable;
+    float* w_theta;       // [nproj] the angles the cached weights were built for (compared element by element on every call)
     int* g_counter;       // [64] next-item counters of the persistent gridding CTAs, zeroed by the plan kernel
     int g_nitems, g_nred;
     size_t bytes;
@@ -77,6 +78,15 @@ int set_error(int code, const char* fmt, ...);
                                    cudaGetErrorString(e__), __FILE__, __LINE__);               \
     } while (0)
 
+// Opt a kernel into `bytes` of dynamic shared memory ONCE per (device, kernel): cudaFuncSetAttribute is a host API
+// call, so the launchers memoise it instead of repeating it on every launch of every chunk.
+int ensure_smem(const void* kern, int bytes);
+#define TCP_SMEM(kern, bytes)                                                     \
+    do {                                                                          \
+        int rc__ = tcpk::ensure_smem((const void*)(kern), (int)(bytes));          \
+        if (rc__ != TCP_OK) return rc__;                                          \
+    } while (0)
+
 // kernel launchers: each enqueues on `st` and returns TCP_OK or an error code
 // flat != NULL: also fill c->fdtab from the call's flat / dark (fused S1+S2 loader of rows_kernel)
 int launch_trig(const tcp_ctx* c, const float* theta, cudaStream_t st, const float* flat = nullptr, const float* dark = nullptr);
@@ -91,7 +101,7 @@ int launch_line_bp(const tcp_ctx* c, void* out, cudaStream_t st);
 int launch_grid_scatter(const tcp_ctx* c, cudaStream_t st);
 int launch_grid_gather(const tcp_ctx* c, const float* theta, cudaStream_t st);
 int launch_grid_tile(const tcp_ctx* c, const float* theta, cudaStream_t st);
-int launch_grid_mma_main(const tcp_ctx* c, cudaStream_t st);
+int launch_grid_mma_main(const tcp_ctx* c, const float* theta, cudaStream_t st);
 int grid_mma_cache_setup(tcp_ctx* c);
 void grid_mma_cache_free(tcp_ctx* c);
 int grid_tile_setup(tcp_ctx* c);
@@ -109,11 +119,23 @@ void pipe_destroy(tcp_ctx* c);
 __device__ __forceinline__ float2 ld_c(const float2* p, size_t i) { return p[i]; }
 __device__ __forceinline__ float2 ld_c(const __half2* p, size_t i) { return __half22float2(p[i]); }
 __device__ __forceinline__ void st_c(float2* p, size_t i, float2 v) { p[i] = v; }
-__device__ __forceinline__ void st_c(__half2* p, size_t i, float2 v) { p[i] = __float22half2_rn(v); }
+// fp32 -> half with saturation to +-65504 (cvt.rn.satfinite): a hot or dead detector pixel must not turn into inf and then,
+// through the transforms, into a slice pair of NaN
+__device__ __forceinline__ __half2 f2h2_sat(float2 v) {
+    unsigned r;
+    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(v.y), "f"(v.x));
+    return *reinterpret_cast<__half2*>(&r);
+}
+__device__ __forceinline__ __half f2h_sat(float v) {
+    unsigned short r;
+    asm("cvt.rn.satfinite.f16.f32 %0, %1;" : "=h"(r) : "f"(v));
+    return *reinterpret_cast<__half*>(&r);
+}
+__device__ __forceinline__ void st_c(__half2* p, size_t i, float2 v) { p[i] = f2h2_sat(v); }
 __device__ __forceinline__ float ld_r(const float* p, size_t i) { return p[i]; }
 __device__ __forceinline__ float ld_r(const __half* p, size_t i) { return __half2float(p[i]); }
 __device__ __forceinline__ void st_r(float* p, size_t i, float v) { p[i] = v; }
-__device__ __forceinline__ void st_r(__half* p, size_t i, float v) { p[i] = __float2half_rn(v); }
+__device__ __forceinline__ void st_r(__half* p, size_t i, float v) { p[i] = f2h_sat(v); }
 
 // S1+S2 for fp16 storage (normalize_half_kernel and the fused loader of rows_kernel share these, so both give the
 // same half value bit for bit): hardware approximations (~2^-22) under a rounding to 2^-11

@@ -11,6 +11,7 @@ import synthgen as sg
 pytestmark = pytest.mark.gpu
 
 FP32_GATE = 1e-5
+FP32_GATE_MAX = 5e-5     # of max |oracle|: fp32 rounding of ~40 sequential stages, see DESIGN.md section 3
 FP16_GATE_L2 = 5e-3
 FP16_GATE_MAX = 1e-2
 
@@ -19,6 +20,18 @@ def rl2(a, b):
     a = np.asarray(a).astype(np.complex128 if np.iscomplexobj(a) or np.iscomplexobj(b) else np.float64)
     b = np.asarray(b).astype(a.dtype)
     return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def check(got, ref, dtype="f32", vol=None, tag=None):
+    """One slice against the oracle at north_star's gates.  fp32: rel-L2 <= 1e-5 (north_star) AND, element by element,
+    max-abs <= FP32_GATE_MAX of max |oracle| over the volume `vol` (a norm alone lets a single wrong
+    pixel through at n >= 512).  fp16 storage: rel-L2 <= 5e-3 and max-abs <= 1e-2 of max |oracle|."""
+    scale = float(np.abs(ref if vol is None else vol).max())
+    e2, emax = rl2(got, ref), float(np.abs(np.asarray(got, np.float64) - ref).max()) / scale
+    if dtype == "f32":
+        assert e2 < FP32_GATE and emax < FP32_GATE_MAX, (tag, e2, emax)
+    else:
+        assert e2 < FP16_GATE_L2 and emax < FP16_GATE_MAX, (tag, e2, emax)
 
 
 def _tcp():
@@ -78,7 +91,7 @@ def test_c1_fp32_stages_and_volume(m):
     # S1..S7
     ref = orc.recon(raw, flat, dark, theta, w.center, w.filter, m, "grid")
     for z in rows:
-        assert rl2(out[z], ref[z]) < FP32_GATE, (z, rl2(out[z], ref[z]))
+        check(out[z], ref[z], "f32")
     r.close()
 
 
@@ -107,9 +120,8 @@ def test_several_pair_groups_and_ragged_chunk(dtype, nz):
     rows = list(range(40, 40 + nz))
     out, _, (raw, flat, dark, theta) = _gpu_recon(w, rows, dtype)
     ref = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, "grid")
-    gate = FP32_GATE if dtype == "f32" else FP16_GATE_L2
     for z in range(nz):
-        assert rl2(out[z], ref[z]) < gate, (z, rl2(out[z], ref[z]))
+        check(out[z], ref[z], dtype, vol=ref, tag=z)
 
 
 def test_limited_and_uneven_angles():
@@ -128,7 +140,7 @@ def test_limited_and_uneven_angles():
     r.close()
     ref = orc.recon(raw, flat, dark, th, w.center, w.filter, 3, "grid")
     for z in range(2):
-        assert rl2(out[z], ref[z]) < FP32_GATE
+        check(out[z], ref[z], "f32")
 
 
 def test_c1_fp16_grid_stage_strip_layout():
@@ -178,7 +190,7 @@ def test_downscaled_configs(cfg, scale, dtype):
     ref = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, "grid")
     if dtype == "f32":
         for z in range(len(rows)):
-            assert rl2(out[z], ref[z]) < FP32_GATE, (cfg, scale, z, rl2(out[z], ref[z]))
+            check(out[z], ref[z], "f32")
     else:
         for z in range(len(rows)):
             assert rl2(out[z], ref[z]) < FP16_GATE_L2, (cfg, scale, z, rl2(out[z], ref[z]))
@@ -193,7 +205,7 @@ def test_filters_and_offcentre(filt):
     out, _, (raw, flat, dark, theta) = _gpu_recon(w, rows, "f32", filt=filt)
     ref = orc.recon(raw, flat, dark, theta, w.center, filt, 3, "grid")
     for z in range(2):
-        assert rl2(out[z], ref[z]) < FP32_GATE
+        check(out[z], ref[z], "f32")
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f16"])
@@ -214,7 +226,7 @@ def test_centre_try_mode(dtype):
     for i, c in enumerate(centers):
         ref = orc.recon(raw, flat, dark, theta, c, w.filter, 3, "grid")[0]
         if dtype == "f32":
-            assert rl2(out[i], ref) < FP32_GATE, (c, rl2(out[i], ref))
+            check(out[i], ref, "f32")
         else:
             assert rl2(out[i], ref) < FP16_GATE_L2, (c, rl2(out[i], ref))
             assert np.abs(out[i] - ref).max() / np.abs(ref).max() < FP16_GATE_MAX
@@ -222,7 +234,7 @@ def test_centre_try_mode(dtype):
     raw8, flat8, dark8, _ = _inputs(w, list(range(8)))
     full = r.recon(*_to_dev(raw8, flat8, dark8, theta)).float().cpu().numpy()
     ref8 = orc.recon(raw8[:, 4:5], flat8[4:5], dark8[4:5], theta, w.center, w.filter, 3, "grid")[0]
-    assert rl2(full[4], ref8) < (FP32_GATE if dtype == "f32" else FP16_GATE_L2)
+    check(full[4], ref8, dtype)
     with pytest.raises(tcp.TcpError):
         r.recon_try(d[0], d[1], d[2], d[3], [float(w.n)])
     with pytest.raises(tcp.TcpError):
@@ -248,7 +260,7 @@ def test_line_summation_operator(dtype, cfg, scale, nz):
     scale_v = np.abs(ref).max()
     for z in range(nz):
         if dtype == "f32":
-            assert rl2(out[z], ref[z]) < FP32_GATE, (z, rl2(out[z], ref[z]))
+            check(out[z], ref[z], "f32")
         else:
             assert rl2(out[z], ref[z]) < FP16_GATE_L2, (z, rl2(out[z], ref[z]))
             assert np.abs(out[z] - ref[z]).max() / scale_v < FP16_GATE_MAX
@@ -256,7 +268,7 @@ def test_line_summation_operator(dtype, cfg, scale, nz):
     r.set_algorithm("fourier")
     out2 = r.recon(*_to_dev(raw, flat, dark, theta)).float().cpu().numpy()
     ref2 = orc.recon(raw[:, :1], flat[:1], dark[:1], theta, w.center, w.filter, 3, "grid")[0]
-    assert rl2(out2[0], ref2) < (FP32_GATE if dtype == "f32" else FP16_GATE_L2)
+    check(out2[0], ref2, dtype)
     r.close()
 
 
@@ -278,13 +290,12 @@ def test_edge_padding(dtype, alg):
     ref = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, method, pad="edge")
     refz = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, method)
     assert rl2(ref[1], refz[1]) > 1e-2                       # the option matters on this input
-    gate = FP32_GATE if dtype == "f32" else FP16_GATE_L2
     for z in range(3):
-        assert rl2(out[z], ref[z]) < gate, (z, rl2(out[z], ref[z]))
+        check(out[z], ref[z], dtype, vol=ref, tag=z)
     r.set_pad("zero")
     outz = r.recon(*dev).float().cpu().numpy()
     for z in range(3):
-        assert rl2(outz[z], refz[z]) < gate
+        check(outz[z], refz[z], dtype, vol=refz, tag=z)
     r.close()
 
 
@@ -314,7 +325,7 @@ def test_recon_under_cuda_graph_capture(dtype):
     torch.cuda.synchronize()
     assert torch.equal(out, eager)
     ref = orc.recon(raw[:, :1], flat[:1], dark[:1], theta, w.center, w.filter, 3, "grid")[0]
-    assert rl2(out[0].float().cpu().numpy(), ref) < (FP32_GATE if dtype == "f32" else FP16_GATE_L2)
+    check(out[0].float().cpu().numpy(), ref, dtype)
     r.close()
 
 
@@ -337,11 +348,11 @@ def test_fused_filter_option(dtype, pad):
     gate = FP32_GATE if dtype == "f32" else FP16_GATE_L2
     assert rl2(ref[2], lit[2]) > 10 * gate or dtype == "f16"
     for z in range(5):
-        assert rl2(out[z], ref[z]) < gate, (z, rl2(out[z], ref[z]))
+        check(out[z], ref[z], dtype, vol=ref, tag=z)
     r.set_filter_fused(False)
     out2 = r.recon(*dev).float().cpu().numpy()
     for z in range(5):
-        assert rl2(out2[z], lit[z]) < gate
+        check(out2[z], lit[z], dtype, vol=lit, tag=z)
     r.close()
 
 
@@ -411,7 +422,7 @@ def test_pipeline_host_matches_direct():
         assert np.array_equal(out_h[sl], d.cpu().numpy())
     ref = orc.recon(np.ascontiguousarray(raw[:, 20:22]), flat[20:22], dark[20:22], theta, w.center, w.filter, 3, "grid")
     for z in range(2):
-        assert rl2(out_h[20 + z], ref[z]) < FP32_GATE
+        check(out_h[20 + z], ref[z], "f32")
     r.close()
     # the partial last chunk runs as a chunk of its own size: equal to a 2-slice context, bit for bit
     r2 = tcp.Recon(w.n, w.nproj, 2, w.center, "f32", w.filter)
@@ -501,13 +512,13 @@ def test_angle_weights_for_unequally_spaced_angles(dtype, alg):
     assert rl2(plain[0], ref[0]) > 0.05                      # the weights matter for these angles
     for z in range(3):
         if dtype == "f32":
-            assert rl2(out[z], ref[z]) < FP32_GATE, (z, rl2(out[z], ref[z]))
+            check(out[z], ref[z], "f32")
         else:
             assert rl2(out[z], ref[z]) < FP16_GATE_L2
             assert np.abs(out[z] - ref[z]).max() / np.abs(ref).max() < FP16_GATE_MAX
     if alg == "fourier":
         t = r.recon_try(dev[0][:, 1:2].contiguous(), dev[1][1:2], dev[2][1:2], dev[3], [w.center, w.center + 1.5]).float().cpu().numpy()
-        assert rl2(t[0], ref[1]) < (FP32_GATE if dtype == "f32" else FP16_GATE_L2)
+        check(t[0], ref[1], dtype)
         r.set_angle_weights(False)
         again = r.recon(*dev).float().cpu().numpy()
         assert np.array_equal(again, base)
@@ -540,14 +551,14 @@ def test_degenerate_cases(dtype, case):
     elif case == "centre_at_edges":
         theta, centers = sg.make_theta(12), [0.0, float(n - 1)]
     else:
-        theta, centers = sg.make_theta(9), [30.25]
+        # fp16 storage holds |f| < 1.9 per pixel: with 90 projections a p = 13.8 sample
+        # backprojects to ~0.15 per pixel, inside that range, and the clamps of S1 are compared at the fp16 gates
+        theta, centers = sg.make_theta(9 if dtype == "f32" else 90), [30.25]
     nproj = theta.size
     flat = rng.uniform(20000, 30000, (nz, n)).astype(np.float32)
     dark = rng.uniform(90, 110, (nz, n)).astype(np.float32)
     raw = np.rint((flat - dark)[None] * np.exp(-rng.uniform(0.0, 1.5, (nproj, nz, n))) + dark[None]).astype(np.uint16)
     if case == "guards":
-        if dtype != "f32":
-            pytest.skip("p = 13.8 rows leave the range the fp16 scaling is set for (DESIGN.md: |f| < 1.9 per pixel)")
         raw[0, 0, 3], raw[1, 0, 4], raw[2, 0, 5] = 0, 65535, 50
         flat[0, 9] = dark[0, 9]
     for c in centers:
@@ -557,10 +568,35 @@ def test_degenerate_cases(dtype, case):
         ref = orc.recon(raw, flat, dark, theta, c, "ramp", 3, "grid")
         assert np.isfinite(out).all()
         if dtype == "f32":
-            assert rl2(out[0], ref[0]) < FP32_GATE, (case, c, rl2(out[0], ref[0]))
+            check(out[0], ref[0], "f32")
         else:
             assert rl2(out[0], ref[0]) < FP16_GATE_L2, (case, c, rl2(out[0], ref[0]))
             assert np.abs(out[0] - ref[0]).max() / np.abs(ref).max() < FP16_GATE_MAX
+
+
+@pytest.mark.parametrize("dtype", ["f16", "f16_out32"])
+def test_fp16_storage_saturates_instead_of_overflowing(dtype):
+    """A dead detector pixel (raw = 0 in every projection, p = 13.8: a ring through the whole slice) and a hot one on
+    few projections drive |f| Phi^2 S past 65504, the largest half.  Every half store of the path saturates
+    (cvt.rn.satfinite: sinogram, spectrum, grid, pass-1, output), so the result stays finite -- no inf in the grid,
+    hence no NaN slice pair after S6 -- and the slice that shares the complex transform with the damaged one is
+    reconstructed as if it were alone, away from where the damaged slice saturates."""
+    tcp = _tcp()
+    n, nz, nproj = 64, 2, 9
+    rng = np.random.default_rng(78)
+    theta = sg.make_theta(nproj)
+    flat = rng.uniform(20000, 30000, (nz, n)).astype(np.float32)
+    dark = rng.uniform(90, 110, (nz, n)).astype(np.float32)
+    raw = np.rint((flat - dark)[None] * np.exp(-rng.uniform(0.0, 1.5, (nproj, nz, n))) + dark[None]).astype(np.uint16)
+    raw[:, 0, 20] = 0                       # dead pixel of slice 0
+    raw[0:2, 0, 40] = 65535                 # hot pixel on two projections
+    r = tcp.Recon(n, nproj, nz, 31.5, dtype, "ramp", 3)
+    out = r.recon(*_to_dev(raw, flat, dark, theta)).float().cpu().numpy()
+    r.close()
+    assert np.isfinite(out).all()
+    ref = orc.recon(raw, flat, dark, theta, 31.5, "ramp", 3, "grid")
+    assert np.abs(ref[0]).max() > 1.0       # the damaged slice does leave the range fp16 storage is scaled for
+    check(out[1], ref[1], dtype, tag="partner slice")
 
 
 def test_empty_inputs_are_refused():
@@ -606,7 +642,7 @@ def test_detector_width_not_a_power_of_two(dtype, cfg, scale, lo, hi):
     scale_v = np.abs(ref).max()
     for z in range(len(rows)):
         if dtype == "f32":
-            assert rl2(out[z], ref[z]) < FP32_GATE, (z, rl2(out[z], ref[z]))
+            check(out[z], ref[z], "f32")
         else:
             assert rl2(out[z], ref[z]) < FP16_GATE_L2, (z, rl2(out[z], ref[z]))
             assert np.abs(out[z] - ref[z]).max() / scale_v < FP16_GATE_MAX
@@ -636,7 +672,7 @@ def test_detector_width_variants_pipeline_try_line_and_errors():
     ref = orc.recon_padded(raw[:, :7], flat[:7], dark[:7], theta, c, w.filter, 3, "grid")
     assert out_h.shape == (7, ndet, ndet)
     for z in range(7):
-        assert rl2(out_h[z].numpy(), ref[z]) < FP32_GATE
+        check(out_h[z].numpy(), ref[z], "f32")
     # try mode
     centers = [c - 2.0, c, c + 1.5]
     d = _to_dev(np.ascontiguousarray(raw[:, 3:4]), flat[3:4], dark[3:4], theta)
@@ -644,7 +680,7 @@ def test_detector_width_variants_pipeline_try_line_and_errors():
     assert t.shape == (3, ndet, ndet)
     for i, ci in enumerate(centers):
         ri = orc.recon_padded(raw[:, 3:4], flat[3:4], dark[3:4], theta, ci, w.filter, 3, "grid")[0]
-        assert rl2(t[i], ri) < FP32_GATE, (ci, rl2(t[i], ri))
+        check(t[i], ri, "f32")
     with pytest.raises(tcp.TcpError):
         r.recon_try(d[0], d[1], d[2], d[3], [float(ndet)])        # centre range is the caller's detector
     # LineRec
@@ -652,7 +688,7 @@ def test_detector_width_variants_pipeline_try_line_and_errors():
     o = r.recon(*_to_dev(np.ascontiguousarray(raw[:, :4]), flat[:4], dark[:4], theta)).cpu().numpy()
     rl = orc.recon_padded(raw[:, :4], flat[:4], dark[:4], theta, c, w.filter, 3, "lin")
     for z in range(4):
-        assert rl2(o[z], rl[z]) < FP32_GATE
+        check(o[z], rl[z], "f32")
     r.close()
     # a power of two: tcp_create_det == tcp_create_ex
     raw8, flat8, dark8, _ = _inputs(w, rows)
@@ -707,8 +743,9 @@ def test_pipeline_slice_ranges_equal_the_whole_volume():
 
 
 # ------------------------------------------------------------------ BASELINE full sizes, bench launch configuration
-@pytest.mark.parametrize("cfg,nz,tcfft", [("C4", 32, 0), ("C4", 32, 4), ("C5", 32, 0)])
-def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft):
+@pytest.mark.parametrize("cfg,nz,tcfft,where", [("C4", 32, 0, "mid"), ("C4", 32, 0, "first"), ("C4", 32, 0, "last"), ("C4", 32, 4, "mid"),
+                                                ("C5", 32, 0, "mid"), ("C5", 32, 0, "first"), ("C5", 32, 0, "last")])
+def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft, where):
     """C4 (2048^2, 2048 projections, fp16, one 32-slice chunk exactly as bench.py launches it: tcgen05
     gridding with 16 pairs per accumulator group) and C5 (4096^2, 4000 projections, M = 8192, off-centre,
     fp16 -> fp32 output).  Inputs are manufactured on the GPU (synthgen.make_counts_torch, frame averaging
@@ -717,7 +754,7 @@ def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft):
     DFT-as-GEMM on the tensor cores (opt-in, TCP_OPT_TCFFT; same gates)."""
     tcp = _tcp()
     w = sg.make_workload(cfg)
-    z0 = w.nz_total // 2 - nz // 2
+    z0 = {"mid": w.nz_total // 2 - nz // 2, "first": 0, "last": w.nz_total - nz}[where]
     rows = list(range(z0, z0 + nz))
     raw_d, ff, df = sg.make_counts_torch(w, rows, device="cuda")
     flat_d = torch.empty((nz, w.n), dtype=torch.float32, device="cuda")
@@ -732,7 +769,7 @@ def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft):
     torch.cuda.synchronize()
     out = out.float().cpu().numpy()
     r.close()
-    sample = sorted({0, 1, nz // 2, nz - 1})
+    sample = sorted({0, 1, nz // 2, nz - 1}) if where == "mid" else [0, nz - 1]     # first / last chunk: the stack's end slices (phantom edge, air rows)
     raw_h = raw_d.view(torch.int16)[:, sample].contiguous().cpu().numpy().view(np.uint16)
     ref = orc.recon(raw_h, flat_d[sample].cpu().numpy(), dark_d[sample].cpu().numpy(), theta, w.center, w.filter, 3, "grid")
     scale = np.abs(ref).max()
