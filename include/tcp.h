@@ -53,9 +53,11 @@ enum { TCP_WS_SINOGRAM = 0, TCP_WS_SPECTRUM = 1, TCP_WS_GRID = 2, TCP_WS_PASS1 =
  * default for TCP_F16 / TCP_F16_OUT32); GATHER: per-cell gather (atomics-free, slow; cross-check);
  * SCATTER_ATOMIC: fp32 atomics (TCP_F32 only; cross-check) */
 enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1, TCP_GRID_TILE = 2, TCP_GRID_MMA = 3 };
-/* TCP_OPT_TCFFT: bit mask of the transforms run as DFT-as-GEMM on the tensor cores (fp16 storage and
- * M = 4096 only; elsewhere the option must be 0): 1 = detector-row kernel (S3 + S4), 2 = column pass,
- * 4 = row pass of the inverse 2D transform.  Default: all that apply. */
+/* TCP_OPT_TCFFT: bit mask of the transforms whose radix-16 butterflies run on the tensor cores (warp-level
+ * mma.sync on fp16 operands, fp32 accumulation; fp16 storage and M = 4096 only, elsewhere the mask must be 0):
+ * 1 = detector-row kernel (S1..S4), 2 = column pass and 4 = row pass of the inverse 2D transform (these two
+ * switch together: 6).  Default: all that apply (7 at M = 4096 with fp16 storage, else 0); 0 = the fp32
+ * CUDA-core Stockham transforms.  Same stages and gates either way. */
 /* TCP_OPT_ALGORITHM ("--reconstruction-algorithm"): TCP_ALG_FOURIER = FourierRec, the
  * gridding path this library is about (default); TCP_ALG_LINE = LineRec, direct line summation with linear
  * interpolation (O(N^4)): S1-S3 as before, then the backprojection sum per pixel.
@@ -150,7 +152,7 @@ int tcp_normalize(tcp_ctx* ctx, const uint16_t* raw_u16, const float* flat, cons
  *   TCP_WS_SINOGRAM [nz][nproj][n] real; TCP_WS_SPECTRUM [npair][nproj][M] complex (FFT order,
  *   scaled by tcp_scale()); TCP_WS_GRID [npair][M l2][M l1] complex (or strip-major, tcp_grid_strip); TCP_WS_PASS1
  *   [npair][M/W][n iy][W l1] complex, W = min(32, max(2, 16384/M)) (the column pass works on strips of W
- *   columns and stores them contiguously); TCP_WS_TRIG [nproj] double2. */
+ *   columns and stores them contiguously), or row pairs (tcp_pass1_layout); TCP_WS_TRIG [nproj] double2. */
 int tcp_workspace(tcp_ctx* ctx, int which, void** ptr, size_t* bytes);
 /* Copy an intermediate into the caller's device buffer dst (>= the size tcp_workspace reports),
  * asynchronously on `stream` (tests only). */
@@ -158,6 +160,13 @@ int tcp_read_workspace(tcp_ctx* ctx, int which, void* dst, size_t dst_bytes, tcp
 /* Layout of TCP_WS_GRID: 0 = [npair][M l2][M l1]; W > 0 = strip-major [npair][M/W][M l2][W l1] (the
  * tensor-core gridding writes strips of W columns so that the column pass of S6 reads contiguously). */
 int tcp_grid_strip(const tcp_ctx* ctx);
+/* Layout of TCP_WS_PASS1: 0 = strips [npair][M/W][n iy][W l1]; 1 = row pairs [npair][n/2][M l1][2 rows] (the
+ * tensor-core transforms, TCP_OPT_TCFFT & 6). */
+int tcp_pass1_layout(const tcp_ctx* ctx);
+/* Test helper for the tensor-core transform itself: `batch` lines of 4096 half2 (re, im) -> 4096 float2 each,
+ * X[k] = sum_i x[i] e^{-/+ 2 pi i ik/4096} (inverse != 0: +, unnormalised), natural order on both sides.
+ * TCP_EUNSUPPORTED unless the context has fp16 storage and M = 4096. */
+int tcp_fft_lines(tcp_ctx* ctx, const void* in_half2, void* out_float2, int batch, int inverse, tcp_stream_t stream);
 /* Power-of-two factor by which SPECTRUM/GRID/PASS1 are scaled relative to S4's G (1 in fp32). */
 double tcp_scale(const tcp_ctx* ctx);
 /* Total device bytes the context allocated; kernels launched by one tcp_recon. */

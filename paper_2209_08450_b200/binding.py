@@ -21,7 +21,7 @@ EXPORTS = [
     "tcp_mean_frames_u16", "tcp_normalize", "tcp_workspace", "tcp_read_workspace", "tcp_scale", "tcp_grid_strip",
     "tcp_workspace_bytes", "tcp_launches_per_recon", "tcp_set_option", "tcp_profile_collect",
     "tcp_recon_volume_host", "tcp_recon_try", "tcp_create_det", "tcp_padded_n",
-    "tcp_recon_volume_host_rows", "tcp_slice_range", "tcp_check_angles",
+    "tcp_recon_volume_host_rows", "tcp_slice_range", "tcp_check_angles", "tcp_pass1_layout", "tcp_fft_lines",
 ]
 
 
@@ -87,6 +87,10 @@ def lib():
     L.tcp_check_angles.argtypes = [vp, ci]
     L.tcp_slice_range.restype = ci
     L.tcp_slice_range.argtypes = [ci, ci, ci, C.POINTER(ci), C.POINTER(ci)]
+    L.tcp_pass1_layout.restype = ci
+    L.tcp_pass1_layout.argtypes = [vp]
+    L.tcp_fft_lines.restype = ci
+    L.tcp_fft_lines.argtypes = [vp, vp, vp, ci, ci, vp]
     L.tcp_recon_try.restype = ci
     L.tcp_recon_try.argtypes = [vp, vp, vp, vp, vp, C.POINTER(cf), ci, vp, vp]
     _lib = L
@@ -250,7 +254,8 @@ class Recon:
         _check(lib().tcp_set_option(self.h, 3, {"fourier": 0, "line": 1}[name]))
 
     def set_tcfft(self, mask: int):
-        """TCP_OPT_TCFFT: which transforms run on the tensor cores (1 rows, 2 column pass, 4 row pass)."""
+        """TCP_OPT_TCFFT: which transforms run their butterflies on the tensor cores (1 rows, 6 = both passes of the
+        inverse 2D transform; default 7 where available: fp16 storage at M = 4096; 0 = fp32 CUDA-core transforms)."""
         _check(lib().tcp_set_option(self.h, 2, int(mask)))
 
     STAGES = ("trig", "normalize", "rows", "grid", "ifft_cols", "ifft_rows")
@@ -310,6 +315,16 @@ class Recon:
                                    out.data_ptr(), _stream(stream)))
         return out
 
+    def fft_lines(self, x_half2: torch.Tensor, inverse=False, stream=None) -> torch.Tensor:
+        """tcp_fft_lines: [batch][4096][2] half (re, im) -> [batch][4096] complex64 through the tensor-core transform."""
+        _dev(x_half2, torch.float16)
+        batch = x_half2.shape[0]
+        if tuple(x_half2.shape) != (batch, 4096, 2):
+            raise TcpError("expected shape (batch, 4096, 2)")
+        out = torch.empty((batch, 4096, 2), dtype=torch.float32, device=x_half2.device)
+        _check(lib().tcp_fft_lines(self.h, x_half2.data_ptr(), out.data_ptr(), batch, 1 if inverse else 0, _stream(stream)))
+        return torch.view_as_complex(out)
+
     def normalize(self, raw_u16, flat, dark, stream=None):
         raw_u16 = _as_u16(raw_u16)
         _dev(raw_u16, torch.uint16, (self.nproj, self.nz, self.n))
@@ -334,7 +349,9 @@ class Recon:
             w = int(lib().tcp_grid_strip(self.h))
             if w:       # strip-major [npair][M/w][M l2][w l1] -> [npair][M l2][M l1]
                 v = v.view(npair, M // w, M, w, 2).permute(0, 2, 1, 3, 4).reshape(npair, M, M, 2)
-        if name == "pass1":     # strip-major [npair][M/w][n iy][w l1] -> [npair][n iy][M l1]
+        if name == "pass1" and int(lib().tcp_pass1_layout(self.h)) == 1:   # row pairs [npair][n/2][M l1][2] -> [npair][n iy][M l1]
+            v = v.view(npair, n // 2, M, 2, 2).permute(0, 1, 3, 2, 4).reshape(npair, n, M, 2)
+        elif name == "pass1":   # strip-major [npair][M/w][n iy][w l1] -> [npair][n iy][M l1]
             w = min(32, max(2, 16384 // M))
             v = v.view(npair, M // w, n, w, 2).permute(0, 2, 1, 3, 4).reshape(npair, n, M, 2)
         return torch.complex(v[..., 0], v[..., 1])

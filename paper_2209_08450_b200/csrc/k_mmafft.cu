@@ -1,0 +1,381 @@
+// k_mmafft.cu -- the three transform kernels of the fp16 path at M = 4096 with their radix-16 butterflies on the
+// tensor cores (mmafft.cuh): S1+S2+S3+S4 per detector row (rows_mma_kernel), and the two passes of the inverse 2D
+// transform S6 with S7 fused (cols_mma_kernel, irows_mma_kernel).  Same stages, tables and layouts at the HBM
+// boundaries as k_rows.cu / k_ifft2.cu except the pass-1 array, which holds ROW PAIRS here:
+//   pass1[pair][iy / 2][l1][iy % 2]   (half2)
+// so that the column pass stores 32 contiguous bytes per thread (4 columns x 2 rows) and the row pass, which
+// transforms rows iy and iy + 1 in one CTA, loads both with one 8-byte access per element.
+#include <math.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "mmafft.cuh"
+#include "umma.cuh"
+#include "tcp_internal.h"
+
+namespace tcpk {
+
+using namespace mf;
+
+static const double kPiM = 3.14159265358979323846264338327950288;
+
+// ------------------------------------------------------------------------------------------------ tables (host, fp64)
+static int inmap(int variant, int q) {                   // input digit held in K slot q' (mmafft.cuh "MMA mapping")
+    if (variant == AV_NAT) return q;
+    const int c = q & 3, i = q >> 2;                     // pass 3 loads digits (2c, 2c+1) and (8+2c, 9+2c) as 8-byte pairs
+    return (i & 1) + 2 * c + 8 * (i >> 1);
+}
+static int outmap(int variant, int t, int r) {           // output digit of tile t, row r (re) and r + 8 (im)
+    if (variant == AV_LOC) return t == 0 ? (r < 4 ? r : r + 8) : r + 4;
+    return r + 8 * t;
+}
+static void build_atab(std::vector<uint32_t>& tab) {
+    tab.assign(ATAB_WORDS, 0u);
+    auto h16 = [](double v) { return (uint32_t)__half_as_ushort(__float2half_rn((float)v)); };
+    for (int v = 0; v < AV_COUNT; ++v)
+        for (int lane = 0; lane < 32; ++lane) {
+            const int g = lane >> 2, c = lane & 3;
+            for (int t = 0; t < 2; ++t)
+                for (int s = 0; s < 2; ++s)
+                    for (int r = 0; r < 4; ++r) {
+                        const int row = g + 8 * (r & 1);                    // tile row
+                        const int q = 8 * s + c + 4 * (r >> 1);             // K slot: columns 2q (re), 2q + 1 (im)
+                        const int o = outmap(v, t, row & 7), j = inmap(v, q);
+                        const double a = 2.0 * kPiM * (double)((o * j) & 15) / 16.0;
+                        const double fr = GAMMA * cos(a), fi = -GAMMA * sin(a);   // W_16^(o j) = fr + i fi
+                        // re row: (fr, -fi) . (x_re, x_im); im row: (fi, fr)
+                        const double e0 = row < 8 ? fr : fi, e1 = row < 8 ? -fi : fr;
+                        tab[((size_t)v * 32 + lane) * 16 + t * 8 + s * 4 + r] = h16(e0) | (h16(e1) << 16);
+                    }
+        }
+}
+
+int mmafft_setup(tcp_ctx* c) {
+    c->mf_ok = 0;
+    if (!c->half_store || c->M != N) return TCP_OK;
+    std::vector<uint32_t> tab;
+    build_atab(tab);
+    TCP_CUDA_CHECK(cudaMalloc((void**)&c->mf_atab, tab.size() * sizeof(uint32_t)));
+    TCP_CUDA_CHECK(cudaMemcpy(c->mf_atab, tab.data(), tab.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    c->bytes += tab.size() * sizeof(uint32_t);
+    c->mf_ok = TCP_TCFFT_ROWS | TCP_TCFFT_COLS | TCP_TCFFT_IROWS;
+    return TCP_OK;
+}
+void mmafft_free(tcp_ctx* c) { cudaFree(c->mf_atab); }
+
+// The filtered row rides fp16 operands between the transforms: Q = H P is stored as 2^12 (H / M) P (typical
+// magnitude 1) and the factor is undone in the phase table.
+constexpr float kRowScale = 4096.f;
+
+// ------------------------------------------------------------------------------------------------ detector rows
+template <bool PAD_EDGE, bool RAW>
+__global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restrict__ sino, __half2* __restrict__ spec,
+                                                          const float2* __restrict__ tw, const uint32_t* __restrict__ atab,
+                                                          const float* __restrict__ hfilt, const float2* __restrict__ ptab, int nproj,
+                                                          int nz, int try_mode, const float* __restrict__ wq,
+                                                          const uint16_t* __restrict__ raw, const float2* __restrict__ fdtab, int nunits) {
+    constexpr int n = N / 2;
+    extern __shared__ __align__(16) uint32_t L[];
+    float2* T1TAB = reinterpret_cast<float2*>(L + 1 * N);               // pass-1 twiddle table behind the lines
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, c = lane & 3;
+    // persistent CTAs: the thread's butterfly fragments and twiddles (scattered table reads) are set up once
+    AFrag An, Al;
+    load_afrag(An, atab, AV_NAT, lane);
+    load_afrag(Al, atab, AV_LO, lane);
+    Twid T;
+    load_twid(T, T1TAB, tw, warp, g, c, (float)(1.0 / GAMMA), (float)(1.0 / (GAMMA * GAMMA)));
+    __syncwarp();
+    auto from_line = [&](int k) { return L[swz<1>(k)]; };
+    const float2* ptab0 = ptab;
+#pragma unroll 1
+    for (int unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
+    const int j = unit % nproj, pair = unit / nproj;
+    const int zA = try_mode ? 0 : 2 * pair, zB = try_mode ? nz : 2 * pair + 1;
+    const bool hasB = zB < nz;
+    const int zBs = hasB ? zB : zA;
+    ptab = try_mode ? ptab0 + (size_t)pair * N : ptab0;
+    const float wj = wq ? __ldg(&wq[j]) : 1.f;
+
+    // ---- stage the two rows as half2 (pA, pB): 8 detector pixels per thread, 128-bit loads
+    {
+        const int i0 = tid * 8;
+        float a[8], b[8];
+        if constexpr (RAW) {
+            const uint4 ra = __ldg(reinterpret_cast<const uint4*>(raw + ((size_t)j * nz + zA) * n + i0));
+            const uint4 rb = __ldg(reinterpret_cast<const uint4*>(raw + ((size_t)j * nz + zBs) * n + i0));
+            const unsigned ua[4] = {ra.x, ra.y, ra.z, ra.w}, ub[4] = {rb.x, rb.y, rb.z, rb.w};
+            const float4* fa = reinterpret_cast<const float4*>(fdtab + (size_t)zA * n + i0);
+            const float4* fb = reinterpret_cast<const float4*>(fdtab + (size_t)zBs * n + i0);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float4 da = __ldg(fa + q), db = __ldg(fb + q);      // (rcp, dark) of pixels 2q, 2q + 1
+                // S1+S2 with the arithmetic of normalize_half_kernel (tcp_internal.h), rounded to the storage type
+                a[2 * q] = -0.69314718055994531f * fast_lg2(fmaxf((u16f(ua[q] & 0xffffu) - da.y) * da.x, 1e-6f));
+                a[2 * q + 1] = -0.69314718055994531f * fast_lg2(fmaxf((u16f(ua[q] >> 16) - da.w) * da.z, 1e-6f));
+                b[2 * q] = -0.69314718055994531f * fast_lg2(fmaxf((u16f(ub[q] & 0xffffu) - db.y) * db.x, 1e-6f));
+                b[2 * q + 1] = -0.69314718055994531f * fast_lg2(fmaxf((u16f(ub[q] >> 16) - db.w) * db.z, 1e-6f));
+            }
+#pragma unroll
+            for (int q = 0; q < 8; ++q) { a[q] = __half2float(__float2half_rn(a[q])); b[q] = __half2float(__float2half_rn(b[q])); }
+        } else {
+            const uint4 ha = __ldg(reinterpret_cast<const uint4*>(sino + ((size_t)zA * nproj + j) * n + i0));
+            const uint4 hb = __ldg(reinterpret_cast<const uint4*>(sino + ((size_t)zBs * nproj + j) * n + i0));
+            const unsigned ua[4] = {ha.x, ha.y, ha.z, ha.w}, ub[4] = {hb.x, hb.y, hb.z, hb.w};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float2 fa = __half22float2(*reinterpret_cast<const __half2*>(&ua[q])), fb = __half22float2(*reinterpret_cast<const __half2*>(&ub[q]));
+                a[2 * q] = fa.x; a[2 * q + 1] = fa.y; b[2 * q] = fb.x; b[2 * q + 1] = fb.y;
+            }
+        }
+        uint32_t w[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) w[q] = pack_h2(a[q] * wj, hasB ? b[q] * wj : 0.f);
+        uint4* dst = reinterpret_cast<uint4*>(&L[swz<1>(i0)]);
+        dst[0] = make_uint4(w[0], w[1], w[2], w[3]);
+        dst[1] = make_uint4(w[4], w[5], w[6], w[7]);
+    }
+    __syncthreads();
+    if constexpr (PAD_EDGE) {     // padding samples of the filter stage: the nearest edge of the periodic row
+        const uint32_t last = L[swz<1>(n - 1)], first = L[swz<1>(0)];
+        const uint32_t v = tid < NT / 2 ? last : first;
+        uint4* dst = reinterpret_cast<uint4*>(&L[swz<1>(n + tid * 8)]);
+        dst[0] = make_uint4(v, v, v, v);
+        dst[1] = make_uint4(v, v, v, v);
+        __syncthreads();
+    }
+
+    // ---- transform 1: spectrum of the padded row, times 2^12 H / M
+    pass1<1, false, !PAD_EDGE, false>(L, An, T, warp, g, c, from_line);
+    __syncthreads();
+    pass2<1, false>(L, An, T, warp, g, c);
+    __syncthreads();
+    pass3<1, false, false, true>(L, Al, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
+        const float2 h = __ldg(reinterpret_cast<const float2*>(hfilt + k0));
+        const float h0 = h.x * kRowScale, h1 = h.y * kRowScale;
+        *reinterpret_cast<uint2*>(&L[swz<1>(k0)]) = make_uint2(pack_h2(y0[0].x * h0, y0[0].y * h0), pack_h2(y1[0].x * h1, y1[0].y * h1));
+    });
+    __syncthreads();
+    // ---- transform 2 (inverse): the filtered row, cropped to the detector (only tile 0 = samples below n is computed)
+    flip_afrag(An);
+    flip_afrag(Al);
+    pass1<1, true, false, false>(L, An, T, warp, g, c, from_line);
+    __syncthreads();
+    pass2<1, true>(L, An, T, warp, g, c);
+    __syncthreads();
+    pass3<1, true, false, true>(L, Al, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
+        *reinterpret_cast<uint2*>(&L[swz<1>(k0)]) = make_uint2(pack_h2(y0[0].x, y0[0].y), pack_h2(y1[0].x, y1[0].y));
+    });
+    __syncthreads();
+    // ---- transform 3: spectrum of the zero-padded filtered row, centre phase and scale on store
+    flip_afrag(An);
+    flip_afrag(Al);
+    pass1<1, false, true, false>(L, An, T, warp, g, c, from_line);
+    __syncthreads();
+    pass2<1, false>(L, An, T, warp, g, c);
+    __syncthreads();
+    __half2* out = spec + ((size_t)pair * nproj + j) * N;
+    pass3<1, false, false, false>(L, Al, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
+        const float4 p = __ldg(reinterpret_cast<const float4*>(ptab + k0));
+        const float s = 1.f / kRowScale;
+        const float2 v0 = make_float2((y0[0].x * p.x - y0[0].y * p.y) * s, (y0[0].x * p.y + y0[0].y * p.x) * s);
+        const float2 v1 = make_float2((y1[0].x * p.z - y1[0].y * p.w) * s, (y1[0].x * p.w + y1[0].y * p.z) * s);
+        *reinterpret_cast<uint2*>(out + k0) = make_uint2(pack_h2(v0.x, v0.y), pack_h2(v1.x, v1.y));
+    });
+    __syncthreads();                      // the line is free for the next unit's rows
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ column pass of S6
+// One CTA = one strip of 4 adjacent columns of the strip-major grid [pair][M/4][M l2][4 l1]: a thread's 16-byte load is
+// the 4 columns of one row, the team transforms the 4 columns with shared twiddles, and only the central n outputs are
+// computed in the last pass (tile 0 of the AV_LOC fragments).
+__global__ void __launch_bounds__(NT, 2) cols_mma_kernel(const uint4* __restrict__ grid, uint2* __restrict__ p1arr,
+                                                          const float2* __restrict__ tw, const uint32_t* __restrict__ atab, int nunits) {
+    constexpr int n = N / 2;
+    extern __shared__ __align__(16) uint32_t L[];
+    float2* T1TAB = reinterpret_cast<float2*>(L + 4 * N);               // pass-1 twiddle table behind the lines
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, c = lane & 3;
+    AFrag An, Ac;
+    load_afrag(An, atab, AV_NAT, lane);
+    flip_afrag(An);
+    load_afrag(Ac, atab, AV_LOC, lane);
+    flip_afrag(Ac);
+    Twid T;
+    load_twid(T, T1TAB, tw, warp, g, c, (float)(1.0 / GAMMA), (float)(1.0 / (GAMMA * GAMMA)));
+    __syncwarp();
+#pragma unroll 1
+    for (int unit = blockIdx.x; unit < nunits; unit += gridDim.x) {       // unit = pair (N / 4) + strip: consecutive blocks of the grid
+    const int strip = unit % (N / 4), pair = unit / (N / 4);
+    const uint4* src = grid + (size_t)unit * N;
+    pass1<4, true, false, true>(L, An, T, warp, g, c, [&](int k) { return __ldg(src + k); });
+    if (unit + (int)gridDim.x < nunits) {        // the next unit of this CTA: a contiguous 64 KB block, 2 cache lines per thread
+        const char* nx = reinterpret_cast<const char*>(src + (size_t)gridDim.x * N) + tid * 256;
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(nx));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(nx + 128));
+    }
+    __syncthreads();
+    pass2<4, true>(L, An, T, warp, g, c);
+    __syncthreads();
+    uint2* dst = p1arr + (size_t)pair * (n / 2) * N + 4 * strip;
+    pass3<4, true, true, false>(L, Ac, warp, g, c, [&](int k0, const float2(&y0)[4], const float2(&y1)[4]) {
+        const int iy0 = k0 < n / 2 ? k0 + n / 2 : k0 - (N - n / 2);       // even; rows iy0 and iy0 + 1 are one pair
+        uint4* d = reinterpret_cast<uint4*>(dst + (size_t)(iy0 >> 1) * N);
+        d[0] = make_uint4(pack_h2(y0[0].x, y0[0].y), pack_h2(y1[0].x, y1[0].y), pack_h2(y0[1].x, y0[1].y), pack_h2(y1[1].x, y1[1].y));
+        d[1] = make_uint4(pack_h2(y0[2].x, y0[2].y), pack_h2(y1[2].x, y1[2].y), pack_h2(y0[3].x, y0[3].y), pack_h2(y1[3].x, y1[3].y));
+    });
+    __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ row pass of S6 + S7
+__device__ __forceinline__ void st_out2(__half* p, float a, float b) { *reinterpret_cast<uint32_t*>(p) = pack_h2(a, b); }
+__device__ __forceinline__ void st_out2(float* p, float a, float b) { *reinterpret_cast<float2*>(p) = make_float2(a, b); }
+
+// The next unit's row pair (a contiguous 32 KB block of the pass-1 array) arrives by bulk asynchronous copies (TMA) in a
+// staging buffer while the current one is in passes 2 and 3: 16 blocks of 256 elements, each followed by 4 elements
+// (32 bytes) of padding, which makes the stride-256 reads of pass 1 bank-conflict free.
+constexpr int IROWS_BLK = 256 * 8 + 32;
+constexpr int IROWS_STAGE = 16 * IROWS_BLK;
+
+template <class TO>
+__global__ void __launch_bounds__(NT, 2) irows_mma_kernel(const uint2* __restrict__ p1arr, TO* __restrict__ out,
+                                                           const float2* __restrict__ tw, const uint32_t* __restrict__ atab,
+                                                           const float* __restrict__ deax, const float* __restrict__ deay, int nz, int nunits) {
+    constexpr int n = N / 2;
+    extern __shared__ __align__(16) uint32_t L[];
+    float2* T1TAB = reinterpret_cast<float2*>(L + 2 * N);               // pass-1 twiddle table behind the lines
+    unsigned char* S = reinterpret_cast<unsigned char*>(L + 2 * N) + T1_BYTES;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(S + IROWS_STAGE);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, c = lane & 3;
+    auto fetch = [&](int unit) {                                          // thread 0 only
+        mbar_expect_tx(bar, 2 * N * 4);
+        const unsigned char* src = reinterpret_cast<const unsigned char*>(p1arr + (size_t)unit * N);
+#pragma unroll 1
+        for (int b = 0; b < 16; ++b) bulk_g2s(S + b * IROWS_BLK, src + b * 2048, 2048, bar);
+    };
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        fence_mbar_init();
+    }
+    __syncthreads();
+    if (tid == 0 && (int)blockIdx.x < nunits) fetch(blockIdx.x);
+    AFrag An, Ac;
+    load_afrag(An, atab, AV_NAT, lane);
+    flip_afrag(An);
+    load_afrag(Ac, atab, AV_LOC, lane);
+    flip_afrag(Ac);
+    Twid T;
+    load_twid(T, T1TAB, tw, warp, g, c, (float)(1.0 / GAMMA), (float)(1.0 / (GAMMA * GAMMA)));
+    __syncwarp();
+    uint32_t phase = 0;
+#pragma unroll 1
+    for (int unit = blockIdx.x; unit < nunits; unit += gridDim.x) {       // unit = pair (n / 2) + row pair rp: rows iy = 2 rp, 2 rp + 1
+    const int rp = unit % (n / 2), pair = unit / (n / 2);
+    mbar_wait(bar, phase);
+    phase ^= 1;
+    pass1<2, true, false, false>(L, An, T, warp, g, c, [&](int k) { return *reinterpret_cast<const uint2*>(S + (k >> 8) * IROWS_BLK + (k & 255) * 8); });
+    __syncthreads();                      // the staging buffer is free, the lines are complete
+    if (tid == 0 && unit + (int)gridDim.x < nunits) {
+        fence_proxy_async();
+        fetch(unit + gridDim.x);
+    }
+    pass2<2, true>(L, An, T, warp, g, c);
+    __syncthreads();
+    const int zA = 2 * pair, zB = 2 * pair + 1;
+    const bool hasB = zB < nz;
+    const float dy0 = __ldg(&deay[2 * rp]), dy1 = __ldg(&deay[2 * rp + 1]);
+    TO* oA = out + ((size_t)zA * n + 2 * rp) * n;
+    TO* oB = out + ((size_t)zB * n + 2 * rp) * n;
+    pass3<2, true, true, false>(L, Ac, warp, g, c, [&](int k0, const float2(&y0)[2], const float2(&y1)[2]) {
+        const int ix = k0 < n / 2 ? k0 + n / 2 : k0 - (N - n / 2);
+        const float2 dx = __ldg(reinterpret_cast<const float2*>(deax + ix));
+#pragma unroll
+        for (int l = 0; l < 2; ++l) {
+            const float d0 = (l ? dy1 : dy0) * dx.x, d1 = (l ? dy1 : dy0) * dx.y;
+            st_out2(oA + (size_t)l * n + ix, y0[l].x * d0, y1[l].x * d1);
+            if (hasB) st_out2(oB + (size_t)l * n + ix, y0[l].y * d0, y1[l].y * d1);
+        }
+    });
+    __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ test helper
+// batch lines of N half2 -> N float2, natural order both sides (tcp_fft_lines)
+template <bool INV>
+__global__ void __launch_bounds__(NT, 2) fft_lines_kernel(const uint32_t* __restrict__ in, float2* __restrict__ out,
+                                                           const float2* __restrict__ tw, const uint32_t* __restrict__ atab) {
+    extern __shared__ __align__(16) uint32_t L[];
+    float2* T1TAB = reinterpret_cast<float2*>(L + 1 * N);               // pass-1 twiddle table behind the lines
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, c = lane & 3;
+    const uint32_t* src = in + (size_t)blockIdx.x * N;
+    float2* dst = out + (size_t)blockIdx.x * N;
+    AFrag An, Al;
+    load_afrag(An, atab, AV_NAT, lane);
+    load_afrag(Al, atab, AV_LO, lane);
+    if (INV) { flip_afrag(An); flip_afrag(Al); }
+    Twid T;
+    load_twid(T, T1TAB, tw, warp, g, c, (float)(1.0 / GAMMA), (float)(1.0 / (GAMMA * GAMMA)));
+    __syncwarp();
+    pass1<1, INV, false, true>(L, An, T, warp, g, c, [&](int k) { return __ldg(src + k); });
+    __syncthreads();
+    pass2<1, INV>(L, An, T, warp, g, c);
+    __syncthreads();
+    pass3<1, false, false, false>(L, Al, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
+        *reinterpret_cast<float4*>(dst + k0) = make_float4(y0[0].x, y0[0].y, y1[0].x, y1[0].y);
+    });
+}
+
+// ------------------------------------------------------------------------------------------------ launchers
+int launch_rows_mma(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw) {
+    const size_t smem = (size_t)N * 4 + T1_BYTES;
+    auto kern = raw ? (c->pad ? rows_mma_kernel<true, true> : rows_mma_kernel<false, true>)
+                    : (c->pad ? rows_mma_kernel<true, false> : rows_mma_kernel<false, false>);
+    TCP_SMEM(kern, smem);
+    const int nunits = c->nproj * c->npair;
+    kern<<<std::min(nunits, 2 * c->nsm), NT, smem, st>>>((const __half*)c->sino, (__half2*)c->spec, c->tw, c->mf_atab, c->hfilt,
+                                                         c->try_ptab ? c->try_ptab : c->ptab, c->nproj, c->nz, c->try_ptab ? 1 : 0,
+                                                         c->angle_weights ? c->wq : nullptr, raw, c->fdtab, nunits);
+    TCP_CUDA_CHECK(cudaGetLastError());
+    return TCP_OK;
+}
+
+int launch_cols_mma(const tcp_ctx* c, cudaStream_t st) {
+    const size_t smem = (size_t)4 * N * 4 + T1_BYTES;
+    TCP_SMEM(cols_mma_kernel, smem);
+    const int nunits = (N / 4) * c->npair;
+    cols_mma_kernel<<<std::min(nunits, 2 * c->nsm), NT, smem, st>>>((const uint4*)c->grid, (uint2*)c->pass1, c->tw, c->mf_atab, nunits);
+    TCP_CUDA_CHECK(cudaGetLastError());
+    return TCP_OK;
+}
+
+int launch_irows_mma(const tcp_ctx* c, void* out, cudaStream_t st) {
+    const size_t smem = (size_t)2 * N * 4 + T1_BYTES + IROWS_STAGE + 16;
+    const int nunits = (N / 4) * c->npair;
+    const int grid = std::min(nunits, 2 * c->nsm);
+    if (c->half_out) {
+        TCP_SMEM(irows_mma_kernel<__half>, smem);
+        irows_mma_kernel<__half><<<grid, NT, smem, st>>>((const uint2*)c->pass1, (__half*)out, c->tw, c->mf_atab, c->deax, c->deay, c->nz, nunits);
+    } else {
+        TCP_SMEM(irows_mma_kernel<float>, smem);
+        irows_mma_kernel<float><<<grid, NT, smem, st>>>((const uint2*)c->pass1, (float*)out, c->tw, c->mf_atab, c->deax, c->deay, c->nz, nunits);
+    }
+    TCP_CUDA_CHECK(cudaGetLastError());
+    return TCP_OK;
+}
+
+int launch_fft_lines(const tcp_ctx* c, const void* in, void* out, int batch, int inverse, cudaStream_t st) {
+    const size_t smem = (size_t)N * 4 + T1_BYTES;
+    if (inverse) {
+        TCP_SMEM(fft_lines_kernel<true>, smem);
+        fft_lines_kernel<true><<<batch, NT, smem, st>>>((const uint32_t*)in, (float2*)out, c->tw, c->mf_atab);
+    } else {
+        TCP_SMEM(fft_lines_kernel<false>, smem);
+        fft_lines_kernel<false><<<batch, NT, smem, st>>>((const uint32_t*)in, (float2*)out, c->tw, c->mf_atab);
+    }
+    TCP_CUDA_CHECK(cudaGetLastError());
+    return TCP_OK;
+}
+
+}  // namespace tcpk

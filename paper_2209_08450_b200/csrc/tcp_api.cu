@@ -11,7 +11,6 @@
 #include <mutex>
 #include <vector>
 
-#include "tcfft.cuh"
 #include "tcp_internal.h"
 
 namespace tcpk {
@@ -146,21 +145,9 @@ static int build_context(tcp_ctx* c) {
     if ((rc = upload(&c->deax, dx, &c->bytes))) return rc;
     if ((rc = upload(&c->deay, dy, &c->bytes))) return rc;
 
-    if (c->tcfft_ok) {
-        std::vector<__half> am;
-        tcfft::build_tables(am);
-        __half* dam = nullptr;
-        if ((rc = upload(&dam, am, &c->bytes))) return rc;
-        c->tc_amat = dam;
-        std::vector<float> hs(M);
-        std::vector<float2> ps(M);
-        for (int k = 0; k < M; ++k) {
-            hs[k] = hf[k] * 64.f;
-            ps[k] = make_float2(pt[k].x / 64.f, pt[k].y / 64.f);
-        }
-        if ((rc = upload(&c->tc_hfilt, hs, &c->bytes))) return rc;
-        if ((rc = upload(&c->tc_ptab, ps, &c->bytes))) return rc;
-    }
+    if ((rc = mmafft_setup(c))) return rc;
+    c->tcfft_ok = c->mf_ok;
+    c->tcfft = c->tcfft_ok;      // default: every transform that can runs its butterflies on the tensor cores
 
     // gather tiles, heaviest (closest to DC) first: sample density falls as 1/radius
     const int T = 16, tx = M / T;
@@ -184,6 +171,14 @@ static int build_context(tcp_ctx* c) {
     c->ntiles = (int)order.size();
     if ((rc = upload(&c->tile_order, order, &c->bytes))) return rc;
     return grid_tile_setup(c);
+}
+
+// which transforms take the tensor-core butterflies (TCP_OPT_TCFFT; k_mmafft.cu): the row kernel unless the uncropped
+// filter option is on; the two passes of S6 together (they share the row-pair layout of the pass-1 array) when the
+// grid is strip-major with strips of 4 columns, i.e. written by the tensor-core gridding
+static bool rows_on_mma(const tcp_ctx* c) { return (c->tcfft & TCP_TCFFT_ROWS) && !(c->filter_fused && !c->try_ptab); }
+static bool ifft2_on_mma(const tcp_ctx* c) {
+    return (c->tcfft & (TCP_TCFFT_COLS | TCP_TCFFT_IROWS)) == (TCP_TCFFT_COLS | TCP_TCFFT_IROWS) && c->grid_strip == 4;
 }
 
 // tcp_recon_try: candidate centres of up to kMax / 2 pairs by value (a negative entry = no slice B in the last pair)
@@ -252,8 +247,6 @@ static tcp_ctx* create_impl(int n, int ndet, int pad_l, int nproj, int nz_chunk,
     c->grid_strip = (c->grid_impl == TCP_GRID_MMA) ? cols_strip_width(c->M) : 0;
     cudaGetDevice(&c->device);
     cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, c->device);
-    c->tcfft_ok = (c->half_store && c->M == 4096) ? TCP_TCFFT_IROWS : 0;
-    c->tcfft = 0;   // measured slower than the CUDA-core transforms: opt-in through TCP_OPT_TCFFT
     int rc_pad = TCP_OK;
     if (ndet != n) rc_pad = dev_alloc(&c->out_pad, (size_t)nz_chunk * n * n * (c->half_out ? 2 : 4), &c->bytes);
     if (rc_pad != TCP_OK || build_context(c) != TCP_OK || setup_kernel_attributes(c) != TCP_OK) {
@@ -299,7 +292,7 @@ void tcp_destroy(tcp_ctx* c) {
     cudaFree(c->tile_order);
     cudaFree(c->try_buf);
     cudaFree(c->out_pad);
-    cudaFree(c->tc_amat); cudaFree(c->tc_hfilt); cudaFree(c->tc_ptab);
+    mmafft_free(c);
     grid_tile_free(c);
     free(c);
 }
@@ -339,16 +332,18 @@ int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* d
         TCP_MARK(6);
         return TCP_OK;
     }
-    if ((rc = fused_s12 ? launch_rows(c, st, raw, flat, dark) : launch_rows(c, st))) return rc;
+    if (rows_on_mma(c)) rc = launch_rows_mma(c, st, fused_s12 ? raw : nullptr);
+    else rc = fused_s12 ? launch_rows(c, st, raw, flat, dark) : launch_rows(c, st);
+    if (rc) return rc;
     TCP_MARK(3);
     if (c->grid_impl == TCP_GRID_SCATTER_ATOMIC) rc = launch_grid_scatter(c, st);
     else if (c->grid_impl == TCP_GRID_GATHER) rc = launch_grid_gather(c, theta, st);
     else rc = launch_grid_tile(c, theta, st);
     if (rc) return rc;
     TCP_MARK(4);
-    if ((rc = launch_ifft_cols(c, st))) return rc;
+    if ((rc = ifft2_on_mma(c) ? launch_cols_mma(c, st) : launch_ifft_cols(c, st))) return rc;
     TCP_MARK(5);
-    if ((rc = (c->tcfft & TCP_TCFFT_IROWS) ? launch_ifft_rows_tc(c, out, st) : launch_ifft_rows(c, out, st))) return rc;
+    if ((rc = ifft2_on_mma(c) ? launch_irows_mma(c, out, st) : launch_ifft_rows(c, out, st))) return rc;
     if (c->out_pad && (rc = launch_crop_out(c, c->nz, user_out, st))) return rc;
     TCP_MARK(6);
 #undef TCP_MARK
@@ -385,14 +380,13 @@ int tcp_recon_try(tcp_ctx* c, const uint16_t* raw, const float* flat, const floa
     if ((rc = launch_normalize(&one, raw, flat, dark, st))) return rc;
     tcp_ctx t = *c;                   // ncenter output "slices"
     t.nz = ncenter; t.npair = npair; t.try_ptab = c->try_buf;
-    t.tcfft = 0;
-    if ((rc = launch_rows(&t, st))) return rc;
+    if ((rc = rows_on_mma(&t) ? launch_rows_mma(&t, st, nullptr) : launch_rows(&t, st))) return rc;
     if (c->grid_impl == TCP_GRID_SCATTER_ATOMIC) rc = launch_grid_scatter(&t, st);
     else if (c->grid_impl == TCP_GRID_GATHER) rc = launch_grid_gather(&t, theta, st);
     else rc = launch_grid_tile(&t, theta, st);
     if (rc) return rc;
-    if ((rc = launch_ifft_cols(&t, st))) return rc;
-    if ((rc = launch_ifft_rows(&t, c->out_pad ? c->out_pad : out, st))) return rc;
+    if ((rc = ifft2_on_mma(&t) ? launch_cols_mma(&t, st) : launch_ifft_cols(&t, st))) return rc;
+    if ((rc = ifft2_on_mma(&t) ? launch_irows_mma(&t, c->out_pad ? c->out_pad : out, st) : launch_ifft_rows(&t, c->out_pad ? c->out_pad : out, st))) return rc;
     return c->out_pad ? launch_crop_out(c, ncenter, out, st) : TCP_OK;
 }
 
@@ -452,6 +446,12 @@ int tcp_read_workspace(tcp_ctx* c, int which, void* dst, size_t dst_bytes, tcp_s
 }
 
 double tcp_scale(const tcp_ctx* c) { return c ? c->scale : 0.0; }
+int tcp_pass1_layout(const tcp_ctx* c) { return c && ifft2_on_mma(c) ? 1 : 0; }
+int tcp_fft_lines(tcp_ctx* c, const void* in_half2, void* out_float2, int batch, int inverse, tcp_stream_t stream) {
+    if (!c || !in_half2 || !out_float2 || batch < 1) return set_error(TCP_EINVAL, "bad argument");
+    if (!c->mf_ok) return set_error(TCP_EUNSUPPORTED, "tensor-core transforms need fp16 storage and M = 4096");
+    return launch_fft_lines(c, in_half2, out_float2, batch, inverse, (cudaStream_t)stream);
+}
 int tcp_grid_strip(const tcp_ctx* c) { return c ? c->grid_strip : 0; }
 size_t tcp_workspace_bytes(const tcp_ctx* c) { return c ? c->bytes : 0; }
 
@@ -493,6 +493,8 @@ int tcp_set_option(tcp_ctx* c, int option, int value) {
     }
     if (option == TCP_OPT_TCFFT) {
         if (value & ~c->tcfft_ok) return set_error(TCP_EUNSUPPORTED, "tensor-core transforms %d not available here (mask %d)", value, c->tcfft_ok);
+        if (((value & TCP_TCFFT_COLS) != 0) != ((value & TCP_TCFFT_IROWS) != 0))
+            return set_error(TCP_EINVAL, "the two passes of the inverse 2D transform switch together (mask 6)");
         c->tcfft = value;
         return TCP_OK;
     }

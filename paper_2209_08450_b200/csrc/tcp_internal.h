@@ -22,8 +22,10 @@ struct tcp_ctx {
     int algorithm;        // TCP_ALG_FOURIER (gridding, default) | TCP_ALG_LINE (direct line summation)
     int grid_strip;       // 0: grid rows are contiguous; W > 0: strip-major [pair][M/W][M l2][W l1] (tcgen05 gridding)
     int device, nsm;      // CUDA device and its SM count
-    int tcfft;            // TCP_TCFFT_* mask of transforms on the tensor cores (k_tcfft.cu)
-    int tcfft_ok;         // the mask this context supports
+    int tcfft;            // TCP_TCFFT_* mask of transforms whose butterflies run on the tensor cores (k_mmafft.cu)
+    int tcfft_ok;         // the mask this context supports (fp16 storage, M = 4096)
+    int mf_ok;            // = tcfft_ok, set by mmafft_setup
+    uint32_t* mf_atab;    // mmafft.cuh: butterfly-matrix fragments [variant][lane][16]
     // workspaces (device)
     void* sino;           // [nz][nproj][n]      float | half
     void* spec;           // [npair][nproj][M]   float2 | half2   (S * G of stage S4, FFT order)
@@ -43,9 +45,6 @@ struct tcp_ctx {
     float2* try_buf;      // its device storage, [ceil(nz/2)][M], allocated on first use
     float* deax;          // [n] 1 / (S * Phi(x))
     float* deay;          // [n] 1 / Phi(y)
-    void* tc_amat;        // tcfft.cuh: DFT-64 matrix, 128 x 128 half in operand block order
-    float* tc_hfilt;      // [M] 2^6 H[k] / M   (the filtered row rides fp16 operands: keep it off the subnormals)
-    float2* tc_ptab;      // [M] ptab / 2^6
     int* tile_order;      // gather gridding: tiles sorted by decreasing work
     int ntiles;
     // tile gridding (k_grid_tile.cu): work items, split-tile reduce list, partial tiles, per-call plan
@@ -109,7 +108,12 @@ void grid_tile_free(tcp_ctx* c);
 int launch_ifft_cols(const tcp_ctx* c, cudaStream_t st);
 int cols_strip_width(int M);
 int launch_ifft_rows(const tcp_ctx* c, void* out, cudaStream_t st);
-int launch_ifft_rows_tc(const tcp_ctx* c, void* out, cudaStream_t st);
+int mmafft_setup(tcp_ctx* c);
+void mmafft_free(tcp_ctx* c);
+int launch_rows_mma(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw);
+int launch_cols_mma(const tcp_ctx* c, cudaStream_t st);
+int launch_irows_mma(const tcp_ctx* c, void* out, cudaStream_t st);
+int launch_fft_lines(const tcp_ctx* c, const void* in, void* out, int batch, int inverse, cudaStream_t st);
 int launch_crop_out(const tcp_ctx* c, int nslices, void* out, cudaStream_t st);
 int launch_mean_frames(const uint16_t* frames, int nframes, int nz, int n, float* mean, cudaStream_t st);
 int setup_kernel_attributes(const tcp_ctx* c);

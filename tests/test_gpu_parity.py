@@ -65,6 +65,37 @@ def _gpu_recon(w, rows, dtype, m=3, filt=None, impl=None, keep=False):
     return res, None, (raw, flat, dark, theta)
 
 
+# ------------------------------------------------------------------ the tensor-core transform on its own
+@pytest.mark.parametrize("inverse", [False, True])
+def test_mma_fft_lines_against_the_dft(inverse):
+    """tcp_fft_lines: the length-4096 transform whose radix-16 butterflies run as mma.sync products (mmafft.cuh), on its
+    own, against the DFT definition in fp64 (numpy.fft of the same fp16 inputs; the oracle's orc.fft on the first lines).
+    Index and sign conventions: a delta at i0 gives e^{-/+ 2 pi i k i0 / N} exactly; a constant gives N delta_k.  Random
+    lines: operands are rounded to fp16 once per pass, so rel-L2 stays at a few 2^-11."""
+    tcp = _tcp()
+    N, B = 4096, 24
+    rng = np.random.default_rng(5)
+    x = (rng.standard_normal((B, N)) + 1j * rng.standard_normal((B, N)))
+    x[0] = 0; x[0, 1] = 1.0                       # delta at 1
+    x[1] = 0; x[1, 2049] = 1j                     # delta in the upper half
+    x[2] = 1.0 - 0.5j                             # constant
+    x[3, N // 2:] = 0                             # zero-padded, as the row kernel's inputs
+    x[4] *= 100.0                                 # large
+    x[5] *= 1e-2                                  # small
+    xh = np.stack([x.real, x.imag], -1).astype(np.float16)
+    xq = xh[..., 0].astype(np.float64) + 1j * xh[..., 1].astype(np.float64)
+    r = tcp.Recon(2048, 8, 2, 1024.0, "f16", "ramp")
+    got = r.fft_lines(torch.from_numpy(xh).cuda(), inverse=inverse).cpu().numpy().astype(np.complex128)
+    r.close()
+    ref = np.fft.ifft(xq, axis=1) * N if inverse else np.fft.fft(xq, axis=1)
+    for b in range(2):
+        o = orc.fft(xq[b], sign=+1 if inverse else -1)
+        assert rl2(o, ref[b]) < 1e-12
+    for b in range(B):
+        assert rl2(got[b], ref[b]) < 1.5e-3, (b, rl2(got[b], ref[b]))
+    assert np.abs(got[0] - ref[0]).max() < 2e-3 and np.abs(got[2] - ref[2]).max() < 2e-3 * N
+
+
 # ------------------------------------------------------------------ C1, stage by stage
 @pytest.mark.parametrize("m", [3, 4])
 def test_c1_fp32_stages_and_volume(m):
@@ -743,15 +774,17 @@ def test_pipeline_slice_ranges_equal_the_whole_volume():
 
 
 # ------------------------------------------------------------------ BASELINE full sizes, bench launch configuration
-@pytest.mark.parametrize("cfg,nz,tcfft,where", [("C4", 32, 0, "mid"), ("C4", 32, 0, "first"), ("C4", 32, 0, "last"), ("C4", 32, 4, "mid"),
-                                                ("C5", 32, 0, "mid"), ("C5", 32, 0, "first"), ("C5", 32, 0, "last")])
+@pytest.mark.parametrize("cfg,nz,tcfft,where", [("C4", 32, None, "mid"), ("C4", 32, None, "first"), ("C4", 32, None, "last"),
+                                                ("C4", 32, 0, "mid"), ("C4", 32, 1, "mid"), ("C4", 32, 6, "mid"),
+                                                ("C5", 32, None, "mid"), ("C5", 32, None, "first"), ("C5", 32, None, "last")])
 def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft, where):
     """C4 (2048^2, 2048 projections, fp16, one 32-slice chunk exactly as bench.py launches it: tcgen05
     gridding with 16 pairs per accumulator group) and C5 (4096^2, 4000 projections, M = 8192, off-centre,
     fp16 -> fp32 output).  Inputs are manufactured on the GPU (synthgen.make_counts_torch, frame averaging
     through tcp_mean_frames_u16) and the SAME arrays go to the oracle, which reconstructs a sample of the
-    chunk's slices one by one.  tcfft = 4 additionally runs the row pass of the inverse 2D transform as
-    DFT-as-GEMM on the tensor cores (opt-in, TCP_OPT_TCFFT; same gates)."""
+    chunk's slices one by one.  tcfft: TCP_OPT_TCFFT, which transforms run their butterflies on the tensor cores
+    (None = the default, every transform at M = 4096; 0 = the fp32 CUDA-core transforms; 1 = the row kernel only;
+    6 = the inverse 2D transform only): same gates for every combination."""
     tcp = _tcp()
     w = sg.make_workload(cfg)
     z0 = {"mid": w.nz_total // 2 - nz // 2, "first": 0, "last": w.nz_total - nz}[where]
@@ -763,7 +796,7 @@ def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft, where):
     tcp.tcp_mean_frames_u16(df.contiguous(), dark_d)
     theta = w.theta
     r = tcp.Recon(w.n, w.nproj, nz, w.center, w.dtype, w.filter, 3)
-    if tcfft:
+    if tcfft is not None:
         r.set_tcfft(tcfft)
     out = r.recon(raw_d.contiguous(), flat_d, dark_d, torch.from_numpy(theta).cuda())
     torch.cuda.synchronize()
@@ -774,5 +807,6 @@ def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft, where):
     ref = orc.recon(raw_h, flat_d[sample].cpu().numpy(), dark_d[sample].cpu().numpy(), theta, w.center, w.filter, 3, "grid")
     scale = np.abs(ref).max()
     for i, z in enumerate(sample):
+        print("full size %s tcfft=%s %s slice %d: rel-L2 %.3e max-abs %.3e" % (cfg, tcfft, where, z, rl2(out[z], ref[i]), np.abs(out[z] - ref[i]).max() / scale))
         assert rl2(out[z], ref[i]) < FP16_GATE_L2, (cfg, z, rl2(out[z], ref[i]))
         assert np.abs(out[z] - ref[i]).max() / scale < FP16_GATE_MAX
