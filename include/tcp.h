@@ -160,9 +160,13 @@ int tcp_read_workspace(tcp_ctx* ctx, int which, void* dst, size_t dst_bytes, tcp
 /* Layout of TCP_WS_GRID: 0 = [npair][M l2][M l1]; W > 0 = strip-major [npair][M/W][M l2][W l1] (the
  * tensor-core gridding writes strips of W columns so that the column pass of S6 reads contiguously). */
 int tcp_grid_strip(const tcp_ctx* ctx);
-/* Layout of TCP_WS_PASS1: 0 = strips [npair][M/W][n iy][W l1]; 1 = row pairs [npair][n/2][M l1][2 rows] (the
- * tensor-core transforms, TCP_OPT_TCFFT & 6). */
+/* Layouts under the tensor-core transforms of the inverse 2D transform (TCP_OPT_TCFFT & 6), which copy a whole line
+ * set into shared memory in bulk and therefore want it stored in their bank-swizzled order (mmafft.cuh, swz<NL>):
+ * tcp_pass1_layout: 0 = TCP_WS_PASS1 in strips [npair][M/W][n iy][W l1]; 1 = row pairs [npair][n/2][position][2 rows]
+ * with column l1 at position swz<2>(l1).  tcp_grid_swizzled: 1 = row l2 of every TCP_WS_GRID strip sits at position
+ * swz<4>(l2) of its strip (0 = at l2). */
 int tcp_pass1_layout(const tcp_ctx* ctx);
+int tcp_grid_swizzled(const tcp_ctx* ctx);
 /* Test helper for the tensor-core transform itself: `batch` lines of 4096 half2 (re, im) -> 4096 float2 each,
  * X[k] = sum_i x[i] e^{-/+ 2 pi i ik/4096} (inverse != 0: +, unnormalised), natural order on both sides.
  * TCP_EUNSUPPORTED unless the context has fp16 storage and M = 4096. */

@@ -89,12 +89,26 @@ def lib():
     L.tcp_slice_range.argtypes = [ci, ci, ci, C.POINTER(ci), C.POINTER(ci)]
     L.tcp_pass1_layout.restype = ci
     L.tcp_pass1_layout.argtypes = [vp]
+    L.tcp_grid_swizzled.restype = ci
+    L.tcp_grid_swizzled.argtypes = [vp]
     L.tcp_fft_lines.restype = ci
     L.tcp_fft_lines.argtypes = [vp, vp, vp, ci, ci, vp]
     L.tcp_recon_try.restype = ci
     L.tcp_recon_try.argtypes = [vp, vp, vp, vp, vp, C.POINTER(cf), ci, vp, vp]
     _lib = L
     return L
+
+
+def _swz(nl: int, size: int):
+    """Position of element k of a line in the layouts the tensor-core transforms read (mmafft.cuh swz<NL>; marshalling of
+    test read-backs only): the inverse permutation is the same function (an XOR with bits it does not change)."""
+    import numpy as np
+    k = np.arange(size, dtype=np.int64)
+    if nl == 2:
+        f = lambda x: np.where(x & 1, 12, 0) ^ np.where(x & 2, 5, 0)
+        return k ^ f((k >> 8) & 3) ^ f((k >> 4) & 3)
+    f = lambda x: ((x & 3) << 1) | (x & 1)
+    return k ^ f((k >> 8) & 3) ^ f((k >> 4) & 3)
 
 
 def tcp_last_error() -> str:
@@ -348,9 +362,14 @@ class Recon:
         if name == "grid":
             w = int(lib().tcp_grid_strip(self.h))
             if w:       # strip-major [npair][M/w][M l2][w l1] -> [npair][M l2][M l1]
-                v = v.view(npair, M // w, M, w, 2).permute(0, 2, 1, 3, 4).reshape(npair, M, M, 2)
-        if name == "pass1" and int(lib().tcp_pass1_layout(self.h)) == 1:   # row pairs [npair][n/2][M l1][2] -> [npair][n iy][M l1]
-            v = v.view(npair, n // 2, M, 2, 2).permute(0, 1, 3, 2, 4).reshape(npair, n, M, 2)
+                v = v.view(npair, M // w, M, w, 2)
+                if int(lib().tcp_grid_swizzled(self.h)):    # row l2 of a strip is stored at position swz<4>(l2)
+                    v = v[:, :, torch.from_numpy(_swz(4, M)).to(v.device)]
+                v = v.permute(0, 2, 1, 3, 4).reshape(npair, M, M, 2)
+        if name == "pass1" and int(lib().tcp_pass1_layout(self.h)) == 1:
+            # row pairs [npair][n/2][position swz<2>(l1)][2 rows] -> [npair][n iy][M l1]
+            v = v.view(npair, n // 2, M, 2, 2)[:, :, torch.from_numpy(_swz(2, M)).to(v.device)]
+            v = v.permute(0, 1, 3, 2, 4).reshape(npair, n, M, 2)
         elif name == "pass1":   # strip-major [npair][M/w][n iy][w l1] -> [npair][n iy][M l1]
             w = min(32, max(2, 16384 // M))
             v = v.view(npair, M // w, n, w, 2).permute(0, 2, 1, 3, 4).reshape(npair, n, M, 2)

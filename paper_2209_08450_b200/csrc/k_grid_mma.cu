@@ -33,6 +33,7 @@
 #include <algorithm>
 
 #include "grid_common.cuh"
+#include "mmafft.cuh"
 #include "umma.cuh"
 #include "tcp_internal.h"
 
@@ -90,7 +91,7 @@ template <int MH, int NN, int MODE>
 __global__ void __launch_bounds__(32 * CW, 16 / CW)
     grid_mma_kernel(const __half2* __restrict__ spec, __half2* __restrict__ grid, float2* __restrict__ partial,
                     const float4* __restrict__ trigf, const int2* __restrict__ plan, const int4* __restrict__ items,
-                    int nproj, int M, int npair, float alpha2, int strip_log2, int nitems, int* __restrict__ counter,
+                    int nproj, int M, int npair, float alpha2, int strip_log2, int rswz, int nitems, int* __restrict__ counter,
                     const int* __restrict__ wstate, int* __restrict__ wcount, const int* __restrict__ woff,
                     uint4* __restrict__ wrec, unsigned* __restrict__ wsamp) {
     if (MODE == GM_DIRECT && wstate[WS_USABLE]) return;
@@ -389,7 +390,7 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
             }
             const int ry = (gb >> 1) * SUBY + ly, rx = (gb & 1) * SUBX + lx;    // region-relative cell
             if (item.z < 0) {
-                const int gr = TY0 + ry, gc = TX0 + rx;
+                const int gr = rswz ? mf::swz<4>(TY0 + ry) : TY0 + ry, gc = TX0 + rx;      // row position inside the strip
                 // strip-major grid (strip width 2^strip_log2 columns) or row-major (strip_log2 < 0)
                 const size_t cell = strip_log2 >= 0 ? ((((size_t)(gc >> strip_log2) * M + gr) << strip_log2) + (gc & ((1 << strip_log2) - 1)))
                                                     : (size_t)gr * M + gc;
@@ -480,7 +481,7 @@ static int launch_mma_mode(const tcp_ctx* c, cudaStream_t st) {
     if (ctas < 1) ctas = 1;
     dim3 grid(ctas, ny, nz);
     kern<<<grid, 32 * CW, L::total, st>>>((const __half2*)c->spec, (__half2*)c->grid, c->g_partial, c->trigf, c->g_plan, c->g_items,
-                                       c->nproj, c->M, c->npair, (float)(alpha * 1.4426950408889634), c->grid_strip ? (int)log2((double)c->grid_strip) : -1,
+                                       c->nproj, c->M, c->npair, (float)(alpha * 1.4426950408889634), c->grid_strip ? (int)log2((double)c->grid_strip) : -1, ifft2_on_mma(c) ? 1 : 0,
                                        c->g_nitems, c->g_counter, c->w_state, c->w_count, c->w_off, c->w_rec, c->w_samp);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;

@@ -27,6 +27,7 @@
 #include <vector>
 
 #include "grid_common.cuh"
+#include "mmafft.cuh"
 #include "tcp_internal.h"
 
 namespace tcpk {
@@ -321,7 +322,7 @@ __global__ void __launch_bounds__(NTHR, 2)
 // red: x = tile, y = first slot, z = S.  One CTA per (split tile, pair); a thread sums 4 cells.
 template <class TC>
 __global__ void __launch_bounds__(NTHR) grid_reduce_kernel(const float2* __restrict__ partial, TC* __restrict__ grid,
-                                                           const int4* __restrict__ red, int M, int npair, int strip) {
+                                                           const int4* __restrict__ red, int M, int npair, int strip, int rswz) {
     const int4 r = red[blockIdx.x];
     const int pair = blockIdx.y, tiles = M / TS;
     const int row = threadIdx.x >> 3, col = (threadIdx.x & 7) * 4;
@@ -339,7 +340,7 @@ __global__ void __launch_bounds__(NTHR) grid_reduce_kernel(const float2* __restr
 #pragma unroll
     for (int e = 0; e < 4; ++e) {
         const int c1 = gc + e;
-        st_c(g, strip ? ((size_t)(c1 / strip) * M + gr) * strip + (c1 % strip) : (size_t)gr * M + c1, a[e]);
+        st_c(g, strip ? ((size_t)(c1 / strip) * M + (rswz ? mf::swz<4>(gr) : gr)) * strip + (c1 % strip) : (size_t)gr * M + c1, a[e]);
     }
 }
 
@@ -441,9 +442,9 @@ int launch_grid_tile(const tcp_ctx* c, const float* theta, cudaStream_t st) {
     if (rc) return rc;
     if (c->g_nred) {
         if (c->half_store)
-            grid_reduce_kernel<__half2><<<dim3(c->g_nred, c->npair), NTHR, 0, st>>>(c->g_partial, (__half2*)c->grid, c->g_red, c->M, c->npair, c->grid_strip);
+            grid_reduce_kernel<__half2><<<dim3(c->g_nred, c->npair), NTHR, 0, st>>>(c->g_partial, (__half2*)c->grid, c->g_red, c->M, c->npair, c->grid_strip, ifft2_on_mma(c) ? 1 : 0);
         else
-            grid_reduce_kernel<float2><<<dim3(c->g_nred, c->npair), NTHR, 0, st>>>(c->g_partial, (float2*)c->grid, c->g_red, c->M, c->npair, c->grid_strip);
+            grid_reduce_kernel<float2><<<dim3(c->g_nred, c->npair), NTHR, 0, st>>>(c->g_partial, (float2*)c->grid, c->g_red, c->M, c->npair, c->grid_strip, ifft2_on_mma(c) ? 1 : 0);
         TCP_CUDA_CHECK(cudaGetLastError());
     }
     return TCP_OK;

@@ -86,7 +86,9 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
     Twid T;
     load_twid(T, T1TAB, tw, warp, g, c, (float)(1.0 / GAMMA), (float)(1.0 / (GAMMA * GAMMA)));
     __syncwarp();
-    auto from_line = [&](int k) { return L[swz<1>(k)]; };
+    Offs<1> O;
+    make_offs<1>(O, warp, g, c);
+    auto no_in = [](int) { return 0u; };
     const float2* ptab0 = ptab;
 #pragma unroll 1
     for (int unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
@@ -146,11 +148,11 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
     }
 
     // ---- transform 1: spectrum of the padded row, times 2^12 H / M
-    pass1<1, false, !PAD_EDGE, false>(L, An, T, warp, g, c, from_line);
+    pass1<1, false, !PAD_EDGE, true>(L, An, T, O, warp, g, c, no_in);
     __syncthreads();
-    pass2<1, false>(L, An, T, warp, g, c);
+    pass2<1, false>(L, An, T, O);
     __syncthreads();
-    pass3<1, false, false, true>(L, Al, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
+    pass3<1, false, false, true>(L, Al, O, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
         const float2 h = __ldg(reinterpret_cast<const float2*>(hfilt + k0));
         const float h0 = h.x * kRowScale, h1 = h.y * kRowScale;
         *reinterpret_cast<uint2*>(&L[swz<1>(k0)]) = make_uint2(pack_h2(y0[0].x * h0, y0[0].y * h0), pack_h2(y1[0].x * h1, y1[0].y * h1));
@@ -159,23 +161,23 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
     // ---- transform 2 (inverse): the filtered row, cropped to the detector (only tile 0 = samples below n is computed)
     flip_afrag(An);
     flip_afrag(Al);
-    pass1<1, true, false, false>(L, An, T, warp, g, c, from_line);
+    pass1<1, true, false, true>(L, An, T, O, warp, g, c, no_in);
     __syncthreads();
-    pass2<1, true>(L, An, T, warp, g, c);
+    pass2<1, true>(L, An, T, O);
     __syncthreads();
-    pass3<1, true, false, true>(L, Al, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
+    pass3<1, true, false, true>(L, Al, O, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
         *reinterpret_cast<uint2*>(&L[swz<1>(k0)]) = make_uint2(pack_h2(y0[0].x, y0[0].y), pack_h2(y1[0].x, y1[0].y));
     });
     __syncthreads();
     // ---- transform 3: spectrum of the zero-padded filtered row, centre phase and scale on store
     flip_afrag(An);
     flip_afrag(Al);
-    pass1<1, false, true, false>(L, An, T, warp, g, c, from_line);
+    pass1<1, false, true, true>(L, An, T, O, warp, g, c, no_in);
     __syncthreads();
-    pass2<1, false>(L, An, T, warp, g, c);
+    pass2<1, false>(L, An, T, O);
     __syncthreads();
     __half2* out = spec + ((size_t)pair * nproj + j) * N;
-    pass3<1, false, false, false>(L, Al, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
+    pass3<1, false, false, false>(L, Al, O, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
         const float4 p = __ldg(reinterpret_cast<const float4*>(ptab + k0));
         const float s = 1.f / kRowScale;
         const float2 v0 = make_float2((y0[0].x * p.x - y0[0].y * p.y) * s, (y0[0].x * p.y + y0[0].y * p.x) * s);
@@ -187,15 +189,28 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
 }
 
 // ------------------------------------------------------------------------------------------------ column pass of S6
-// One CTA = one strip of 4 adjacent columns of the strip-major grid [pair][M/4][M l2][4 l1]: a thread's 16-byte load is
-// the 4 columns of one row, the team transforms the 4 columns with shared twiddles, and only the central n outputs are
-// computed in the last pass (tile 0 of the AV_LOC fragments).
+// One unit = one strip of 4 adjacent columns of the strip-major grid [pair][M/4][M l2][4 l1], whose rows the gridding
+// kernel stores at position swz<4>(l2) (tcp_internal.h: ifft2_on_mma): the 64 KB block is exactly the team's 4
+// interleaved lines, and ONE bulk asynchronous copy (TMA) brings it in.  Persistent CTAs; while one CTA of an SM waits for
+// its copy the others transform.  Only the central n outputs are computed in the last pass (tile 0 of the AV_LOC fragments).
+// Output: pass1[pair][iy / 2][swz<2>(l1)][iy % 2] -- the row pass loads its lines the same way.  A thread holds 32
+// contiguous bytes (4 columns x 2 rows); lane pairs swap halves so that every 16-byte store instruction fills whole sectors.
 __global__ void __launch_bounds__(NT, 2) cols_mma_kernel(const uint4* __restrict__ grid, uint2* __restrict__ p1arr,
                                                           const float2* __restrict__ tw, const uint32_t* __restrict__ atab, int nunits) {
     constexpr int n = N / 2;
-    extern __shared__ __align__(16) uint32_t L[];
-    float2* T1TAB = reinterpret_cast<float2*>(L + 4 * N);               // pass-1 twiddle table behind the lines
+    extern __shared__ __align__(128) uint32_t L[];
+    float2* T1TAB = reinterpret_cast<float2*>(L + 4 * N);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(reinterpret_cast<unsigned char*>(T1TAB) + T1_BYTES);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, c = lane & 3;
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        fence_mbar_init();
+    }
+    __syncthreads();
+    if (tid == 0 && (int)blockIdx.x < nunits) {
+        mbar_expect_tx(bar, 4 * N * 4);
+        bulk_g2s(L, grid + (size_t)blockIdx.x * N, 4 * N * 4, bar);
+    }
     AFrag An, Ac;
     load_afrag(An, atab, AV_NAT, lane);
     flip_afrag(An);
@@ -204,27 +219,55 @@ __global__ void __launch_bounds__(NT, 2) cols_mma_kernel(const uint4* __restrict
     Twid T;
     load_twid(T, T1TAB, tw, warp, g, c, (float)(1.0 / GAMMA), (float)(1.0 / (GAMMA * GAMMA)));
     __syncwarp();
+    Offs<4> O;
+    make_offs<4>(O, warp, g, c);
+    auto no_in = [](int) { return make_uint4(0u, 0u, 0u, 0u); };
+    uint32_t phase = 0;
 #pragma unroll 1
     for (int unit = blockIdx.x; unit < nunits; unit += gridDim.x) {       // unit = pair (N / 4) + strip: consecutive blocks of the grid
     const int strip = unit % (N / 4), pair = unit / (N / 4);
-    const uint4* src = grid + (size_t)unit * N;
-    pass1<4, true, false, true>(L, An, T, warp, g, c, [&](int k) { return __ldg(src + k); });
-    if (unit + (int)gridDim.x < nunits) {        // the next unit of this CTA: a contiguous 64 KB block, 2 cache lines per thread
-        const char* nx = reinterpret_cast<const char*>(src + (size_t)gridDim.x * N) + tid * 256;
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(nx));
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(nx + 128));
-    }
+    mbar_wait(bar, phase);
+    phase ^= 1;
+    pass1<4, true, false, true>(L, An, T, O, warp, g, c, no_in);
     __syncthreads();
-    pass2<4, true>(L, An, T, warp, g, c);
+    pass2<4, true>(L, An, T, O);
     __syncthreads();
-    uint2* dst = p1arr + (size_t)pair * (n / 2) * N + 4 * strip;
-    pass3<4, true, true, false>(L, Ac, warp, g, c, [&](int k0, const float2(&y0)[4], const float2(&y1)[4]) {
+    // columns 4 strip + l sit at swz<2>(4 strip + l) = base + (l ^ x1) of their row pair
+    const int sw = swz<2>(4 * strip), x1 = sw & 1;
+    unsigned char* dst = reinterpret_cast<unsigned char*>(p1arr + (size_t)pair * (n / 2) * N + (sw & ~3));
+    pass3<4, true, true, false>(L, Ac, O, warp, g, c, [&](int k0, const float2(&y0)[4], const float2(&y1)[4]) {
         const int iy0 = k0 < n / 2 ? k0 + n / 2 : k0 - (N - n / 2);       // even; rows iy0 and iy0 + 1 are one pair
-        uint4* d = reinterpret_cast<uint4*>(dst + (size_t)(iy0 >> 1) * N);
-        d[0] = make_uint4(pack_h2(y0[0].x, y0[0].y), pack_h2(y1[0].x, y1[0].y), pack_h2(y0[1].x, y0[1].y), pack_h2(y1[1].x, y1[1].y));
-        d[1] = make_uint4(pack_h2(y0[2].x, y0[2].y), pack_h2(y1[2].x, y1[2].y), pack_h2(y0[3].x, y0[3].y), pack_h2(y1[3].x, y1[3].y));
+        uint32_t w[8];                                                     // the thread's 32 bytes: [position][row]
+#pragma unroll
+        for (int l = 0; l < 4; ++l) {
+            const int pos = l ^ x1;
+            const uint32_t a = pack_h2(y0[l].x, y0[l].y), b = pack_h2(y1[l].x, y1[l].y);
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (q == pos) { w[2 * q] = a; w[2 * q + 1] = b; }
+        }
+        // lanes c and c ^ 1 hold the chunks of row pairs iy0 / 2 and iy0 / 2 +- 1: the even lane takes both first halves,
+        // the odd lane both second halves, so that each of the two store instructions writes whole 32-byte sectors
+        const bool odd = c & 1;
+        uint32_t r[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) r[q] = __shfl_xor_sync(0xffffffffu, odd ? w[q] : w[4 + q], 1);
+        unsigned char* mine = dst + (size_t)(iy0 >> 1) * (N * 8);
+        unsigned char* other = odd ? mine - N * 8 : mine + N * 8;
+        if (!odd) {
+            *reinterpret_cast<uint4*>(mine) = make_uint4(w[0], w[1], w[2], w[3]);
+            *reinterpret_cast<uint4*>(other) = make_uint4(r[0], r[1], r[2], r[3]);
+        } else {
+            *reinterpret_cast<uint4*>(other + 16) = make_uint4(r[0], r[1], r[2], r[3]);
+            *reinterpret_cast<uint4*>(mine + 16) = make_uint4(w[4], w[5], w[6], w[7]);
+        }
     });
-    __syncthreads();
+    __syncthreads();                      // the lines are free for the next unit
+    if (tid == 0 && unit + (int)gridDim.x < nunits) {
+        fence_proxy_async();
+        mbar_expect_tx(bar, 4 * N * 4);
+        bulk_g2s(L, grid + (size_t)(unit + gridDim.x) * N, 4 * N * 4, bar);
+    }
     }
 }
 
@@ -232,34 +275,28 @@ __global__ void __launch_bounds__(NT, 2) cols_mma_kernel(const uint4* __restrict
 __device__ __forceinline__ void st_out2(__half* p, float a, float b) { *reinterpret_cast<uint32_t*>(p) = pack_h2(a, b); }
 __device__ __forceinline__ void st_out2(float* p, float a, float b) { *reinterpret_cast<float2*>(p) = make_float2(a, b); }
 
-// The next unit's row pair (a contiguous 32 KB block of the pass-1 array) arrives by bulk asynchronous copies (TMA) in a
-// staging buffer while the current one is in passes 2 and 3: 16 blocks of 256 elements, each followed by 4 elements
-// (32 bytes) of padding, which makes the stride-256 reads of pass 1 bank-conflict free.
-constexpr int IROWS_BLK = 256 * 8 + 32;
-constexpr int IROWS_STAGE = 16 * IROWS_BLK;
-
+// One unit = one row pair (iy, iy + 1) of one slice pair: a contiguous 32 KB block of the pass-1 array, columns already
+// at their swizzled positions (cols_mma_kernel), brought in by one bulk asynchronous copy.
 template <class TO>
 __global__ void __launch_bounds__(NT, 2) irows_mma_kernel(const uint2* __restrict__ p1arr, TO* __restrict__ out,
                                                            const float2* __restrict__ tw, const uint32_t* __restrict__ atab,
                                                            const float* __restrict__ deax, const float* __restrict__ deay, int nz, int nunits) {
     constexpr int n = N / 2;
-    extern __shared__ __align__(16) uint32_t L[];
-    float2* T1TAB = reinterpret_cast<float2*>(L + 2 * N);               // pass-1 twiddle table behind the lines
-    unsigned char* S = reinterpret_cast<unsigned char*>(L + 2 * N) + T1_BYTES;
-    uint64_t* bar = reinterpret_cast<uint64_t*>(S + IROWS_STAGE);
+    extern __shared__ __align__(128) uint32_t L0[];                       // two line sets: the next unit arrives while this one is transformed
+    float2* T1TAB = reinterpret_cast<float2*>(L0 + 2 * 2 * N);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(reinterpret_cast<unsigned char*>(T1TAB) + T1_BYTES);   // [2]
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, c = lane & 3;
-    auto fetch = [&](int unit) {                                          // thread 0 only
-        mbar_expect_tx(bar, 2 * N * 4);
-        const unsigned char* src = reinterpret_cast<const unsigned char*>(p1arr + (size_t)unit * N);
-#pragma unroll 1
-        for (int b = 0; b < 16; ++b) bulk_g2s(S + b * IROWS_BLK, src + b * 2048, 2048, bar);
+    auto fetch = [&](int unit, int b) {                                   // thread 0 only
+        mbar_expect_tx(&bar[b], 2 * N * 4);
+        bulk_g2s(L0 + b * 2 * N, p1arr + (size_t)unit * N, 2 * N * 4, &bar[b]);
     };
     if (tid == 0) {
-        mbar_init(bar, 1);
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
         fence_mbar_init();
     }
     __syncthreads();
-    if (tid == 0 && (int)blockIdx.x < nunits) fetch(blockIdx.x);
+    if (tid == 0 && (int)blockIdx.x < nunits) fetch(blockIdx.x, 0);
     AFrag An, Ac;
     load_afrag(An, atab, AV_NAT, lane);
     flip_afrag(An);
@@ -268,26 +305,31 @@ __global__ void __launch_bounds__(NT, 2) irows_mma_kernel(const uint2* __restric
     Twid T;
     load_twid(T, T1TAB, tw, warp, g, c, (float)(1.0 / GAMMA), (float)(1.0 / (GAMMA * GAMMA)));
     __syncwarp();
-    uint32_t phase = 0;
+    Offs<2> O;
+    make_offs<2>(O, warp, g, c);
+    auto no_in = [](int) { return make_uint2(0u, 0u); };
+    int it = 0;
 #pragma unroll 1
-    for (int unit = blockIdx.x; unit < nunits; unit += gridDim.x) {       // unit = pair (n / 2) + row pair rp: rows iy = 2 rp, 2 rp + 1
+    for (int unit = blockIdx.x; unit < nunits; unit += gridDim.x, ++it) { // unit = pair (n / 2) + row pair rp: rows iy = 2 rp, 2 rp + 1
     const int rp = unit % (n / 2), pair = unit / (n / 2);
-    mbar_wait(bar, phase);
-    phase ^= 1;
-    pass1<2, true, false, false>(L, An, T, warp, g, c, [&](int k) { return *reinterpret_cast<const uint2*>(S + (k >> 8) * IROWS_BLK + (k & 255) * 8); });
-    __syncthreads();                      // the staging buffer is free, the lines are complete
+    const int b = it & 1;
+    uint32_t* L = L0 + b * 2 * N;
+    // the other line set was last read in pass 3 of the previous unit, which every thread left through the barrier below
     if (tid == 0 && unit + (int)gridDim.x < nunits) {
         fence_proxy_async();
-        fetch(unit + gridDim.x);
+        fetch(unit + gridDim.x, b ^ 1);
     }
-    pass2<2, true>(L, An, T, warp, g, c);
+    mbar_wait(&bar[b], (it >> 1) & 1);
+    pass1<2, true, false, true>(L, An, T, O, warp, g, c, no_in);
+    __syncthreads();
+    pass2<2, true>(L, An, T, O);
     __syncthreads();
     const int zA = 2 * pair, zB = 2 * pair + 1;
     const bool hasB = zB < nz;
     const float dy0 = __ldg(&deay[2 * rp]), dy1 = __ldg(&deay[2 * rp + 1]);
     TO* oA = out + ((size_t)zA * n + 2 * rp) * n;
     TO* oB = out + ((size_t)zB * n + 2 * rp) * n;
-    pass3<2, true, true, false>(L, Ac, warp, g, c, [&](int k0, const float2(&y0)[2], const float2(&y1)[2]) {
+    pass3<2, true, true, false>(L, Ac, O, warp, g, c, [&](int k0, const float2(&y0)[2], const float2(&y1)[2]) {
         const int ix = k0 < n / 2 ? k0 + n / 2 : k0 - (N - n / 2);
         const float2 dx = __ldg(reinterpret_cast<const float2*>(deax + ix));
 #pragma unroll
@@ -297,7 +339,7 @@ __global__ void __launch_bounds__(NT, 2) irows_mma_kernel(const uint2* __restric
             if (hasB) st_out2(oB + (size_t)l * n + ix, y0[l].y * d0, y1[l].y * d1);
         }
     });
-    __syncthreads();
+    __syncthreads();                      // this line set is free
     }
 }
 
@@ -318,11 +360,13 @@ __global__ void __launch_bounds__(NT, 2) fft_lines_kernel(const uint32_t* __rest
     Twid T;
     load_twid(T, T1TAB, tw, warp, g, c, (float)(1.0 / GAMMA), (float)(1.0 / (GAMMA * GAMMA)));
     __syncwarp();
-    pass1<1, INV, false, true>(L, An, T, warp, g, c, [&](int k) { return __ldg(src + k); });
+    Offs<1> O;
+    make_offs<1>(O, warp, g, c);
+    pass1<1, INV, false, false>(L, An, T, O, warp, g, c, [&](int k) { return __ldg(src + k); });
     __syncthreads();
-    pass2<1, INV>(L, An, T, warp, g, c);
+    pass2<1, INV>(L, An, T, O);
     __syncthreads();
-    pass3<1, false, false, false>(L, Al, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
+    pass3<1, false, false, false>(L, Al, O, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
         *reinterpret_cast<float4*>(dst + k0) = make_float4(y0[0].x, y0[0].y, y1[0].x, y1[0].y);
     });
 }
@@ -342,7 +386,7 @@ int launch_rows_mma(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw) {
 }
 
 int launch_cols_mma(const tcp_ctx* c, cudaStream_t st) {
-    const size_t smem = (size_t)4 * N * 4 + T1_BYTES;
+    const size_t smem = (size_t)4 * N * 4 + T1_BYTES + 16;
     TCP_SMEM(cols_mma_kernel, smem);
     const int nunits = (N / 4) * c->npair;
     cols_mma_kernel<<<std::min(nunits, 2 * c->nsm), NT, smem, st>>>((const uint4*)c->grid, (uint2*)c->pass1, c->tw, c->mf_atab, nunits);
@@ -351,7 +395,7 @@ int launch_cols_mma(const tcp_ctx* c, cudaStream_t st) {
 }
 
 int launch_irows_mma(const tcp_ctx* c, void* out, cudaStream_t st) {
-    const size_t smem = (size_t)2 * N * 4 + T1_BYTES + IROWS_STAGE + 16;
+    const size_t smem = (size_t)2 * 2 * N * 4 + T1_BYTES + 16;
     const int nunits = (N / 4) * c->npair;
     const int grid = std::min(nunits, 2 * c->nsm);
     if (c->half_out) {

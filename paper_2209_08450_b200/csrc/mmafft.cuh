@@ -76,14 +76,39 @@ template <int NL>
 __device__ __forceinline__ typename Vec<NL>::T* elem(uint32_t* L, int k) { return reinterpret_cast<typename Vec<NL>::T*>(L + NL * swz<NL>(k)); }
 
 struct AFrag { uint32_t a[2][2][4]; };                    // [tile][K step][register]
-// Twiddles of a thread: pass 2's four sit in registers; pass 1's sixteen in a per-CTA shared-memory table
-// t1[slot = 4 group + 2 tile + e][thread] (float2: consecutive threads, consecutive 8 bytes: conflict free), which
-// keeps the kernels at two CTAs per SM without spills.
+// Twiddles of a thread.  Pass 2 needs four (registers).  Pass 1 needs sixteen, W^(d2 beta) with beta = 8 warp + 64 group
+// + 2c + e: the four of group 0 sit in a small shared-memory table base[2 tile + e][thread] and the others follow by the
+// recurrence W^(d2 (beta + 64)) = W^(d2 beta) W_64^(d2), whose two factors step[tile] are registers.
+typedef unsigned long long f32x2_t;
+struct Tw2s { f32x2_t r, i; };
 struct Twid {
-    const float2* t1;                                     // this thread's column of the table: t1[slot * NT]
-    float2 t2[2][2];                                      // pass 2: [tile][e]
+    const float2* base;                                   // this thread's column: base[(2 t + e) * NT]
+    float2 step[2];
+    Tw2s t2[2];                                           // pass 2: [tile], butterflies 2c and 2c + 1 packed (real parts, imaginary parts)
 };
-constexpr int T1_BYTES = 16 * NT * 8;
+constexpr int T1_BYTES = 4 * NT * 8;
+
+// Byte offsets of the thread's accesses into the lines (element k of NL lines at byte 4 NL swz(k)).  In every pattern the
+// bits the swizzle reads and flips come from the thread's own indices, never from the group, tile or input counters, so
+// an access is one of these offsets plus a compile-time immediate.
+template <int NL>
+struct Offs {
+    uint32_t r1, w1[2], r2, w2[2], r3[4];
+};
+template <int NL>
+__device__ __forceinline__ void make_offs(Offs<NL>& o, int warp, int g, int c) {
+    o.r1 = 4 * NL * swz<NL>(256 * c + 8 * warp + g);                           // + 4 NL (1024 i + 64 grp)
+    const int b2 = 256 * (warp >> 1) + 8 * (warp & 1);
+    o.r2 = 4 * NL * swz<NL>(b2 + 16 * c + g);                                  // + 4 NL (1024 grp + 64 i)
+    const int b3 = 256 * (8 * (warp & 1) + g) + 16 * (warp >> 1) + 2 * c;
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+        o.w1[e] = 4 * NL * swz<NL>(256 * g + 8 * warp + 2 * c + e);            // + 4 NL (2048 t + 64 grp)
+        o.w2[e] = 4 * NL * swz<NL>(b2 + 16 * g + 2 * c + e);                   // + 4 NL (1024 grp + 128 t)
+        o.r3[e] = 4 * NL * swz<NL>(b3 + e);                                    // + 4 NL 64 grp
+        o.r3[2 + e] = 4 * NL * swz<NL>(b3 + 8 + e);
+    }
+}
 
 __device__ __forceinline__ void load_afrag(AFrag& f, const uint32_t* __restrict__ atab, int variant, int lane) {
     const uint4* p = reinterpret_cast<const uint4*>(atab + ((size_t)variant * 32 + lane) * 16);
@@ -109,24 +134,20 @@ __device__ __forceinline__ void flip_afrag(AFrag& f) {
 __device__ __forceinline__ void load_twid(Twid& T, float2* t1tab, const float2* __restrict__ tw, int warp, int g, int c, float s1, float s2) {
     float2* mine = t1tab + (warp * 32 + g * 4 + c);
 #pragma unroll
-    for (int grp = 0; grp < 4; ++grp)
-#pragma unroll
-        for (int t = 0; t < 2; ++t)
-#pragma unroll
-            for (int e = 0; e < 2; ++e) {
-                const int d2 = g + 8 * t, beta = 8 * warp + 64 * grp + 2 * c + e;
-                const float2 w = __ldg(&tw[(d2 * beta) & (N - 1)]);
-                mine[(4 * grp + 2 * t + e) * NT] = make_float2(w.x * s1, w.y * s1);
-            }
-    T.t1 = mine;
-#pragma unroll
-    for (int t = 0; t < 2; ++t)
+    for (int t = 0; t < 2; ++t) {
+        const int d2 = g + 8 * t;
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-            const int d1 = g + 8 * t, d0 = 8 * (warp & 1) + 2 * c + e;
-            const float2 w = __ldg(&tw[(16 * d1 * d0) & (N - 1)]);
-            T.t2[t][e] = make_float2(w.x * s2, w.y * s2);
+            const float2 w = __ldg(&tw[(d2 * (8 * warp + 2 * c + e)) & (N - 1)]);
+            mine[(2 * t + e) * NT] = make_float2(w.x * s1, w.y * s1);
         }
+        const float2 v0 = __ldg(&tw[(16 * d2 * (8 * (warp & 1) + 2 * c)) & (N - 1)]);
+        const float2 v1 = __ldg(&tw[(16 * d2 * (8 * (warp & 1) + 2 * c + 1)) & (N - 1)]);
+        asm("mov.b64 %0, {%1, %2};" : "=l"(T.t2[t].r) : "f"(v0.x * s2), "f"(v1.x * s2));
+        asm("mov.b64 %0, {%1, %2};" : "=l"(T.t2[t].i) : "f"(v0.y * s2), "f"(v1.y * s2));
+        T.step[t] = __ldg(&tw[(64 * d2) & (N - 1)]);
+    }
+    T.base = mine;
 }
 
 __device__ __forceinline__ void mma_z(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
@@ -145,6 +166,29 @@ __device__ __forceinline__ uint32_t pack_h2(float re, float im) {
     asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(im), "f"(re));
     return r;
 }
+// Packed fp32 pairs (sm_100 FMUL2 / FFMA2: two fp32 operations per issued instruction).  The accumulator of an MMA holds
+// {re, re', im, im'} of two adjacent butterflies, so a pair of complex twiddle products is 2 FMUL2 + 2 FFMA2.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void unpk2(f32x2 v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ f32x2 neg2(f32x2 a) { return a ^ 0x8000000080000000ull; }
+// twiddles of two adjacent butterflies: real parts, imaginary parts
+struct Tw2 { f32x2 r, i; };
+// acc = {re0, re1, im0, im1} times the twiddle pair (or its conjugate), packed to two half2 (re, im) words
+template <bool INV>
+__device__ __forceinline__ void twmul2(const float (&acc)[4], const Tw2& w, uint32_t& h0, uint32_t& h1) {
+    const f32x2 re = pk2(acc[0], acc[1]), im = pk2(acc[2], acc[3]);
+    const f32x2 yr = fma2(im, INV ? w.i : neg2(w.i), mul2(re, w.r));      // re wr -/+ im wi
+    const f32x2 yi = fma2(re, INV ? neg2(w.i) : w.i, mul2(im, w.r));      // im wr +/- re wi
+    float r0, r1, i0, i1;
+    unpk2(yr, r0, r1);
+    unpk2(yi, i0, i1);
+    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(h0) : "f"(i0), "f"(r0));
+    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(h1) : "f"(i1), "f"(r1));
+}
+
 template <bool INV>
 __device__ __forceinline__ float2 twmul(float re, float im, float2 w) {       // (re + i im) w, or times conj(w)
     return INV ? make_float2(fmaf(im, w.y, re * w.x), fmaf(-re, w.y, im * w.x))
@@ -164,18 +208,36 @@ __device__ __forceinline__ void bfly(float (&acc)[2][4], const AFrag& A, uint32_
 
 constexpr int groups_per_batch(int NL) { return 4 / NL; }
 
-// pass 1 (stride 256).  in(k): the Vec<NL> at natural index k (from the lines, or straight from global memory);
-// outputs go to the lines.  GLOBAL_IN: the inputs of the next batch are requested before the current one is transformed.
-template <int NL, bool INV, bool KPRUNE, bool GLOBAL_IN, class In>
-__device__ __forceinline__ void pass1(uint32_t* L, const AFrag& A, const Twid& T, int warp, int g, int c, In in) {
+template <int NL>
+__device__ __forceinline__ typename Vec<NL>::T& at(uint32_t* L, uint32_t byte_off) {
+    return *reinterpret_cast<typename Vec<NL>::T*>(reinterpret_cast<unsigned char*>(L) + byte_off);
+}
+// store the packed outputs at natural indices k0 (even) and k0 + 1 of all lines; o[e] = byte offset of k0 + e
+template <int NL>
+__device__ __forceinline__ void put2(uint32_t* L, const uint32_t (&o)[2], uint32_t imm, const uint32_t (&w0)[NL], const uint32_t (&w1)[NL]) {
+    if constexpr (NL == 1) {
+        at<2>(L, o[0] + imm) = make_uint2(w0[0], w1[0]);          // one line: k0 and k0 + 1 are adjacent words
+    } else {
+        vmake(at<NL>(L, o[0] + imm), w0);
+        vmake(at<NL>(L, o[1] + imm), w1);
+    }
+}
+
+// pass 1 (stride 256).  SRC_LINES: the inputs are in the lines (in place); otherwise in(k) returns the Vec<NL> at natural
+// index k from somewhere else (a staging buffer, global memory).  Outputs go to the lines.
+template <int NL, bool INV, bool KPRUNE, bool SRC_LINES, class In>
+__device__ __forceinline__ void pass1(uint32_t* L, const AFrag& A, const Twid& T, const Offs<NL>& O, int warp, int g, int c, In in) {
     using V = typename Vec<NL>::T;
     constexpr int GB = groups_per_batch(NL), NB = 4 / GB, NI = KPRUNE ? 2 : 4;
-    V nxt[GB][4];
-    if constexpr (GLOBAL_IN) {
+    Tw2 cur[2];
+    f32x2 sx[2], sy[2];
 #pragma unroll
-        for (int q = 0; q < GB; ++q)
-#pragma unroll
-            for (int i = 0; i < NI; ++i) nxt[q][i] = in((c + 4 * i) * 256 + 8 * warp + 64 * q + g);
+    for (int t = 0; t < 2; ++t) {
+        const float2 a = T.base[(2 * t) * NT], b = T.base[(2 * t + 1) * NT];
+        cur[t].r = pk2(a.x, b.x);
+        cur[t].i = pk2(a.y, b.y);
+        sx[t] = pk2(T.step[t].x, T.step[t].x);
+        sy[t] = pk2(T.step[t].y, T.step[t].y);
     }
 #pragma unroll
     for (int bt = 0; bt < NB; ++bt) {
@@ -184,17 +246,9 @@ __device__ __forceinline__ void pass1(uint32_t* L, const AFrag& A, const Twid& T
         for (int q = 0; q < GB; ++q)
 #pragma unroll
             for (int i = 0; i < NI; ++i) {
-                if constexpr (GLOBAL_IN) v[q][i] = nxt[q][i];
+                if constexpr (SRC_LINES) v[q][i] = at<NL>(L, O.r1 + 4 * NL * (1024 * i + 64 * (bt * GB + q)));
                 else v[q][i] = in((c + 4 * i) * 256 + 8 * warp + 64 * (bt * GB + q) + g);
             }
-        if constexpr (GLOBAL_IN) {
-            if (bt + 1 < NB) {
-#pragma unroll
-                for (int q = 0; q < GB; ++q)
-#pragma unroll
-                    for (int i = 0; i < NI; ++i) nxt[q][i] = in((c + 4 * i) * 256 + 8 * warp + 64 * ((bt + 1) * GB + q) + g);
-            }
-        }
         float acc[GB][NL][2][4];
 #pragma unroll
         for (int q = 0; q < GB; ++q)
@@ -203,24 +257,17 @@ __device__ __forceinline__ void pass1(uint32_t* L, const AFrag& A, const Twid& T
                 bfly<KPRUNE, false>(acc[q][l], A, vget(v[q][0], l), vget(v[q][1], l), KPRUNE ? 0u : vget(v[q][2], l), KPRUNE ? 0u : vget(v[q][3], l));
 #pragma unroll
         for (int q = 0; q < GB; ++q) {
-            const int grp = bt * GB + q, beta0 = 8 * warp + 64 * grp;
+            const int grp = bt * GB + q;
 #pragma unroll
             for (int t = 0; t < 2; ++t) {
                 uint32_t w0[NL], w1[NL];
-                const float2 ta = T.t1[(4 * grp + 2 * t) * NT], tb = T.t1[(4 * grp + 2 * t + 1) * NT];
 #pragma unroll
-                for (int l = 0; l < NL; ++l) {
-                    const float2 y0 = twmul<INV>(acc[q][l][t][0], acc[q][l][t][2], ta);
-                    const float2 y1 = twmul<INV>(acc[q][l][t][1], acc[q][l][t][3], tb);
-                    w0[l] = pack_h2(y0.x, y0.y);
-                    w1[l] = pack_h2(y1.x, y1.y);
-                }
-                const int k0 = (g + 8 * t) * 256 + beta0 + 2 * c;
-                if constexpr (NL == 1) {
-                    *reinterpret_cast<uint2*>(L + swz<1>(k0)) = make_uint2(w0[0], w1[0]);      // k0 even: k0, k0 + 1 are adjacent words
-                } else {
-                    vmake(*elem<NL>(L, k0), w0);
-                    vmake(*elem<NL>(L, k0 + 1), w1);
+                for (int l = 0; l < NL; ++l) twmul2<INV>(acc[q][l][t], cur[t], w0[l], w1[l]);
+                put2<NL>(L, O.w1, 4 * NL * (2048 * t + 64 * grp), w0, w1);
+                if (grp < 3) {          // next group: beta + 64, i.e. times step = sx + i sy
+                    const f32x2 nr = fma2(cur[t].i, neg2(sy[t]), mul2(cur[t].r, sx[t]));
+                    cur[t].i = fma2(cur[t].r, sy[t], mul2(cur[t].i, sx[t]));
+                    cur[t].r = nr;
                 }
             }
         }
@@ -229,61 +276,42 @@ __device__ __forceinline__ void pass1(uint32_t* L, const AFrag& A, const Twid& T
 
 // pass 2 (stride 16), in place
 template <int NL, bool INV>
-__device__ __forceinline__ void pass2(uint32_t* L, const AFrag& A, const Twid& T, int warp, int g, int c) {
+__device__ __forceinline__ void pass2(uint32_t* L, const AFrag& A, const Twid& T, const Offs<NL>& O) {
     using V = typename Vec<NL>::T;
     constexpr int GB = groups_per_batch(NL), NB = 4 / GB;
 #pragma unroll
     for (int bt = 0; bt < NB; ++bt) {
         V v[GB][4];
 #pragma unroll
-        for (int q = 0; q < GB; ++q) {
-            const int base = ((warp >> 1) + 4 * (bt * GB + q)) * 256 + 8 * (warp & 1);
+        for (int q = 0; q < GB; ++q)
 #pragma unroll
-            for (int i = 0; i < 4; ++i) v[q][i] = *elem<NL>(L, base + (c + 4 * i) * 16 + g);
-        }
+            for (int i = 0; i < 4; ++i) v[q][i] = at<NL>(L, O.r2 + 4 * NL * (1024 * (bt * GB + q) + 64 * i));
         float acc[GB][NL][2][4];
 #pragma unroll
         for (int q = 0; q < GB; ++q)
 #pragma unroll
             for (int l = 0; l < NL; ++l) bfly<false, false>(acc[q][l], A, vget(v[q][0], l), vget(v[q][1], l), vget(v[q][2], l), vget(v[q][3], l));
 #pragma unroll
-        for (int q = 0; q < GB; ++q) {
-            const int base = ((warp >> 1) + 4 * (bt * GB + q)) * 256 + 8 * (warp & 1);
+        for (int q = 0; q < GB; ++q)
 #pragma unroll
             for (int t = 0; t < 2; ++t) {
                 uint32_t w0[NL], w1[NL];
 #pragma unroll
-                for (int l = 0; l < NL; ++l) {
-                    const float2 y0 = twmul<INV>(acc[q][l][t][0], acc[q][l][t][2], T.t2[t][0]);
-                    const float2 y1 = twmul<INV>(acc[q][l][t][1], acc[q][l][t][3], T.t2[t][1]);
-                    w0[l] = pack_h2(y0.x, y0.y);
-                    w1[l] = pack_h2(y1.x, y1.y);
-                }
-                const int k0 = base + (g + 8 * t) * 16 + 2 * c;
-                if constexpr (NL == 1) {
-                    *reinterpret_cast<uint2*>(L + swz<1>(k0)) = make_uint2(w0[0], w1[0]);
-                } else {
-                    vmake(*elem<NL>(L, k0), w0);
-                    vmake(*elem<NL>(L, k0 + 1), w1);
-                }
+                for (int l = 0; l < NL; ++l) twmul2<INV>(acc[q][l][t], Tw2{T.t2[t].r, T.t2[t].i}, w0[l], w1[l]);
+                put2<NL>(L, O.w2, 4 * NL * (1024 * (bt * GB + q) + 128 * t), w0, w1);
             }
-        }
     }
 }
 
 // pass 3 (stride 1): the thread's inputs of group grp: digits (2c, 2c + 1) and (8 + 2c, 9 + 2c) of butterfly d2 = 8 h + g
 template <int NL>
-__device__ __forceinline__ void pass3_load(uint32_t* L, int grp, int warp, int g, int c, typename Vec<NL>::T (&v)[4]) {
-    const int slot = (8 * (warp & 1) + g) * 256 + ((warp >> 1) + 4 * grp) * 16;
+__device__ __forceinline__ void pass3_load(uint32_t* L, const Offs<NL>& O, int grp, typename Vec<NL>::T (&v)[4]) {
     if constexpr (NL == 1) {
-        const uint2 lo = *reinterpret_cast<const uint2*>(L + swz<1>(slot + 2 * c));
-        const uint2 hi = *reinterpret_cast<const uint2*>(L + swz<1>(slot + 8 + 2 * c));
+        const uint2 lo = at<2>(L, O.r3[0] + 4 * 64 * grp), hi = at<2>(L, O.r3[2] + 4 * 64 * grp);
         v[0] = lo.x; v[1] = lo.y; v[2] = hi.x; v[3] = hi.y;
     } else {
-        v[0] = *elem<NL>(L, slot + 2 * c);
-        v[1] = *elem<NL>(L, slot + 2 * c + 1);
-        v[2] = *elem<NL>(L, slot + 8 + 2 * c);
-        v[3] = *elem<NL>(L, slot + 9 + 2 * c);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) v[j] = at<NL>(L, O.r3[j] + 4 * NL * 64 * grp);
     }
 }
 // natural index of the thread's first output (butterfly 2c) of tile t: o 256 + d1 16 + 8 h + 2c; the second is + 1.
@@ -297,15 +325,16 @@ __device__ __forceinline__ int pass3_index(int t, int grp, int warp, int g, int 
 // epi(k0, y0[NL], y1[NL]) gets the NL lines of the team together.  TO_LINES (one line): the epilogue writes the line
 // itself, so every input of the team is loaded before a block barrier and only then transformed.
 template <int NL, bool MPRUNE, bool CENTRE, bool TO_LINES, class Epi>
-__device__ __forceinline__ void pass3(uint32_t* L, const AFrag& A, int warp, int g, int c, Epi epi) {
+__device__ __forceinline__ void pass3(uint32_t* L, const AFrag& A, const Offs<NL>& O, int warp, int g, int c, Epi epi) {
     using V = typename Vec<NL>::T;
     constexpr int GB = groups_per_batch(NL), NB = 4 / GB, NTILE = MPRUNE ? 1 : 2;
     static_assert(!TO_LINES || NL == 1, "line-to-line pass 3 is used by the row kernel only");
+    const int kbase = pass3_index<CENTRE>(0, 0, warp, g, c);
 #pragma unroll
     for (int bt = 0; bt < NB; ++bt) {
         V v[GB][4];
 #pragma unroll
-        for (int q = 0; q < GB; ++q) pass3_load<NL>(L, bt * GB + q, warp, g, c, v[q]);
+        for (int q = 0; q < GB; ++q) pass3_load<NL>(L, O, bt * GB + q, v[q]);
         if constexpr (TO_LINES) __syncthreads();          // NB == 1: all inputs of the team are in registers
         float acc[GB][NL][2][4];
 #pragma unroll
@@ -322,7 +351,7 @@ __device__ __forceinline__ void pass3(uint32_t* L, const AFrag& A, int warp, int
                     y0[l] = make_float2(acc[q][l][t][0], acc[q][l][t][2]);
                     y1[l] = make_float2(acc[q][l][t][1], acc[q][l][t][3]);
                 }
-                epi(pass3_index<CENTRE>(t, bt * GB + q, warp, g, c), y0, y1);
+                epi(kbase + 2048 * t + 64 * (bt * GB + q), y0, y1);
             }
     }
 }

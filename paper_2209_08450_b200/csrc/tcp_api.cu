@@ -177,9 +177,6 @@ static int build_context(tcp_ctx* c) {
 // filter option is on; the two passes of S6 together (they share the row-pair layout of the pass-1 array) when the
 // grid is strip-major with strips of 4 columns, i.e. written by the tensor-core gridding
 static bool rows_on_mma(const tcp_ctx* c) { return (c->tcfft & TCP_TCFFT_ROWS) && !(c->filter_fused && !c->try_ptab); }
-static bool ifft2_on_mma(const tcp_ctx* c) {
-    return (c->tcfft & (TCP_TCFFT_COLS | TCP_TCFFT_IROWS)) == (TCP_TCFFT_COLS | TCP_TCFFT_IROWS) && c->grid_strip == 4;
-}
 
 // tcp_recon_try: candidate centres of up to kMax / 2 pairs by value (a negative entry = no slice B in the last pair)
 struct TryCentres {
@@ -447,6 +444,7 @@ int tcp_read_workspace(tcp_ctx* c, int which, void* dst, size_t dst_bytes, tcp_s
 
 double tcp_scale(const tcp_ctx* c) { return c ? c->scale : 0.0; }
 int tcp_pass1_layout(const tcp_ctx* c) { return c && ifft2_on_mma(c) ? 1 : 0; }
+int tcp_grid_swizzled(const tcp_ctx* c) { return c && ifft2_on_mma(c) ? 1 : 0; }
 int tcp_fft_lines(tcp_ctx* c, const void* in_half2, void* out_float2, int batch, int inverse, tcp_stream_t stream) {
     if (!c || !in_half2 || !out_float2 || batch < 1) return set_error(TCP_EINVAL, "bad argument");
     if (!c->mf_ok) return set_error(TCP_EUNSUPPORTED, "tensor-core transforms need fp16 storage and M = 4096");

@@ -66,6 +66,13 @@ struct tcp_ctx {
     struct Pipe* pipe;
 };
 
+// The tensor-core transforms of the inverse 2D transform (k_mmafft.cu) take their input lines straight into their
+// swizzled shared-memory layout with one bulk copy, so their producers store rows pre-permuted: the gridding writes
+// row l2 of a grid strip at position swz<4>(l2), the column pass writes column l1 of a row pair at swz<2>(l1).
+static inline bool ifft2_on_mma(const tcp_ctx* c) {
+    return (c->tcfft & (TCP_TCFFT_COLS | TCP_TCFFT_IROWS)) == (TCP_TCFFT_COLS | TCP_TCFFT_IROWS) && c->grid_strip == 4;
+}
+
 namespace tcpk {
 
 int set_error(int code, const char* fmt, ...);
