@@ -74,12 +74,43 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
                                                           const float2* __restrict__ tw, const uint32_t* __restrict__ atab,
                                                           const float* __restrict__ hfilt, const float2* __restrict__ ptab, int nproj,
                                                           int nz, int try_mode, const float* __restrict__ wq,
-                                                          const uint16_t* __restrict__ raw, const float2* __restrict__ fdtab, int nunits) {
+                                                          const uint16_t* __restrict__ raw, const float2* __restrict__ fdtab, int npair_try) {
     constexpr int n = N / 2;
     extern __shared__ __align__(16) uint32_t L[];
     float2* T1TAB = reinterpret_cast<float2*>(L + 1 * N);               // pass-1 twiddle table behind the lines
+    // per-thread copies of the tables the epilogues and the loader need, [slot][thread] (conflict free, and a shared-memory
+    // wavefront moves 128 bytes where the L1 path of a global load moves a 32-byte sector per cycle)
+    float2* HT = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(T1TAB) + T1_BYTES);   // 2^12 H/M at (k0, k0 + 1) of the 8 output pairs
+    float4* PT = reinterpret_cast<float4*>(HT + 8 * NT);                // phase table / 2^12 at the same indices
+    float4* FD = PT + 8 * NT;                                           // RAW: (1/(flat-dark), dark) of the thread's 8 pixels, slices A and B
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, c = lane & 3;
-    // persistent CTAs: the thread's butterfly fragments and twiddles (scattered table reads) are set up once
+    // persistent CTAs: a CTA stays with ONE slice pair (blockIdx % npair), so everything that depends on the thread and the
+    // pair only -- butterfly fragments, twiddles, filter, phase and flat/dark tables -- is set up once
+    const int npair_grid = npair_try;                                  // slice pairs of the call
+    const int pair = blockIdx.x % npair_grid, jstart = blockIdx.x / npair_grid, jstep = gridDim.x / npair_grid;
+    const int zA = try_mode ? 0 : 2 * pair, zB = try_mode ? nz : 2 * pair + 1;
+    const bool hasB = zB < nz;
+    const int zBs = hasB ? zB : zA;
+    if (try_mode) ptab += (size_t)pair * N;
+    {
+        const int kbase = pass3_index<false>(0, 0, warp, g, c);
+#pragma unroll
+        for (int sl = 0; sl < 8; ++sl) {
+            const int k0 = kbase + 2048 * (sl & 1) + 64 * (sl >> 1);
+            const float2 h = __ldg(reinterpret_cast<const float2*>(hfilt + k0));
+            HT[sl * NT + tid] = make_float2(h.x * kRowScale, h.y * kRowScale);
+            const float4 p = __ldg(reinterpret_cast<const float4*>(ptab + k0));
+            const float s = 1.f / kRowScale;
+            PT[sl * NT + tid] = make_float4(p.x * s, p.y * s, p.z * s, p.w * s);
+        }
+        if constexpr (RAW) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                FD[q * NT + tid] = __ldg(reinterpret_cast<const float4*>(fdtab + (size_t)zA * n + tid * 8) + q);
+                FD[(4 + q) * NT + tid] = __ldg(reinterpret_cast<const float4*>(fdtab + (size_t)zBs * n + tid * 8) + q);
+            }
+        }
+    }
     AFrag An, Al;
     load_afrag(An, atab, AV_NAT, lane);
     load_afrag(Al, atab, AV_LO, lane);
@@ -89,14 +120,10 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
     Offs<1> O;
     make_offs<1>(O, warp, g, c);
     auto no_in = [](int) { return 0u; };
-    const float2* ptab0 = ptab;
+    const int kbase = pass3_index<false>(0, 0, warp, g, c);
+    auto slot_of = [&](int k0) { return 2 * (((k0 - kbase) >> 6) & 3) + ((k0 - kbase) >> 11); };   // folds to a constant per call site
 #pragma unroll 1
-    for (int unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
-    const int j = unit % nproj, pair = unit / nproj;
-    const int zA = try_mode ? 0 : 2 * pair, zB = try_mode ? nz : 2 * pair + 1;
-    const bool hasB = zB < nz;
-    const int zBs = hasB ? zB : zA;
-    ptab = try_mode ? ptab0 + (size_t)pair * N : ptab0;
+    for (int j = jstart; j < nproj; j += jstep) {
     const float wj = wq ? __ldg(&wq[j]) : 1.f;
 
     // ---- stage the two rows as half2 (pA, pB): 8 detector pixels per thread, 128-bit loads
@@ -107,11 +134,9 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
             const uint4 ra = __ldg(reinterpret_cast<const uint4*>(raw + ((size_t)j * nz + zA) * n + i0));
             const uint4 rb = __ldg(reinterpret_cast<const uint4*>(raw + ((size_t)j * nz + zBs) * n + i0));
             const unsigned ua[4] = {ra.x, ra.y, ra.z, ra.w}, ub[4] = {rb.x, rb.y, rb.z, rb.w};
-            const float4* fa = reinterpret_cast<const float4*>(fdtab + (size_t)zA * n + i0);
-            const float4* fb = reinterpret_cast<const float4*>(fdtab + (size_t)zBs * n + i0);
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                const float4 da = __ldg(fa + q), db = __ldg(fb + q);      // (rcp, dark) of pixels 2q, 2q + 1
+                const float4 da = FD[q * NT + tid], db = FD[(4 + q) * NT + tid];      // (rcp, dark) of pixels 2q, 2q + 1
                 // S1+S2 with the arithmetic of normalize_half_kernel (tcp_internal.h), rounded to the storage type
                 a[2 * q] = -0.69314718055994531f * fast_lg2(fmaxf((u16f(ua[q] & 0xffffu) - da.y) * da.x, 1e-6f));
                 a[2 * q + 1] = -0.69314718055994531f * fast_lg2(fmaxf((u16f(ua[q] >> 16) - da.w) * da.z, 1e-6f));
@@ -153,8 +178,8 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
     pass2<1, false>(L, An, T, O);
     __syncthreads();
     pass3<1, false, false, true>(L, Al, O, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
-        const float2 h = __ldg(reinterpret_cast<const float2*>(hfilt + k0));
-        const float h0 = h.x * kRowScale, h1 = h.y * kRowScale;
+        const float2 h = HT[slot_of(k0) * NT + tid];
+        const float h0 = h.x, h1 = h.y;
         *reinterpret_cast<uint2*>(&L[swz<1>(k0)]) = make_uint2(pack_h2(y0[0].x * h0, y0[0].y * h0), pack_h2(y1[0].x * h1, y1[0].y * h1));
     });
     __syncthreads();
@@ -178,10 +203,9 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
     __syncthreads();
     __half2* out = spec + ((size_t)pair * nproj + j) * N;
     pass3<1, false, false, false>(L, Al, O, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
-        const float4 p = __ldg(reinterpret_cast<const float4*>(ptab + k0));
-        const float s = 1.f / kRowScale;
-        const float2 v0 = make_float2((y0[0].x * p.x - y0[0].y * p.y) * s, (y0[0].x * p.y + y0[0].y * p.x) * s);
-        const float2 v1 = make_float2((y1[0].x * p.z - y1[0].y * p.w) * s, (y1[0].x * p.w + y1[0].y * p.z) * s);
+        const float4 p = PT[slot_of(k0) * NT + tid];
+        const float2 v0 = make_float2(y0[0].x * p.x - y0[0].y * p.y, y0[0].x * p.y + y0[0].y * p.x);
+        const float2 v1 = make_float2(y1[0].x * p.z - y1[0].y * p.w, y1[0].x * p.w + y1[0].y * p.z);
         *reinterpret_cast<uint2*>(out + k0) = make_uint2(pack_h2(v0.x, v0.y), pack_h2(v1.x, v1.y));
     });
     __syncthreads();                      // the line is free for the next unit's rows
@@ -373,14 +397,15 @@ __global__ void __launch_bounds__(NT, 2) fft_lines_kernel(const uint32_t* __rest
 
 // ------------------------------------------------------------------------------------------------ launchers
 int launch_rows_mma(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw) {
-    const size_t smem = (size_t)N * 4 + T1_BYTES;
+    const size_t smem = (size_t)N * 4 + T1_BYTES + 8 * NT * (8 + 16 + (raw ? 16 : 0));
     auto kern = raw ? (c->pad ? rows_mma_kernel<true, true> : rows_mma_kernel<false, true>)
                     : (c->pad ? rows_mma_kernel<true, false> : rows_mma_kernel<false, false>);
     TCP_SMEM(kern, smem);
-    const int nunits = c->nproj * c->npair;
-    kern<<<std::min(nunits, 2 * c->nsm), NT, smem, st>>>((const __half*)c->sino, (__half2*)c->spec, c->tw, c->mf_atab, c->hfilt,
-                                                         c->try_ptab ? c->try_ptab : c->ptab, c->nproj, c->nz, c->try_ptab ? 1 : 0,
-                                                         c->angle_weights ? c->wq : nullptr, raw, c->fdtab, nunits);
+    // gridDim = npair x (CTAs per pair): every CTA keeps one slice pair and strides over the projections
+    const int per_pair = std::max(1, std::min(c->nproj, (2 * c->nsm) / c->npair));
+    kern<<<c->npair * per_pair, NT, smem, st>>>((const __half*)c->sino, (__half2*)c->spec, c->tw, c->mf_atab, c->hfilt,
+                                                c->try_ptab ? c->try_ptab : c->ptab, c->nproj, c->nz, c->try_ptab ? 1 : 0,
+                                                c->angle_weights ? c->wq : nullptr, raw, c->fdtab, c->npair);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }
