@@ -49,6 +49,12 @@ def lib():
         _lib.orc_kernel_alpha.restype = C.c_double
         _lib.orc_kernel_alpha.argtypes = [C.c_int]
         _lib.orc_num_threads.restype = C.c_int
+        _lib.orc_kernel_phi.restype = C.c_double
+        _lib.orc_kernel_phi.argtypes = [C.c_int, C.c_double]
+        _lib.orc_kernel_phihat.restype = C.c_double
+        _lib.orc_kernel_phihat.argtypes = [C.c_int, C.c_double, C.c_int]
+        _lib.orc_bessel_i0.restype = C.c_double
+        _lib.orc_bessel_i0.argtypes = [C.c_double]
     return _lib
 
 
@@ -74,6 +80,23 @@ def num_threads() -> int:
 
 def kernel_alpha(m: int = DEFAULT_M) -> float:
     return float(lib().orc_kernel_alpha(int(m)))
+
+
+KB = 16     # kernel code = half-width m (Gaussian) or KB + m (Kaiser-Bessel window); every `m` argument below takes a code
+
+
+def kernel_phi(code: int, t: float) -> float:
+    """Interpolation weight phi(t) of the kernel `code` (0 outside the open box |t| < m)."""
+    return float(lib().orc_kernel_phi(int(code), float(t)))
+
+
+def kernel_phihat(code: int, x: float, M: int) -> float:
+    """Continuous transform of phi at x / M cycles per grid cell (the deapodisation factor of image coordinate x)."""
+    return float(lib().orc_kernel_phihat(int(code), float(x), int(M)))
+
+
+def bessel_i0(z: float) -> float:
+    return float(lib().orc_bessel_i0(float(z)))
 
 
 def dft(x, sign=-1):

@@ -32,6 +32,50 @@ void orc_spectrum_fused(const double*, int, int, double, int, int, cplx*);
 static inline double kernel_alpha(int m) { return PI / (std::sqrt(2.0) * (double)m); }
 double orc_kernel_alpha(int m) { return kernel_alpha(m); }
 
+// The (phi, Phi^) pair as one switch, so that a narrower kernel can be swapped in "in both implementations at once"
+// (reading Q21).  The kernel argument of every function below is a CODE:
+//   m            (1..15)   Gaussian of half-width m, exactly the arithmetic above (unchanged);
+//   16 + m                 Kaiser-Bessel window of half-width m (the textbook gridding kernel of the NUFFT literature the
+//                          paper's Fourier method cites):
+//                            phi(t)  = I0(beta sqrt(1 - (t/m)^2)) / I0(beta)  for |t| < m, else 0,
+//                            Phi^(x) = (2m / I0(beta)) sinh(z) / z,  z = sqrt(beta^2 - (2 pi m x / M)^2)   (its exact transform),
+//                            beta    = pi sqrt((2m/sigma)^2 (sigma - 1/2)^2 - 0.8),  sigma = 2 the oversampling (Beatty et al. 2005).
+static inline int k_half(int code) { return code & 15; }
+static inline bool k_is_kb(int code) { return (code >> 4) == 1; }
+static inline double kb_beta(int m) { return PI * std::sqrt((double)m * (double)m * 2.25 - 0.8); }
+// modified Bessel function of order 0 by its power series sum ((z/2)^2)^k / (k!)^2 (all terms positive: no cancellation)
+static double bessel_i0(double z) {
+    const double q = 0.25 * z * z;
+    double term = 1.0, sum = 1.0;
+    for (int k = 1; k < 200; ++k) {
+        term *= q / ((double)k * (double)k);
+        sum += term;
+        if (term < 1e-18 * sum) break;
+    }
+    return sum;
+}
+static double k_phi(int code, double t) {                 // interpolation weight at distance t, zero outside the open box
+    const int m = k_half(code);
+    if (!(std::fabs(t) < (double)m)) return 0.0;
+    if (!k_is_kb(code)) return std::exp(-kernel_alpha(m) * t * t);
+    const double beta = kb_beta(m), u = 1.0 - (t / (double)m) * (t / (double)m);
+    return bessel_i0(beta * std::sqrt(u > 0.0 ? u : 0.0)) / bessel_i0(beta);
+}
+static double k_phihat(int code, double x, int M) {       // continuous transform of phi at frequency x / M cycles per cell
+    const int m = k_half(code);
+    if (!k_is_kb(code)) {
+        const double alpha = kernel_alpha(m);
+        return std::sqrt(PI / alpha) * std::exp(-PI * PI * x * x / (alpha * (double)M * (double)M));
+    }
+    const double beta = kb_beta(m), a = 2.0 * PI * (double)m * x / (double)M, z2 = beta * beta - a * a;
+    const double z = std::sqrt(std::fabs(z2));
+    const double sh = z2 > 0.0 ? (z < 1e-8 ? 1.0 : std::sinh(z) / z) : (z < 1e-8 ? 1.0 : std::sin(z) / z);
+    return 2.0 * (double)m * sh / bessel_i0(beta);
+}
+double orc_kernel_phi(int code, double t) { return k_phi(code, t); }
+double orc_kernel_phihat(int code, double x, int M) { return k_phihat(code, x, M); }
+double orc_bessel_i0(double z) { return bessel_i0(z); }
+
 // ---------------------------------------------------------------------------
 // B_exact: the sum that gridding approximates (adjoint type-1 non-uniform DFT):
 //   f[iy][ix] = Re sum_j sum_k G[j][k] exp(2 pi i (k/M) (x cos_j + y sin_j)),  k signed.
@@ -116,8 +160,8 @@ void orc_project_lin_adjoint(const double* f, const float* theta, int nproj, int
 // ---------------------------------------------------------------------------
 static inline int wrap(long l, int M) { long r = l % M; return (int)(r < 0 ? r + M : r); }
 
-void orc_grid(const cplx* G, const float* theta, int nproj, int n, int m, cplx* F) {
-    const int M = 2 * n;
+void orc_grid(const cplx* G, const float* theta, int nproj, int n, int code, cplx* F) {
+    const int M = 2 * n, m = k_half(code);
     const double alpha = kernel_alpha(m);
     for (size_t i = 0; i < (size_t)M * M; ++i) F[i] = 0.0;
     std::vector<double> w1(2 * m), w2(2 * m);
@@ -129,6 +173,11 @@ void orc_grid(const cplx* G, const float* theta, int nproj, int n, int m, cplx* 
             long l01 = (long)std::floor(nu1), l02 = (long)std::floor(nu2);
             for (int a = -m + 1; a <= m; ++a) {   // candidates floor(nu)-m+1 .. floor(nu)+m
                 double t1 = (double)(l01 + a) - nu1, t2 = (double)(l02 + a) - nu2;
+                if (k_is_kb(code)) {
+                    w1[a + m - 1] = k_phi(code, t1);
+                    w2[a + m - 1] = k_phi(code, t2);
+                    continue;
+                }
                 w1[a + m - 1] = (std::fabs(t1) < (double)m) ? std::exp(-alpha * t1 * t1) : 0.0;
                 w2[a + m - 1] = (std::fabs(t2) < (double)m) ? std::exp(-alpha * t2 * t2) : 0.0;
             }
@@ -146,8 +195,8 @@ void orc_grid(const cplx* G, const float* theta, int nproj, int n, int m, cplx* 
 
 // Literal transpose of S5 (gather with the same weights), for P8:
 //   G*[j][k] = sum_taps w_1 w_2 F[l2 mod M][l1 mod M].
-void orc_grid_adjoint(const cplx* F, const float* theta, int nproj, int n, int m, cplx* G) {
-    const int M = 2 * n;
+void orc_grid_adjoint(const cplx* F, const float* theta, int nproj, int n, int code, cplx* G) {
+    const int M = 2 * n, m = k_half(code);
     const double alpha = kernel_alpha(m);
     for (int j = 0; j < nproj; ++j) {
         double cs = std::cos((double)theta[j]), sn = std::sin((double)theta[j]);
@@ -161,7 +210,7 @@ void orc_grid_adjoint(const cplx* F, const float* theta, int nproj, int n, int m
                     double t1 = (double)(l01 + a1) - nu1, t2 = (double)(l02 + a2) - nu2;
                     if (std::fabs(t1) >= (double)m || std::fabs(t2) >= (double)m) continue;
                     acc += F[(size_t)wrap(l02 + a2, M) * M + wrap(l01 + a1, M)] *
-                           (std::exp(-alpha * t1 * t1) * std::exp(-alpha * t2 * t2));
+                           (k_is_kb(code) ? k_phi(code, t1) * k_phi(code, t2) : std::exp(-alpha * t1 * t1) * std::exp(-alpha * t2 * t2));
                 }
             G[(size_t)j * M + k] = acc;
         }
@@ -194,14 +243,15 @@ void orc_fft2(const cplx* F, int M, int sign, cplx* g) {
 //   f[iy][ix] = g[y mod M][x mod M] / (Phi^(x) Phi^(y)),  x = ix - n/2, y = iy - n/2.
 // Real part -> fre; imaginary part (second slice of a packed pair) -> fim if not NULL.
 // ---------------------------------------------------------------------------
-void orc_deapod_crop(const cplx* g, int n, int m, double* fre, double* fim) {
-    const int M = 2 * n;
+void orc_deapod_crop(const cplx* g, int n, int code, double* fre, double* fim) {
+    const int M = 2 * n, m = k_half(code);
     const double alpha = kernel_alpha(m);
     for (int iy = 0; iy < n; ++iy)
         for (int ix = 0; ix < n; ++ix) {
             double x = ix - n / 2, y = iy - n / 2;
             double px = std::sqrt(PI / alpha) * std::exp(-PI * PI * x * x / (alpha * (double)M * (double)M));
             double py = std::sqrt(PI / alpha) * std::exp(-PI * PI * y * y / (alpha * (double)M * (double)M));
+            if (k_is_kb(code)) { px = k_phihat(code, x, M); py = k_phihat(code, y, M); }
             cplx v = g[(size_t)wrap((long)y, M) * M + wrap((long)x, M)] / (px * py);
             fre[(size_t)iy * n + ix] = v.real();
             if (fim) fim[(size_t)iy * n + ix] = v.imag();
@@ -209,8 +259,8 @@ void orc_deapod_crop(const cplx* g, int n, int m, double* fre, double* fim) {
 }
 
 // Literal transpose of S7 (divide, zero-embed at (y mod M, x mod M)), for P8.
-void orc_deapod_crop_adjoint(const double* fre, const double* fim, int n, int m, cplx* g) {
-    const int M = 2 * n;
+void orc_deapod_crop_adjoint(const double* fre, const double* fim, int n, int code, cplx* g) {
+    const int M = 2 * n, m = k_half(code);
     const double alpha = kernel_alpha(m);
     for (size_t i = 0; i < (size_t)M * M; ++i) g[i] = 0.0;
     for (int iy = 0; iy < n; ++iy)
@@ -218,6 +268,7 @@ void orc_deapod_crop_adjoint(const double* fre, const double* fim, int n, int m,
             double x = ix - n / 2, y = iy - n / 2;
             double px = std::sqrt(PI / alpha) * std::exp(-PI * PI * x * x / (alpha * (double)M * (double)M));
             double py = std::sqrt(PI / alpha) * std::exp(-PI * PI * y * y / (alpha * (double)M * (double)M));
+            if (k_is_kb(code)) { px = k_phihat(code, x, M); py = k_phihat(code, y, M); }
             cplx v(fre[(size_t)iy * n + ix], fim ? fim[(size_t)iy * n + ix] : 0.0);
             g[(size_t)wrap((long)y, M) * M + wrap((long)x, M)] = v / (px * py);
         }
