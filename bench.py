@@ -86,7 +86,12 @@ class ClockSampler:
 
 
 KERNEL_NAMES = {"normalize": "normalize_half_kernel / normalize_kernel", "rows": "rows_kernel", "ifft_cols": "ifft_cols_pf_kernel / ifft_cols_kernel",
-                "ifft_rows": "ifft_rows_kernel"}
+                "ifft_rows": "ifft_rows_kernel", "grid": "grid_tile_kernel"}
+KERNEL_NAMES_MMA = {"rows": "rows_mma_kernel", "ifft_cols": "cols_mma_kernel", "ifft_rows": "irows_mma_kernel", "grid": "grid_mma_kernel"}
+
+
+def kernel_label(m):
+    return "Kaiser-Bessel half-width %d" % (m & 15) if m >> 4 else "Gaussian half-width %d" % m
 
 
 def stage_model(w, nz, m, half_store, half_out, fused_s12=False):
@@ -103,10 +108,11 @@ def stage_model(w, nz, m, half_store, half_out, fused_s12=False):
     if fused_s12:
         return {
             "rows": {"bytes": P * nz * n * 2 + npair * P * M * bc, "flops": 3 * fft * npair * P + 10.0 * P * nz * n},
-            "grid": {"bytes": npair * P * M * bc + npair * M * M * bc, "flops": 4.0 * (2 * m) ** 2 * npair * P * M},
+            "grid": {"bytes": npair * P * M * bc + npair * M * M * bc, "flops": 4.0 * (2 * (m & 15)) ** 2 * npair * P * M},
             "ifft_cols": {"bytes": npair * M * M * bc + npair * n * M * bc, "flops": fft * npair * M},
             "ifft_rows": {"bytes": npair * n * M * bc + nz * n * n * bo, "flops": fft * npair * n},
         }
+    m = m & 15                              # kernel code -> half-width (taps per axis = 2 m)
     return {
         "normalize": {"bytes": P * nz * n * (2 + br), "flops": 10.0 * P * nz * n},
         "rows": {"bytes": P * nz * n * br + npair * P * M * bc, "flops": 3 * fft * npair * P},
@@ -187,6 +193,59 @@ def replica_slices(nz_total, nz_chunk, world):
     (rounded down to whole chunks); the job's voxel count is world times that."""
     nz = nz_total - nz_total % nz_chunk
     return nz, world * nz
+
+
+def measure_config(name, dtype, m, steps, warmup, dev, hbm_gbs):
+    """Compute-only throughput of another BASELINE.json config (whole volume resident in HBM, CUDA events around the
+    chunk loop, per-kernel events from the library): the `configs` entries of the bench line."""
+    import torch
+    import synthgen as sg
+    import paper_2209_08450_b200 as tcp
+
+    w = sg.make_workload(name, dtype=dtype)
+    nzc, n = w.nz_chunk, w.n
+    nz_total = w.nz_total - w.nz_total % nzc
+    nchunks = nz_total // nzc
+    half_store, half_out = w.dtype != "f32", w.dtype == "f16"
+    raw, flat, dark, _ = build_volume(w, nz_total, dev)
+    theta = torch.from_numpy(w.theta).to(dev)
+    out = torch.empty((nz_total, n, n), dtype=torch.float16 if half_out else torch.float32, device=dev)
+    r = tcp.Recon(n, w.nproj, nzc, w.center, w.dtype, w.filter, m)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        for ch in range(nchunks):
+            r.recon(raw[ch], flat[ch], dark[ch], theta, out=out[ch * nzc:(ch + 1) * nzc], stream=stream)
+
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    r.set_profile(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stage_ms, ncalls = {k: 0.0 for k in r.STAGES}, 0
+    e0.record(stream)
+    for _ in range(steps):
+        step()
+        ms, nc = r.profile_collect()
+        for k in ms:
+            stage_ms[k] += ms[k]
+        ncalls += nc
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_step = e0.elapsed_time(e1) / steps
+    r.set_profile(False)
+    launches = r.launches_per_recon
+    r.close()
+    whole = sum(v["bytes"] for v in stage_model(w, nzc, m, half_store, half_out).values()) * nchunks
+    res = {"workload": "%s: %d proj x %d x %d u16 -> %d^2 x %d voxels, %s, %d-slice chunks, %s, %s filter"
+                       % (w.name, w.nproj, nz_total, n, n, nz_total, w.dtype, nzc, kernel_label(m), w.filter),
+           "value": float(nz_total) * n * n / (ms_step * 1e-3) / 1e9, "unit": "GVoxel/s", "ms_per_step": ms_step,
+           "slices_per_s": nz_total / (ms_step * 1e-3), "steps": steps, "warmup": warmup,
+           "whole_path_hbm_frac": whole / (ms_step * 1e-3) / 1e9 / hbm_gbs, "launches_per_chunk": launches,
+           "ms_per_chunk": {k: stage_ms[k] / max(ncalls, 1) for k in stage_ms}}
+    del raw, flat, dark, out
+    torch.cuda.empty_cache()
+    return res
 
 
 def run_ours(args, rank, world, local_rank):
@@ -302,11 +361,14 @@ def run_ours(args, rank, world, local_rank):
 
     if rank != 0:
         return
-    # ---- roofline of the dominant kernel
+    # ---- roofline of the dominant kernel.  Denominators are MEASURED: the HBM copy rate of MEASURED_PEAKS.json and the
+    # fp32 FFMA / fp16 mma.sync issue rates of this GPU at this moment (tcp_measure_rates; both kernels are in the library).
     hbm_gbs, sm_max_mhz, which = _peaks()
+    fp32_peak, hmma_peak = tcp.tcp_measure_rates()
     fused_s12 = half_store and not args.fused_filter and args.algorithm == "fourier"      # tcp.h: TCP_OPT_FUSE_NORMALIZE
+    on_mma = half_store and n == 2048 and args.algorithm == "fourier"                     # tcp.h: TCP_OPT_TCFFT default
     model = stage_model(w, nzc, m, half_store, half_out, fused_s12)
-    alu_peak = 148 * 128 * 2 * sm_max_mhz * 1e6 / 1e12        # fp32 FMA lanes x 2 flop x clock, TFLOP/s
+    alu_peak = fp32_peak
     kernels = {}
     for k in model:
         t = stage_ms[k] / max(ncalls, 1) * 1e-3               # average launch duration, s
@@ -314,9 +376,9 @@ def run_ours(args, rank, world, local_rank):
                       "GBps": model[k]["bytes"] / t / 1e9 if t > 0 else None,
                       "TFLOPps": model[k]["flops"] / t / 1e12 if t > 0 else None,
                       # fractions of roofline: algorithmic bytes against the measured HBM peak, algorithmic flops
-                      # (5 N log2 N per transform, 4 per gridding tap, pair and sample) against the fp32 CUDA-core peak
-                      "hbm_frac": model[k]["bytes"] / t / 1e9 / hbm_gbs if t > 0 else None,
-                      "fp32_frac": model[k]["flops"] / t / 1e12 / alu_peak if t > 0 else None}
+                      # (5 N log2 N per transform, 4 per gridding tap, pair and sample) against the measured fp32 peak
+                      "frac_hbm": model[k]["bytes"] / t / 1e9 / hbm_gbs if t > 0 else None,
+                      "frac_alu": model[k]["flops"] / t / 1e12 / alu_peak if t > 0 else None}
     dom = max(model, key=lambda k: stage_ms[k])
     traffic = None           # DRAM bytes per launch of the dominant kernel from the committed ncu capture
     try:
@@ -326,24 +388,19 @@ def run_ours(args, rank, world, local_rank):
                     traffic = int(ln.split(",")[1])
     except Exception:
         pass
-    if dom == "grid":
-        # the gridding kernel is bound by CUDA-core instruction issue (weight generation), not by HBM and not
-        # by the tensor pipe (profiles/): its roofline is the fp32 FMA peak against the ALGORITHMIC flops of
-        # the gridding sum, 4 flops per tap, pair and sample
-        roof = {"kernel": "grid_mma_kernel" if half_store else "grid_tile_kernel", "bound": "alu",
-                "achieved": kernels[dom]["TFLOPps"], "peak": alu_peak,
-                "unit": "TFLOP/s", "frac": kernels[dom]["TFLOPps"] / alu_peak, "traffic": traffic,
-                "peak_source": "148 SMs x 128 fp32 lanes x 2 x %.0f MHz (DESIGN.md)" % sm_max_mhz}
-    elif (kernels[dom]["fp32_frac"] or 0) > (kernels[dom]["hbm_frac"] or 0):
-        # a transform kernel closer to the fp32 CUDA-core roof (5 N log2 N flops per transform) than to the HBM roof
-        # (the Stockham kernels are bound by FMA issue and the shared-memory data pipe)
-        roof = {"kernel": KERNEL_NAMES.get(dom, dom), "bound": "alu", "achieved": kernels[dom]["TFLOPps"], "peak": alu_peak,
-                "unit": "TFLOP/s", "frac": kernels[dom]["TFLOPps"] / alu_peak, "traffic": traffic,
-                "hbm_frac": kernels[dom]["hbm_frac"],
-                "peak_source": "148 SMs x 128 fp32 lanes x 2 x %.0f MHz (DESIGN.md)" % sm_max_mhz}
-    else:
-        roof = {"kernel": KERNEL_NAMES.get(dom, dom), "bound": "hbm", "achieved": kernels[dom]["GBps"], "peak": hbm_gbs, "unit": "GB/s",
-                "frac": kernels[dom]["GBps"] / hbm_gbs, "traffic": traffic, "peak_source": "MEASURED_PEAKS.json (%s)" % which}
+    names = dict(KERNEL_NAMES, **(KERNEL_NAMES_MMA if on_mma else ({"grid": "grid_mma_kernel"} if half_store else {})))
+    # SURVEY 8(d) assigns the roofs: normalise and the 2D transform passes HBM, gridding "plain ALUs / smem / L2", the
+    # row kernel "HBM if half2 math; else fp32 ALUs".  Both fractions are reported for every kernel; `bound` names the
+    # roof 8(d) assigns to the dominant one and `frac` is the fraction of that roof.
+    assigned = {"normalize": "hbm", "rows": "alu", "grid": "alu", "ifft_cols": "hbm", "ifft_rows": "hbm"}[dom]
+    roof = {"kernel": names.get(dom, dom), "bound": assigned,
+            "achieved": kernels[dom]["TFLOPps"] if assigned == "alu" else kernels[dom]["GBps"],
+            "peak": alu_peak if assigned == "alu" else hbm_gbs, "unit": "TFLOP/s" if assigned == "alu" else "GB/s",
+            "frac": kernels[dom]["frac_alu"] if assigned == "alu" else kernels[dom]["frac_hbm"],
+            "frac_hbm": kernels[dom]["frac_hbm"], "frac_alu": kernels[dom]["frac_alu"], "traffic": traffic,
+            "peak_source": "fp32: tcp_measure_rates (FFMA issue rate measured in this run); HBM: MEASURED_PEAKS.json (%s)" % which,
+            "peaks": {"hbm_GBps": hbm_gbs, "fp32_TFLOPps": fp32_peak, "hmma_f16_TFLOPps": hmma_peak,
+                      "fp32_nominal_TFLOPps": 148 * 128 * 2 * sm_max_mhz * 1e6 / 1e12}}
     # whole path: SURVEY 8(d)'s algorithmic figure of the method (40 B/voxel at C4), whether or not a stage is fused away
     whole_bytes = sum(v["bytes"] for v in stage_model(w, nzc, m, half_store, half_out).values()) * nchunks
     if fused_s12:
@@ -352,8 +409,10 @@ def run_ours(args, rank, world, local_rank):
         "metric": "reconstructed GVoxel/s", "value": value, "unit": "GVoxel/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": {"f32": "f32", "f16": "f16", "f16_out32": "f16"}[w.dtype], "data": "synthetic",
-        "config": {"workload": "%s: %d proj x %d x %d u16 -> %d^2 x %d voxels, %s, %d-slice chunks, m=%d, %s filter"
-                   % (w.name, w.nproj, nz_total, n, n, nz_total, w.dtype, nzc, m, w.filter) + variant,
+        "config": {"workload": "%s: %d proj x %d x %d u16 -> %d^2 x %d voxels, %s, %d-slice chunks, %s, %s filter"
+                   % (w.name, w.nproj, nz_total, n, n, nz_total, w.dtype, nzc, kernel_label(m), w.filter) + variant,
+                   "gridding_kernel": kernel_label(m) + " (tcp_create_ex code %d)" % m,
+                   "transforms": "radix-16 butterflies on mma.sync (TCP_OPT_TCFFT = 7)" if on_mma else "fp32 Stockham on the CUDA cores",
                    "l2": "inputs larger than L2 (%.1f GB raw resident in HBM)" % (raw.numel() * 2 / 1e9),
                    "replicas": world},
         "slices_per_s": world * nz_total / (ms_step * 1e-3),
@@ -371,6 +430,17 @@ def run_ours(args, rank, world, local_rank):
         if not variant:      # the oracle leg reconstructs the contract's default chain
             cb["parity_rel_l2_max"] = max(err)
         line["cpu_baseline"] = cb
+    if args.configs and world == 1 and not variant:
+        # the other configs of BASELINE.json, compute-only, in the same run (the headline config is the line itself)
+        r.close()
+        del raw, flat, dark, out
+        torch.cuda.empty_cache()
+        line["configs"] = []
+        for name, dt in (("C1", None), ("C2", "f32"), ("C2", "f16"), ("C3", None), ("C5", None)):
+            try:
+                line["configs"].append(measure_config(name, dt, m, 2, 3, dev, hbm_gbs))
+            except Exception as e:        # a config that does not fit this box is reported, not fatal
+                line["configs"].append({"workload": name, "error": str(e)[:200]})
     print(json.dumps(line))
 
 
@@ -419,7 +489,7 @@ def run_reference(args, rank, world):
         "impl": "reference", "metric": "reconstructed GVoxel/s", "value": v, "unit": "GVoxel/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "%s: %d proj x %d px, m=%d, %s filter (bounded sample)" % (w.name, w.nproj, w.n, m, w.filter)},
+        "config": {"workload": "%s: %d proj x %d px, %s, %s filter (bounded sample)" % (w.name, w.nproj, w.n, kernel_label(m), w.filter)},
         "cpu_baseline": {"value": v, "unit": "GVoxel/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": v, "unit": "GVoxel/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -435,7 +505,10 @@ def main():
     ap.add_argument("--workload", default="C4")
     ap.add_argument("--nz", type=int, default=0, help="override the number of slices in the volume")
     ap.add_argument("--nz-chunk", type=int, default=0)
-    ap.add_argument("--m", type=int, default=3, help="gridding kernel half-width")
+    ap.add_argument("--m", type=int, default=16 + 2,
+                    help="gridding kernel code of tcp_create_ex: 3, 4 = Gaussian half-width; 16 + 2 (default), 16 + 3 = Kaiser-Bessel")
+    ap.add_argument("--no-configs", dest="configs", action="store_false",
+                    help="skip the compute-only runs of the other BASELINE.json configs (the `configs` key)")
     ap.add_argument("--e2e-nz", type=int, default=0,
                     help="slices streamed through the host pipeline per step (0: the whole volume; halved if pinned host memory runs out)")
     ap.add_argument("--dtype", default="", choices=["", "f32", "f16", "f16_out32"],

@@ -108,8 +108,14 @@ enum { TCP_ST_TRIG = 0, TCP_ST_NORMALIZE = 1, TCP_ST_ROWS = 2, TCP_ST_GRID = 3, 
  * Returns NULL on error (see tcp_last_error). */
 tcp_ctx* tcp_create(int n, int nproj, int nz_chunk, float center, int dtype, int filter);
 
-/* As tcp_create, with the gridding kernel half-width m in {3, 4} (taps per axis = 2m;
- * 0 = default 3, which meets the 2e-3 gridding-vs-exact gate with 3x margin). */
+/* As tcp_create, with the gridding kernel as a code m (taps per axis = 2 x half-width):
+ *   0            the default, 3;
+ *   3, 4         Gaussian phi(t) = exp(-alpha t^2) of that half-width (3 meets the 2e-3 gridding-vs-exact gate with 2.7x margin);
+ *   16 + 2, 16 + 3   TCP_KERNEL_KB + half-width: Kaiser-Bessel window phi(t) = I0(beta sqrt(1 - (t/m)^2)) / I0(beta),
+ *                beta = pi sqrt(2.25 m^2 - 0.8), deapodised by its exact transform (the "accuracy controls" of PAPER.md:173,
+ *                DESIGN.md reading Q21).  Half-width 2 reaches 3.9e-4 of the exact sum on the C1 phantom with 16 taps
+ *                per sample where the Gaussian needs 36 for 7.4e-4.  Tile and tensor-core griddings only. */
+enum { TCP_KERNEL_GAUSS = 0, TCP_KERNEL_KB = 16 };
 tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, int filter, int m);
 
 /* Detector width that is not a power of two ("16-bit data are additionally padded/unpadded to
@@ -171,6 +177,11 @@ int tcp_grid_swizzled(const tcp_ctx* ctx);
  * X[k] = sum_i x[i] e^{-/+ 2 pi i ik/4096} (inverse != 0: +, unnormalised), natural order on both sides.
  * TCP_EUNSUPPORTED unless the context has fp16 storage and M = 4096. */
 int tcp_fft_lines(tcp_ctx* ctx, const void* in_half2, void* out_float2, int batch, int inverse, tcp_stream_t stream);
+/* Measurement helper (blocks, ~20 ms, current device, default stream): issue-rate micro-benchmarks for the arithmetic
+ * roofs bench.py reports against.  *fp32_tflops (HOST): FFMA throughput with 16 independent chains per thread;
+ * *hmma_tflops (HOST): mma.sync m16n8k16 fp16 -> fp32 throughput with 8 independent chains per warp (the instruction of
+ * the tensor-core transforms).  Both at the clocks of the moment. */
+int tcp_measure_rates(double* fp32_tflops, double* hmma_tflops);
 /* Power-of-two factor by which SPECTRUM/GRID/PASS1 are scaled relative to S4's G (1 in fp32). */
 double tcp_scale(const tcp_ctx* ctx);
 /* Total device bytes the context allocated; kernels launched by one tcp_recon. */

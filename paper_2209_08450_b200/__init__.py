@@ -23,6 +23,7 @@ from .binding import (  # noqa: F401
     tcp_slice_range,
     tcp_check_angles,
     tcp_last_error,
+    tcp_measure_rates,
     DTYPES,
     FILTERS,
     EXPORTS,

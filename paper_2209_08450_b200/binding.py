@@ -21,7 +21,7 @@ EXPORTS = [
     "tcp_mean_frames_u16", "tcp_normalize", "tcp_workspace", "tcp_read_workspace", "tcp_scale", "tcp_grid_strip",
     "tcp_workspace_bytes", "tcp_launches_per_recon", "tcp_set_option", "tcp_profile_collect",
     "tcp_recon_volume_host", "tcp_recon_try", "tcp_create_det", "tcp_padded_n",
-    "tcp_recon_volume_host_rows", "tcp_slice_range", "tcp_check_angles", "tcp_pass1_layout", "tcp_fft_lines",
+    "tcp_recon_volume_host_rows", "tcp_slice_range", "tcp_check_angles", "tcp_pass1_layout", "tcp_grid_swizzled", "tcp_fft_lines", "tcp_measure_rates",
 ]
 
 
@@ -93,6 +93,8 @@ def lib():
     L.tcp_grid_swizzled.argtypes = [vp]
     L.tcp_fft_lines.restype = ci
     L.tcp_fft_lines.argtypes = [vp, vp, vp, ci, ci, vp]
+    L.tcp_measure_rates.restype = ci
+    L.tcp_measure_rates.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.tcp_recon_try.restype = ci
     L.tcp_recon_try.argtypes = [vp, vp, vp, vp, vp, C.POINTER(cf), ci, vp, vp]
     _lib = L
@@ -139,6 +141,13 @@ def tcp_create(n, nproj, nz_chunk, center, dtype, filter):
     if not h:
         raise TcpError("tcp_create failed: " + tcp_last_error())
     return h
+
+
+def tcp_measure_rates():
+    """(fp32 FFMA TFLOP/s, fp16 mma.sync TFLOP/s) measured on the current device (tcp_measure_rates)."""
+    a, b = C.c_double(0.0), C.c_double(0.0)
+    _check(lib().tcp_measure_rates(C.byref(a), C.byref(b)))
+    return float(a.value), float(b.value)
 
 
 def tcp_create_ex(n, nproj, nz_chunk, center, dtype, filter, m):

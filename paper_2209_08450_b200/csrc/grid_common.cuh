@@ -25,6 +25,21 @@ __device__ __forceinline__ float ex2_approx(float x) {
     return y;
 }
 
+// Kaiser-Bessel window (kernel code 16 + m, reading Q21): phi(d) = I0(beta sqrt(u)) / I0(beta), u = 1 - (d/m)^2,
+// from a table of phi over u in [0, 1] (KB_NTAB intervals, built in fp64 at create) with linear interpolation:
+// |error| <= h^2 / 8 max|phi''(u)| = 4e-7 at beta = 13.9, below the fp32 path's 1e-5 gate.
+constexpr int KB_NTAB = 4096;
+__device__ __forceinline__ float kb_weight(const float* __restrict__ tab, float d, float inv_m2) {
+    const float u = fmaxf(fmaf(-d * d, inv_m2, 1.f), 0.f) * (float)KB_NTAB;
+    const int i = min((int)u, KB_NTAB - 1);
+    const float a = __ldg(tab + i), b = __ldg(tab + i + 1);
+    return fmaf(u - (float)i, b - a, a);
+}
+// weight of one tap at distance d: Gaussian 2^(-k2 d^2) (kbtab == NULL, k2 = alpha log2 e) or the table (k2 = 1 / m^2)
+__device__ __forceinline__ float tap_weight(const float* __restrict__ kbtab, float d, float k2) {
+    return kbtab ? kb_weight(kbtab, d, k2) : ex2_approx(-k2 * d * d);
+}
+
 template <class TC> __device__ __forceinline__ TC czero();
 template <> __device__ __forceinline__ float2 czero<float2>() { return make_float2(0.f, 0.f); }
 template <> __device__ __forceinline__ __half2 czero<__half2>() { return __floats2half2_rn(0.f, 0.f); }

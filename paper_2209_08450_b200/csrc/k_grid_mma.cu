@@ -93,7 +93,7 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                     const float4* __restrict__ trigf, const int2* __restrict__ plan, const int4* __restrict__ items,
                     int nproj, int M, int npair, float alpha2, int strip_log2, int rswz, int nitems, int* __restrict__ counter,
                     const int* __restrict__ wstate, int* __restrict__ wcount, const int* __restrict__ woff,
-                    uint4* __restrict__ wrec, unsigned* __restrict__ wsamp) {
+                    uint4* __restrict__ wrec, unsigned* __restrict__ wsamp, const float* __restrict__ kbtab) {
     if (MODE == GM_DIRECT && wstate[WS_USABLE]) return;
     if (MODE == GM_CACHED && !wstate[WS_USABLE]) return;
     if (MODE == GM_COUNT && !wstate[WS_REBUILD]) return;
@@ -325,7 +325,7 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                     const float ax0 = (float)SX - flx, ay0 = (float)SY - fly;
                     auto wgt = [&](float a, float frac, float hi) {
                         const float d = a - frac;
-                        const float w = ex2_approx(-alpha2 * d * d);
+                        const float w = tap_weight(kbtab, d, alpha2);
                         return (a >= lo && a <= hi) ? w : 0.f;
                     };
                     unsigned wx[SUBX / 2], wy[SUBY / 2];
@@ -481,8 +481,8 @@ static int launch_mma_mode(const tcp_ctx* c, cudaStream_t st) {
     if (ctas < 1) ctas = 1;
     dim3 grid(ctas, ny, nz);
     kern<<<grid, 32 * CW, L::total, st>>>((const __half2*)c->spec, (__half2*)c->grid, c->g_partial, c->trigf, c->g_plan, c->g_items,
-                                       c->nproj, c->M, c->npair, (float)(alpha * 1.4426950408889634), c->grid_strip ? (int)log2((double)c->grid_strip) : -1, ifft2_on_mma(c) ? 1 : 0,
-                                       c->g_nitems, c->g_counter, c->w_state, c->w_count, c->w_off, c->w_rec, c->w_samp);
+                                       c->nproj, c->M, c->npair, c->kbtab ? (float)(1.0 / ((double)MH * MH)) : (float)(alpha * 1.4426950408889634), c->grid_strip ? (int)log2((double)c->grid_strip) : -1, ifft2_on_mma(c) ? 1 : 0,
+                                       c->g_nitems, c->g_counter, c->w_state, c->w_count, c->w_off, c->w_rec, c->w_samp, c->kbtab);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }
@@ -539,6 +539,7 @@ void grid_mma_cache_free(tcp_ctx* c) {
 int launch_grid_mma_main(const tcp_ctx* c, const float* theta, cudaStream_t st) {
     if (!c->half_store) return set_error(TCP_EUNSUPPORTED, "tensor-core gridding needs fp16 storage");
     const bool wide = c->npair > 8;
+    if (c->m == 2) return wide ? launch_mma_t<2, 32>(c, theta, st) : launch_mma_t<2, 16>(c, theta, st);
     if (c->m == 3) return wide ? launch_mma_t<3, 32>(c, theta, st) : launch_mma_t<3, 16>(c, theta, st);
     return wide ? launch_mma_t<4, 32>(c, theta, st) : launch_mma_t<4, 16>(c, theta, st);
 }

@@ -94,7 +94,7 @@ template <int MH, int NP, class TC>
 __global__ void __launch_bounds__(NTHR, 2)
     grid_tile_kernel(const TC* __restrict__ spec, TC* __restrict__ grid, float2* __restrict__ partial,
                      const double2* __restrict__ trig, const int2* __restrict__ plan, const int4* __restrict__ items,
-                     int nproj, int M, int npair, float alpha2) {
+                     int nproj, int M, int npair, float alpha2, const float* __restrict__ kbtab) {
     constexpr int KL = chord_len(MH);
     constexpr int PB = batch_records<TC>();
     constexpr int GW = NP * (int)sizeof(TC) / 16;           // uint4 words of spectrum per sample
@@ -241,8 +241,8 @@ __global__ void __launch_bounds__(NTHR, 2)
                     // tap offsets: e = a - 1/2 (a = l - floor(nu), valid -m+1..m <=> |e| < m); d = l - nu
                     const float exa = cxa - mt.x, exb = exa + 1.f, eya = cya - mt.z, eyb = eya + 1.f;
                     const float dxa = exa - mt.y, dxb = dxa + 1.f, dya = eya - mt.w, dyb = dya + 1.f;
-                    float wxa = ex2_approx(-alpha2 * dxa * dxa), wxb = ex2_approx(-alpha2 * dxb * dxb);
-                    float wya = ex2_approx(-alpha2 * dya * dya), wyb = ex2_approx(-alpha2 * dyb * dyb);
+                    float wxa = tap_weight(kbtab, dxa, alpha2), wxb = tap_weight(kbtab, dxb, alpha2);
+                    float wya = tap_weight(kbtab, dya, alpha2), wyb = tap_weight(kbtab, dyb, alpha2);
                     wxa = (fabsf(exa) < (float)MH) ? wxa : 0.f;
                     wxb = (fabsf(exb) < (float)MH) ? wxb : 0.f;
                     wya = (fabsf(eya) < (float)MH) ? wya : 0.f;
@@ -419,7 +419,7 @@ static int launch_tile_t(const tcp_ctx* c, cudaStream_t st) {
     const double alpha = 3.14159265358979323846 / (1.4142135623730951 * MH);
     dim3 grid(c->g_nitems, (c->npair + NP - 1) / NP);
     kern<<<grid, NTHR, smem, st>>>((const TC*)c->spec, (TC*)c->grid, c->g_partial, c->trig, c->g_plan, c->g_items, c->nproj,
-                                   c->M, c->npair, (float)(alpha * 1.4426950408889634));
+                                   c->M, c->npair, c->kbtab ? (float)(1.0 / ((double)MH * MH)) : (float)(alpha * 1.4426950408889634), c->kbtab);
     TCP_CUDA_CHECK(cudaGetLastError());
     return TCP_OK;
 }
@@ -437,6 +437,7 @@ int launch_grid_tile(const tcp_ctx* c, const float* theta, cudaStream_t st) {
     TCP_CUDA_CHECK(cudaGetLastError());
     int rc;
     if (c->grid_impl == TCP_GRID_MMA) rc = launch_grid_mma_main(c, theta, st);
+    else if (c->m == 2) rc = c->half_store ? launch_tile_np<2, __half2>(c, st) : launch_tile_np<2, float2>(c, st);
     else if (c->m == 3) rc = c->half_store ? launch_tile_np<3, __half2>(c, st) : launch_tile_np<3, float2>(c, st);
     else rc = c->half_store ? launch_tile_np<4, __half2>(c, st) : launch_tile_np<4, float2>(c, st);
     if (rc) return rc;

@@ -11,6 +11,7 @@
 #include <mutex>
 #include <vector>
 
+#include "grid_common.cuh"
 #include "tcp_internal.h"
 
 namespace tcpk {
@@ -135,10 +136,28 @@ static int build_context(tcp_ctx* c) {
     }
 
     const double alpha = kPi / (sqrt(2.0) * (double)m);
+    // Kaiser-Bessel window (tcp_create_ex kernel code 16 + m; reading Q21): beta = pi sqrt(2.25 m^2 - 0.8),
+    // phi(t) = I0(beta sqrt(1 - (t/m)^2)) / I0(beta), Phi(x) = (2m / I0(beta)) sinh(z) / z with z^2 = beta^2 - (2 pi m x / M)^2
+    const double beta = kPi * sqrt(2.25 * (double)m * (double)m - 0.8);
+    auto i0 = [](double z) {
+        const double q = 0.25 * z * z;
+        double term = 1.0, sum = 1.0;
+        for (int k = 1; k < 200 && term > 1e-18 * sum; ++k) { term *= q / ((double)k * (double)k); sum += term; }
+        return sum;
+    };
+    if (c->kernel == 1) {
+        std::vector<float> kb(tcpk::KB_NTAB + 1);
+        for (int i = 0; i <= tcpk::KB_NTAB; ++i) kb[i] = (float)(i0(beta * sqrt((double)i / (double)tcpk::KB_NTAB)) / i0(beta));
+        if ((rc = upload(&c->kbtab, kb, &c->bytes))) return rc;
+    }
     std::vector<float> dx(n), dy(n);
     for (int i = 0; i < n; ++i) {
         double x = (double)(i - n / 2);
         double phi = sqrt(kPi / alpha) * exp(-kPi * kPi * x * x / (alpha * (double)M * (double)M));
+        if (c->kernel == 1) {
+            const double a = 2.0 * kPi * (double)m * x / (double)M, z = sqrt(beta * beta - a * a);     // |x| <= n/2: a <= pi m / 2 < beta
+            phi = 2.0 * (double)m * sinh(z) / (z * i0(beta));
+        }
         dy[i] = (float)(1.0 / phi);
         dx[i] = (float)(1.0 / (phi * c->scale));
     }
@@ -213,6 +232,9 @@ const char* tcp_last_error(void) { return g_err; }
 static tcp_ctx* create_impl(int n, int ndet, int pad_l, int nproj, int nz_chunk, float center, int dtype, int filter, int m) {
     g_err[0] = 0;
     if (m == 0) m = 3;
+    const int kernel = m >> 4;            // kernel code: half-width (Gaussian) or 16 + half-width (Kaiser-Bessel)
+    m &= 15;
+    if (kernel > 1 || (kernel == 1 && m != 2 && m != 3)) { set_error(TCP_EINVAL, "kernel code %d: Kaiser-Bessel half-width must be 2 or 3", m | (kernel << 4)); return nullptr; }
     if (n < 64 || n > 4096 || (n & (n - 1)) != 0) {
         set_error(TCP_EINVAL, "n=%d must be a power of two in [64, 4096]", n);
         return nullptr;
@@ -222,7 +244,7 @@ static tcp_ctx* create_impl(int n, int ndet, int pad_l, int nproj, int nz_chunk,
     center += (float)pad_l;
     if (dtype < TCP_F32 || dtype > TCP_F16_OUT32) { set_error(TCP_EINVAL, "unknown dtype %d", dtype); return nullptr; }
     if (filter < TCP_FILTER_RAMP || filter > TCP_FILTER_HAMMING) { set_error(TCP_EINVAL, "unknown filter %d", filter); return nullptr; }
-    if (m != 3 && m != 4) { set_error(TCP_EINVAL, "kernel half-width m=%d must be 3 or 4", m); return nullptr; }
+    if (kernel == 0 && m != 3 && m != 4) { set_error(TCP_EINVAL, "kernel half-width m=%d must be 3 or 4", m); return nullptr; }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         cudaGetLastError();
@@ -232,7 +254,7 @@ static tcp_ctx* create_impl(int n, int ndet, int pad_l, int nproj, int nz_chunk,
     tcp_ctx* c = (tcp_ctx*)calloc(1, sizeof(tcp_ctx));
     if (!c) { set_error(TCP_ENOMEM, "out of host memory"); return nullptr; }
     c->n = n; c->M = 2 * n; c->nproj = nproj; c->nz = nz_chunk; c->npair = (nz_chunk + 1) / 2;
-    c->dtype = dtype; c->filter = filter; c->m = m; c->center = center;
+    c->dtype = dtype; c->filter = filter; c->m = m; c->kernel = kernel; c->center = center;
     c->ndet = ndet; c->pad_l = pad_l;
     c->fuse_norm = 1;
     c->half_store = dtype != TCP_F32;
@@ -287,6 +309,7 @@ void tcp_destroy(tcp_ctx* c) {
     cudaFree(c->sino); cudaFree(c->spec); cudaFree(c->grid); cudaFree(c->pass1); cudaFree(c->trig); cudaFree(c->trigf); cudaFree(c->wq); cudaFree(c->fdtab);
     cudaFree(c->tw); cudaFree(c->hfilt); cudaFree(c->ptab); cudaFree(c->ftab); cudaFree(c->deax); cudaFree(c->deay);
     cudaFree(c->tile_order);
+    cudaFree(c->kbtab);
     cudaFree(c->try_buf);
     cudaFree(c->out_pad);
     mmafft_free(c);
@@ -457,6 +480,8 @@ int tcp_set_option(tcp_ctx* c, int option, int value) {
     if (!c) return set_error(TCP_EINVAL, "NULL context");
     if (option == TCP_OPT_GRID_IMPL) {
         if (value < TCP_GRID_GATHER || value > TCP_GRID_MMA) return set_error(TCP_EINVAL, "bad grid impl %d", value);
+        if ((c->kernel == 1 || c->m == 2) && value != TCP_GRID_TILE && value != TCP_GRID_MMA)
+            return set_error(TCP_EUNSUPPORTED, "the Kaiser-Bessel kernel is built into the tile and tensor-core griddings only");
         if (value == TCP_GRID_SCATTER_ATOMIC && c->half_store) return set_error(TCP_EUNSUPPORTED, "scatter gridding supports TCP_F32 only");
         if (value == TCP_GRID_MMA && !c->half_store) return set_error(TCP_EUNSUPPORTED, "tensor-core gridding needs fp16 storage");
         c->grid_impl = value;

@@ -9,6 +9,8 @@
 
 struct tcp_ctx {
     int n, M, nproj, nz, npair, dtype, filter, m;
+    int kernel;           // gridding kernel family: 0 Gaussian, 1 Kaiser-Bessel (tcp_create_ex code 16 + m)
+    float* kbtab;         // Kaiser-Bessel: phi over u = 1 - (d/m)^2, KB_NTAB + 1 samples (NULL for the Gaussian)
     float center;         // rotation centre in the padded row (caller's centre + pad_l)
     int ndet, pad_l;      // tcp_create_det: caller's detector width / image side, air samples left of it (ndet == n, 0 otherwise)
     void* out_pad;        // [nz][n][n] in the output dtype when ndet != n (the central ndet x ndet pixels are then copied out)

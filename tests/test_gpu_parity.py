@@ -97,8 +97,9 @@ def test_mma_fft_lines_against_the_dft(inverse):
 
 
 # ------------------------------------------------------------------ C1, stage by stage
-@pytest.mark.parametrize("m", [3, 4])
+@pytest.mark.parametrize("m", [3, 4, 16 + 2, 16 + 3])
 def test_c1_fp32_stages_and_volume(m):
+    """m: kernel code (3, 4: Gaussian half-width; 16 + 2, 16 + 3: Kaiser-Bessel window, reading Q21)."""
     w = sg.make_workload("C1")
     rows = list(range(w.nz_total))
     out, r, (raw, flat, dark, theta) = _gpu_recon(w, rows, "f32", m=m, keep=True)
@@ -124,6 +125,29 @@ def test_c1_fp32_stages_and_volume(m):
     for z in rows:
         check(out[z], ref[z], "f32")
     r.close()
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f16", "f16_out32"])
+@pytest.mark.parametrize("cfg,scale,nz", [("C1", 1, 8), ("C2", 4, 5), ("C3", 4, 18)])
+def test_kaiser_bessel_kernel(dtype, cfg, scale, nz):
+    """The half-width-2 Kaiser-Bessel kernel (tcp_create_ex code 16 + 2: 16 taps per sample instead of 36) through both
+    production griddings (CUDA-core tile kernel for fp32, tensor cores for fp16 storage) against the oracle with the same
+    kernel code, at the gates of north_star; odd and multi-group chunks, an off-centre axis (C3)."""
+    w = sg.make_workload(cfg, scale=scale)
+    rows = list(range(min(nz, w.nz_total)))
+    out, _, (raw, flat, dark, theta) = _gpu_recon(w, rows, dtype, m=16 + 2)
+    ref = orc.recon(raw, flat, dark, theta, w.center, w.filter, 16 + 2, "grid")
+    for z in range(len(rows)):
+        check(out[z], ref[z], "f32" if dtype == "f32" else dtype, vol=ref, tag=z)
+    tcp = _tcp()
+    r = tcp.Recon(w.n, w.nproj, 2, w.center, dtype, w.filter, 16 + 2)
+    for impl in ("gather", "scatter"):
+        with pytest.raises(tcp.TcpError):
+            r.set_grid_impl(impl)
+    r.close()
+    for bad in (16 + 4, 16 + 1, 32 + 2, 2):
+        with pytest.raises(tcp.TcpError):
+            tcp.tcp_create_ex(w.n, w.nproj, 2, w.center, dtype, w.filter, bad)
 
 
 def test_c1_gridding_implementations_agree():
@@ -775,7 +799,7 @@ def test_pipeline_slice_ranges_equal_the_whole_volume():
 
 # ------------------------------------------------------------------ BASELINE full sizes, bench launch configuration
 @pytest.mark.parametrize("cfg,nz,tcfft,where", [("C4", 32, None, "mid"), ("C4", 32, None, "first"), ("C4", 32, None, "last"),
-                                                ("C4", 32, 0, "mid"), ("C4", 32, 1, "mid"), ("C4", 32, 6, "mid"),
+                                                ("C4", 32, 0, "mid"), ("C4", 32, 1, "mid"), ("C4", 32, 6, "mid"), ("C4kb", 32, None, "mid"),
                                                 ("C5", 32, None, "mid"), ("C5", 32, None, "first"), ("C5", 32, None, "last")])
 def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft, where):
     """C4 (2048^2, 2048 projections, fp16, one 32-slice chunk exactly as bench.py launches it: tcgen05
@@ -786,6 +810,8 @@ def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft, where):
     (None = the default, every transform at M = 4096; 0 = the fp32 CUDA-core transforms; 1 = the row kernel only;
     6 = the inverse 2D transform only): same gates for every combination."""
     tcp = _tcp()
+    kcode = 16 + 2 if cfg.endswith("kb") else 3          # "C4kb": C4 with the half-width-2 Kaiser-Bessel kernel
+    cfg = cfg[:2]
     w = sg.make_workload(cfg)
     z0 = {"mid": w.nz_total // 2 - nz // 2, "first": 0, "last": w.nz_total - nz}[where]
     rows = list(range(z0, z0 + nz))
@@ -795,7 +821,7 @@ def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft, where):
     tcp.tcp_mean_frames_u16(ff.contiguous(), flat_d)
     tcp.tcp_mean_frames_u16(df.contiguous(), dark_d)
     theta = w.theta
-    r = tcp.Recon(w.n, w.nproj, nz, w.center, w.dtype, w.filter, 3)
+    r = tcp.Recon(w.n, w.nproj, nz, w.center, w.dtype, w.filter, kcode)
     if tcfft is not None:
         r.set_tcfft(tcfft)
     out = r.recon(raw_d.contiguous(), flat_d, dark_d, torch.from_numpy(theta).cuda())
@@ -804,7 +830,7 @@ def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft, where):
     r.close()
     sample = sorted({0, 1, nz // 2, nz - 1}) if where == "mid" else [0, nz - 1]     # first / last chunk: the stack's end slices (phantom edge, air rows)
     raw_h = raw_d.view(torch.int16)[:, sample].contiguous().cpu().numpy().view(np.uint16)
-    ref = orc.recon(raw_h, flat_d[sample].cpu().numpy(), dark_d[sample].cpu().numpy(), theta, w.center, w.filter, 3, "grid")
+    ref = orc.recon(raw_h, flat_d[sample].cpu().numpy(), dark_d[sample].cpu().numpy(), theta, w.center, w.filter, kcode, "grid")
     scale = np.abs(ref).max()
     for i, z in enumerate(sample):
         print("full size %s tcfft=%s %s slice %d: rel-L2 %.3e max-abs %.3e" % (cfg, tcfft, where, z, rl2(out[z], ref[i]), np.abs(out[z] - ref[i]).max() / scale))
