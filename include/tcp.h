@@ -66,7 +66,9 @@ enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1, TCP_GRID_TILE = 2, TCP_
 /* TCP_OPT_PAD: the n padding samples of the filter stage S3 (the padding "allows for
  * suppressing artifacts when processing samples not fitting into the detector field of view"):
  * TCP_PAD_ZERO (default, the reading of north_star) or TCP_PAD_EDGE = the nearest detector edge value of
- * the periodic length-2n row (p[n-1] for n <= i < 3n/2, p[0] after).  Stage S4 always zero-pads. */
+ * the periodic length-2n row (p[n-1] for n <= i < 3n/2, p[0] after).  Stage S4 always zero-pads.  TCP_PAD_EDGE is
+ * refused (TCP_EUNSUPPORTED) on a tcp_create_det context whose width is not a power of two: there the row is
+ * already padded with air, and its edge samples are not the detector's. */
 /* TCP_OPT_FILTER_FUSED (0 default | 1): the second reading of "filter, then Fourier backprojection" (DESIGN.md
  * Q6): filter and spectrum have the same length M = 2n, so S3 + S4 collapse to G = C H FFT_M(padded row) x phase
  * with NO crop of the filtered row in between: one transform per row instead of three, and a slightly different

@@ -506,6 +506,10 @@ int tcp_set_option(tcp_ctx* c, int option, int value) {
     }
     if (option == TCP_OPT_PAD) {
         if (value != TCP_PAD_ZERO && value != TCP_PAD_EDGE) return set_error(TCP_EINVAL, "unknown padding %d", value);
+        // tcp_create_det rows carry air (p = 0) around the detector inside the power-of-two row, so replicating the
+        // ROW's edge samples would pad with zeros and silently bring the truncation artefacts back: refuse instead
+        if (value == TCP_PAD_EDGE && c->ndet != c->n)
+            return set_error(TCP_EUNSUPPORTED, "TCP_PAD_EDGE needs a power-of-two detector width (tcp_create_det pads the row with air)");
         c->pad = value;
         return TCP_OK;
     }

@@ -738,6 +738,8 @@ def test_detector_width_variants_pipeline_try_line_and_errors():
         check(t[i], ri, "f32")
     with pytest.raises(tcp.TcpError):
         r.recon_try(d[0], d[1], d[2], d[3], [float(ndet)])        # centre range is the caller's detector
+    with pytest.raises(tcp.TcpError):                              # the padded row's edges are air, not the detector's
+        r.set_pad("edge")
     # LineRec
     r.set_algorithm("line")
     o = r.recon(*_to_dev(np.ascontiguousarray(raw[:, :4]), flat[:4], dark[:4], theta)).cpu().numpy()
