@@ -10,7 +10,7 @@ pairs are in the C++ files; the wrappers of those only marshal numpy arrays.  Th
 small functions do their arithmetic here in numpy (double precision), each citing
 the reading it follows and pinned by its own test: `angle_weights` (trapezoid
 weights, reading Q20, pin P11), `padded_size` and `recon_padded` (detector width not
-a power of two, reading Q19, pin P10).
+a power of two, reading Q19, pin P10).  `recon_pre` only chains calls.
 """
 from __future__ import annotations
 
@@ -22,7 +22,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liboracle.so")
-_SRC = [os.path.join(_HERE, "oracle.cpp"), os.path.join(_HERE, "oracle_bp.cpp")]
+_SRC = [os.path.join(_HERE, "oracle.cpp"), os.path.join(_HERE, "oracle_bp.cpp"), os.path.join(_HERE, "oracle_pre.cpp")]
 
 FILTERS = {"ramp": 0, "shepp": 1, "parzen": 2, "cosine": 3, "hann": 4, "hamming": 5}
 METHODS = {"grid": 0, "exact": 1, "lin": 2}
@@ -280,6 +280,37 @@ def recon(raw, flat, dark, theta, center, filt="ramp", m=DEFAULT_M, method="grid
                     C.c_double(center), C.c_int(FILTERS[filt]), C.c_int(PADS[pad] | (2 if fused else 0)), C.c_int(m), C.c_int(METHODS[method]),
                     _p(out))
     return out
+
+
+def remove_zingers(p, dif):
+    """orc_zinger (reading Q22): p f64 [nz][nproj][n] -> copy with every sample that lies more than `dif` below the
+    median of its 3 x 3 (projection, pixel) neighbourhood replaced by that median."""
+    p = _f64(p)
+    nz, nproj, n = p.shape
+    out = np.empty_like(p)
+    lib().orc_zinger(_p(p), C.c_int(nz), C.c_int(nproj), C.c_int(n), C.c_double(dif), _p(out))
+    return out
+
+
+def remove_rings(p, alpha, return_r=False):
+    """orc_ring_ti (reading Q23): p f64 [nz][nproj][n] -> p minus the per-pixel offsets r[nz][n] estimated from the
+    angle-averaged profile by the closed-form Tikhonov formula (A + alpha I) r = A pbar, A = D2^T D2."""
+    p = _f64(p)
+    nz, nproj, n = p.shape
+    out, r = np.empty_like(p), np.empty((nz, n))
+    lib().orc_ring_ti(_p(p), C.c_int(nz), C.c_int(nproj), C.c_int(n), C.c_double(alpha), _p(out), _p(r))
+    return (out, r) if return_r else out
+
+
+def recon_pre(raw, flat, dark, theta, center, filt="ramp", m=DEFAULT_M, method="grid", zinger_dif=0.0, ring_alpha=0.0):
+    """S1+S2, then the optional pre-processing steps in the order zingers, rings (each off when its parameter is 0),
+    then S3..S7: the chain tcp_recon runs with TCP_PARAM_ZINGER_DIF / TCP_PARAM_RING_ALPHA set."""
+    p = neglog(raw, _f32(flat), _f32(dark))
+    if zinger_dif > 0:
+        p = remove_zingers(p, zinger_dif)
+    if ring_alpha > 0:
+        p = remove_rings(p, ring_alpha)
+    return fbp_from_sino(p, theta, center, filt=filt, m=m, method=method)
 
 
 def padded_size(ndet: int) -> tuple[int, int]:

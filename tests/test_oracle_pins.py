@@ -619,3 +619,73 @@ def test_golden_c1_oracle_samples():
     assert scale > 1e-3
     for k, v in stored.items():
         assert abs(now[k] - v) <= 1e-12 * scale, (k, now[k], v)
+
+
+# ---------------------------------------------------------------- P13 / P14: pre-processing filters
+def test_p13_zinger_removal():
+    """Reading Q22 ("zinger artifacts reduction (Rivers, 1998)").  (a) the 3 x 3 median with clamped edges
+    against numpy.median on every window of a small random array (dif = -inf replaces everything by its median);
+    (b) dif = +inf changes nothing, bit for bit; (c) on a smooth sinogram with injected isolated low samples (bright
+    detector hits) exactly those samples are replaced, every other sample stays bit-identical, and the replaced ones
+    land within the local variation of the true value; (d) HIGH outliers (dead pixels) are not zingers and stay."""
+    rng = np.random.default_rng(13)
+    p = rng.standard_normal((2, 7, 9))
+    med = orc.remove_zingers(p, -1e300)
+    for z in range(2):
+        pp = np.pad(p[z], 1, mode="edge")
+        for j in range(7):
+            for i in range(9):
+                assert med[z, j, i] == np.median(pp[j:j + 3, i:i + 3])
+    assert np.array_equal(orc.remove_zingers(p, 1e300), p)
+    jj, ii = np.meshgrid(np.arange(40), np.arange(64), indexing="ij")
+    smooth = (1.5 + 0.5 * np.sin(ii / 9.0) * np.cos(jj / 7.0))[None]
+    bad = smooth.copy()
+    hits = [(3, 5), (10, 40), (0, 0), (39, 63), (20, 21)]
+    for j, i in hits:
+        bad[0, j, i] -= 1.0
+    bad[0, 30, 30] += 1.0                                   # a high outlier
+    out = orc.remove_zingers(bad, 0.3)
+    changed = {(int(j), int(i)) for j, i in zip(*np.nonzero(out[0] != bad[0]))}
+    assert changed == set(hits)
+    for j, i in hits:
+        assert abs(out[0, j, i] - smooth[0, j, i]) < 0.08        # the local variation of the smooth sinogram over one sample
+    assert out[0, 30, 30] == bad[0, 30, 30]
+
+
+def test_p14_ring_removal_closed_form():
+    """Reading Q23 (ring removal "with an analytical formula by V. Titarenko").  (a) the banded solve against
+    numpy.linalg.solve on the dense normal equations (A + alpha I) r = A pbar built from an explicit second-difference
+    matrix; (b) a profile linear in the detector index has D2 pbar = 0: r = 0 and the sinogram is unchanged; (c) the
+    correction is the same for every projection and only depends on the angle mean; (d) the filter is linear, and away from
+    the detector edges it is the high-pass lambda_k / (lambda_k + alpha), lambda_k = 16 sin^4(pi k / n), of the profile:
+    a single bad column of height h keeps the fraction (1/n) sum_k alpha / (lambda_k + alpha) of h (6 % at alpha = 1e-3:
+    the smooth bump the regulariser cannot tell from the object), spread as a broad bump lower than that everywhere else."""
+    rng = np.random.default_rng(14)
+    nz, nproj, n, alpha = 2, 11, 37, 0.05
+    p = rng.standard_normal((nz, nproj, n))
+    out, r = orc.remove_rings(p, alpha, return_r=True)
+    D2 = np.zeros((n - 2, n))
+    for i in range(n - 2):
+        D2[i, i:i + 3] = (1.0, -2.0, 1.0)
+    A = D2.T @ D2
+    for z in range(nz):
+        ref = np.linalg.solve(A + alpha * np.eye(n), A @ p[z].mean(0))
+        assert np.abs(r[z] - ref).max() < 1e-12
+        assert np.abs(out[z] - (p[z] - ref[None])).max() < 1e-12
+    lin = (0.3 + 0.01 * np.arange(n))[None, None, :] * np.ones((1, nproj, 1))
+    o2, r2 = orc.remove_rings(lin, alpha, return_r=True)
+    assert np.abs(r2).max() < 1e-12 and np.abs(o2 - lin).max() < 1e-12
+    n, nproj, h = 256, 60, 0.05
+    ii = np.arange(n)
+    smooth = 2.0 * np.sqrt(np.maximum(0.0, 1.0 - ((ii - 128) / 100.0) ** 2))[None, None, :] * np.ones((1, nproj, 1))
+    smooth = smooth + 0.05 * np.sin(ii / 30.0)[None, None, :] * np.cos(np.arange(nproj) / 5.0)[None, :, None]
+    bad = smooth.copy()
+    bad[0, :, 77] += h
+    o3 = orc.remove_rings(bad, 1e-3)
+    base = orc.remove_rings(smooth, 1e-3)
+    lam = 16.0 * np.sin(np.pi * np.arange(n) / n) ** 4
+    keep = float(np.mean(1e-3 / (lam + 1e-3)))
+    left = (o3 - base)[0]
+    assert np.abs(left - left[0][None]).max() < 1e-12                 # the same correction in every projection
+    assert left[0, 77] == pytest.approx(keep * h, rel=0.05) and keep < 0.08
+    assert np.abs(left[0][np.r_[0:77, 78:n]]).max() < left[0, 77]
