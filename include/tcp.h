@@ -190,6 +190,20 @@ double tcp_scale(const tcp_ctx* ctx);
 size_t tcp_workspace_bytes(const tcp_ctx* ctx);
 int tcp_launches_per_recon(const tcp_ctx* ctx);
 int tcp_set_option(tcp_ctx* ctx, int option, int value);
+/* Real-valued parameters.  Pre-processing of the sinogram between S2 and S3, each step off at 0 (default),
+ * applied in this order by tcp_recon, tcp_recon_try and the host pipeline, all algorithms; with either on, S1+S2 run as
+ * their own kernel (TCP_OPT_FUSE_NORMALIZE is ignored).  TCP_EUNSUPPORTED on a tcp_create_det context whose width is
+ * not a power of two; TCP_EINVAL for a negative or non-finite value.
+ *   TCP_PARAM_ZINGER_DIF  "zinger artifacts reduction (Rivers, 1998)", reading Q22: a sample of p = -ln t that
+ *       lies more than `value` below the median of its 3 x 3 (projection, detector pixel) neighbourhood (indices
+ *       clamped at the array edges, medians taken on the unmodified sinogram) is replaced by that median: an isolated
+ *       bright detector hit is an isolated low sample of p.
+ *   TCP_PARAM_RING_ALPHA  ring removal "with an analytical formula by V. Titarenko", reading Q23: per slice, the offset
+ *       r[i] of detector pixel i common to all projections is estimated from the angle-averaged profile pbar as the
+ *       minimiser of ||D2 (pbar - r)||^2 + value ||r||^2 (D2 = second differences), in closed form
+ *       (D2^T D2 + value I) r = D2^T D2 pbar, and subtracted from every projection. */
+enum { TCP_PARAM_ZINGER_DIF = 0, TCP_PARAM_RING_ALPHA = 1 };
+int tcp_set_param(tcp_ctx* ctx, int param, double value);
 
 /* Rotation-centre "try" mode ("--reconstruction-type try": one slice reconstructed for a
  * set of candidate centres, for visual choice).  raw_u16 [nproj][1][n], flat / dark [n], theta [nproj] are

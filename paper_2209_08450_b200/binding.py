@@ -21,7 +21,7 @@ EXPORTS = [
     "tcp_mean_frames_u16", "tcp_normalize", "tcp_workspace", "tcp_read_workspace", "tcp_scale", "tcp_grid_strip",
     "tcp_workspace_bytes", "tcp_launches_per_recon", "tcp_set_option", "tcp_profile_collect",
     "tcp_recon_volume_host", "tcp_recon_try", "tcp_create_det", "tcp_padded_n",
-    "tcp_recon_volume_host_rows", "tcp_slice_range", "tcp_check_angles", "tcp_pass1_layout", "tcp_grid_swizzled", "tcp_fft_lines", "tcp_measure_rates",
+    "tcp_recon_volume_host_rows", "tcp_slice_range", "tcp_check_angles", "tcp_pass1_layout", "tcp_grid_swizzled", "tcp_fft_lines", "tcp_measure_rates", "tcp_set_param",
 ]
 
 
@@ -93,6 +93,8 @@ def lib():
     L.tcp_grid_swizzled.argtypes = [vp]
     L.tcp_fft_lines.restype = ci
     L.tcp_fft_lines.argtypes = [vp, vp, vp, ci, ci, vp]
+    L.tcp_set_param.restype = ci
+    L.tcp_set_param.argtypes = [vp, ci, C.c_double]
     L.tcp_measure_rates.restype = ci
     L.tcp_measure_rates.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.tcp_recon_try.restype = ci
@@ -275,6 +277,14 @@ class Recon:
     def set_algorithm(self, name: str):
         """TCP_OPT_ALGORITHM: "fourier" (FourierRec, default) or "line" (LineRec, direct line summation)."""
         _check(lib().tcp_set_option(self.h, 3, {"fourier": 0, "line": 1}[name]))
+
+    def set_zinger(self, dif: float):
+        """TCP_PARAM_ZINGER_DIF: zinger removal threshold on p = -ln t (0 = off)."""
+        _check(lib().tcp_set_param(self.h, 0, float(dif)))
+
+    def set_ring(self, alpha: float):
+        """TCP_PARAM_RING_ALPHA: regularisation of the closed-form ring estimate (0 = off)."""
+        _check(lib().tcp_set_param(self.h, 1, float(alpha)))
 
     def set_tcfft(self, mask: int):
         """TCP_OPT_TCFFT: which transforms run their butterflies on the tensor cores (1 rows, 6 = both passes of the

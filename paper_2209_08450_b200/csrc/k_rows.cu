@@ -221,7 +221,8 @@ static int launch_rows_m(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw,
 // S1+S2 can ride the loader of rows_kernel: fp16 storage (the fused value is the stored half, bit for bit), the default
 // chain (not the uncropped-filter option, not the try mode), the caller's rows as wide as the transform's
 bool rows_fuses_normalize(const tcp_ctx* c) {
-    return c->fuse_norm && c->half_store && c->algorithm == TCP_ALG_FOURIER && !c->filter_fused && !c->try_ptab && c->ndet == c->n;
+    return c->fuse_norm && c->half_store && c->algorithm == TCP_ALG_FOURIER && !c->filter_fused && !c->try_ptab && c->ndet == c->n &&
+           !(c->zinger_dif > 0.0) && !(c->ring_alpha > 0.0);       // pre-processing works on the sinogram workspace
 }
 
 int launch_rows(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw, const float* flat, const float* dark) {

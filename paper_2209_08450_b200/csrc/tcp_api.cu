@@ -310,6 +310,7 @@ void tcp_destroy(tcp_ctx* c) {
     cudaFree(c->tw); cudaFree(c->hfilt); cudaFree(c->ptab); cudaFree(c->ftab); cudaFree(c->deax); cudaFree(c->deay);
     cudaFree(c->tile_order);
     cudaFree(c->kbtab);
+    cudaFree(c->pre_buf);
     cudaFree(c->try_buf);
     cudaFree(c->out_pad);
     mmafft_free(c);
@@ -341,6 +342,7 @@ int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* d
     if ((rc = fused_s12 ? launch_trig(c, theta, st, flat, dark) : launch_trig(c, theta, st))) return rc;
     TCP_MARK(1);
     if (!fused_s12 && (rc = launch_normalize(c, raw, flat, dark, st))) return rc;
+    if ((c->zinger_dif > 0.0 || c->ring_alpha > 0.0) && (rc = launch_pre(c, st))) return rc;
     TCP_MARK(2);
     if (c->algorithm == TCP_ALG_LINE) {       // LineRec: filter (timed as "rows"), backprojection (timed as "grid")
         if ((rc = launch_filter(c, st))) return rc;
@@ -398,6 +400,7 @@ int tcp_recon_try(tcp_ctx* c, const uint16_t* raw, const float* flat, const floa
     one.nz = 1; one.npair = 1;
     if ((rc = launch_trig(c, theta, st))) return rc;
     if ((rc = launch_normalize(&one, raw, flat, dark, st))) return rc;
+    if ((c->zinger_dif > 0.0 || c->ring_alpha > 0.0) && (rc = launch_pre(&one, st))) return rc;
     tcp_ctx t = *c;                   // ncenter output "slices"
     t.nz = ncenter; t.npair = npair; t.try_ptab = c->try_buf;
     if ((rc = rows_on_mma(&t) ? launch_rows_mma(&t, st, nullptr) : launch_rows(&t, st))) return rc;
@@ -429,7 +432,7 @@ int tcp_profile_collect(tcp_ctx* c, double* ms_sum, int* ncalls) {
 
 int tcp_launches_per_recon(const tcp_ctx* c) {
     if (!c) return 0;
-    const int crop = (c->out_pad ? 1 : 0) - (rows_fuses_normalize(c) ? 1 : 0);   // tcp_create_det: + the cut-out copy; fused S1+S2: - normalise
+    const int crop = (c->out_pad ? 1 : 0) - (rows_fuses_normalize(c) ? 1 : 0) + (c->zinger_dif > 0.0 ? 1 : 0) + (c->ring_alpha > 0.0 ? 3 : 0);   // tcp_create_det: + the cut-out copy; fused S1+S2: - normalise
     if (c->algorithm == TCP_ALG_LINE) return 4 + crop;                   // trig, normalise, filter, backprojection
     if (c->grid_impl == TCP_GRID_MMA)       // + plan, cache decide (+ count, scan, fill, cached kernel: most exit at once) (+ reduce)
         return 8 + (c->w_cap > 0 ? 4 : 0) + (c->g_nred ? 1 : 0) + crop;
@@ -475,6 +478,22 @@ int tcp_fft_lines(tcp_ctx* c, const void* in_half2, void* out_float2, int batch,
 }
 int tcp_grid_strip(const tcp_ctx* c) { return c ? c->grid_strip : 0; }
 size_t tcp_workspace_bytes(const tcp_ctx* c) { return c ? c->bytes : 0; }
+
+int tcp_set_param(tcp_ctx* c, int param, double value) {
+    if (!c) return set_error(TCP_EINVAL, "NULL context");
+    if (!(value >= 0.0) || !(value - value == 0.0)) return set_error(TCP_EINVAL, "parameter value %g must be finite and >= 0", value);
+    if (value > 0.0 && c->ndet != c->n) return set_error(TCP_EUNSUPPORTED, "pre-processing needs a power-of-two detector width");
+    if (param == TCP_PARAM_ZINGER_DIF) { c->zinger_dif = value; return TCP_OK; }
+    if (param == TCP_PARAM_RING_ALPHA) {
+        if (value > 0.0 && !c->pre_buf) {
+            int rc = dev_alloc((void**)&c->pre_buf, (size_t)c->nz * c->n * 6 * sizeof(double), &c->bytes);
+            if (rc) return rc;
+        }
+        c->ring_alpha = value;
+        return TCP_OK;
+    }
+    return set_error(TCP_EINVAL, "unknown parameter %d", param);
+}
 
 int tcp_set_option(tcp_ctx* c, int option, int value) {
     if (!c) return set_error(TCP_EINVAL, "NULL context");

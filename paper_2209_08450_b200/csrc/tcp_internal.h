@@ -37,6 +37,9 @@ struct tcp_ctx {
     float4* trigf;        // [nproj] (cos hi, cos lo, sin hi, sin lo): float-float split of trig
     float* wq;            // [nproj] quadrature weight of every projection relative to pi/nproj (trig_kernel, every call)
     float2* fdtab;        // [nz][n] (1 / max(flat - dark, eps_d), dark) of the call, written by trig_kernel for the fused S1+S2 loader
+    double zinger_dif;    // TCP_PARAM_ZINGER_DIF (0: off) and TCP_PARAM_RING_ALPHA (0: off): pre-processing between S2 and S3 (k_pre.cu)
+    double ring_alpha;
+    double* pre_buf;      // ring removal: [nz][n] angle means + [nz][5][n] solver work, allocated when the option is first set
     int fuse_norm;        // TCP_OPT_FUSE_NORMALIZE: S1+S2 in the loader of rows_kernel where that applies (fp16 storage)
     int angle_weights;    // TCP_OPT_ANGLE_WEIGHTS: the row kernels scale projection j by wq[j] (unequally spaced angles)
     // tables (device), built in fp64 on the host at create
@@ -105,6 +108,7 @@ int launch_rows(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw = nullptr
                 const float* dark = nullptr);
 bool rows_fuses_normalize(const tcp_ctx* c);
 int launch_filter(const tcp_ctx* c, cudaStream_t st);
+int launch_pre(const tcp_ctx* c, cudaStream_t st);          // zinger / ring removal on the sinogram workspace
 int launch_line_bp(const tcp_ctx* c, void* out, cudaStream_t st);
 int launch_grid_scatter(const tcp_ctx* c, cudaStream_t st);
 int launch_grid_gather(const tcp_ctx* c, const float* theta, cudaStream_t st);

@@ -838,3 +838,63 @@ def test_full_size_chunk_sampled_against_oracle(cfg, nz, tcfft, where):
         print("full size %s tcfft=%s %s slice %d: rel-L2 %.3e max-abs %.3e" % (cfg, tcfft, where, z, rl2(out[z], ref[i]), np.abs(out[z] - ref[i]).max() / scale))
         assert rl2(out[z], ref[i]) < FP16_GATE_L2, (cfg, z, rl2(out[z], ref[i]))
         assert np.abs(out[z] - ref[i]).max() / scale < FP16_GATE_MAX
+
+
+# ------------------------------------------------------------------ pre-processing between S2 and S3
+@pytest.mark.parametrize("dtype", ["f32", "f16"])
+@pytest.mark.parametrize("which", ["zinger", "ring", "both"])
+def test_preprocessing_zingers_and_rings(dtype, which):
+    """TCP_PARAM_ZINGER_DIF / TCP_PARAM_RING_ALPHA against the oracle's recon_pre (readings Q22, Q23; pins
+    P13, P14).  Input: C2 at quarter size with bright detector hits (counts x 3 on isolated samples: p lower by ln 3, far
+    from the 0.3 threshold on either side, so the fp32 and fp64 decisions agree) and two miscalibrated detector columns
+    (+2 %, -3 % gain in every projection: rings).  Gates of north_star; the options must matter on this input; 5 slices
+    (an odd chunk); try mode and LineRec run the same steps; padded-detector contexts and bad values are refused."""
+    tcp = _tcp()
+    w = sg.make_workload("C2", scale=4)
+    rows = list(range(30, 35))
+    raw, flat, dark, theta = _inputs(w, rows)
+    rng = np.random.default_rng(31)
+    raw = raw.astype(np.float64)
+    for _ in range(40):
+        j, z, i = rng.integers(w.nproj), rng.integers(len(rows)), rng.integers(w.n)
+        raw[j, z, i] = (raw[j, z, i] - dark[z, i]) * 3.0 + dark[z, i]
+    raw[:, :, 40] = (raw[:, :, 40] - dark[None, :, 40]) * 1.02 + dark[None, :, 40]
+    raw[:, :, 77] = (raw[:, :, 77] - dark[None, :, 77]) * 0.97 + dark[None, :, 77]
+    raw = np.clip(np.rint(raw), 0, 65535).astype(np.uint16)
+    zd = 0.3 if which in ("zinger", "both") else 0.0
+    ra = 2e-3 if which in ("ring", "both") else 0.0
+    r = tcp.Recon(w.n, w.nproj, len(rows), w.center, dtype, w.filter, 3)
+    dev = _to_dev(raw, flat, dark, theta)
+    plain = r.recon(*dev).float().cpu().numpy()
+    r.set_zinger(zd)
+    r.set_ring(ra)
+    out = r.recon(*dev).float().cpu().numpy()
+    ref = orc.recon_pre(raw, flat, dark, theta, w.center, w.filter, 3, "grid", zinger_dif=zd, ring_alpha=ra)
+    ref0 = orc.recon(raw, flat, dark, theta, w.center, w.filter, 3, "grid")
+    assert rl2(ref[2], ref0[2]) > 2e-2                      # the steps matter on this input
+    assert rl2(plain[2], ref0[2]) < (FP32_GATE if dtype == "f32" else FP16_GATE_L2)
+    for z in range(len(rows)):
+        check(out[z], ref[z], dtype, vol=ref, tag=(which, z))
+    # the sinogram workspace after the steps
+    p = orc.neglog(raw, flat, dark)
+    if zd:
+        p = orc.remove_zingers(p, zd)
+    if ra:
+        p = orc.remove_rings(p, ra)
+    sino = r.workspace("sinogram").float().cpu().numpy()
+    assert np.abs(sino - p).max() < (3e-6 if dtype == "f32" else 2e-3) * max(1.0, np.abs(p).max())
+    # try mode and LineRec take the same steps
+    t = r.recon_try(dev[0][:, 2:3].contiguous(), dev[1][2:3], dev[2][2:3], dev[3], [w.center]).float().cpu().numpy()
+    check(t[0], ref[2], dtype, vol=ref, tag="try")
+    r.set_algorithm("line")
+    ol = r.recon(*dev).float().cpu().numpy()
+    rl_ = orc.recon_pre(raw, flat, dark, theta, w.center, w.filter, 3, "lin", zinger_dif=zd, ring_alpha=ra)
+    check(ol[1], rl_[1], dtype, vol=rl_, tag="line")
+    for bad in (-1.0, float("nan")):
+        with pytest.raises(tcp.TcpError):
+            r.set_zinger(bad)
+    r.close()
+    rp = tcp.Recon(100, w.nproj, 2, 50.0, dtype, w.filter, 3)
+    with pytest.raises(tcp.TcpError):
+        rp.set_ring(1e-3)
+    rp.close()
