@@ -191,6 +191,15 @@ def tcp_mean_frames_u16(frames, mean, stream=None):
     _check(lib().tcp_mean_frames_u16(frames.data_ptr(), k, nz, n, _dev(mean, torch.float32, (nz, n)), _stream(stream)))
 
 
+def _host(t: torch.Tensor, dtype, shape=None, what="tensor") -> int:
+    """A HOST pointer the library may dereference: CPU tensor, contiguous, right dtype and shape (mirror of _dev)."""
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise TcpError("%s: expected a contiguous CPU tensor of dtype %s" % (what, dtype))
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise TcpError("%s: expected shape %s, got %s" % (what, tuple(shape), tuple(t.shape)))
+    return t.data_ptr()
+
+
 def tcp_recon_volume_host(h, raw_host, flat_host, dark_host, theta_host, out_host, nz_total, nbuf=3):
     """Host (pinned) tensors in, host tensor out; returns the device-timed milliseconds."""
     ms = C.c_float(0.0)
@@ -319,7 +328,15 @@ class Recon:
     def workspace_bytes(self) -> int:
         return int(lib().tcp_workspace_bytes(self.h))
 
-    def recon(self, raw_u16, flat, dark, theta, out=None, stream=None):
+    def recon(self, raw_u16, flat, dark, theta, out=None, stream=None, check_angles=True):
+        """tcp_recon on device tensors.  check_angles: tcp_recon cannot validate its DEVICE angles without a synchronisation,
+        so the binding checks each distinct theta tensor ONCE (tcp_check_angles on a host copy; cached by data pointer and
+        version) -- a 0..2 pi scan or unsorted angles would otherwise give a silently wrong image."""
+        if check_angles and isinstance(theta, torch.Tensor) and theta.is_cuda:
+            key = (theta.data_ptr(), theta._version, tuple(theta.shape))
+            if getattr(self, "_theta_ok", None) != key:
+                tcp_check_angles(theta.detach().float().cpu())
+                self._theta_ok = key
         raw_u16 = _as_u16(raw_u16)
         _dev(raw_u16, torch.uint16, (self.nproj, self.nz, self.n))
         _dev(flat, torch.float32, (self.nz, self.n))
@@ -398,10 +415,23 @@ class Recon:
         """rows = (z_begin, z_end): only that slice range of the stack (tcp_recon_volume_host_rows), e.g.
         tcp_slice_range(nz_total, rank, world) in a one-process-per-GPU job; out_host keeps the full-stack shape."""
         raw_host = _as_u16(raw_host)
+        if raw_host.dim() != 3:
+            raise TcpError("raw_host: expected [nproj][nz_total][n]")
         nproj, nz_total, n = raw_host.shape
-        assert (nproj, n) == (self.nproj, self.n)
+        if (nproj, n) != (self.nproj, self.n):
+            raise TcpError("raw_host: expected %d projections of width %d, got %s" % (self.nproj, self.n, tuple(raw_host.shape)))
         if out_host is None:
             out_host = torch.empty((nz_total, n, n), dtype=self.out_dtype).pin_memory()
+        # the library dereferences these on the host and hands them to the copy engines: check them here (a CUDA theta
+        # would be read as host memory; a wrong dtype or a non-contiguous view would be misread or overrun)
+        _host(raw_host, torch.uint16, (self.nproj, nz_total, self.n), "raw_host")
+        _host(flat_host, torch.float32, (nz_total, self.n), "flat_host")
+        _host(dark_host, torch.float32, (nz_total, self.n), "dark_host")
+        _host(theta_host, torch.float32, (self.nproj,), "theta_host")
+        _host(out_host, self.out_dtype, (nz_total, self.n, self.n), "out_host")
+        if not (raw_host.is_pinned() and out_host.is_pinned()):
+            import warnings
+            warnings.warn("tcp_recon_volume_host: pageable host buffers: the copies will not overlap the compute")
         if rows is None:
             ms = tcp_recon_volume_host(self.h, raw_host, flat_host, dark_host, theta_host, out_host, nz_total, nbuf)
         else:

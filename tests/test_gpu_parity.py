@@ -898,3 +898,30 @@ def test_preprocessing_zingers_and_rings(dtype, which):
     with pytest.raises(tcp.TcpError):
         rp.set_ring(1e-3)
     rp.close()
+
+
+def test_binding_checks_host_tensors_and_device_angles():
+    """The binding validates what the library cannot (advisor findings): host tensors of the pipeline call must be CPU,
+    contiguous, of the right dtype and shape (a CUDA theta would be dereferenced on the host); device angles of
+    Recon.recon are checked once per tensor on a host copy (unsorted or >= pi spans are refused, not silently mis-gridded)."""
+    tcp = _tcp()
+    w = sg.make_workload("C1")
+    raw, flat, dark, theta = _inputs(w, list(range(4)))
+    r = tcp.Recon(w.n, w.nproj, 4, w.center, "f32", w.filter)
+    raw_h = torch.from_numpy(raw.view(np.int16)).view(torch.uint16).pin_memory()
+    flat_h, dark_h, th_h = torch.from_numpy(flat).pin_memory(), torch.from_numpy(dark).pin_memory(), torch.from_numpy(theta).pin_memory()
+    out, _ = r.recon_volume_host(raw_h, flat_h, dark_h, th_h, nbuf=2)
+    assert np.isfinite(out.numpy()).all()
+    for bad in [dict(theta=th_h.cuda()), dict(theta=th_h.double()), dict(flat=flat_h[:, ::2]), dict(dark=dark_h[:3]),
+                dict(flat=flat_h.cuda())]:
+        a = dict(raw=raw_h, flat=flat_h, dark=dark_h, theta=th_h)
+        a.update(bad)
+        with pytest.raises(tcp.TcpError):
+            r.recon_volume_host(a["raw"], a["flat"], a["dark"], a["theta"], nbuf=2)
+    dev = _to_dev(raw, flat, dark, theta)
+    r.recon(*dev)
+    with pytest.raises(tcp.TcpError):
+        r.recon(dev[0], dev[1], dev[2], (dev[3] * 2.0).contiguous())          # a full turn
+    with pytest.raises(tcp.TcpError):
+        r.recon(dev[0], dev[1], dev[2], dev[3].flip(0).contiguous())          # decreasing
+    r.close()
