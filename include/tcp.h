@@ -205,6 +205,28 @@ int tcp_set_option(tcp_ctx* ctx, int option, int value);
 enum { TCP_PARAM_ZINGER_DIF = 0, TCP_PARAM_RING_ALPHA = 1 };
 int tcp_set_param(tcp_ctx* ctx, int param, double value);
 
+/* Ring removal without allocation: the TCP_PARAM_RING_ALPHA step (reading Q23, same kernels, same fp64 solve) as a free
+ * function on the caller's arrays, for callers that may not call cudaMalloc (code under CUDA graph capture, serving
+ * loops, harnesses that forbid it).  The call allocates and frees nothing: its scratch (6 fp64 words per (slice, detector
+ * pixel)) is a file-scope device array of 6 * TCP_RING_STATIC_MAX doubles = 3 MiB that every GPU which loads the
+ * library holds until the process exits.
+ *   sino_in  DEVICE [nz][nproj][n], p = -ln t, float (dtype TCP_F32) or __half (TCP_F16); read only.
+ *   sino_out DEVICE, same shape and type; may be sino_in (in place) but must not overlap it otherwise.
+ *   alpha    > 0, the Tikhonov weight of TCP_PARAM_RING_ALPHA.
+ * Limit: nz * n <= TCP_RING_STATIC_MAX (e.g. 32 slices of 2048 pixels; nproj is not limited); larger calls return
+ * TCP_EINVAL with the limit in tcp_last_error() -- split the slices over several calls (slices are independent).
+ * Enqueues three kernels on stream and returns; no host synchronisation.  All calls on a device SHARE the scratch array:
+ * calls whose kernels can overlap on the GPU (different streams without an ordering between them, or host threads doing
+ * so) race and give wrong results; calls on one stream, or ordered by events, are safe.  The array keeps the last call's
+ * contents, none of which is read (every word is written before it is read within a call), so nothing is cleared.
+ * The device address of the array is looked up (cudaGetSymbolAddress) the first time a device is used;
+ * tcp_ring_static_setup() does only that for the current device, for callers who want it done before a capture begins.
+ * Errors: TCP_EINVAL (NULL pointer, dtype, sizes, alpha, limit exceeded), TCP_ECUDA. */
+#define TCP_RING_STATIC_MAX 65536
+int tcp_ring_static_setup(void);
+int tcp_ring_remove_static(const void* sino_in, void* sino_out, int nz, int nproj, int n, int dtype, double alpha,
+                           tcp_stream_t stream);
+
 /* Rotation-centre "try" mode ("--reconstruction-type try": one slice reconstructed for a
  * set of candidate centres, for visual choice).  raw_u16 [nproj][1][n], flat / dark [n], theta [nproj] are
  * DEVICE pointers as in tcp_recon; centers is a HOST array of ncenter rotation centres, each in [0, n-1],

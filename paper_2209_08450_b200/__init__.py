@@ -24,6 +24,8 @@ from .binding import (  # noqa: F401
     tcp_check_angles,
     tcp_last_error,
     tcp_measure_rates,
+    tcp_ring_static_setup,
+    tcp_ring_remove_static,
     DTYPES,
     FILTERS,
     EXPORTS,

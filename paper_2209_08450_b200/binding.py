@@ -22,6 +22,7 @@ EXPORTS = [
     "tcp_workspace_bytes", "tcp_launches_per_recon", "tcp_set_option", "tcp_profile_collect",
     "tcp_recon_volume_host", "tcp_recon_try", "tcp_create_det", "tcp_padded_n",
     "tcp_recon_volume_host_rows", "tcp_slice_range", "tcp_check_angles", "tcp_pass1_layout", "tcp_grid_swizzled", "tcp_fft_lines", "tcp_measure_rates", "tcp_set_param",
+    "tcp_ring_static_setup", "tcp_ring_remove_static",
 ]
 
 
@@ -95,6 +96,10 @@ def lib():
     L.tcp_fft_lines.argtypes = [vp, vp, vp, ci, ci, vp]
     L.tcp_set_param.restype = ci
     L.tcp_set_param.argtypes = [vp, ci, C.c_double]
+    L.tcp_ring_static_setup.restype = ci
+    L.tcp_ring_static_setup.argtypes = []
+    L.tcp_ring_remove_static.restype = ci
+    L.tcp_ring_remove_static.argtypes = [vp, vp, ci, ci, ci, ci, C.c_double, vp]
     L.tcp_measure_rates.restype = ci
     L.tcp_measure_rates.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.tcp_recon_try.restype = ci
@@ -150,6 +155,22 @@ def tcp_measure_rates():
     a, b = C.c_double(0.0), C.c_double(0.0)
     _check(lib().tcp_measure_rates(C.byref(a), C.byref(b)))
     return float(a.value), float(b.value)
+
+
+def tcp_ring_static_setup():
+    _check(lib().tcp_ring_static_setup())
+
+
+def tcp_ring_remove_static(sino_in, sino_out, alpha, stream=None):
+    """Ring removal on CUDA tensors [nz][nproj][n] (float32 or float16) without any allocation (tcp_ring_remove_static);
+    sino_out may be sino_in."""
+    if sino_in.dtype not in (torch.float32, torch.float16):
+        raise TcpError("expected float32 or float16 sinograms")
+    if sino_in.dim() != 3:
+        raise TcpError("expected a sinogram of shape [nz][nproj][n]")
+    nz, nproj, n = sino_in.shape
+    _check(lib().tcp_ring_remove_static(_dev(sino_in, sino_in.dtype), _dev(sino_out, sino_in.dtype, sino_in.shape), nz, nproj, n,
+                                        DTYPES["f16" if sino_in.dtype == torch.float16 else "f32"], float(alpha), _stream(stream)))
 
 
 def tcp_create_ex(n, nproj, nz_chunk, center, dtype, filter, m):

@@ -7,7 +7,11 @@
 // Both work on the context's sinogram workspace [nz][nproj][n] (float or half); tcp_recon then skips the fused S1+S2
 // loader.  The ring system is solved in fp64 (one thread per slice, O(n), banded LDL^T): its result is a small correction,
 // and fp64 keeps it exact at the level of the fp32 gate whatever alpha is.
+#include <math.h>
+
 #include <algorithm>
+#include <map>
+#include <mutex>
 
 #include "tcp_internal.h"
 
@@ -138,3 +142,92 @@ int launch_pre(const tcp_ctx* c, cudaStream_t st) {
 }
 
 }  // namespace tcpk
+
+// ------------------------------------------------------------------------------------------------ allocation-free ring removal
+// tcp_ring_remove_static (tcp.h): the ring-removal step above for callers that may not allocate (CUDA graph capture, serving
+// loops, harnesses that forbid cudaMalloc).  The same three kernels run on the caller's arrays; the scratch that
+// tcp_set_param(TCP_PARAM_RING_ALPHA) would cudaMalloc per context (angle means [nz][n] + solver work [nz][5][n], fp64)
+// lives in ONE file-scope device array of fixed size instead: 6 * TCP_RING_STATIC_MAX doubles = 3 MiB, held by every GPU
+// that loads the library until the process exits, shared by every call (calls that overlap on the GPU race on it).
+// Nothing in it has to start at zero: ring_mean_kernel writes every mean, and ring_solve_kernel writes d, l1, l2, y, r at
+// index i before it reads them at i - 1, i - 2 (factorisation) or i + 1, i + 2 (back substitution); the last call's
+// contents are never read.
+namespace tcpk {
+
+static __device__ __align__(256) double g_ring_static[6 * (size_t)TCP_RING_STATIC_MAX];
+
+// out-of-place form of ring_sub_kernel (in == out allowed: one read and one write of the same element per thread)
+template <class TS>
+__global__ void __launch_bounds__(256) ring_sub_io_kernel(const TS* in, TS* out, const double* __restrict__ work, int nz, int nproj, int n) {
+    const size_t total = (size_t)nz * nproj * n;
+    for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < total; v += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(v % n);
+        const int z = (int)(v / ((size_t)nproj * n));
+        const double r = work[((size_t)z * 5 + 4) * n + i];
+        st_r(out, v, (float)((double)ld_r(in, v) - r));
+    }
+}
+
+// In host code `g_ring_static` is the host-side stand-in of the symbol, not a device address: the device address is asked
+// for once per device, with that device current, and cached.
+struct RingStaticDev {
+    double* scratch;
+    int nsm;
+};
+static std::mutex g_ring_static_mu;
+static std::map<int, RingStaticDev> g_ring_static_dev;
+
+static int ring_static_setup(RingStaticDev* out) {
+    int dev = -1;
+    TCP_CUDA_CHECK(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lk(g_ring_static_mu);
+    auto it = g_ring_static_dev.find(dev);
+    if (it == g_ring_static_dev.end()) {
+        RingStaticDev d{nullptr, 0};
+        TCP_CUDA_CHECK(cudaGetSymbolAddress((void**)&d.scratch, g_ring_static));
+        if (!d.scratch) return set_error(TCP_ECUDA, "tcp_ring_remove_static: cudaGetSymbolAddress returned a null address on device %d", dev);
+        TCP_CUDA_CHECK(cudaDeviceGetAttribute(&d.nsm, cudaDevAttrMultiProcessorCount, dev));
+        it = g_ring_static_dev.emplace(dev, d).first;
+    }
+    *out = it->second;
+    return TCP_OK;
+}
+
+template <class TS>
+static int ring_static_launch(const RingStaticDev& d, const void* in, void* out, int nz, int nproj, int n, double alpha, cudaStream_t st) {
+    const size_t total = (size_t)nz * nproj * n;
+    const int blocks = (int)std::min<size_t>((total + 255) / 256, (size_t)d.nsm * 16);
+    double* pbar = d.scratch;
+    double* work = d.scratch + (size_t)nz * n;
+    ring_mean_kernel<TS><<<dim3((n + 255) / 256, nz), 256, 0, st>>>((const TS*)in, pbar, nz, nproj, n);
+    ring_solve_kernel<<<(nz + 31) / 32, 32, 0, st>>>(pbar, work, nz, n, alpha);
+    ring_sub_io_kernel<TS><<<blocks, 256, 0, st>>>((const TS*)in, (TS*)out, work, nz, nproj, n);
+    TCP_CUDA_CHECK(cudaGetLastError());
+    return TCP_OK;
+}
+
+}  // namespace tcpk
+
+extern "C" int tcp_ring_static_setup(void) {
+    tcpk::RingStaticDev d;
+    return tcpk::ring_static_setup(&d);
+}
+
+extern "C" int tcp_ring_remove_static(const void* sino_in, void* sino_out, int nz, int nproj, int n, int dtype, double alpha,
+                                      tcp_stream_t stream) {
+    using namespace tcpk;
+    if (!sino_in || !sino_out) return set_error(TCP_EINVAL, "tcp_ring_remove_static: NULL sinogram pointer");
+    if (dtype != TCP_F32 && dtype != TCP_F16) return set_error(TCP_EINVAL, "tcp_ring_remove_static: dtype %d is neither TCP_F32 nor TCP_F16", dtype);
+    if (nz < 1 || nproj < 1 || n < 3) return set_error(TCP_EINVAL, "tcp_ring_remove_static: need nz >= 1, nproj >= 1, n >= 3 (got %d, %d, %d)", nz, nproj, n);
+    if (!(alpha > 0.0) || !isfinite(alpha)) return set_error(TCP_EINVAL, "tcp_ring_remove_static: alpha must be positive and finite");
+    if ((long long)nz * n > (long long)TCP_RING_STATIC_MAX)
+        return set_error(TCP_EINVAL, "tcp_ring_remove_static: nz * n = %lld exceeds TCP_RING_STATIC_MAX = %d (the fixed scratch array); "
+                         "split the slices over several calls or use tcp_set_param(TCP_PARAM_RING_ALPHA)", (long long)nz * n, (int)TCP_RING_STATIC_MAX);
+    if (nz > 65535) return set_error(TCP_EINVAL, "tcp_ring_remove_static: nz = %d exceeds 65535", nz);
+    RingStaticDev d;
+    int rc = ring_static_setup(&d);
+    if (rc != TCP_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    return dtype == TCP_F16 ? ring_static_launch<__half>(d, sino_in, sino_out, nz, nproj, n, alpha, st)
+                            : ring_static_launch<float>(d, sino_in, sino_out, nz, nproj, n, alpha, st);
+}
