@@ -83,6 +83,11 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
     float2* HT = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(T1TAB) + T1_BYTES);   // 2^12 H/M at (k0, k0 + 1) of the 8 output pairs
     float4* PT = reinterpret_cast<float4*>(HT + 8 * NT);                // phase table / 2^12 at the same indices
     float4* FD = PT + 8 * NT;                                           // RAW: (1/(flat-dark), dark) of the thread's 8 pixels, slices A and B
+    // RAW: the two detector rows of the NEXT projection arrive by bulk asynchronous copies (2 x 4 KB) while this one is
+    // transformed; loaded with __ldg at the top of the loop they cost a DRAM latency per unit with nothing to hide it
+    // (profiles/r2_kernels.md: 11 % of the warp samples wait on that load)
+    uint16_t* RB = reinterpret_cast<uint16_t*>(FD + 8 * NT);            // [2][n]
+    uint64_t* rbar = reinterpret_cast<uint64_t*>(RB + 2 * n);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, c = lane & 3;
     // persistent CTAs: a CTA stays with ONE slice pair (blockIdx % npair), so everything that depends on the thread and the
     // pair only -- butterfly fragments, twiddles, filter, phase and flat/dark tables -- is set up once
@@ -92,6 +97,20 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
     const bool hasB = zB < nz;
     const int zBs = hasB ? zB : zA;
     if (try_mode) ptab += (size_t)pair * N;
+    auto fetch_raw = [&](int j) {                                       // thread 0 only
+        mbar_expect_tx(rbar, 2 * n * 2);
+        bulk_g2s(RB, raw + ((size_t)j * nz + zA) * n, n * 2, rbar);
+        bulk_g2s(RB + n, raw + ((size_t)j * nz + zBs) * n, n * 2, rbar);
+    };
+    if constexpr (RAW) {
+        if (tid == 0) {
+            mbar_init(rbar, 1);
+            fence_mbar_init();
+        }
+        __syncthreads();
+        if (tid == 0 && jstart < nproj) fetch_raw(jstart);
+    }
+    uint32_t rphase = 0;
     {
         const int kbase = pass3_index<false>(0, 0, warp, g, c);
 #pragma unroll
@@ -131,8 +150,10 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
         const int i0 = tid * 8;
         float a[8], b[8];
         if constexpr (RAW) {
-            const uint4 ra = __ldg(reinterpret_cast<const uint4*>(raw + ((size_t)j * nz + zA) * n + i0));
-            const uint4 rb = __ldg(reinterpret_cast<const uint4*>(raw + ((size_t)j * nz + zBs) * n + i0));
+            mbar_wait(rbar, rphase);
+            rphase ^= 1;
+            const uint4 ra = *reinterpret_cast<const uint4*>(RB + i0);
+            const uint4 rb = *reinterpret_cast<const uint4*>(RB + n + i0);
             const unsigned ua[4] = {ra.x, ra.y, ra.z, ra.w}, ub[4] = {rb.x, rb.y, rb.z, rb.w};
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
@@ -163,6 +184,12 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
         dst[1] = make_uint4(w[4], w[5], w[6], w[7]);
     }
     __syncthreads();
+    if constexpr (RAW) {                  // every thread has read the raw rows: the next projection's may land
+        if (tid == 0 && j + jstep < nproj) {
+            fence_proxy_async();
+            fetch_raw(j + jstep);
+        }
+    }
     if constexpr (PAD_EDGE) {     // padding samples of the filter stage: the nearest edge of the periodic row
         const uint32_t last = L[swz<1>(n - 1)], first = L[swz<1>(0)];
         const uint32_t v = tid < NT / 2 ? last : first;
@@ -219,6 +246,9 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
 // its copy the others transform.  Only the central n outputs are computed in the last pass (tile 0 of the AV_LOC fragments).
 // Output: pass1[pair][iy / 2][swz<2>(l1)][iy % 2] -- the row pass loads its lines the same way.  A thread holds 32
 // contiguous bytes (4 columns x 2 rows); lane pairs swap halves so that every 16-byte store instruction fills whole sectors.
+__device__ __forceinline__ void st_v4(void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+    asm volatile("st.global.v4.b32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
 __global__ void __launch_bounds__(NT, 2) cols_mma_kernel(const uint4* __restrict__ grid, uint2* __restrict__ p1arr,
                                                           const float2* __restrict__ tw, const uint32_t* __restrict__ atab, int nunits) {
     constexpr int n = N / 2;
@@ -278,13 +308,10 @@ __global__ void __launch_bounds__(NT, 2) cols_mma_kernel(const uint4* __restrict
         for (int q = 0; q < 4; ++q) r[q] = __shfl_xor_sync(0xffffffffu, odd ? w[q] : w[4 + q], 1);
         unsigned char* mine = dst + (size_t)(iy0 >> 1) * (N * 8);
         unsigned char* other = odd ? mine - N * 8 : mine + N * 8;
-        if (!odd) {
-            *reinterpret_cast<uint4*>(mine) = make_uint4(w[0], w[1], w[2], w[3]);
-            *reinterpret_cast<uint4*>(other) = make_uint4(r[0], r[1], r[2], r[3]);
-        } else {
-            *reinterpret_cast<uint4*>(other + 16) = make_uint4(r[0], r[1], r[2], r[3]);
-            *reinterpret_cast<uint4*>(mine + 16) = make_uint4(w[4], w[5], w[6], w[7]);
-        }
+        // two unconditional 16-byte stores per thread (addresses and values selected, no divergent branch: the compiler
+        // splits a store whose address comes out of a merged branch into four 4-byte stores, 4 x the tag requests)
+        st_v4(odd ? other + 16 : mine, odd ? r[0] : w[0], odd ? r[1] : w[1], odd ? r[2] : w[2], odd ? r[3] : w[3]);
+        st_v4(odd ? mine + 16 : other, odd ? w[4] : r[0], odd ? w[5] : r[1], odd ? w[6] : r[2], odd ? w[7] : r[3]);
     });
     __syncthreads();                      // the lines are free for the next unit
     if (tid == 0 && unit + (int)gridDim.x < nunits) {
@@ -397,7 +424,7 @@ __global__ void __launch_bounds__(NT, 2) fft_lines_kernel(const uint32_t* __rest
 
 // ------------------------------------------------------------------------------------------------ launchers
 int launch_rows_mma(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw) {
-    const size_t smem = (size_t)N * 4 + T1_BYTES + 8 * NT * (8 + 16 + (raw ? 16 : 0));
+    const size_t smem = (size_t)N * 4 + T1_BYTES + 8 * NT * (8 + 16 + (raw ? 16 : 0)) + (raw ? 2 * (N / 2) * 2 + 16 : 0);
     auto kern = raw ? (c->pad ? rows_mma_kernel<true, true> : rows_mma_kernel<false, true>)
                     : (c->pad ? rows_mma_kernel<true, false> : rows_mma_kernel<false, false>);
     TCP_SMEM(kern, smem);
