@@ -69,6 +69,11 @@ void mmafft_free(tcp_ctx* c) { cudaFree(c->mf_atab); }
 constexpr float kRowScale = 4096.f;
 
 // ------------------------------------------------------------------------------------------------ detector rows
+// negate the imaginary output rows (registers 1, 3) of tile 0: the transform then returns the conjugate of its result
+__device__ __forceinline__ void conj_tile0(AFrag& f) {
+#pragma unroll
+    for (int s = 0; s < 2; ++s) { f.a[0][s][1] ^= 0x80008000u; f.a[0][s][3] ^= 0x80008000u; }
+}
 template <bool PAD_EDGE, bool RAW>
 __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restrict__ sino, __half2* __restrict__ spec,
                                                           const float2* __restrict__ tw, const uint32_t* __restrict__ atab,
@@ -204,26 +209,26 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
     __syncthreads();
     pass2<1, false>(L, An, T, O);
     __syncthreads();
+    // the epilogue stores conj(Q): the inverse transform below is conj(FFT(conj(Q))), i.e. a FORWARD transform whose
+    // pass-3 fragments have their imaginary rows negated (4 sign flips instead of 64 to turn both fragment sets around)
     pass3<1, false, false, true>(L, Al, O, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
         const float2 h = HT[slot_of(k0) * NT + tid];
         const float h0 = h.x, h1 = h.y;
-        *reinterpret_cast<uint2*>(&L[swz<1>(k0)]) = make_uint2(pack_h2(y0[0].x * h0, y0[0].y * h0), pack_h2(y1[0].x * h1, y1[0].y * h1));
+        *reinterpret_cast<uint2*>(&L[swz<1>(k0)]) = make_uint2(pack_h2(y0[0].x * h0, y0[0].y * -h0), pack_h2(y1[0].x * h1, y1[0].y * -h1));
     });
     __syncthreads();
-    // ---- transform 2 (inverse): the filtered row, cropped to the detector (only tile 0 = samples below n is computed)
-    flip_afrag(An);
-    flip_afrag(Al);
-    pass1<1, true, false, true>(L, An, T, O, warp, g, c, no_in);
+    // ---- transform 2 (inverse, see above): the filtered row, cropped to the detector (only tile 0 = samples below n is computed)
+    pass1<1, false, false, true>(L, An, T, O, warp, g, c, no_in);
     __syncthreads();
-    pass2<1, true>(L, An, T, O);
+    pass2<1, false>(L, An, T, O);
     __syncthreads();
+    conj_tile0(Al);
     pass3<1, true, false, true>(L, Al, O, warp, g, c, [&](int k0, const float2(&y0)[1], const float2(&y1)[1]) {
         *reinterpret_cast<uint2*>(&L[swz<1>(k0)]) = make_uint2(pack_h2(y0[0].x, y0[0].y), pack_h2(y1[0].x, y1[0].y));
     });
+    conj_tile0(Al);
     __syncthreads();
     // ---- transform 3: spectrum of the zero-padded filtered row, centre phase and scale on store
-    flip_afrag(An);
-    flip_afrag(Al);
     pass1<1, false, true, true>(L, An, T, O, warp, g, c, no_in);
     __syncthreads();
     pass2<1, false>(L, An, T, O);
