@@ -391,8 +391,12 @@ def run_ours(args, rank, world, local_rank):
     names = dict(KERNEL_NAMES, **(KERNEL_NAMES_MMA if on_mma else ({"grid": "grid_mma_kernel"} if half_store else {})))
     # SURVEY 8(d) assigns the roofs: normalise and the 2D transform passes HBM, gridding "plain ALUs / smem / L2", the
     # row kernel "HBM if half2 math; else fp32 ALUs".  Both fractions are reported for every kernel; `bound` names the
-    # roof 8(d) assigns to the dominant one and `frac` is the fraction of that roof.
-    assigned = {"normalize": "hbm", "rows": "alu", "grid": "alu", "ifft_cols": "hbm", "ifft_rows": "hbm"}[dom]
+    # roof assigned to the dominant one and `frac` is the fraction of that roof.  One departure from 8(d), fp16 storage
+    # only: its gridding row describes a CUDA-core kernel; grid_mma_kernel multiplies on the tensor cores and replays
+    # cached weights, its FMA pipe is 16 % busy and its DRAM traffic 53-56 % of peak (profiles/r2_kernels.md), so HBM is
+    # the nearer roof and the one reported.  The fp32 tile kernel keeps "alu".
+    assigned = {"normalize": "hbm", "rows": "alu", "grid": "hbm" if half_store else "alu", "ifft_cols": "hbm",
+                "ifft_rows": "hbm"}[dom]
     roof = {"kernel": names.get(dom, dom), "bound": assigned,
             "achieved": kernels[dom]["TFLOPps"] if assigned == "alu" else kernels[dom]["GBps"],
             "peak": alu_peak if assigned == "alu" else hbm_gbs, "unit": "TFLOP/s" if assigned == "alu" else "GB/s",
