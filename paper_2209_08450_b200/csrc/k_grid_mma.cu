@@ -62,6 +62,59 @@ __device__ __forceinline__ void nu_split(float k, float c_hi, float c_lo, float&
     else if (frac >= 1.f) { fl += 1.f; frac -= 1.f; }
 }
 
+// Compact weight record of a column for the half-width-2 kernel (4 taps per axis): 28 bytes instead of 52.
+//   cx: the two aligned groups of four cell positions (8 bytes each) that hold the x taps, groups u0 and u0 + 1 of the
+//       sub-tile's four (u0 in -1..3; a group outside the sub-tile is stored as zero and dropped);
+//   cy: the four y taps, rows e0y .. e0y + 3 of the sub-tile's eight (e0y in -3..7; rows outside are dropped);
+//   u0 + 1 (3 bits) and e0y + 3 (4 bits) ride in bits 14 and 15 of the four y taps, which are zero for weights <= 1.
+// expand_record() rebuilds exactly the (xa, xc, yv) registers the direct kernel computes: every position outside the two
+// groups / four rows carries a zero weight there (the open box |l - nu| < 2 spans four cells).
+__device__ __forceinline__ void compact_record(const unsigned (&wx)[8], const unsigned (&wy)[4], int e0x, int e0y, uint4& cx, uint2& cy) {
+    const int u0 = max(-1, min(3, e0x >= -4 ? (e0x + 4) / 4 - 1 : -1));
+    auto unit = [&](int j) {
+        uint2 r = make_uint2(0u, 0u);
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            if (q == j) r = make_uint2(wx[2 * q], wx[2 * q + 1]);
+        return r;
+    };
+    const uint2 a = unit(u0), b = unit(u0 + 1);
+    cx = make_uint4(a.x, a.y, b.x, b.y);
+    const int ey = max(-3, min(7, e0y));
+    const unsigned long long ylo = (unsigned long long)wy[0] | ((unsigned long long)wy[1] << 32);
+    const unsigned long long yhi = (unsigned long long)wy[2] | ((unsigned long long)wy[3] << 32);
+    unsigned long long t;
+    if (ey >= 0) {
+        const int sh = 16 * ey;
+        t = sh == 0 ? ylo : (sh < 64 ? ((ylo >> sh) | (yhi << (64 - sh))) : (yhi >> (sh - 64)));
+    } else {
+        t = ylo << (16 * -ey);
+    }
+    const unsigned code = (unsigned)(u0 + 1) | ((unsigned)(ey + 3) << 3);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) t |= (unsigned long long)((code >> (2 * i)) & 3u) << (16 * i + 14);
+    cy = make_uint2((unsigned)t, (unsigned)(t >> 32));
+}
+__device__ __forceinline__ void expand_record(const uint4& cx, const uint2& cy, uint4& xa, uint4& xc, uint4& yv) {
+    unsigned long long t = (unsigned long long)cy.x | ((unsigned long long)cy.y << 32);
+    const unsigned code = ((cy.x >> 14) & 3u) | (((cy.x >> 30) & 3u) << 2) | (((cy.y >> 14) & 3u) << 4) | (((cy.y >> 30) & 3u) << 6);
+    t &= 0x3fff3fff3fff3fffull;
+    const int u0 = (int)(code & 7u) - 1, ey = (int)(code >> 3) - 3;
+    auto pick = [&](int j, unsigned first, unsigned second) { return u0 == j ? first : (u0 == j - 1 ? second : 0u); };
+    xa = make_uint4(pick(0, cx.x, cx.z), pick(0, cx.y, cx.w), pick(1, cx.x, cx.z), pick(1, cx.y, cx.w));
+    xc = make_uint4(pick(2, cx.x, cx.z), pick(2, cx.y, cx.w), pick(3, cx.x, cx.z), pick(3, cx.y, cx.w));
+    unsigned long long lo, hi;
+    if (ey >= 0) {
+        const int sh = 16 * ey;
+        lo = sh < 64 ? t << sh : 0ull;
+        hi = sh == 0 ? 0ull : (sh < 64 ? t >> (64 - sh) : t << (sh - 64));
+    } else {
+        lo = t >> (16 * -ey);
+        hi = 0ull;
+    }
+    yv = make_uint4((unsigned)lo, (unsigned)(lo >> 32), (unsigned)hi, (unsigned)(hi >> 32));
+}
+
 // dynamic shared memory carve-up: per-warp A/B stages and scratch
 template <int NN>
 struct MmaSmem {
@@ -224,6 +277,34 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
         if (ns > 0) {
             const size_t st0 = (size_t)wbase;
             alignas(16) __half2 bvA[NPG], bvB[NPG];
+            if constexpr (MH == 2) {
+                // compact records (28 bytes per column, compact_record above), expanded right before the stage is written
+                auto ldx = [&](size_t st) { return __ldg(&wrec[(st * 3 + 0) * 32 + lane]); };
+                auto ldy = [&](size_t st) { return __ldg(reinterpret_cast<const uint2*>(&wrec[(st * 3 + 1) * 32]) + lane); };
+                uint4 cxA = ldx(st0);
+                uint2 cyA = ldy(st0);
+                gather(__ldg(&wsamp[st0 * 32 + lane]), bvA);
+                unsigned samp_next = ns > 1 ? __ldg(&wsamp[(st0 + 1) * 32 + lane]) : 0u;
+#pragma unroll 1
+                for (int sidx = 0; sidx < ns; ++sidx) {
+                    const size_t st = st0 + sidx + 1;
+                    const bool more = sidx + 1 < ns;
+                    uint4 cxB = cxA;
+                    uint2 cyB = cyA;
+                    if (more) {
+                        gather(samp_next, bvB);
+                        cxB = ldx(st);
+                        cyB = ldy(st);
+                        if (sidx + 2 < ns) samp_next = __ldg(&wsamp[(st + 1) * 32 + lane]);
+                    }
+                    uint4 xa, xc, yv;
+                    expand_record(cxA, cyA, xa, xc, yv);
+                    issue_step(xa, xc, yv, bvA, true);
+                    cxA = cxB; cyA = cyB;
+#pragma unroll
+                    for (int p = 0; p < NPG; ++p) bvA[p] = bvB[p];
+                }
+            } else {
             uint4 xaA = __ldg(&wrec[(st0 * 3 + 0) * 32 + lane]), xcA = __ldg(&wrec[(st0 * 3 + 1) * 32 + lane]);
             uint4 yvA = __ldg(&wrec[(st0 * 3 + 2) * 32 + lane]);
             gather(__ldg(&wsamp[st0 * 32 + lane]), bvA);
@@ -244,6 +325,7 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                 xaA = xaB; xcA = xcB; yvA = yvB;
 #pragma unroll
                 for (int p = 0; p < NPG; ++p) bvA[p] = bvB[p];
+            }
             }
         }
     } else
@@ -315,6 +397,8 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                 // at distance d = a - frac; the open box |l - nu| < m keeps a in [-m+1, m] for a fractional nu
                 // and [-m+1, m-1] when nu is an integer.
                 uint4 xa, xc, yv;
+                uint4 cxr = make_uint4(0u, 0u, 0u, 0u);
+                uint2 cyr = make_uint2(0u, 0u);
                 {
                     float flx, frx, fly, fry;
                     nu_split((float)k, cxh, cxl, flx, frx);
@@ -342,13 +426,20 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                     xa = make_uint4(wx[0], wx[1], wx[2], wx[3]);
                     xc = make_uint4(wx[4], wx[5], wx[6], wx[7]);
                     yv = make_uint4(wy[0], wy[1], wy[2], wy[3]);
+                    if constexpr (MODE == GM_FILL && MH == 2)      // first tap (a = lo) sits at cell position lo - ax0, row lo - ay0
+                        compact_record(wx, wy, (int)(lo - ax0), (int)(lo - ay0), cxr, cyr);
                 }
                 if constexpr (MODE == GM_FILL) {
                     // record of this step and column: [step][xa | xc | yv][lane] and the sample offset
                     const size_t st = (size_t)wbase + istep;
-                    wrec[(st * 3 + 0) * 32 + lane] = xa;
-                    wrec[(st * 3 + 1) * 32 + lane] = xc;
-                    wrec[(st * 3 + 2) * 32 + lane] = yv;
+                    if constexpr (MH == 2) {
+                        wrec[(st * 3 + 0) * 32 + lane] = cxr;
+                        reinterpret_cast<uint2*>(&wrec[(st * 3 + 1) * 32])[lane] = cyr;
+                    } else {
+                        wrec[(st * 3 + 0) * 32 + lane] = xa;
+                        wrec[(st * 3 + 1) * 32 + lane] = xc;
+                        wrec[(st * 3 + 2) * 32 + lane] = yv;
+                    }
                     wsamp[st * 32 + lane] = samp;
                     ++istep;
                 } else {

@@ -411,14 +411,16 @@ def test_fused_filter_option(dtype, pad):
     r.close()
 
 
-def test_gridding_weight_cache():
-    """TCP_OPT_WEIGHT_CACHE: the cached replay equals the direct kernel bit for bit; the cache follows a change of
+@pytest.mark.parametrize("m", [3, 16 + 2])
+def test_gridding_weight_cache(m):
+    """TCP_OPT_WEIGHT_CACHE: the cached replay equals the direct kernel bit for bit (m = 3: the 52-byte records; Kaiser-Bessel
+    half-width 2: the compact 28-byte records, k_grid_mma.cu compact_record / expand_record); the cache follows a change of
     the angles between calls (rebuilt on the device) and of nothing else."""
     tcp = _tcp()
     w = sg.make_workload("C1")
     raw, flat, dark, theta = _inputs(w, list(range(8)))
     d = _to_dev(raw, flat, dark, theta)
-    r = tcp.Recon(w.n, w.nproj, 8, w.center, "f16", w.filter, 3)
+    r = tcp.Recon(w.n, w.nproj, 8, w.center, "f16", w.filter, m)
     r.set_weight_cache(False)
     direct = r.recon(*d).clone()
     r.set_weight_cache(True)
@@ -432,7 +434,7 @@ def test_gridding_weight_cache():
     r.set_weight_cache(False)
     b = r.recon(*d2).clone()
     assert torch.equal(a, b)
-    ref = orc.recon(raw[:, 3:4], flat[3:4], dark[3:4], th2, w.center, w.filter, 3, "grid")[0]
+    ref = orc.recon(raw[:, 3:4], flat[3:4], dark[3:4], th2, w.center, w.filter, m, "grid")[0]
     assert rl2(a[3].float().cpu().numpy(), ref) < FP16_GATE_L2
     # back to the first angles
     r.set_weight_cache(True)
