@@ -140,7 +140,10 @@ int tcp_padded_n(const tcp_ctx* ctx);
  *   flat, dark [nz_chunk][n] float32, already averaged over frames
  *   theta   [nproj] float32 radians, strictly increasing, spanning less than pi
  *   out     [nz_chunk][n][n], float32 (TCP_F32, TCP_F16_OUT32) or IEEE half (TCP_F16)
- * One tcp_recon may be in flight per context.  Bitwise reproducible run to run. */
+ * One tcp_recon may be in flight per context.  Bitwise reproducible run to run.
+ * Alignment: on a power-of-two context (tcp_create, tcp_create_ex) raw_u16, flat, dark and out must be 16-byte aligned
+ * (rows move as 16-byte vectors and bulk copies; cudaMalloc and torch allocations are 256-byte aligned, and so is every
+ * whole-chunk view of them): TCP_EINVAL otherwise.  tcp_create_det contexts of other widths take any element alignment. */
 int tcp_recon(tcp_ctx* ctx, const uint16_t* raw_u16, const float* flat, const float* dark,
               const float* theta, void* out, tcp_stream_t stream);
 

@@ -326,6 +326,9 @@ int tcp_normalize(tcp_ctx* c, const uint16_t* raw, const float* flat, const floa
 int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* dark, const float* theta, void* out,
               tcp_stream_t stream) {
     if (!c || !raw || !flat || !dark || !theta || !out) return set_error(TCP_EINVAL, "NULL argument");
+    // the kernels move rows with 16-byte loads, stores and bulk copies (tcp.h: alignment of the device arrays)
+    if (c->ndet == c->n && (((uintptr_t)raw | (uintptr_t)flat | (uintptr_t)dark | (uintptr_t)out) & 15))
+        return set_error(TCP_EINVAL, "raw_u16, flat, dark and out must be 16-byte aligned");
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
     void* const user_out = out;
@@ -376,6 +379,8 @@ int tcp_recon_try(tcp_ctx* c, const uint16_t* raw, const float* flat, const floa
                   const float* centers, int ncenter, void* out, tcp_stream_t stream) {
     if (!c || !raw || !flat || !dark || !theta || !centers || !out) return set_error(TCP_EINVAL, "NULL argument");
     if (c->algorithm != TCP_ALG_FOURIER) return set_error(TCP_EUNSUPPORTED, "tcp_recon_try is FourierRec only");
+    if (c->ndet == c->n && (((uintptr_t)raw | (uintptr_t)flat | (uintptr_t)dark | (uintptr_t)out) & 15))
+        return set_error(TCP_EINVAL, "raw_u16, flat, dark and out must be 16-byte aligned");
     if (ncenter < 1 || ncenter > c->nz) return set_error(TCP_EINVAL, "ncenter=%d outside [1, nz_chunk=%d]", ncenter, c->nz);
     for (int i = 0; i < ncenter; ++i)
         if (!(centers[i] >= 0.f && centers[i] <= (float)(c->ndet - 1)))

@@ -926,4 +926,9 @@ def test_binding_checks_host_tensors_and_device_angles():
         r.recon(dev[0], dev[1], dev[2], (dev[3] * 2.0).contiguous())          # a full turn
     with pytest.raises(tcp.TcpError):
         r.recon(dev[0], dev[1], dev[2], dev[3].flip(0).contiguous())          # decreasing
+    # tcp.h: on a power-of-two context the device arrays must be 16-byte aligned (rows move as 16-byte vectors / bulk copies)
+    shifted = torch.empty(dev[1].numel() + 1, dtype=torch.float32, device="cuda")[1:].view_as(dev[1])
+    shifted.copy_(dev[1])
+    with pytest.raises(tcp.TcpError, match="16-byte"):
+        r.recon(dev[0], shifted, dev[2], dev[3])
     r.close()
