@@ -62,54 +62,62 @@ __device__ __forceinline__ void nu_split(float k, float c_hi, float c_lo, float&
     else if (frac >= 1.f) { fl += 1.f; frac -= 1.f; }
 }
 
-// Compact weight record of a column for the half-width-2 kernel (4 taps per axis): 28 bytes instead of 52.
-//   cx: the two aligned groups of four cell positions (8 bytes each) that hold the x taps, groups u0 and u0 + 1 of the
-//       sub-tile's four (u0 in -1..3; a group outside the sub-tile is stored as zero and dropped);
-//   cy: the four y taps, rows e0y .. e0y + 3 of the sub-tile's eight (e0y in -3..7; rows outside are dropped);
-//   u0 + 1 (3 bits) and e0y + 3 (4 bits) ride in bits 14 and 15 of the four y taps, which are zero for weights <= 1.
-// expand_record() rebuilds exactly the (xa, xc, yv) registers the direct kernel computes: every position outside the two
-// groups / four rows carries a zero weight there (the open box |l - nu| < 2 spans four cells).
-__device__ __forceinline__ void compact_record(const unsigned (&wx)[8], const unsigned (&wy)[4], int e0x, int e0y, uint4& cx, uint2& cy) {
-    const int u0 = max(-1, min(3, e0x >= -4 ? (e0x + 4) / 4 - 1 : -1));
-    auto unit = [&](int j) {
-        uint2 r = make_uint2(0u, 0u);
+// Compact weight record of a column for the half-width-2 kernel (4 taps per axis): one uint4 + the sample offset = 20 bytes
+// instead of 52.
+//   (x, y) of the uint4: the four x taps, cell positions ex .. ex + 3 of the sub-tile's sixteen (ex in -4..16; taps whose
+//       position falls outside the sub-tile are stored as zero and dropped);
+//   (z, w): the four y taps, rows ey .. ey + 3 of the sub-tile's eight (ey in -3..7);
+//   ex + 4 (5 bits) and ey + 3 (4 bits) ride in bits 14 and 15 of the taps, which are zero for weights <= 1.
+// expand_record() rebuilds exactly the (xa, xc, yv) registers the direct kernel computes: every position outside the four
+// cells / four rows carries a zero weight there (the open box |l - nu| < 2 spans four cells).
+__device__ __forceinline__ uint4 compact_record(const unsigned (&wx)[8], const unsigned (&wy)[4], int e0x, int e0y) {
+    const int ex = max(-4, min(16, e0x));
+    unsigned long long tx = 0ull;
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
-            if (q == j) r = make_uint2(wx[2 * q], wx[2 * q + 1]);
-        return r;
-    };
-    const uint2 a = unit(u0), b = unit(u0 + 1);
-    cx = make_uint4(a.x, a.y, b.x, b.y);
+    for (int i = 0; i < 4; ++i) {
+        const int cell = ex + i;
+        unsigned h = 0u;
+#pragma unroll
+        for (int q = 0; q < 16; ++q)
+            if (q == cell) h = (q & 1) ? (wx[q >> 1] >> 16) : (wx[q >> 1] & 0xffffu);
+        tx |= (unsigned long long)h << (16 * i);
+    }
     const int ey = max(-3, min(7, e0y));
     const unsigned long long ylo = (unsigned long long)wy[0] | ((unsigned long long)wy[1] << 32);
     const unsigned long long yhi = (unsigned long long)wy[2] | ((unsigned long long)wy[3] << 32);
-    unsigned long long t;
+    unsigned long long ty;
     if (ey >= 0) {
         const int sh = 16 * ey;
-        t = sh == 0 ? ylo : (sh < 64 ? ((ylo >> sh) | (yhi << (64 - sh))) : (yhi >> (sh - 64)));
+        ty = sh == 0 ? ylo : (sh < 64 ? ((ylo >> sh) | (yhi << (64 - sh))) : (yhi >> (sh - 64)));
     } else {
-        t = ylo << (16 * -ey);
+        ty = ylo << (16 * -ey);
     }
-    const unsigned code = (unsigned)(u0 + 1) | ((unsigned)(ey + 3) << 3);
+    const unsigned cxd = (unsigned)(ex + 4), cyd = (unsigned)(ey + 3);
 #pragma unroll
-    for (int i = 0; i < 4; ++i) t |= (unsigned long long)((code >> (2 * i)) & 3u) << (16 * i + 14);
-    cy = make_uint2((unsigned)t, (unsigned)(t >> 32));
+    for (int i = 0; i < 3; ++i) tx |= (unsigned long long)((cxd >> (2 * i)) & 3u) << (16 * i + 14);
+#pragma unroll
+    for (int i = 0; i < 2; ++i) ty |= (unsigned long long)((cyd >> (2 * i)) & 3u) << (16 * i + 14);
+    return make_uint4((unsigned)tx, (unsigned)(tx >> 32), (unsigned)ty, (unsigned)(ty >> 32));
 }
-__device__ __forceinline__ void expand_record(const uint4& cx, const uint2& cy, uint4& xa, uint4& xc, uint4& yv) {
-    unsigned long long t = (unsigned long long)cy.x | ((unsigned long long)cy.y << 32);
-    const unsigned code = ((cy.x >> 14) & 3u) | (((cy.x >> 30) & 3u) << 2) | (((cy.y >> 14) & 3u) << 4) | (((cy.y >> 30) & 3u) << 6);
-    t &= 0x3fff3fff3fff3fffull;
-    const int u0 = (int)(code & 7u) - 1, ey = (int)(code >> 3) - 3;
+__device__ __forceinline__ void expand_record(const uint4& rec, uint4& xa, uint4& xc, uint4& yv) {
+    const unsigned cxd = ((rec.x >> 14) & 3u) | (((rec.x >> 30) & 3u) << 2) | (((rec.y >> 14) & 3u) << 4);
+    const unsigned cyd = ((rec.z >> 14) & 3u) | (((rec.z >> 30) & 3u) << 2);
+    const unsigned long long tx = ((unsigned long long)rec.x | ((unsigned long long)rec.y << 32)) & 0x3fff3fff3fff3fffull;
+    const unsigned long long ty = ((unsigned long long)rec.z | ((unsigned long long)rec.w << 32)) & 0x3fff3fff3fff3fffull;
+    // x: the taps start at cell ex = 4 u0 + r: groups u0 and u0 + 1 of the sub-tile's four groups of four cells
+    const int u0 = (int)(cxd >> 2) - 1, shx = 16 * (int)(cxd & 3u), ey = (int)cyd - 3;
+    const unsigned long long ga = tx << shx, gb = shx ? tx >> (64 - shx) : 0ull;
+    const unsigned a0 = (unsigned)ga, a1 = (unsigned)(ga >> 32), b0 = (unsigned)gb, b1 = (unsigned)(gb >> 32);
     auto pick = [&](int j, unsigned first, unsigned second) { return u0 == j ? first : (u0 == j - 1 ? second : 0u); };
-    xa = make_uint4(pick(0, cx.x, cx.z), pick(0, cx.y, cx.w), pick(1, cx.x, cx.z), pick(1, cx.y, cx.w));
-    xc = make_uint4(pick(2, cx.x, cx.z), pick(2, cx.y, cx.w), pick(3, cx.x, cx.z), pick(3, cx.y, cx.w));
+    xa = make_uint4(pick(0, a0, b0), pick(0, a1, b1), pick(1, a0, b0), pick(1, a1, b1));
+    xc = make_uint4(pick(2, a0, b0), pick(2, a1, b1), pick(3, a0, b0), pick(3, a1, b1));
     unsigned long long lo, hi;
     if (ey >= 0) {
         const int sh = 16 * ey;
-        lo = sh < 64 ? t << sh : 0ull;
-        hi = sh == 0 ? 0ull : (sh < 64 ? t >> (64 - sh) : t << (sh - 64));
+        lo = sh < 64 ? ty << sh : 0ull;
+        hi = sh == 0 ? 0ull : (sh < 64 ? ty >> (64 - sh) : ty << (sh - 64));
     } else {
-        lo = t >> (16 * -ey);
+        lo = ty >> (16 * -ey);
         hi = 0ull;
     }
     yv = make_uint4((unsigned)lo, (unsigned)(lo >> 32), (unsigned)hi, (unsigned)(hi >> 32));
@@ -278,29 +286,25 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
             const size_t st0 = (size_t)wbase;
             alignas(16) __half2 bvA[NPG], bvB[NPG];
             if constexpr (MH == 2) {
-                // compact records (28 bytes per column, compact_record above), expanded right before the stage is written
-                auto ldx = [&](size_t st) { return __ldg(&wrec[(st * 3 + 0) * 32 + lane]); };
-                auto ldy = [&](size_t st) { return __ldg(reinterpret_cast<const uint2*>(&wrec[(st * 3 + 1) * 32]) + lane); };
-                uint4 cxA = ldx(st0);
-                uint2 cyA = ldy(st0);
+                // compact records (20 bytes per column, compact_record above), expanded right before the stage is written
+                auto ldr = [&](size_t st) { return __ldg(&wrec[st * 32 + lane]); };       // records of consecutive steps are contiguous
+                uint4 recA = ldr(st0);
                 gather(__ldg(&wsamp[st0 * 32 + lane]), bvA);
                 unsigned samp_next = ns > 1 ? __ldg(&wsamp[(st0 + 1) * 32 + lane]) : 0u;
 #pragma unroll 1
                 for (int sidx = 0; sidx < ns; ++sidx) {
                     const size_t st = st0 + sidx + 1;
                     const bool more = sidx + 1 < ns;
-                    uint4 cxB = cxA;
-                    uint2 cyB = cyA;
+                    uint4 recB = recA;
                     if (more) {
                         gather(samp_next, bvB);
-                        cxB = ldx(st);
-                        cyB = ldy(st);
+                        recB = ldr(st);
                         if (sidx + 2 < ns) samp_next = __ldg(&wsamp[(st + 1) * 32 + lane]);
                     }
                     uint4 xa, xc, yv;
-                    expand_record(cxA, cyA, xa, xc, yv);
+                    expand_record(recA, xa, xc, yv);
                     issue_step(xa, xc, yv, bvA, true);
-                    cxA = cxB; cyA = cyB;
+                    recA = recB;
 #pragma unroll
                     for (int p = 0; p < NPG; ++p) bvA[p] = bvB[p];
                 }
@@ -398,7 +402,6 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                 // and [-m+1, m-1] when nu is an integer.
                 uint4 xa, xc, yv;
                 uint4 cxr = make_uint4(0u, 0u, 0u, 0u);
-                uint2 cyr = make_uint2(0u, 0u);
                 {
                     float flx, frx, fly, fry;
                     nu_split((float)k, cxh, cxl, flx, frx);
@@ -427,14 +430,13 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                     xc = make_uint4(wx[4], wx[5], wx[6], wx[7]);
                     yv = make_uint4(wy[0], wy[1], wy[2], wy[3]);
                     if constexpr (MODE == GM_FILL && MH == 2)      // first tap (a = lo) sits at cell position lo - ax0, row lo - ay0
-                        compact_record(wx, wy, (int)(lo - ax0), (int)(lo - ay0), cxr, cyr);
+                        cxr = compact_record(wx, wy, (int)(lo - ax0), (int)(lo - ay0));
                 }
                 if constexpr (MODE == GM_FILL) {
                     // record of this step and column: [step][xa | xc | yv][lane] and the sample offset
                     const size_t st = (size_t)wbase + istep;
                     if constexpr (MH == 2) {
-                        wrec[(st * 3 + 0) * 32 + lane] = cxr;
-                        reinterpret_cast<uint2*>(&wrec[(st * 3 + 1) * 32])[lane] = cyr;
+                        wrec[st * 32 + lane] = cxr;
                     } else {
                         wrec[(st * 3 + 0) * 32 + lane] = xa;
                         wrec[(st * 3 + 1) * 32 + lane] = xc;
