@@ -68,8 +68,8 @@ __device__ __forceinline__ void nu_split(float k, float c_hi, float c_lo, float&
 //       position falls outside the sub-tile are stored as zero and dropped);
 //   (z, w): the four y taps, rows ey .. ey + 3 of the sub-tile's eight (ey in -3..7);
 //   ex + 4 (5 bits) and ey + 3 (4 bits) ride in bits 14 and 15 of the taps, which are zero for weights <= 1.
-// expand_record() rebuilds exactly the (xa, xc, yv) registers the direct kernel computes: every position outside the four
-// cells / four rows carries a zero weight there (the open box |l - nu| < 2 spans four cells).
+// The replay rebuilds exactly the A stage the direct kernel writes: every position outside the four cells / four rows
+// carries a zero weight there (the open box |l - nu| < 2 spans four cells).
 __device__ __forceinline__ uint4 compact_record(const unsigned (&wx)[8], const unsigned (&wy)[4], int e0x, int e0y) {
     const int ex = max(-4, min(16, e0x));
     unsigned long long tx = 0ull;
@@ -99,28 +99,21 @@ __device__ __forceinline__ uint4 compact_record(const unsigned (&wx)[8], const u
     for (int i = 0; i < 2; ++i) ty |= (unsigned long long)((cyd >> (2 * i)) & 3u) << (16 * i + 14);
     return make_uint4((unsigned)tx, (unsigned)(tx >> 32), (unsigned)ty, (unsigned)(ty >> 32));
 }
-__device__ __forceinline__ void expand_record(const uint4& rec, uint4& xa, uint4& xc, uint4& yv) {
+// What the replay needs of a record (issue_step_taps below): the x weights of the 16 cell positions, the four y taps as
+// they are and the row of the first one.
+__device__ __forceinline__ void expand_record_x(const uint4& rec, uint4& xa, uint4& xc, unsigned& ty01, unsigned& ty23, int& ey) {
     const unsigned cxd = ((rec.x >> 14) & 3u) | (((rec.x >> 30) & 3u) << 2) | (((rec.y >> 14) & 3u) << 4);
     const unsigned cyd = ((rec.z >> 14) & 3u) | (((rec.z >> 30) & 3u) << 2);
     const unsigned long long tx = ((unsigned long long)rec.x | ((unsigned long long)rec.y << 32)) & 0x3fff3fff3fff3fffull;
-    const unsigned long long ty = ((unsigned long long)rec.z | ((unsigned long long)rec.w << 32)) & 0x3fff3fff3fff3fffull;
-    // x: the taps start at cell ex = 4 u0 + r: groups u0 and u0 + 1 of the sub-tile's four groups of four cells
-    const int u0 = (int)(cxd >> 2) - 1, shx = 16 * (int)(cxd & 3u), ey = (int)cyd - 3;
+    const int u0 = (int)(cxd >> 2) - 1, shx = 16 * (int)(cxd & 3u);
     const unsigned long long ga = tx << shx, gb = shx ? tx >> (64 - shx) : 0ull;
     const unsigned a0 = (unsigned)ga, a1 = (unsigned)(ga >> 32), b0 = (unsigned)gb, b1 = (unsigned)(gb >> 32);
     auto pick = [&](int j, unsigned first, unsigned second) { return u0 == j ? first : (u0 == j - 1 ? second : 0u); };
     xa = make_uint4(pick(0, a0, b0), pick(0, a1, b1), pick(1, a0, b0), pick(1, a1, b1));
     xc = make_uint4(pick(2, a0, b0), pick(2, a1, b1), pick(3, a0, b0), pick(3, a1, b1));
-    unsigned long long lo, hi;
-    if (ey >= 0) {
-        const int sh = 16 * ey;
-        lo = sh < 64 ? ty << sh : 0ull;
-        hi = sh == 0 ? 0ull : (sh < 64 ? ty >> (64 - sh) : ty << (sh - 64));
-    } else {
-        lo = ty >> (16 * -ey);
-        hi = 0ull;
-    }
-    yv = make_uint4((unsigned)lo, (unsigned)(lo >> 32), (unsigned)hi, (unsigned)(hi >> 32));
+    ty01 = rec.z & 0x3fff3fffu;
+    ty23 = rec.w & 0x3fff3fffu;
+    ey = (int)cyd - 3;
 }
 
 // dynamic shared memory carve-up: per-warp A/B stages and scratch
@@ -264,6 +257,56 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
         __syncwarp();
     };
 
+    // the same stage from a compact record (half-width 2, cached replay): only the four tap rows ey .. ey + 3 are multiplied
+    // out, the four other rows (ey + 4 .. ey + 7 modulo 8) are stored as zeros; a tap row that falls outside the sub-tile
+    // lands, with a zero weight, on a row that is zero anyway.  No branch, half the products; bit-identical to issue_step.
+    auto issue_step_taps = [&](const uint4& rec, const __half2* bv) {
+        uint4 xa, xc;
+        unsigned ty01, ty23;
+        int ey;
+        expand_record_x(rec, xa, xc, ty01, ty23, ey);
+        if (nstep > 0) mbar_wait(bar, (nstep - 1) & 1);
+        {
+            unsigned char* brow = Bw + (cl >> 3) * L::B_LBO + (cl & 7) * 16;
+            const uint4* vv = reinterpret_cast<const uint4*>(bv);
+#pragma unroll
+            for (int q = 0; q < GW; ++q) *reinterpret_cast<uint4*>(brow + q * 128) = vv[q];
+        }
+        {
+            unsigned char* arow = Aw + (cl >> 3) * A_LBO + (cl & 7) * 16;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int r = ey + i;
+                unsigned char* dst = arow + ((r & 7) << 8);
+                if (i < 4) {
+                    const unsigned w = i < 2 ? ty01 : ty23;
+                    unsigned y2 = (i & 1) ? __byte_perm(w, 0, 0x3232) : __byte_perm(w, 0, 0x1010);
+                    y2 = (unsigned)r < 8u ? y2 : 0u;
+                    auto mul = [&](unsigned x) {
+                        const __half2 pr = __hmul2(*reinterpret_cast<const __half2*>(&x), *reinterpret_cast<const __half2*>(&y2));
+                        return *reinterpret_cast<const unsigned*>(&pr);
+                    };
+                    *reinterpret_cast<uint4*>(dst) = make_uint4(mul(xa.x), mul(xa.y), mul(xa.z), mul(xa.w));
+                    *reinterpret_cast<uint4*>(dst + 128) = make_uint4(mul(xc.x), mul(xc.y), mul(xc.z), mul(xc.w));
+                } else {
+                    *reinterpret_cast<uint4*>(dst) = make_uint4(0u, 0u, 0u, 0u);
+                    *reinterpret_cast<uint4*>(dst + 128) = make_uint4(0u, 0u, 0u, 0u);
+                }
+            }
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            umma_f16(acc, adesc0, bdesc0, IDESC, istep > 0 ? 1u : 0u);
+            umma_f16(acc, adesc1, bdesc1, IDESC, 1u);
+            umma_commit(bar);
+        }
+        ++nstep;
+        ++istep;
+        __syncwarp();
+    };
+
     // persistent CTA: items claimed from a counter, heaviest regions first (TMEM allocation, barrier set-up and
     // launch cost once per CTA, not per item)
     int* const ctr = counter + (MODE * 16 + blockIdx.y * gridDim.z + blockIdx.z);
@@ -286,7 +329,7 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
             const size_t st0 = (size_t)wbase;
             alignas(16) __half2 bvA[NPG], bvB[NPG];
             if constexpr (MH == 2) {
-                // compact records (20 bytes per column, compact_record above), expanded right before the stage is written
+                // compact records (20 bytes per column, compact_record above), expanded as the stage is written
                 auto ldr = [&](size_t st) { return __ldg(&wrec[st * 32 + lane]); };       // records of consecutive steps are contiguous
                 uint4 recA = ldr(st0);
                 gather(__ldg(&wsamp[st0 * 32 + lane]), bvA);
@@ -301,9 +344,7 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                         recB = ldr(st);
                         if (sidx + 2 < ns) samp_next = __ldg(&wsamp[(st + 1) * 32 + lane]);
                     }
-                    uint4 xa, xc, yv;
-                    expand_record(recA, xa, xc, yv);
-                    issue_step(xa, xc, yv, bvA, true);
+                    issue_step_taps(recA, bvA);
                     recA = recB;
 #pragma unroll
                     for (int p = 0; p < NPG; ++p) bvA[p] = bvB[p];
