@@ -310,44 +310,92 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
     // persistent CTA: items claimed from a counter, heaviest regions first (TMEM allocation, barrier set-up and
     // launch cost once per CTA, not per item)
     int* const ctr = counter + (MODE * 16 + blockIdx.y * gridDim.z + blockIdx.z);
+    // Replay of the compact records: a warp runs only ~4 steps per item, so the chain claim -> item -> step offset -> first
+    // record -> gather (dependent global-load latencies) weighs on every item.  The NEXT item is claimed at the top of the
+    // current one (the atomic's result is not touched until the steps are done), and its header and first record are loaded
+    // under the current item's epilogue.
+    constexpr bool AHEAD = MODE == GM_CACHED && MH == 2;
+    auto ldr = [&](size_t st) { return __ldg(&wrec[st * 32 + lane]); };       // compact records of consecutive steps are contiguous
+    int it_n = 0, ns_n = 0, wbase_n = 0, claimed = 0;
+    int4 item_n = make_int4(0, 0, 0, 0);
+    uint4 rec_n = make_uint4(0u, 0u, 0u, 0u);
+    unsigned samp_n = 0u, samp2_n = 0u;
+    auto load_header = [&]() {
+        ns_n = 0;
+        if (it_n < nitems) {
+            item_n = items[it_n];
+            ns_n = wcount[it_n * NSUB + sub];
+            wbase_n = woff[it_n * NSUB + sub];
+        }
+    };
+    auto load_first = [&]() {
+        if (ns_n > 0) {
+            rec_n = ldr((size_t)wbase_n);
+            samp_n = __ldg(&wsamp[(size_t)wbase_n * 32 + lane]);
+            samp2_n = ns_n > 1 ? __ldg(&wsamp[((size_t)wbase_n + 1) * 32 + lane]) : 0u;
+        }
+    };
+    if constexpr (AHEAD) {
+        if (tid == 0) misc[13] = (uint32_t)atomicAdd(ctr, 1);
+        __syncthreads();
+        it_n = (int)misc[13];
+        load_header();
+        load_first();
+        __syncthreads();                 // everyone has read misc[13] before thread 0 writes the next claim
+    }
 #pragma unroll 1
     for (;;) {
-    if (tid == 0) misc[12] = (uint32_t)atomicAdd(ctr, 1);
-    __syncthreads();
-    const int it = (int)misc[12];
-    if (it >= nitems) break;
-    const int4 item = items[it];
+    int it;
+    if constexpr (AHEAD) {
+        it = it_n;
+        if (it >= nitems) break;
+        if (tid == 0) claimed = atomicAdd(ctr, 1);
+    } else {
+        if (tid == 0) misc[12] = (uint32_t)atomicAdd(ctr, 1);
+        __syncthreads();
+        it = (int)misc[12];
+        if (it >= nitems) break;
+    }
+    const int4 item = AHEAD ? item_n : items[it];
     const int tile = item.x, split = item.y & 0xffff, nsplit = item.y >> 16;
     const int TX0 = (tile % tiles) * TS, TY0 = (tile / tiles) * TS;
     istep = 0;
-    const int wbase = (MODE == GM_FILL || MODE == GM_CACHED) ? woff[it * NSUB + sub] : 0;
+    const int wbase = AHEAD ? wbase_n : ((MODE == GM_FILL || MODE == GM_CACHED) ? woff[it * NSUB + sub] : 0);
     if constexpr (MODE == GM_CACHED) {
-        // replay, software-pipelined two deep: the gather of step s + 1 and the sample offsets of step s + 2 are in
-        // flight while step s is staged (a step is otherwise two dependent global-load latencies with nothing to hide them)
-        const int ns = wcount[it * NSUB + sub];
+        // replay, software-pipelined: the gathers of the next step(s) and the sample offsets of the one after are in flight
+        // while step s is staged (a step is otherwise two dependent global-load latencies with nothing to hide them)
+        const int ns = AHEAD ? ns_n : wcount[it * NSUB + sub];
         if (ns > 0) {
             const size_t st0 = (size_t)wbase;
             alignas(16) __half2 bvA[NPG], bvB[NPG];
             if constexpr (MH == 2) {
                 // compact records (20 bytes per column, compact_record above), expanded as the stage is written
-                auto ldr = [&](size_t st) { return __ldg(&wrec[st * 32 + lane]); };       // records of consecutive steps are contiguous
-                uint4 recA = ldr(st0);
-                gather(__ldg(&wsamp[st0 * 32 + lane]), bvA);
-                unsigned samp_next = ns > 1 ? __ldg(&wsamp[(st0 + 1) * 32 + lane]) : 0u;
+                if constexpr (!AHEAD) {
+                    rec_n = ldr(st0);
+                    samp_n = __ldg(&wsamp[st0 * 32 + lane]);
+                    samp2_n = ns > 1 ? __ldg(&wsamp[(st0 + 1) * 32 + lane]) : 0u;
+                }
+                // three deep: the gathers of steps s + 1 and s + 2 are in flight while step s is staged
+                alignas(16) __half2 bvC[NPG];
+                uint4 recA = rec_n, recB = rec_n, recC = rec_n;
+                gather(samp_n, bvA);
+                unsigned samp_next = 0u;
+                if (ns > 1) {
+                    gather(samp2_n, bvB);
+                    recB = ldr(st0 + 1);
+                    if (ns > 2) samp_next = __ldg(&wsamp[(st0 + 2) * 32 + lane]);
+                }
 #pragma unroll 1
                 for (int sidx = 0; sidx < ns; ++sidx) {
-                    const size_t st = st0 + sidx + 1;
-                    const bool more = sidx + 1 < ns;
-                    uint4 recB = recA;
-                    if (more) {
-                        gather(samp_next, bvB);
-                        recB = ldr(st);
-                        if (sidx + 2 < ns) samp_next = __ldg(&wsamp[(st + 1) * 32 + lane]);
+                    if (sidx + 2 < ns) {
+                        gather(samp_next, bvC);
+                        recC = ldr(st0 + sidx + 2);
+                        if (sidx + 3 < ns) samp_next = __ldg(&wsamp[(st0 + sidx + 3) * 32 + lane]);
                     }
                     issue_step_taps(recA, bvA);
-                    recA = recB;
+                    recA = recB; recB = recC;
 #pragma unroll
-                    for (int p = 0; p < NPG; ++p) bvA[p] = bvB[p];
+                    for (int p = 0; p < NPG; ++p) { bvA[p] = bvB[p]; bvB[p] = bvC[p]; }
                 }
             } else {
             uint4 xaA = __ldg(&wrec[(st0 * 3 + 0) * 32 + lane]), xcA = __ldg(&wrec[(st0 * 3 + 1) * 32 + lane]);
@@ -499,9 +547,16 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
     // ---- this warp's MMAs complete (commits complete in order: wait for the last one)
     if (istep > 0) mbar_wait(bar, (nstep - 1) & 1);
     if (lane == 0) misc[1 + warp] = istep;
+    if constexpr (AHEAD) {
+        if (tid == 0) misc[13] = (uint32_t)claimed;
+    }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    if constexpr (AHEAD) {               // header of the next item: in flight during the first half of the epilogue
+        it_n = (int)misc[13];
+        load_header();
+    }
 
     // ---- epilogue: TMEM -> registers -> grid (or partial tile).  A warp can read only its own lane
     // quarter of TMEM: warp w takes rows 32 (w & 3) .. +31 of CW / (CW / 4) of the CTA's sub-tiles
@@ -512,6 +567,9 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
         const size_t pstride = (size_t)M * M;
 #pragma unroll 1
         for (int bb = 0; bb < PER; ++bb) {
+            if constexpr (AHEAD) {
+                if (bb == PER / 2) load_first();                // first record of the next item: in flight during the second half
+            }
             const int b = hsel * PER + bb;                      // accumulator inside the CTA
             const int gb = (int)blockIdx.z * CW + b;            // sub-tile inside the region
             uint32_t r[NN];
