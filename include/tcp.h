@@ -111,12 +111,14 @@ enum { TCP_ST_TRIG = 0, TCP_ST_NORMALIZE = 1, TCP_ST_ROWS = 2, TCP_ST_GRID = 3, 
 tcp_ctx* tcp_create(int n, int nproj, int nz_chunk, float center, int dtype, int filter);
 
 /* As tcp_create, with the gridding kernel as a code m (taps per axis = 2 x half-width):
- *   0            the default, 3;
+ *   0            the default (what tcp_create and tcp_create_det's m = 0 use): 16 + 2, see below;
  *   3, 4         Gaussian phi(t) = exp(-alpha t^2) of that half-width (3 meets the 2e-3 gridding-vs-exact gate with 2.7x margin);
  *   16 + 2, 16 + 3   TCP_KERNEL_KB + half-width: Kaiser-Bessel window phi(t) = I0(beta sqrt(1 - (t/m)^2)) / I0(beta),
  *                beta = pi sqrt(2.25 m^2 - 0.8), deapodised by its exact transform (the "accuracy controls" of PAPER.md:173,
  *                DESIGN.md reading Q21).  Half-width 2 reaches 3.9e-4 of the exact sum on the C1 phantom with 16 taps
- *                per sample where the Gaussian needs 36 for 7.4e-4.  Tile and tensor-core griddings only. */
+ *                per sample where the Gaussian needs 36 for 7.4e-4: more accurate and less work, hence the default
+ *                (the oracle takes the same code).  Tile and tensor-core griddings only: TCP_GRID_GATHER and
+ *                TCP_GRID_SCATTER_ATOMIC need a Gaussian context. */
 enum { TCP_KERNEL_GAUSS = 0, TCP_KERNEL_KB = 16 };
 tcp_ctx* tcp_create_ex(int n, int nproj, int nz_chunk, float center, int dtype, int filter, int m);
 

@@ -231,7 +231,7 @@ const char* tcp_last_error(void) { return g_err; }
 // n: the power of two the transforms run on; ndet <= n: the caller's detector width (tcp_create_det), embedded at pad_l
 static tcp_ctx* create_impl(int n, int ndet, int pad_l, int nproj, int nz_chunk, float center, int dtype, int filter, int m) {
     g_err[0] = 0;
-    if (m == 0) m = 3;
+    if (m == 0) m = TCP_KERNEL_KB + 2;    // the default: Kaiser-Bessel, half-width 2 (tcp.h)
     const int kernel = m >> 4;            // kernel code: half-width (Gaussian) or 16 + half-width (Kaiser-Bessel)
     m &= 15;
     if (kernel > 1 || (kernel == 1 && m != 2 && m != 3)) { set_error(TCP_EINVAL, "kernel code %d: Kaiser-Bessel half-width must be 2 or 3", m | (kernel << 4)); return nullptr; }

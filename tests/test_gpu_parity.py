@@ -477,7 +477,7 @@ def test_pipeline_host_matches_direct():
         d = r.recon(*_to_dev(np.ascontiguousarray(raw[:, sl]), flat[sl], dark[sl], theta))
         torch.cuda.synchronize()
         assert np.array_equal(out_h[sl], d.cpu().numpy())
-    ref = orc.recon(np.ascontiguousarray(raw[:, 20:22]), flat[20:22], dark[20:22], theta, w.center, w.filter, 3, "grid")
+    ref = orc.recon(np.ascontiguousarray(raw[:, 20:22]), flat[20:22], dark[20:22], theta, w.center, w.filter, orc.KB + 2, "grid")   # default kernel
     for z in range(2):
         check(out_h[20 + z], ref[z], "f32")
     r.close()
