@@ -708,10 +708,11 @@ int grid_mma_cache_setup(tcp_ctx* c) {
     const size_t cap = (size_t)std::min(steps, 2.0e9 / 1.0);
     size_t freeb = 0, totalb = 0;
     cudaMemGetInfo(&freeb, &totalb);
-    const size_t need = cap * (3 * 32 * sizeof(uint4) + 32 * sizeof(unsigned)) + 2 * nent * sizeof(int);
+    const size_t rec = (c->m == 2 ? 1 : 3) * 32 * sizeof(uint4);        // bytes of weight records per step: compact (half-width 2) or 52 per column
+    const size_t need = cap * (rec + 32 * sizeof(unsigned)) + 2 * nent * sizeof(int);
     if (need > freeb / 4) return TCP_OK;                                  // leave the memory to the caller: direct kernel
     if (cudaMalloc((void**)&c->w_count, nent * sizeof(int)) != cudaSuccess || cudaMalloc((void**)&c->w_off, nent * sizeof(int)) != cudaSuccess ||
-        cudaMalloc((void**)&c->w_rec, cap * 3 * 32 * sizeof(uint4)) != cudaSuccess || cudaMalloc((void**)&c->w_samp, cap * 32 * sizeof(unsigned)) != cudaSuccess) {
+        cudaMalloc((void**)&c->w_rec, cap * rec) != cudaSuccess || cudaMalloc((void**)&c->w_samp, cap * 32 * sizeof(unsigned)) != cudaSuccess) {
         cudaGetLastError();
         cudaFree(c->w_count); cudaFree(c->w_off); cudaFree(c->w_rec); cudaFree(c->w_samp);
         c->w_count = c->w_off = nullptr; c->w_rec = nullptr; c->w_samp = nullptr;
