@@ -385,17 +385,22 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                     recB = ldr(st0 + 1);
                     if (ns > 2) samp_next = __ldg(&wsamp[(st0 + 2) * 32 + lane]);
                 }
-#pragma unroll 1
-                for (int sidx = 0; sidx < ns; ++sidx) {
-                    if (sidx + 2 < ns) {
-                        gather(samp_next, bvC);
-                        recC = ldr(st0 + sidx + 2);
-                        if (sidx + 3 < ns) samp_next = __ldg(&wsamp[(st0 + sidx + 3) * 32 + lane]);
+                // the three buffer sets take turns (loop unrolled by three: no register rotation between steps)
+                auto step = [&](int i, const uint4& rcur, const __half2* bcur, uint4& rnew, __half2* bnew) {
+                    if (i + 2 < ns) {
+                        gather(samp_next, bnew);
+                        rnew = ldr(st0 + i + 2);
+                        if (i + 3 < ns) samp_next = __ldg(&wsamp[(st0 + i + 3) * 32 + lane]);
                     }
-                    issue_step_taps(recA, bvA);
-                    recA = recB; recB = recC;
-#pragma unroll
-                    for (int p = 0; p < NPG; ++p) { bvA[p] = bvB[p]; bvB[p] = bvC[p]; }
+                    issue_step_taps(rcur, bcur);
+                };
+#pragma unroll 1
+                for (int sidx = 0; sidx < ns; sidx += 3) {
+                    step(sidx, recA, bvA, recC, bvC);
+                    if (sidx + 1 >= ns) break;
+                    step(sidx + 1, recB, bvB, recA, bvA);
+                    if (sidx + 2 >= ns) break;
+                    step(sidx + 2, recC, bvC, recB, bvB);
                 }
             } else {
             uint4 xaA = __ldg(&wrec[(st0 * 3 + 0) * 32 + lane]), xcA = __ldg(&wrec[(st0 * 3 + 1) * 32 + lane]);
@@ -587,6 +592,8 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
                 const size_t cell = strip_log2 >= 0 ? ((((size_t)(gc >> strip_log2) * M + gr) << strip_log2) + (gc & ((1 << strip_log2) - 1)))
                                                     : (size_t)gr * M + gc;
                 __half2* dst = grid + (size_t)(pg * NPG) * pstride + cell;
+                // (keep the test per plane: a single uniform branch around sixteen back-to-back stores measures 29 % SLOWER -- the
+                // kernel gains from the stores being spread out between the address arithmetic)
 #pragma unroll
                 for (int p = 0; p < NPG; ++p)
                     if (pg * NPG + p < npair) dst[p * pstride] = f2h2_sat(make_float2(__uint_as_float(r[2 * p]), __uint_as_float(r[2 * p + 1])));
