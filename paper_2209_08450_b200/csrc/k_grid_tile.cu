@@ -352,7 +352,7 @@ int grid_tile_setup(tcp_ctx* c) {
     const int M = c->M, n = c->n, tiles = M / TS, MH = c->m;
     const double h = 0.5 * TS + MH, rd = h * 1.4142135623730951;
     const double chord_avg = 0.9 * (TS + 2 * MH);
-    // cap: a fraction of one CTA slot's fair share (148 SMs x 2 CTAs)
+    // cap: a fraction of one CTA slot's fair share (148 SMs x 2 CTAs), see below
     double total = 0;
     std::vector<double> est((size_t)tiles * tiles);
     for (int ty = 0; ty < tiles; ++ty)
@@ -372,7 +372,7 @@ int grid_tile_setup(tcp_ctx* c) {
     // the floor keeps the per-item fixed cost small against its work; a grid with fewer tiles than CTA slots (M <= 512) is
     // bound by the latency of one CTA's walk instead, and splits four times finer (C1: gridding 0.142 -> 0.054 ms)
     const double floor_ = tiles * tiles < 2 * 148 ? 512.0 : 2048.0;
-    const double cap = std::max(floor_, total / (148.0 * 2.0) / 6.0);
+    const double cap = std::max(floor_, total / (148.0 * 2.0) / 3.0);      // a third of a slot's fair share (a sixth measured 9 % slower at C3: more partial tiles to write and sum)
     struct It { double w; int4 v; };
     std::vector<It> its;
     std::vector<int4> red;
