@@ -94,18 +94,27 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
     uint16_t* RB = reinterpret_cast<uint16_t*>(FD + 8 * NT);            // [2][n]
     uint64_t* rbar = reinterpret_cast<uint64_t*>(RB + 2 * n);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, c = lane & 3;
-    // persistent CTAs: a CTA stays with ONE slice pair (blockIdx % npair), so everything that depends on the thread and the
-    // pair only -- butterfly fragments, twiddles, filter, phase and flat/dark tables -- is set up once
+    // persistent CTAs: the npair x nproj units (pair-major) are cut into gridDim.x contiguous runs of equal length, so a CTA
+    // works through consecutive projections of ONE slice pair (two when its run crosses a pair boundary): what depends on the
+    // thread and the pair only -- the flat/dark table, in try mode the phase table -- is set up when the pair changes, the
+    // butterfly fragments, twiddles and the filter table once.  (A fixed pair per CTA left 8 of the 296 CTA slots idle.)
     const int npair_grid = npair_try;                                  // slice pairs of the call
-    const int pair = blockIdx.x % npair_grid, jstart = blockIdx.x / npair_grid, jstep = gridDim.x / npair_grid;
-    const int zA = try_mode ? 0 : 2 * pair, zB = try_mode ? nz : 2 * pair + 1;
-    const bool hasB = zB < nz;
-    const int zBs = hasB ? zB : zA;
-    if (try_mode) ptab += (size_t)pair * N;
-    auto fetch_raw = [&](int j) {                                       // thread 0 only
+    const long long nunit = (long long)npair_grid * nproj;
+    const int u0 = (int)((long long)blockIdx.x * nunit / gridDim.x), u1 = (int)(((long long)blockIdx.x + 1) * nunit / gridDim.x);
+    auto slices_of = [&](int p, int& a, int& bs, bool& hb) {
+        a = try_mode ? 0 : 2 * p;
+        const int b = try_mode ? nz : 2 * p + 1;
+        hb = b < nz;
+        bs = hb ? b : a;
+    };
+    auto fetch_raw = [&](int u) {                                       // thread 0 only
+        const int p = u / nproj, j = u - p * nproj;
+        int a, bs;
+        bool hb;
+        slices_of(p, a, bs, hb);
         mbar_expect_tx(rbar, 2 * n * 2);
-        bulk_g2s(RB, raw + ((size_t)j * nz + zA) * n, n * 2, rbar);
-        bulk_g2s(RB + n, raw + ((size_t)j * nz + zBs) * n, n * 2, rbar);
+        bulk_g2s(RB, raw + ((size_t)j * nz + a) * n, n * 2, rbar);
+        bulk_g2s(RB + n, raw + ((size_t)j * nz + bs) * n, n * 2, rbar);
     };
     if constexpr (RAW) {
         if (tid == 0) {
@@ -113,19 +122,27 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
             fence_mbar_init();
         }
         __syncthreads();
-        if (tid == 0 && jstart < nproj) fetch_raw(jstart);
+        if (tid == 0 && u0 < u1) fetch_raw(u0);
     }
     uint32_t rphase = 0;
-    {
-        const int kbase = pass3_index<false>(0, 0, warp, g, c);
+    const int kbase = pass3_index<false>(0, 0, warp, g, c);
 #pragma unroll
-        for (int sl = 0; sl < 8; ++sl) {
-            const int k0 = kbase + 2048 * (sl & 1) + 64 * (sl >> 1);
-            const float2 h = __ldg(reinterpret_cast<const float2*>(hfilt + k0));
-            HT[sl * NT + tid] = make_float2(h.x * kRowScale, h.y * kRowScale);
-            const float4 p = __ldg(reinterpret_cast<const float4*>(ptab + k0));
-            const float s = 1.f / kRowScale;
-            PT[sl * NT + tid] = make_float4(p.x * s, p.y * s, p.z * s, p.w * s);
+    for (int sl = 0; sl < 8; ++sl) {
+        const int k0 = kbase + 2048 * (sl & 1) + 64 * (sl >> 1);
+        const float2 h = __ldg(reinterpret_cast<const float2*>(hfilt + k0));
+        HT[sl * NT + tid] = make_float2(h.x * kRowScale, h.y * kRowScale);
+    }
+    // the per-thread tables are written and read by the same thread only: no barrier around a change of pair
+    auto setup_pair = [&](int p, int zA, int zBs, bool first) {
+        if (first || try_mode) {
+            const float2* pt = try_mode ? ptab + (size_t)p * N : ptab;
+#pragma unroll
+            for (int sl = 0; sl < 8; ++sl) {
+                const int k0 = kbase + 2048 * (sl & 1) + 64 * (sl >> 1);
+                const float4 v = __ldg(reinterpret_cast<const float4*>(pt + k0));
+                const float s = 1.f / kRowScale;
+                PT[sl * NT + tid] = make_float4(v.x * s, v.y * s, v.z * s, v.w * s);
+            }
         }
         if constexpr (RAW) {
 #pragma unroll
@@ -134,7 +151,7 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
                 FD[(4 + q) * NT + tid] = __ldg(reinterpret_cast<const float4*>(fdtab + (size_t)zBs * n + tid * 8) + q);
             }
         }
-    }
+    };
     AFrag An, Al;
     load_afrag(An, atab, AV_NAT, lane);
     load_afrag(Al, atab, AV_LO, lane);
@@ -144,10 +161,18 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
     Offs<1> O;
     make_offs<1>(O, warp, g, c);
     auto no_in = [](int) { return 0u; };
-    const int kbase = pass3_index<false>(0, 0, warp, g, c);
     auto slot_of = [&](int k0) { return 2 * (((k0 - kbase) >> 6) & 3) + ((k0 - kbase) >> 11); };   // folds to a constant per call site
+    int pair = -1, zA = 0, zBs = 0;
+    bool hasB = false;
 #pragma unroll 1
-    for (int j = jstart; j < nproj; j += jstep) {
+    for (int u = u0; u < u1; ++u) {
+    const int up = u / nproj, j = u - up * nproj;
+    if (up != pair) {
+        const bool first = pair < 0;
+        pair = up;
+        slices_of(pair, zA, zBs, hasB);
+        setup_pair(pair, zA, zBs, first);
+    }
     const float wj = wq ? __ldg(&wq[j]) : 1.f;
 
     // ---- stage the two rows as half2 (pA, pB): 8 detector pixels per thread, 128-bit loads
@@ -190,9 +215,9 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
     }
     __syncthreads();
     if constexpr (RAW) {                  // every thread has read the raw rows: the next projection's may land
-        if (tid == 0 && j + jstep < nproj) {
+        if (tid == 0 && u + 1 < u1) {
             fence_proxy_async();
-            fetch_raw(j + jstep);
+            fetch_raw(u + 1);
         }
     }
     if constexpr (PAD_EDGE) {     // padding samples of the filter stage: the nearest edge of the periodic row
@@ -433,9 +458,9 @@ int launch_rows_mma(const tcp_ctx* c, cudaStream_t st, const uint16_t* raw) {
     auto kern = raw ? (c->pad ? rows_mma_kernel<true, true> : rows_mma_kernel<false, true>)
                     : (c->pad ? rows_mma_kernel<true, false> : rows_mma_kernel<false, false>);
     TCP_SMEM(kern, smem);
-    // gridDim = npair x (CTAs per pair): every CTA keeps one slice pair and strides over the projections
-    const int per_pair = std::max(1, std::min(c->nproj, (2 * c->nsm) / c->npair));
-    kern<<<c->npair * per_pair, NT, smem, st>>>((const __half*)c->sino, (__half2*)c->spec, c->tw, c->mf_atab, c->hfilt,
+    // every CTA takes one contiguous run of the npair x nproj units
+    const int nctas = (int)std::min<long long>((long long)c->npair * c->nproj, 2 * c->nsm);
+    kern<<<nctas, NT, smem, st>>>((const __half*)c->sino, (__half2*)c->spec, c->tw, c->mf_atab, c->hfilt,
                                                 c->try_ptab ? c->try_ptab : c->ptab, c->nproj, c->nz, c->try_ptab ? 1 : 0,
                                                 c->angle_weights ? c->wq : nullptr, raw, c->fdtab, c->npair);
     TCP_CUDA_CHECK(cudaGetLastError());
