@@ -78,7 +78,9 @@ enum { TCP_GRID_GATHER = 0, TCP_GRID_SCATTER_ATOMIC = 1, TCP_GRID_TILE = 2, TCP_
  * (sub-tile, sample), which depend only on theta, n and m, in a device cache built on the first call and
  * rebuilt (on the device, no host synchronisation) whenever the angles passed to tcp_recon change; 0 computes
  * them in every call.  Same results bit for bit.  The cache is keyed by an element-by-element comparison of the call's
- * angles with a device copy of the angles it was built for (no checksum). */
+ * angles with a device copy of the angles it was built for (no checksum), made on the device in every call.  The rebuild
+ * itself (three more kernels) is launched by calls that come after the host has SEEN the verdict (a word of mapped pinned
+ * memory, read without synchronisation): calls with new angles enqueued before that take the uncached kernel. */
 /* TCP_OPT_ANGLE_WEIGHTS (0 default | 1): quadrature weights for angles that are not equally spaced (PAPER.md:61:
  * unlike the log-polar method, the Fourier-based one applies to "non-equally spaced angles", e.g. interlaced
  * scanning).  0: every projection enters with pi/nproj (equispaced half turn).  1: projection j enters with
@@ -191,7 +193,8 @@ int tcp_fft_lines(tcp_ctx* ctx, const void* in_half2, void* out_float2, int batc
 int tcp_measure_rates(double* fp32_tflops, double* hmma_tflops);
 /* Power-of-two factor by which SPECTRUM/GRID/PASS1 are scaled relative to S4's G (1 in fp32). */
 double tcp_scale(const tcp_ctx* ctx);
-/* Total device bytes the context allocated; kernels launched by one tcp_recon. */
+/* Total device bytes the context allocated; kernels one tcp_recon launches in the steady state (a call that may have to
+ * rebuild the weight cache launches three more, see TCP_OPT_WEIGHT_CACHE). */
 size_t tcp_workspace_bytes(const tcp_ctx* ctx);
 int tcp_launches_per_recon(const tcp_ctx* ctx);
 int tcp_set_option(tcp_ctx* ctx, int option, int value);

@@ -620,13 +620,13 @@ __global__ void __launch_bounds__(32 * CW, 16 / CW)
 // angles and raises WS_REBUILD; the count / scan / fill kernels then run (they exit at once otherwise) and WS_USABLE
 // tells the multiply-accumulate kernels which of the two (cached, direct) works.  One block.
 __global__ void __launch_bounds__(1024) wc_decide_kernel(int* __restrict__ state, int enable, const float* __restrict__ theta,
-                                                         float* __restrict__ w_theta, int nproj) {
+                                                         float* __restrict__ w_theta, int nproj, volatile int* hflag) {
     int differ = 0;
     if (enable)
         for (int j = threadIdx.x; j < nproj; j += blockDim.x) differ |= __float_as_uint(theta[j]) != __float_as_uint(w_theta[j]);
     differ = __syncthreads_or(differ);
     if (!enable) {
-        if (threadIdx.x == 0) { state[WS_USABLE] = 0; state[WS_REBUILD] = 0; }
+        if (threadIdx.x == 0) { state[WS_USABLE] = 0; state[WS_REBUILD] = 0; *hflag = 0; }
         return;
     }
     const bool rebuild = !state[WS_USABLE] || differ;
@@ -636,6 +636,7 @@ __global__ void __launch_bounds__(1024) wc_decide_kernel(int* __restrict__ state
     if (threadIdx.x == 0) {
         if (rebuild) state[WS_USABLE] = 0;
         state[WS_REBUILD] = rebuild ? 1 : 0;
+        *hflag = rebuild ? 1 : 0;                        // for the host, whenever it looks (launch_mma_t)
     }
 }
 
@@ -689,11 +690,19 @@ static int launch_mma_mode(const tcp_ctx* c, cudaStream_t st) {
 template <int MH, int NN>
 static int launch_mma_t(const tcp_ctx* c, const float* theta, cudaStream_t st) {
     int rc;
-    wc_decide_kernel<<<1, 1024, 0, st>>>(c->w_state, c->w_cap > 0 && c->w_enable ? 1 : 0, theta, c->w_theta, c->nproj);
+    // The three rebuild kernels (count, scan, fill) exit at once unless wc_decide_kernel raised WS_REBUILD, but even that costs
+    // ~20 us per call.  The host therefore launches them only while the verdict it last SAW (a word of mapped pinned memory that
+    // wc_decide_kernel writes; read here without any synchronisation, so possibly several calls old) says a rebuild is due.  A
+    // change of angles the host has not seen yet is still caught on the device in the same call: wc_decide_kernel clears
+    // WS_USABLE, the cached kernel exits and the direct kernel (same results bit for bit) runs until the rebuild is launched.
+    const bool maybe_rebuild = *c->w_hflag != 0;
+    wc_decide_kernel<<<1, 1024, 0, st>>>(c->w_state, c->w_cap > 0 && c->w_enable ? 1 : 0, theta, c->w_theta, c->nproj, c->w_hflag);
     if (c->w_cap > 0) {
-        if ((rc = launch_mma_mode<MH, 16, GM_COUNT>(c, st))) return rc;
-        wc_scan_kernel<<<1, 1024, 0, st>>>(c->w_count, c->w_off, c->g_nitems * NSUB, c->w_cap, c->w_state);
-        if ((rc = launch_mma_mode<MH, 16, GM_FILL>(c, st))) return rc;
+        if (maybe_rebuild) {
+            if ((rc = launch_mma_mode<MH, 16, GM_COUNT>(c, st))) return rc;
+            wc_scan_kernel<<<1, 1024, 0, st>>>(c->w_count, c->w_off, c->g_nitems * NSUB, c->w_cap, c->w_state);
+            if ((rc = launch_mma_mode<MH, 16, GM_FILL>(c, st))) return rc;
+        }
         if ((rc = launch_mma_mode<MH, NN, GM_CACHED>(c, st))) return rc;
     }
     return launch_mma_mode<MH, NN, GM_DIRECT>(c, st);
@@ -707,6 +716,12 @@ int grid_mma_cache_setup(tcp_ctx* c) {
     c->w_cap = 0;
     if (cudaMalloc((void**)&c->w_state, 4 * sizeof(int)) != cudaSuccess) { cudaGetLastError(); c->w_state = nullptr; return set_error(TCP_ENOMEM, "weight cache state"); }
     cudaMemset(c->w_state, 0, 4 * sizeof(int));
+    {
+        int* hf = nullptr;
+        if (cudaHostAlloc((void**)&hf, sizeof(int), cudaHostAllocMapped) != cudaSuccess) { cudaGetLastError(); return set_error(TCP_ENOMEM, "weight cache host flag"); }
+        *hf = 1;                                                            // nothing built yet
+        c->w_hflag = hf;
+    }
     if (cudaMalloc((void**)&c->w_theta, (size_t)c->nproj * sizeof(float)) != cudaSuccess) { cudaGetLastError(); c->w_theta = nullptr; return set_error(TCP_ENOMEM, "weight cache angles"); }
     cudaMemset(c->w_theta, 0xff, (size_t)c->nproj * sizeof(float));
     c->bytes += 16 + (size_t)c->nproj * sizeof(float);
@@ -732,6 +747,7 @@ int grid_mma_cache_setup(tcp_ctx* c) {
 
 void grid_mma_cache_free(tcp_ctx* c) {
     cudaFree(c->w_state); cudaFree(c->w_theta); cudaFree(c->w_count); cudaFree(c->w_off); cudaFree(c->w_rec); cudaFree(c->w_samp);
+    if (c->w_hflag) cudaFreeHost((void*)c->w_hflag);
 }
 
 // Enqueue the tensor-core gridding of the spectrum into the grid (fp16 storage only); the plan

@@ -439,8 +439,8 @@ int tcp_launches_per_recon(const tcp_ctx* c) {
     if (!c) return 0;
     const int crop = (c->out_pad ? 1 : 0) - (rows_fuses_normalize(c) ? 1 : 0) + (c->zinger_dif > 0.0 ? 1 : 0) + (c->ring_alpha > 0.0 ? 3 : 0);   // tcp_create_det: + the cut-out copy; fused S1+S2: - normalise
     if (c->algorithm == TCP_ALG_LINE) return 4 + crop;                   // trig, normalise, filter, backprojection
-    if (c->grid_impl == TCP_GRID_MMA)       // + plan, cache decide (+ count, scan, fill, cached kernel: most exit at once) (+ reduce)
-        return 8 + (c->w_cap > 0 ? 4 : 0) + (c->g_nred ? 1 : 0) + crop;
+    if (c->grid_impl == TCP_GRID_MMA)       // + plan, cache decide (+ cached kernel) (+ reduce); NOT counted: count, scan, fill of a call that may have to rebuild the cache
+        return 8 + (c->w_cap > 0 ? 1 : 0) + (c->g_nred ? 1 : 0) + crop;
     if (c->grid_impl == TCP_GRID_TILE) return 7 + (c->g_nred ? 1 : 0) + crop;   // + plan (+ reduce)
     return 6 + crop;                                                     // (scatter adds a memset, not a kernel)
 }
