@@ -366,8 +366,12 @@ int grid_tile_setup(tcp_ctx* c) {
                 np = c->nproj;
                 if (rho > rd + 1.0) np = std::min<double>(np, c->nproj * 2.0 * asin(std::min(1.0, rd / rho)) / 3.14159265358979 * 0.75);
             }
-            est[(size_t)ty * tiles + tx] = np * chord_avg + 64.0;        // + fixed per-tile cost
-            total += est[(size_t)ty * tiles + tx];
+            // Samples lie at radius <= n and reach MH cells further; rd bounds the tile's half diagonal plus MH, so a tile whose
+            // centre is more than n + rd + 2 from DC (the corners of the grid, a fifth of it) receives nothing, nor do its periodic
+            // images, which are further still: it gets no work item and is never written; the grid is zeroed once instead.
+            const bool empty = rho - rd > n + 2;
+            est[(size_t)ty * tiles + tx] = empty ? -1.0 : np * chord_avg + 64.0;        // + fixed per-tile cost
+            if (!empty) total += est[(size_t)ty * tiles + tx];
         }
     // the floor keeps the per-item fixed cost small against its work; a grid with fewer tiles than CTA slots (M <= 512) is
     // bound by the latency of one CTA's walk instead, and splits four times finer (C1: gridding 0.142 -> 0.054 ms)
@@ -378,6 +382,7 @@ int grid_tile_setup(tcp_ctx* c) {
     std::vector<int4> red;
     int nslots = 0;
     for (int t = 0; t < tiles * tiles; ++t) {
+        if (est[t] < 0.0) continue;              // no sample can reach the tile: no item, its cells stay zero (tcp_ctx::grid_dirty)
         int S = (int)ceil(est[t] / cap);
         S = std::max(1, std::min(S, std::min(64, c->nproj)));
         int slot0 = -1;

@@ -253,6 +253,7 @@ static tcp_ctx* create_impl(int n, int ndet, int pad_l, int nproj, int nz_chunk,
     }
     tcp_ctx* c = (tcp_ctx*)calloc(1, sizeof(tcp_ctx));
     if (!c) { set_error(TCP_ENOMEM, "out of host memory"); return nullptr; }
+    c->grid_dirty = 1;            // the griddings that skip the empty corner tiles zero the grid on their first call
     c->n = n; c->M = 2 * n; c->nproj = nproj; c->nz = nz_chunk; c->npair = (nz_chunk + 1) / 2;
     c->dtype = dtype; c->filter = filter; c->m = m; c->kernel = kernel; c->center = center;
     c->ndet = ndet; c->pad_l = pad_l;
@@ -323,6 +324,15 @@ int tcp_normalize(tcp_ctx* c, const uint16_t* raw, const float* flat, const floa
     return launch_normalize(c, raw, flat, dark, (cudaStream_t)stream);
 }
 
+// The tile and tensor-core griddings have no work item for the tiles no sample can reach (grid_tile_setup): those cells are
+// zeroed here, once per context and again after any tcp_set_option (which may change the layout or the writer of the grid).
+static int clean_grid(tcp_ctx* c, cudaStream_t st) {
+    if (!c->grid_dirty) return TCP_OK;
+    TCP_CUDA_CHECK(cudaMemsetAsync(c->grid, 0, (size_t)c->npair * c->M * c->M * (c->half_store ? sizeof(__half2) : sizeof(float2)), st));
+    c->grid_dirty = 0;
+    return TCP_OK;
+}
+
 int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* dark, const float* theta, void* out,
               tcp_stream_t stream) {
     if (!c || !raw || !flat || !dark || !theta || !out) return set_error(TCP_EINVAL, "NULL argument");
@@ -363,7 +373,10 @@ int tcp_recon(tcp_ctx* c, const uint16_t* raw, const float* flat, const float* d
     TCP_MARK(3);
     if (c->grid_impl == TCP_GRID_SCATTER_ATOMIC) rc = launch_grid_scatter(c, st);
     else if (c->grid_impl == TCP_GRID_GATHER) rc = launch_grid_gather(c, theta, st);
-    else rc = launch_grid_tile(c, theta, st);
+    else {
+        if ((rc = clean_grid(c, st))) return rc;
+        rc = launch_grid_tile(c, theta, st);
+    }
     if (rc) return rc;
     TCP_MARK(4);
     if ((rc = ifft2_on_mma(c) ? launch_cols_mma(c, st) : launch_ifft_cols(c, st))) return rc;
@@ -411,7 +424,10 @@ int tcp_recon_try(tcp_ctx* c, const uint16_t* raw, const float* flat, const floa
     if ((rc = rows_on_mma(&t) ? launch_rows_mma(&t, st, nullptr) : launch_rows(&t, st))) return rc;
     if (c->grid_impl == TCP_GRID_SCATTER_ATOMIC) rc = launch_grid_scatter(&t, st);
     else if (c->grid_impl == TCP_GRID_GATHER) rc = launch_grid_gather(&t, theta, st);
-    else rc = launch_grid_tile(&t, theta, st);
+    else {
+        if ((rc = clean_grid(c, st))) return rc;        // all npair planes of the context's grid
+        rc = launch_grid_tile(&t, theta, st);
+    }
     if (rc) return rc;
     if ((rc = ifft2_on_mma(&t) ? launch_cols_mma(&t, st) : launch_ifft_cols(&t, st))) return rc;
     if ((rc = ifft2_on_mma(&t) ? launch_irows_mma(&t, c->out_pad ? c->out_pad : out, st) : launch_ifft_rows(&t, c->out_pad ? c->out_pad : out, st))) return rc;
@@ -502,6 +518,7 @@ int tcp_set_param(tcp_ctx* c, int param, double value) {
 
 int tcp_set_option(tcp_ctx* c, int option, int value) {
     if (!c) return set_error(TCP_EINVAL, "NULL context");
+    c->grid_dirty = 1;           // an option may change the grid's layout or writer: the never-written corner tiles are zeroed again
     if (option == TCP_OPT_GRID_IMPL) {
         if (value < TCP_GRID_GATHER || value > TCP_GRID_MMA) return set_error(TCP_EINVAL, "bad grid impl %d", value);
         if ((c->kernel == 1 || c->m == 2) && value != TCP_GRID_TILE && value != TCP_GRID_MMA)

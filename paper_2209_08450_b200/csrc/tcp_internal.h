@@ -59,6 +59,7 @@ struct tcp_ctx {
     int2* g_plan;
     // weight cache of the tcgen05 gridding (k_grid_mma.cu): per-step records, built on the device when theta changes
     int* w_state; int* w_count; int* w_off; uint4* w_rec; unsigned* w_samp; int w_cap, w_enable;
+    int grid_dirty;          // 1: the grid workspace must be zeroed before the next tile / tensor-core gridding (they never write the empty corner tiles)
     volatile int* w_hflag;   // pinned, mapped: the last wc_decide_kernel's verdict (1: the cache must be rebuilt) as the host may see it, late
     float* w_theta;       // [nproj] the angles the cached weights were built for (compared element by element on every call)
     int* g_counter;       // [64] next-item counters of the persistent gridding CTAs, zeroed by the plan kernel
