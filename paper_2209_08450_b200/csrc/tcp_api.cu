@@ -325,7 +325,7 @@ int tcp_normalize(tcp_ctx* c, const uint16_t* raw, const float* flat, const floa
 }
 
 // The tile and tensor-core griddings have no work item for the tiles no sample can reach (grid_tile_setup): those cells are
-// zeroed here, once per context and again after any tcp_set_option (which may change the layout or the writer of the grid).
+// zeroed here, once per context and again after a tcp_set_option that may change the layout or the writer of the grid.
 static int clean_grid(tcp_ctx* c, cudaStream_t st) {
     if (!c->grid_dirty) return TCP_OK;
     TCP_CUDA_CHECK(cudaMemsetAsync(c->grid, 0, (size_t)c->npair * c->M * c->M * (c->half_store ? sizeof(__half2) : sizeof(float2)), st));
@@ -518,7 +518,8 @@ int tcp_set_param(tcp_ctx* c, int param, double value) {
 
 int tcp_set_option(tcp_ctx* c, int option, int value) {
     if (!c) return set_error(TCP_EINVAL, "NULL context");
-    c->grid_dirty = 1;           // an option may change the grid's layout or writer: the never-written corner tiles are zeroed again
+    // these two change the grid's layout or its writer: the corner tiles that are never written must be zeroed again
+    if (option == TCP_OPT_GRID_IMPL || option == TCP_OPT_TCFFT) c->grid_dirty = 1;
     if (option == TCP_OPT_GRID_IMPL) {
         if (value < TCP_GRID_GATHER || value > TCP_GRID_MMA) return set_error(TCP_EINVAL, "bad grid impl %d", value);
         if ((c->kernel == 1 || c->m == 2) && value != TCP_GRID_TILE && value != TCP_GRID_MMA)
