@@ -932,3 +932,31 @@ def test_binding_checks_host_tensors_and_device_angles():
     with pytest.raises(tcp.TcpError, match="16-byte"):
         r.recon(dev[0], shifted, dev[2], dev[3])
     r.close()
+
+
+def test_grid_corners_stay_zero_across_option_changes():
+    """The tile and tensor-core griddings have no work item for the corner tiles no sample can reach; the grid is zeroed once
+    per context and again after an option that changes its layout or writer.  Switching the gridding implementation back
+    and forth on one context (strip-major <-> row-major grid) must therefore reproduce the first result bit for bit, and the
+    corner cells of the grid workspace must read zero."""
+    tcp = _tcp()
+    w = sg.make_workload("C2", scale=2)               # n = 256: the corner tiles exist (M = 512, 16 x 16 tiles)
+    rows = list(range(40, 46))
+    raw, flat, dark, theta = _inputs(w, rows)
+    dev = _to_dev(raw, flat, dark, theta)
+    r = tcp.Recon(w.n, w.nproj, len(rows), w.center, "f16", w.filter)
+    first = r.recon(*dev).clone()
+    g = r.workspace("grid")                             # [npair][M l2][M l1], FFT order
+    M = 2 * w.n
+    assert float(g[:, M // 2 - 8:M // 2 + 8, M // 2 - 8:M // 2 + 8].abs().max()) == 0.0      # |l1|, |l2| ~ n: the far corner
+    assert float(g.abs().max()) > 0.0
+    r.set_grid_impl("tile")
+    tile = r.recon(*dev).clone()
+    r.set_grid_impl("mma")
+    again = r.recon(*dev).clone()
+    assert torch.equal(again, first)
+    ref = orc.recon(raw, flat, dark, theta, w.center, w.filter, orc.KB + 2, "grid")
+    for z in range(len(rows)):
+        check(tile[z].float().cpu().numpy(), ref[z], "f16", vol=ref, tag=("tile", z))
+        check(first[z].float().cpu().numpy(), ref[z], "f16", vol=ref, tag=("mma", z))
+    r.close()
