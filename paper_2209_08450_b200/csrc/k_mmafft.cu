@@ -279,6 +279,11 @@ __global__ void __launch_bounds__(NT, 2) rows_mma_kernel(const __half* __restric
 __device__ __forceinline__ void st_v4(void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
     asm volatile("st.global.v4.b32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
 }
+// Samples lie within radius n of DC and reach at most 4 cells further, so in a strip of columns |x| >= xmin only the rows
+// |l2| < h = sqrt((n + 8)^2 - xmin^2) can be non-zero (a fifth of the grid is corners that the gridding never writes): the
+// rows [0, h) and [M - h, M) come from the grid, the rows between from this block of zeros, which stays in L2.  Row positions
+// are swizzled within aligned groups of 8 (swz<4>), so h is rounded up to a multiple of 8.
+__device__ __align__(128) uint4 g_zero_rows[N];
 __global__ void __launch_bounds__(NT, 2) cols_mma_kernel(const uint4* __restrict__ grid, uint2* __restrict__ p1arr,
                                                           const float2* __restrict__ tw, const uint32_t* __restrict__ atab, int nunits) {
     constexpr int n = N / 2;
@@ -286,15 +291,29 @@ __global__ void __launch_bounds__(NT, 2) cols_mma_kernel(const uint4* __restrict
     float2* T1TAB = reinterpret_cast<float2*>(L + 4 * N);
     uint64_t* bar = reinterpret_cast<uint64_t*>(reinterpret_cast<unsigned char*>(T1TAB) + T1_BYTES);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, c = lane & 3;
+    auto fetch_strip = [&](int unit) {                                    // thread 0 only: 64 KB in one, or in three copies
+        const int l1 = 4 * (unit % (N / 4));
+        const int xmin = l1 < n ? l1 : N - l1 - 3;                        // smallest |x| of the strip's four columns
+        const int R = n + 8;
+        int h = (int)sqrtf((float)(R * R - xmin * xmin)) + 2;
+        h = (h + 7) & ~7;
+        const uint4* src = grid + (size_t)unit * N;
+        uint4* dst = reinterpret_cast<uint4*>(L);
+        mbar_expect_tx(bar, 4 * N * 4);
+        if (2 * h >= N) {
+            bulk_g2s(dst, src, 4 * N * 4, bar);
+        } else {
+            bulk_g2s(dst, src, h * 16, bar);
+            bulk_g2s(dst + h, g_zero_rows, (N - 2 * h) * 16, bar);
+            bulk_g2s(dst + (N - h), src + (N - h), h * 16, bar);
+        }
+    };
     if (tid == 0) {
         mbar_init(bar, 1);
         fence_mbar_init();
     }
     __syncthreads();
-    if (tid == 0 && (int)blockIdx.x < nunits) {
-        mbar_expect_tx(bar, 4 * N * 4);
-        bulk_g2s(L, grid + (size_t)blockIdx.x * N, 4 * N * 4, bar);
-    }
+    if (tid == 0 && (int)blockIdx.x < nunits) fetch_strip(blockIdx.x);
     AFrag An, Ac;
     load_afrag(An, atab, AV_NAT, lane);
     flip_afrag(An);
@@ -346,8 +365,7 @@ __global__ void __launch_bounds__(NT, 2) cols_mma_kernel(const uint4* __restrict
     __syncthreads();                      // the lines are free for the next unit
     if (tid == 0 && unit + (int)gridDim.x < nunits) {
         fence_proxy_async();
-        mbar_expect_tx(bar, 4 * N * 4);
-        bulk_g2s(L, grid + (size_t)(unit + gridDim.x) * N, 4 * N * 4, bar);
+        fetch_strip(unit + gridDim.x);
     }
     }
 }
